@@ -1,0 +1,478 @@
+"""Pins of the CPU oracle against what the mathematics fixes.
+
+None of these retype the oracle's own formulas: they are closed forms from textbooks, Ward identities,
+symmetries, and an independent colour-DRESSED recursion (explicit f^{abc}, T^a, full Feynman rules)
+written here in numpy.  A dropped term, wrong sign, wrong index or transposed operand in
+oracle/me_oracle.c fails at least one of them.
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2510_05392_b200 import inputs
+
+GS = math.sqrt(4 * math.pi * inputs.PARAMS["aS"])
+MT = inputs.PARAMS["mT"]
+
+
+def mdot(a, b):
+    return a[..., 0] * b[..., 0] - (a[..., 1:] * b[..., 1:]).sum(-1)
+
+
+# ---------------------------------------------------------------------------------------------
+# P1: e+ e- -> mu+ mu- per-helicity closed form
+# |M_h|^2 = (1 +- cos th)^2 |e^2 + g_{le} g_{lm} s/(s - mZ^2 + i mZ wZ)|^2 for opposite helicities on
+# each fermion line ("+" if lambda_e- = lambda_mu-, th = angle(e-, mu-)), zero otherwise; me = sum/4.
+def _ee_couplings(P):
+    e2 = 4 * math.pi / P["aEWM1"]
+    e = math.sqrt(e2)
+    sw2 = 1 - P["mW"] ** 2 / P["mZ"] ** 2
+    sw, cw = math.sqrt(sw2), math.sqrt(1 - sw2)
+    return e2, e * (-0.5 + sw2) / (sw * cw), e * sw / cw
+
+
+def test_p1_eemumu_closed_form_and_mask(params):
+    p = inputs.momenta("epem_mupmum", 64)
+    me, mh = oracle.matrix_elements("epem_mupmum", p, params, per_helicity=True)
+    e2, gL, gR = _ee_couplings(params)
+    s = inputs.SQRT_S ** 2
+    prop = s / (s - params["mZ"] ** 2 + 1j * params["mZ"] * params["wZ"])
+    pe, pm = p[:, 1, 1:], p[:, 3, 1:]
+    cos = (pe * pm).sum(-1) / np.linalg.norm(pe, axis=-1) / np.linalg.norm(pm, axis=-1)
+    good = []
+    tot = np.zeros(len(p))
+    for h in range(16):
+        lam = [1 if (h >> (3 - i)) & 1 else -1 for i in range(4)]
+        if lam[0] == lam[1] or lam[2] == lam[3]:
+            assert np.all(mh[:, h] <= 1e-20 * me)
+            continue
+        good.append(h)
+        ge = gL if lam[1] < 0 else gR
+        gm = gL if lam[3] < 0 else gR
+        sign = 1.0 if lam[1] == lam[3] else -1.0
+        val = (1 + sign * cos) ** 2 * abs(e2 + ge * gm * prop) ** 2 / 4
+        np.testing.assert_allclose(mh[:, h], val, rtol=1e-12)
+        tot += val
+    assert good == [5, 6, 9, 10]
+    np.testing.assert_allclose(me, tot, rtol=1e-12)
+
+
+def test_p1_eemumu_qed_limit(params):
+    # decoupled Z (huge mass): me -> e^4 (1 + cos^2 th)
+    P = dict(params, mZ=1e9, mW=0.8e9, wZ=0.0)
+    p = inputs.momenta("epem_mupmum", 32, seed=3)
+    me = oracle.matrix_elements("epem_mupmum", p, P)
+    pe, pm = p[:, 1, 1:], p[:, 3, 1:]
+    cos = (pe * pm).sum(-1) / np.linalg.norm(pe, axis=-1) / np.linalg.norm(pm, axis=-1)
+    e4 = (4 * math.pi / P["aEWM1"]) ** 2
+    np.testing.assert_allclose(me, e4 * (1 + cos ** 2), rtol=1e-9)
+
+
+# ---------------------------------------------------------------------------------------------
+# P2: analytic g g -> t tbar (zero width), e.g. Ellis-Stirling-Webber:
+# me = g^4 [1/(6 t1 t2) - 3/8][t1^2 + t2^2 + rho - rho^2/(4 t1 t2)]
+def test_p2_ggttx_analytic(params):
+    P = dict(params, wT=0.0)
+    p = inputs.momenta("gg_ttx", 256)
+    me = oracle.matrix_elements("gg_ttx", p, P)
+    m = P["mT"]
+    s = mdot(p[:, 0] + p[:, 1], p[:, 0] + p[:, 1])
+    t = mdot(p[:, 0] - p[:, 2], p[:, 0] - p[:, 2])
+    u = mdot(p[:, 0] - p[:, 3], p[:, 0] - p[:, 3])
+    t1, t2, rho = (m * m - t) / s, (m * m - u) / s, 4 * m * m / s
+    ana = GS ** 4 * (1 / (6 * t1 * t2) - 3 / 8) * (t1 ** 2 + t2 ** 2 + rho - rho ** 2 / (4 * t1 * t2))
+    np.testing.assert_allclose(me, ana, rtol=1e-11)
+
+
+# ---------------------------------------------------------------------------------------------
+# helpers: physical polarisation vectors built HERE (not taken from the oracle)
+def _transverse(k, rng):
+    """random complex vector e with e.k = 0 for a massless k (not normalised: Ward identity is linear)."""
+    e = rng.normal(size=4) + 1j * rng.normal(size=4)
+    nref = np.array([1.0, 0.3, -0.5, 0.2])
+    return e - mdot(e, k) / mdot(nref, k) * nref
+
+
+def _gluon_particle(ig):
+    return ig if ig < 2 else ig + 2
+
+
+# P3: Ward identity: eps_i -> k_i kills every partial amplitude (zero width, other gluons transverse)
+@pytest.mark.parametrize("proc,n", [("gg_ttx", 2), ("gg_ttxg", 3), ("gg_ttxgg", 4), ("gg_ttxggg", 5)])
+def test_p3_gauge_invariance(proc, n):
+    p = inputs.momenta(proc, 2, seed=7)[1]
+    rng = np.random.default_rng(11)
+    hel = [1, -1, 1, -1, 1, 1, -1][: n + 2]
+    eps = np.array([_transverse(p[_gluon_particle(i)], rng) for i in range(n)])
+    A0 = oracle.partial_amplitudes(n, p, hel, MT, 0.0, GS, eps_override=eps)
+    scale = np.abs(A0).max()
+    assert scale > 0
+    for ig in range(n):
+        e = eps.copy()
+        e[ig] = p[_gluon_particle(ig)] / 100.0      # k_i (sign and scale irrelevant), same size as eps
+        A1 = oracle.partial_amplitudes(n, p, hel, MT, 0.0, GS, eps_override=e)
+        assert np.abs(A1).max() < 1e-11 * scale, (ig, np.abs(A1).max() / scale)
+    # with a finite width the identity must NOT hold exactly (reading A4): ~1e-3
+    e = eps.copy()
+    e[0] = p[0] / 100.0
+    A2 = oracle.partial_amplitudes(n, p, hel, MT, 1.4915, GS, eps_override=e)
+    assert np.abs(A2).max() > 1e-7 * scale
+
+
+# ---------------------------------------------------------------------------------------------
+# P4: colour-DRESSED recursion with the full Feynman rules (Peskin conventions), numpy, written here.
+#   qqg vertex i g gamma^mu T^a;  ggg vertex g f^{abc}[g^{mn}(k1-k2)^r + g^{nr}(k2-k3)^m + g^{rm}(k3-k1)^n]
+#   gggg vertex -i g^2 [f^{abe}f^{cde}(g^{mr}g^{ns}-g^{ms}g^{nr}) + f^{ace}f^{bde}(g^{mn}g^{rs}-g^{ms}g^{nr})
+#                       + f^{ade}f^{bce}(g^{mn}g^{rs}-g^{mr}g^{ns})]
+#   gluon propagator -i g_{mn} d^{ab}/k^2;  quark propagator i(qslash+m)/(q^2-m^2+i m G)
+# Chiral (Weyl) gamma matrices here -- a third representation, different from the oracle's Dirac one.
+_s0 = np.eye(2, dtype=complex)
+_sig = [np.array([[0, 1], [1, 0]], dtype=complex), np.array([[0, -1j], [1j, 0]]), np.array([[1, 0], [0, -1]], dtype=complex)]
+_Z2 = np.zeros((2, 2), dtype=complex)
+GAM = [np.block([[_Z2, _s0], [_s0, _Z2]])] + [np.block([[_Z2, s], [-s, _Z2]]) for s in _sig]
+METRIC = np.diag([1.0, -1.0, -1.0, -1.0])
+
+
+def _slash(a):
+    return a[0] * GAM[0] - a[1] * GAM[1] - a[2] * GAM[2] - a[3] * GAM[3]
+
+
+def _su3():
+    T = oracle.su3_generators()   # only the generator matrices (data), checked below against the algebra
+    f = np.zeros((8, 8, 8))
+    for a in range(8):
+        for b in range(8):
+            comm = T[a] @ T[b] - T[b] @ T[a]
+            for c in range(8):
+                f[a, b, c] = (-2j * np.trace(comm @ T[c])).real
+    return T, f
+
+
+def test_su3_generators_algebra():
+    T, f = _su3()
+    for a in range(8):
+        for b in range(8):
+            assert abs(np.trace(T[a] @ T[b]) - (0.5 if a == b else 0.0)) < 1e-15
+            comm = T[a] @ T[b] - T[b] @ T[a]
+            np.testing.assert_allclose(comm, 1j * np.einsum("c,cij->ij", f[a, b], T), atol=1e-15)
+    assert abs(f[0, 1, 2] - 1.0) < 1e-15 and abs(f[3, 4, 7] - math.sqrt(3) / 2) < 1e-15
+    # Casimirs: sum_a T^a T^a = 4/3, f^{acd} f^{bcd} = 3 delta^{ab}
+    np.testing.assert_allclose(sum(T[a] @ T[a] for a in range(8)), 4 / 3 * np.eye(3), atol=1e-15)
+    np.testing.assert_allclose(np.einsum("acd,bcd->ab", f, f), 3 * np.eye(8), atol=1e-14)
+
+
+def _weyl_spinors(p, m):
+    """numerical basis of u / v spinors in the chiral representation from projectors (p-slash +- m):
+    returns functions giving ubar(p,lambda) and v(p,lambda) as helicity eigenstates, built by projecting
+    arbitrary vectors -- independent of the oracle's explicit formulas."""
+    E = p[0]
+    pv = p[1:]
+    pp = np.linalg.norm(pv)
+    n = pv / pp
+    Sig = sum(n[i] * np.block([[_sig[i], _Z2], [_Z2, _sig[i]]]) for i in range(3))   # helicity operator (both reps)
+
+    def proj(sign_m, lam, seed):
+        w = np.random.default_rng(seed).normal(size=4) + 1j * np.random.default_rng(seed + 1).normal(size=4)
+        x = (_slash(p) + sign_m * m * np.eye(4)) @ (0.5 * (np.eye(4) + lam * Sig)) @ w
+        x = x / np.sqrt((x.conj() @ x).real) * math.sqrt(2 * E)
+        return x
+
+    def ubar(lam):
+        u = proj(+1, lam, 100)                 # (pslash - m) u = 0  <=>  u in image of (pslash + m)
+        return u.conj() @ GAM[0]
+
+    def v(lam):
+        return proj(-1, -lam, 200)             # (pslash + m) v = 0, spin operator eigenvalue is minus the helicity
+    return ubar, v
+
+
+def _polvec(p, lam):
+    """helicity polarisation vector from scratch: eigenvector of the rotation generator about p."""
+    pv = p[1:]
+    n = pv / np.linalg.norm(pv)
+    # (n.S) with (S_i)_{jk} = -i eps_{ijk}; eigenvector with eigenvalue lam
+    S = np.zeros((3, 3), dtype=complex)
+    epsl = np.zeros((3, 3, 3))
+    epsl[0, 1, 2] = epsl[1, 2, 0] = epsl[2, 0, 1] = 1
+    epsl[0, 2, 1] = epsl[2, 1, 0] = epsl[1, 0, 2] = -1
+    for i in range(3):
+        S += n[i] * (-1j) * epsl[i]
+    w, vec = np.linalg.eig(S)
+    e3 = vec[:, np.argmin(np.abs(w - lam))]
+    return np.concatenate([[0.0], e3 / np.sqrt((e3.conj() @ e3).real)])
+
+
+def _dressed_amplitude(n, p, hel, cols, ci, cj, width, T, f):
+    """i*M for g g -> t tbar (n-2)g with external gluon colours cols, top colour ci, antitop colour cj."""
+    g = GS
+    ks, eps = [], []
+    for ig in range(n):
+        ip = _gluon_particle(ig)
+        e = _polvec(p[ip], hel[ip])
+        if ig >= 2:
+            e = e.conj()
+        eps.append(e)
+        ks.append(p[ip] if ig < 2 else -p[ip])
+    ubar_f, _ = _weyl_spinors(p[2], MT)
+    _, v_f = _weyl_spinors(p[3], MT)
+    ubar, v = ubar_f(hel[2]), v_f(hel[3])
+    full = (1 << n) - 1
+    K = {S: sum(ks[i] for i in range(n) if S >> i & 1) for S in range(1, full + 1)}
+    J = {}   # subset -> [8][4] contravariant current including propagator
+
+    def lower(x):
+        return x * np.array([1.0, -1.0, -1.0, -1.0])
+
+    def subsets(S):
+        sub = (S - 1) & S
+        while sub:
+            yield sub
+            sub = (sub - 1) & S
+
+    for S in sorted(range(1, full + 1), key=lambda s: bin(s).count("1")):
+        bits = [i for i in range(n) if S >> i & 1]
+        if len(bits) == 1:
+            cur = np.zeros((8, 4), dtype=complex)
+            cur[cols[bits[0]]] = eps[bits[0]]
+            J[S] = cur
+            continue
+        cur = np.zeros((8, 4), dtype=complex)
+        k3 = -K[S]
+        for S1 in subsets(S):
+            S2 = S ^ S1
+            if S1 > S2:
+                continue                        # unordered pairs
+            A, B, k1, k2 = J[S1], J[S2], K[S1], K[S2]
+            AB = np.einsum("am,bm->ab", A, lower(B))
+            t1 = np.einsum("ab,r->abr", AB, k1 - k2)
+            t2 = np.einsum("a,br->abr", A @ lower(k2 - k3), B)
+            t3 = np.einsum("b,ar->abr", B @ lower(k3 - k1), A)
+            cur += g * np.einsum("abc,abr->cr", f, t1 + t2 + t3)
+        for S1 in subsets(S):
+            for S2 in subsets(S ^ S1):
+                S3 = S ^ S1 ^ S2
+                if not (S1 < S2 < S3):
+                    continue                    # unordered triples
+                A, B, C = J[S1], J[S2], J[S3]
+                AB = np.einsum("am,bm->ab", A, lower(B))
+                AC = np.einsum("am,cm->ac", A, lower(C))
+                BC = np.einsum("bm,cm->bc", B, lower(C))
+                ff1 = np.einsum("abe,cde->abcd", f, f)
+                ff2 = np.einsum("ace,bde->abcd", f, f)
+                ff3 = np.einsum("ade,bce->abcd", f, f)
+                L1 = np.einsum("ac,bs->abcs", AC, B) - np.einsum("as,bc->abcs", A, BC)
+                L2 = np.einsum("ab,cs->abcs", AB, C) - np.einsum("as,bc->abcs", A, BC)
+                L3 = np.einsum("ab,cs->abcs", AB, C) - np.einsum("ac,bs->abcs", AC, B)
+                cur += -1j * g * g * (np.einsum("abcd,abcs->ds", ff1, L1) + np.einsum("abcd,abcs->ds", ff2, L2)
+                                      + np.einsum("abcd,abcs->ds", ff3, L3))
+        J[S] = cur * (-1j) / mdot(K[S], K[S])
+    # quark line: Psi[S] = row spinor [3 colours][4]
+    Psi = {0: np.zeros((3, 4), dtype=complex)}
+    Psi[0][ci] = ubar
+    for S in sorted(range(1, full), key=lambda s: bin(s).count("1")):
+        acc = np.zeros((3, 4), dtype=complex)
+        for S2 in [S] + list(subsets(S)):
+            S1 = S ^ S2
+            for c in range(8):
+                acc += 1j * g * (T[c].T @ Psi[S1]) @ _slash(J[S2][c])      # (Psi T^c)_l = sum_l' Psi_l' T^c_{l' l}
+        q = p[2] - K[S]
+        prop = 1j * (_slash(q) + MT * np.eye(4)) / (mdot(q, q) - MT ** 2 + 1j * MT * width)
+        Psi[S] = acc @ prop
+    amp = 0
+    for S2 in range(1, full + 1):
+        S1 = full ^ S2
+        for c in range(8):
+            amp += 1j * g * ((T[c].T @ Psi[S1]) @ _slash(J[S2][c]) @ v)[cj]
+    return amp
+
+
+def _decomposed(n, A, cols, ci, cj, T):
+    tot = 0
+    for s, perm in enumerate(itertools.permutations(range(n))):
+        M = np.eye(3, dtype=complex)
+        for gidx in perm:
+            M = M @ T[cols[gidx]]
+        tot += M[ci, cj] * A[s]
+    return tot
+
+
+@pytest.mark.parametrize("proc,n,nsample", [("gg_ttx", 2, 40), ("gg_ttxg", 3, 40), ("gg_ttxgg", 4, 40)])
+def test_p4_colour_dressed_amplitudes(proc, n, nsample):
+    """M^{a1..an}_{ij} from the dressed recursion == sum_sigma (T^sigma)_{ij} A(sigma) up to ONE global phase."""
+    T, f = _su3()
+    p = inputs.momenta(proc, 3, seed=5)[2]
+    rng = np.random.default_rng(3)
+    ratios = []
+    for _ in range(nsample):
+        hel = [int(x) for x in rng.choice([-1, 1], size=n + 2)]
+        cols = [int(x) for x in rng.integers(0, 8, size=n)]
+        ci, cj = int(rng.integers(0, 3)), int(rng.integers(0, 3))
+        A = oracle.partial_amplitudes(n, p, hel, MT, 1.4915, GS)
+        dec = _decomposed(n, A, cols, ci, cj, T)
+        full = _dressed_amplitude(n, p, hel, cols, ci, cj, 1.4915, T, f)
+        # spinor/polarisation phases differ between the two constructions but depend on (hel) only:
+        # compare moduli for every sample ...
+        if abs(dec) < 1e-14 * np.abs(A).max():
+            assert abs(full) < 1e-10 * np.abs(A).max()
+            continue
+        assert abs(abs(full) / abs(dec) - 1) < 1e-9, (hel, cols, ci, cj, full, dec)
+        ratios.append((tuple(hel), full / dec))
+    # (the colour-independence of the phase is checked in test_p4_phase_is_colour_independent)
+    assert len(ratios) >= 2          # most random colour assignments of small n vanish identically
+
+
+def test_p4_phase_is_colour_independent():
+    """For one helicity assignment, full/decomposed must be the same complex number for all colours."""
+    T, f = _su3()
+    n = 3
+    p = inputs.momenta("gg_ttxg", 1, seed=9)[0]
+    hel = [1, -1, -1, 1, 1]
+    A = oracle.partial_amplitudes(n, p, hel, MT, 1.4915, GS)
+    rng = np.random.default_rng(8)
+    rs = []
+    for _ in range(60):
+        cols = [int(x) for x in rng.integers(0, 8, size=n)]
+        ci, cj = int(rng.integers(0, 3)), int(rng.integers(0, 3))
+        dec = _decomposed(n, A, cols, ci, cj, T)
+        if abs(dec) < 1e-12 * np.abs(A).max():
+            continue
+        rs.append(_dressed_amplitude(n, p, hel, cols, ci, cj, 1.4915, T, f) / dec)
+    rs = np.array(rs)
+    assert len(rs) > 10
+    np.testing.assert_allclose(rs, rs[0], rtol=1e-9)
+    assert abs(abs(rs[0]) - 1) < 1e-9
+
+
+def test_p4_full_colour_sum_ggttx(params):
+    """sum over ALL colours of |M|^2 from the dressed recursion == oracle's A^dagger C A, per helicity (n = 2)."""
+    T, f = _su3()
+    n = 2
+    p = inputs.momenta("gg_ttx", 1, seed=2)
+    me, mh = oracle.matrix_elements("gg_ttx", p, params, per_helicity=True)
+    for h in (0b0110, 0b1011, 0b0000):
+        hel = [1 if (h >> (3 - i)) & 1 else -1 for i in range(4)]
+        tot = 0.0
+        for cols in itertools.product(range(8), repeat=n):
+            for ci in range(3):
+                for cj in range(3):
+                    tot += abs(_dressed_amplitude(n, p[0], hel, list(cols), ci, cj, params["wT"], T, f)) ** 2
+        np.testing.assert_allclose(tot / 256.0, mh[0, h], rtol=1e-10)
+
+
+# ---------------------------------------------------------------------------------------------
+# P5: colour-matrix invariants
+def test_p5_colour_matrix_invariants():
+    CF = 4.0 / 3.0
+    expect_den = {2: 3, 3: 9, 4: 54, 5: 324}
+    rowsum = {2: 14 / 3, 3: 60 / 9, 4: 705 / 54, 5: 9300 / 324}
+    for n in (2, 3, 4, 5):
+        C = oracle.color_matrix(n)
+        nperm = math.factorial(n)
+        assert C.shape == (nperm, nperm)
+        assert oracle.me_oracle.color_matrix_max_imag(n) < 1e-12
+        np.testing.assert_allclose(C, C.T, atol=1e-12)
+        np.testing.assert_allclose(np.diag(C), 3 * CF ** n, rtol=1e-13)
+        # adjacent transposition of the last two gluons is lexicographic neighbour 0 <-> 1
+        np.testing.assert_allclose(C[0, 1], -CF ** (n - 1) / 2, rtol=1e-12)
+        ints = C * expect_den[n]
+        np.testing.assert_allclose(ints, np.round(ints), atol=1e-8)
+        np.testing.assert_allclose(C[0].sum(), rowsum[n], rtol=1e-12)
+        w = np.linalg.eigvalsh(C)
+        assert w.min() > 0
+    np.testing.assert_allclose(oracle.color_matrix(2) * 3, [[16, -2], [-2, 16]], atol=1e-12)
+    np.testing.assert_allclose(oracle.color_matrix(3)[0] * 9, [64, -8, -8, 1, 1, 10], atol=1e-11)
+    assert sorted(set(np.round(oracle.color_matrix(4) * 54).astype(int).ravel())) == [-64, -28, -10, -1, 8, 62, 71, 80, 512]
+    n5 = np.round(oracle.color_matrix(5) * 324).astype(int)
+    assert len(set(n5.ravel())) == 24 and n5.min() == -512 and n5.max() == 4096
+
+
+# ---------------------------------------------------------------------------------------------
+# P6: symmetries of me
+def _rotation(rng):
+    q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    L = np.eye(4)
+    L[1:, 1:] = q
+    return L
+
+
+def _boost(beta):
+    b = np.asarray(beta)
+    b2 = b @ b
+    gam = 1 / math.sqrt(1 - b2)
+    L = np.eye(4)
+    L[0, 0] = gam
+    L[0, 1:] = L[1:, 0] = gam * b
+    L[1:, 1:] += (gam - 1) * np.outer(b, b) / b2
+    return L
+
+
+@pytest.mark.parametrize("proc", ["gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "epem_mupmum"])
+def test_p6_lorentz_invariance(proc, params):
+    nev = 2 if proc == "gg_ttxggg" else 4
+    p = inputs.momenta(proc, nev, seed=4)
+    rng = np.random.default_rng(1)
+    R = _rotation(rng)
+    # rotations: exact symmetry also with the fixed top width
+    me = oracle.matrix_elements(proc, p, params)
+    me2 = oracle.matrix_elements(proc, np.einsum("mn,epn->epm", R, p), params)
+    np.testing.assert_allclose(me2, me, rtol=2e-10)
+    # boosts change the helicity-basis polarisation vectors by a gauge transformation, so the sum over
+    # helicities is boost invariant only where the Ward identity holds: zero top width (reading A4)
+    P0 = dict(params, wT=0.0)
+    L = _boost([0.3, -0.2, 0.4]) @ R
+    me = oracle.matrix_elements(proc, p, P0)
+    me2 = oracle.matrix_elements(proc, np.einsum("mn,epn->epm", L, p), P0)
+    np.testing.assert_allclose(me2, me, rtol=2e-10)
+
+
+@pytest.mark.parametrize("proc", ["gg_ttxgg", "gg_ttxggg"])
+def test_p6_bose_symmetry(proc, params):
+    nev = 2
+    p = inputs.momenta(proc, nev, seed=6)
+    me = oracle.matrix_elements(proc, p, params)
+    q = p.copy()
+    q[:, [4, 5]] = p[:, [5, 4]]                    # swap two final gluons
+    np.testing.assert_allclose(oracle.matrix_elements(proc, q, params), me, rtol=1e-11)
+    q = p.copy()
+    q[:, [0, 1]] = p[:, [1, 0]]                    # swap the two beams (now along -z / +z)
+    np.testing.assert_allclose(oracle.matrix_elements(proc, q, params), me, rtol=1e-11)
+
+
+@pytest.mark.parametrize("proc", ["gg_ttx", "gg_ttxg", "gg_ttxgg", "epem_mupmum"])
+def test_p6_parity_per_helicity(proc, params):
+    """spatial inversion maps helicity h to its complement: me_h(p) = me_{~h}(-p)   (QCD; for e+e- the
+    Z coupling violates parity, so only CP-like total statements hold -- there we check me only changes
+    by the known L<->R swap, i.e. it differs, and the helicity mask maps onto itself)."""
+    p = inputs.momenta(proc, 3, seed=8)
+    me, mh = oracle.matrix_elements(proc, p, params, per_helicity=True)
+    q = p.copy()
+    q[..., 1:] *= -1
+    me2, mh2 = oracle.matrix_elements(proc, q, params, per_helicity=True)
+    ncomb = mh.shape[1]
+    if proc == "epem_mupmum":
+        assert np.array_equal((mh > 0), (mh2[:, ::-1] > 0)[:, :])
+        assert np.abs(mh - mh2[:, ::-1]).max() > 1e-3 * mh.max()    # parity IS violated by the Z
+    else:
+        np.testing.assert_allclose(mh2[:, ::-1], mh, rtol=1e-9, atol=1e-14 * mh.max())
+        np.testing.assert_allclose(me2, me, rtol=1e-11)
+    assert ncomb == 2 ** p.shape[1]
+
+
+# ---------------------------------------------------------------------------------------------
+# P10: the oracle's own rounding error: fp64 vs 80-bit long double
+@pytest.mark.parametrize("proc,nev,tol", [("epem_mupmum", 256, 1e-13), ("gg_ttx", 256, 1e-12), ("gg_ttxg", 128, 1e-11),
+                                          ("gg_ttxgg", 64, 1e-11), ("gg_ttxggg", 16, 1e-11)])
+def test_p10_double_vs_long_double(proc, nev, tol, params):
+    p = inputs.momenta(proc, nev)
+    a = oracle.matrix_elements(proc, p, params)
+    b = oracle.matrix_elements(proc, p, params, long_double=True)
+    assert np.max(np.abs(a / b - 1)) < tol
+
+
+def test_denominators():
+    assert oracle.DENOM == {"epem_mupmum": 4.0, "gg_ttx": 256.0, "gg_ttxg": 256.0, "gg_ttxgg": 512.0, "gg_ttxggg": 1536.0}
