@@ -1,0 +1,77 @@
+"""Host-side generator (diagram enumeration, colour algebra, lowering to the diagram program) on CPU.
+
+Pins: Table 2 of the paper (tests/golden/table2_complexity.txt), the oracle's brute-force colour matrix,
+and the oracle's per-helicity matrix elements through the numpy IR evaluator tests/ir_eval.py.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import ir_eval
+import oracle
+from paper_2510_05392_b200 import inputs
+from paper_2510_05392_b200.gen import colour, diagrams
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _table2():
+    rows = {}
+    for line in open(os.path.join(HERE, "golden", "table2_complexity.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, nd, nc, nh, nw = line.split()
+        rows[name] = (int(nd), int(nc), int(nh), int(nw))
+    return rows
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_diagram_and_colour_counts_match_table2(n):
+    t2 = _table2()
+    proc = diagrams.build_process(n)
+    nd, nc, nh, _ = t2[proc.name]
+    assert proc.ndiagrams == nd
+    assert proc.ncolor == nc == math.factorial(n)
+    assert 2 ** proc.npar == nh
+    # every diagram appears in the program, four-gluon vertices as three terms each
+    assert len({a.diagram for a in proc.amps}) == nd
+
+
+def test_diagram_count_recursion_p7():
+    """psi(n) = sum_j C(n,j) g(j) psi(n-j) with g = 1,1,4,25,220,2485 reproduces Table 2 up to 2->6."""
+    g = [len(diagrams.gluon_trees(tuple(range(k)))) for k in range(1, 7)]
+    assert g == [1, 1, 4, 25, 220, 2485]
+    psi = [1]
+    for n in range(1, 7):
+        psi.append(sum(math.comb(n, j) * g[j - 1] * psi[n - j] for j in range(1, n + 1)))
+    t2 = _table2()
+    assert psi[2:7] == [t2[k][0] for k in ("gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "gg_ttxgggg")]
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_exact_colour_matrix_matches_oracle_brute_force(n):
+    C = colour.colour_matrix(n)
+    den = colour.common_denominator(C)
+    assert den == {2: 3, 3: 9, 4: 54, 5: 324}[n]
+    Cf = np.array([[float(x) for x in r] for r in C])
+    np.testing.assert_allclose(Cf, oracle.color_matrix(n), atol=1e-11)
+    ints = np.array([[int(x * den) for x in r] for r in C])
+    assert np.abs(ints).max() <= 4096          # exactly representable in TF32 (11-bit significand incl. hidden bit)
+
+
+@pytest.mark.parametrize("name,n,hels", [("gg_ttx", 2, None), ("gg_ttxg", 3, None), ("gg_ttxgg", 4, None),
+                                         ("gg_ttxggg", 5, (0, 37, 100, 127))])
+def test_program_matches_oracle_per_helicity(name, n, hels, params):
+    proc = diagrams.build_process(n)
+    C = np.array([[float(x) for x in r] for r in colour.colour_matrix(n)])
+    gs = math.sqrt(4 * math.pi * params["aS"])
+    p = inputs.momenta(name, 2, seed=3)
+    _, mh_o = oracle.matrix_elements(name, p, params, per_helicity=True)
+    npar = proc.npar
+    for h in (range(1 << npar) if hels is None else hels):
+        hel = [1 if (h >> (npar - 1 - i)) & 1 else -1 for i in range(npar)]
+        j = ir_eval.evaluate(proc, p[1], hel, params["mT"], params["wT"])
+        mh = (j.conj() @ C @ j).real * gs ** (2 * n) / oracle.DENOM[name]
+        assert abs(mh / mh_o[1][h] - 1) < 1e-10, (h, mh, mh_o[1][h])
