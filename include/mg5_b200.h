@@ -1,0 +1,127 @@
+/* mg5_b200.h -- C ABI of the B200-native leading-order matrix-element engine.
+ *
+ * What the library computes (arxiv 2510.05392; citations are /root/reference/PAPER.md lines):
+ *   "takes as input an array of particle momenta for many events (i.e. 4*npar fptype values for each of
+ *    nevt events), and returns as its output an array of matrix elements (i.e. one fptype value for each
+ *    of nevt events)"                                                        (Sec. 2.2)
+ *   me[e] = (1/denom) sum_{good helicities h} Re( J_h(e)^dagger C J_h(e) )   (PAPER.md:95-98, 117-119, 124,
+ *    Eq. 1 at PAPER.md:264-269), J_h(e) = the ncolor dual amplitudes ("jamps") summed over the process's
+ *    Feynman diagrams.
+ *
+ * Conventions
+ *   - All functions return MG_OK (0) or a negative MG_E* code; nothing throws across this boundary.
+ *     mg_last_error() gives a text for the last failure on that handle (or for a failed init when NULL).
+ *   - Pointers are marked HOST or DEVICE.  The caller owns every buffer it passes; the library owns only
+ *     the opaque handle, its constant tables, and its internal CUDA streams/events.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls that take a
+ *     stream are asynchronous and stream-ordered unless stated otherwise.
+ *   - Momenta: fp64, array-of-structures momenta[nevt][npar][4] = (E, px, py, pz) in GeV; particle order =
+ *     order in the process string (two beams along +z/-z, then the final state); all physical (E > 0).
+ *   - Helicity index h = sum_i b_i 2^(npar-1-i), b_i = 0 <-> helicity -1, 1 <-> +1, particle 0 most
+ *     significant (reading A2).
+ *   - Device must be compute capability 10.x (B200, sm_100a): MG_ENODEV otherwise.  There is no CPU path.
+ */
+#ifndef MG5_B200_H
+#define MG5_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_process mg_process; /* opaque, library-owned */
+
+/* the paper's FPTYPE d / m / f: amplitudes fp64 + colour sum fp64; amplitudes fp64 +
+ * colour sum fp32/TF32; everything fp32 */
+enum { MG_FP64 = 0, MG_MIXED = 1, MG_FP32 = 2 };
+enum { MG_OK = 0, MG_EINVAL = -1, MG_ENODEV = -2, MG_ENOMEM = -3, MG_ECUDA = -4, MG_ESTATE = -5 };
+
+/* colour-sum implementations ("color_sum_kernel" vs "color_sum_blas", here own kernels):
+ *   MG_CS_FUSED  : inside the diagram kernel, scalar ALUs, triangular form; jamps never leave the thread
+ *   MG_CS_TENSOR : jamps written to the workspace as [2][ncolor][nGoodHel*nevt], then ONE
+ *                  tensor-core contraction over all helicities: DMMA (mma.sync f64) in MG_FP64,
+ *                  tcgen05 kind::tf32 with TMEM accumulators in MG_MIXED / MG_FP32 */
+enum { MG_CS_FUSED = 0, MG_CS_TENSOR = 1 };
+
+/* helicity scheduling ("helicity streams"):
+ *   MG_SCHED_GRID    : helicity is a grid dimension of one launch (default)
+ *   MG_SCHED_STREAMS : one launch per good helicity, each on its own library-owned stream, forked from and
+ *                      joined back into the caller's stream with events */
+enum { MG_SCHED_GRID = 0, MG_SCHED_STREAMS = 1 };
+
+/* Create a process.  name: "epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg" (BASELINE.json configs;
+ * Table 2).  Parameters start at the BASELINE.json card.  *out is NULL on failure. */
+int mg_init_process(const char* name, int precision, int device, mg_process** out);
+
+/* Static facts about the process (any pointer may be NULL). ngroups = diagram-group functions in the diagram
+ * kernel. */
+int mg_process_info(const mg_process* p, int* npar, int* ncomb, int* ncolor, int* ndiagrams, int* ngroups);
+
+/* Algorithmic floating-point operations of the diagram stage per (event, helicity) and of the colour sum per
+ * (event, helicity) (dense 2*2*ncolor^2 + 4*ncolor), as counted by the generator. */
+int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_flops);
+
+/* Set model parameters.  keys (HOST strings): "aEWM1" (1/alpha), "mZ", "wZ", "mW", "mT", "wT", "aS".
+ * Derived couplings are recomputed on the host.  Unknown key -> MG_EINVAL, nothing changed. */
+int mg_set_parameters(mg_process* p, const char* const* keys, const double* values, int n);
+
+/* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "block" (threads per block of the diagram kernel,
+ * multiple of 32, <= 256).  Unknown key or bad value -> MG_EINVAL. */
+int mg_set_option(mg_process* p, const char* key, int value);
+
+/* Bytes of DEVICE workspace needed by mg_sigma_batch / mg_helicity_filter for batches of up to nevt events
+ * with the current options and good-helicity list (all ncomb helicities if none is set yet).
+ * Layout inside is private; 256-byte alignment of the base is required. */
+size_t mg_workspace_bytes(const mg_process* p, int nevt);
+
+/* Helicity filter ("a pre-determined set of good helicities whose contribution is non-zero",
+ * PAPER.md:649).  Evaluates every helicity combination on the first nprobe events of d_momenta (DEVICE),
+ * all in one launch, and marks h good iff max_e me_h(e)/sum_h' me_h'(e) > 1e-8 (reading A5).
+ * h_mask (HOST, [ncomb], out) and ngood (HOST, out) may be NULL.  Synchronises the stream.  The list is
+ * stored in the handle. */
+int mg_helicity_filter(mg_process* p, const double* d_momenta, int nprobe, void* d_workspace, size_t ws_bytes,
+                       void* cuda_stream, unsigned char* h_mask, int* ngood);
+
+/* Install a good-helicity mask directly (HOST, [ncomb]); all ones = the paper's
+ * CUDACPP_RUNTIME_GOODHELICITIES=ALL. */
+int mg_set_good_helicities(mg_process* p, const unsigned char* h_mask);
+
+/* One batch: d_momenta (DEVICE, [nevt][npar][4] fp64) -> d_me (DEVICE, [nevt] fp64, GeV^(-2(npar-4))).
+ * If no good-helicity list is set, the filter runs first on min(nevt, 1024) events (this synchronises).
+ * ws_bytes must be >= mg_workspace_bytes(p, nevt).  nevt = 0 is a no-op. */
+int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                   size_t ws_bytes, void* cuda_stream);
+
+/* Same from HOST buffers (pinned memory recommended): copies h_momenta to an internal device buffer, runs the
+ * batch, copies me back, synchronises.  The library allocates and owns the device buffers it needs here. */
+int mg_sigma_batch_host(mg_process* p, const double* h_momenta, int nevt, double* h_me);
+
+/* Per-helicity contributions of the last mg_sigma_batch still held in the workspace:
+ * copies me_h[ngood][nevt] (already divided by denom) to d_out (DEVICE).  For tests. */
+int mg_last_helicity_terms(mg_process* p, int nevt, const void* d_workspace, double* d_out, void* cuda_stream);
+
+/* Device time (ms, CUDA events on the caller's stream) of the stages of the last mg_sigma_batch when option
+ * "timing" = 1: [0] diagram kernels, [1] colour sum (0 when fused), [2] helicity sum.  Synchronises. */
+int mg_last_stage_ms(mg_process* p, float ms[3]);
+
+/* Stand-alone colour sum over rows of jamps already in DEVICE memory, layout [2][ncolor][nrows] (re block,
+ * im block) of the precision's colour-sum type (fp64 for MG_FP64, fp32 otherwise):
+ *   d_out[r] = sum_ij (Re J_i C_ij Re J_j + Im J_i C_ij Im J_j),  C = integer numerators (denominator NOT applied).
+ * impl = MG_CS_FUSED runs the scalar-ALU triangular kernel, MG_CS_TENSOR the tensor-core kernel. */
+int mg_color_sum(mg_process* p, int impl, const void* d_jamps, long nrows, double* d_out, void* cuda_stream);
+
+/* Copy the integer colour matrix numerators [ncolor*ncolor] and the common denominator to HOST memory. */
+int mg_color_matrix(const mg_process* p, int* h_numerators, int* denominator);
+
+/* Micro-benchmarks for roofline denominators (bench.py): kind 0 = fp64 FMA, 1 = fp32 FMA, 2 = DMMA (mma.sync
+ * m8n8k4 f64), 3 = tcgen05 kind::tf32.  Returns achieved TFLOP/s in *tflops.  Synchronous. */
+int mg_measure_peak(int device, int kind, double* tflops);
+
+const char* mg_last_error(const mg_process* p);
+void mg_destroy(mg_process* p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG5_B200_H */

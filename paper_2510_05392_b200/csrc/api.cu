@@ -1,0 +1,472 @@
+// api.cu -- the C ABI of include/mg5_b200.h: handle, parameters, helicity filter, batch scheduling.
+//
+// Host-side flow of one batch:
+//   [first call] helicity filter on a probe batch, every helicity combination in ONE launch
+//   diagram kernel(s): helicity as grid.y (MG_SCHED_GRID) or one launch per helicity on a library stream
+//   colour sum: fused in the diagram kernel (MG_CS_FUSED) or ONE tensor-core contraction over the
+//               nGoodHel*nevt rows of the jamps buffer (MG_CS_TENSOR; csrc/color_sum.cu)
+//   helicity sum kernel: me[e] = sum_h me_h[h][e]  (fixed order: deterministic)
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/mg5_b200.h"
+#include "color_sum.cuh"
+#include "mg_internal.cuh"
+
+using namespace mg;
+
+static thread_local std::string g_init_error;
+
+struct mg_process {
+    const ProcessDesc* d = nullptr;
+    int precision = MG_FP64;
+    int device = 0;
+    // parameters (BASELINE.json card)
+    double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
+    // options
+    int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
+    long jamp_chunk_bytes = 1L << 30;
+    // good helicities
+    std::vector<int> good;
+    int* d_good = nullptr;     // DEVICE [ncomb]
+    int* d_all = nullptr;      // DEVICE [ncomb] = 0..ncomb-1
+    void* d_cmat = nullptr;    // DEVICE [ncolor^2] numerators as the colour-sum type
+    // helicity streams
+    std::vector<cudaStream_t> streams;
+    cudaEvent_t ev_fork = nullptr;
+    std::vector<cudaEvent_t> ev_join;
+    // host-buffer path
+    double* d_mom_own = nullptr; double* d_me_own = nullptr; void* d_ws_own = nullptr;
+    int own_nevt = 0; size_t own_ws = 0;
+    // timing
+    cudaEvent_t ev_t[4] = { nullptr, nullptr, nullptr, nullptr };
+    bool timed = false;
+    std::string err;
+};
+
+static int fail(mg_process* p, int code, const std::string& msg)
+{
+    if (p) p->err = msg; else g_init_error = msg;
+    return code;
+}
+#define CUDA_TRY(p, call)                                                                        \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return fail(p, e_ == cudaErrorMemoryAllocation ? MG_ENOMEM : MG_ECUDA,               \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                     \
+    } while (0)
+
+static size_t cs_elem(const mg_process* p) { return p->precision == MG_FP64 ? 8 : 4; }
+static size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
+static phys<double> make_phys(const mg_process* p)
+{
+    phys<double> ph;
+    ph.mt = p->mT; ph.wt = p->wT; ph.mz = p->mZ; ph.wz = p->wZ;
+    const double ee = sqrt(4.0 * M_PI / p->aEWM1);
+    const double sw2 = 1.0 - p->mW * p->mW / (p->mZ * p->mZ);
+    const double sw = sqrt(sw2), cw = sqrt(1.0 - sw2);
+    ph.ee = ee; ph.gl = ee * (-0.5 + sw2) / (sw * cw); ph.gr = ee * sw / cw;
+    return ph;
+}
+
+static double make_norm(const mg_process* p)
+{
+    const double g2 = 4.0 * M_PI * p->aS;
+    return pow(g2, p->d->coupling_order) / (p->d->denom * p->d->cden);
+}
+
+extern "C" const char* mg_last_error(const mg_process* p) { return p ? p->err.c_str() : g_init_error.c_str(); }
+
+static int upload_tables(mg_process* p)
+{
+    const ProcessDesc* d = p->d;
+    const int n2 = d->ncolor * d->ncolor;
+    if (p->d_cmat) { cudaFree(p->d_cmat); p->d_cmat = nullptr; }
+    CUDA_TRY(p, cudaMalloc(&p->d_cmat, (size_t)n2 * cs_elem(p)));
+    if (p->precision == MG_FP64) {
+        std::vector<double> h(n2);
+        for (int i = 0; i < n2; i++) h[i] = d->cmat[i];
+        CUDA_TRY(p, cudaMemcpy(p->d_cmat, h.data(), n2 * sizeof(double), cudaMemcpyHostToDevice));
+    } else {
+        std::vector<float> h(n2);
+        for (int i = 0; i < n2; i++) h[i] = (float)d->cmat[i];
+        CUDA_TRY(p, cudaMemcpy(p->d_cmat, h.data(), n2 * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    std::vector<int> all(d->ncomb);
+    for (int i = 0; i < d->ncomb; i++) all[i] = i;
+    CUDA_TRY(p, cudaMalloc(&p->d_all, d->ncomb * sizeof(int)));
+    CUDA_TRY(p, cudaMalloc(&p->d_good, d->ncomb * sizeof(int)));
+    CUDA_TRY(p, cudaMemcpy(p->d_all, all.data(), d->ncomb * sizeof(int), cudaMemcpyHostToDevice));
+    return MG_OK;
+}
+
+extern "C" int mg_init_process(const char* name, int precision, int device, mg_process** out)
+{
+    if (!out) return fail(nullptr, MG_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!name) return fail(nullptr, MG_EINVAL, "name is NULL");
+    if (precision < MG_FP64 || precision > MG_FP32) return fail(nullptr, MG_EINVAL, "bad precision");
+    const ProcessDesc* d = nullptr;
+    if (!strcmp(name, "epem_mupmum")) d = desc_epem_mupmum();
+    else if (!strcmp(name, "gg_ttx")) d = desc_gg_ttx();
+    else if (!strcmp(name, "gg_ttxg")) d = desc_gg_ttxg();
+    else if (!strcmp(name, "gg_ttxgg")) d = desc_gg_ttxgg();
+    else if (!strcmp(name, "gg_ttxggg")) d = desc_gg_ttxggg();
+    else return fail(nullptr, MG_EINVAL, std::string("unknown process ") + name);
+#ifdef MG_NO_FP32
+    if (precision == MG_FP32) return fail(nullptr, MG_EINVAL, "library built without MG_FP32");
+#endif
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
+        return fail(nullptr, MG_ENODEV, "no such CUDA device");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(nullptr, MG_ENODEV, "cannot query device");
+    if (prop.major != 10) {
+        char buf[128];
+        snprintf(buf, sizeof buf, "device is sm_%d%d; this library is sm_100a only (no fallback)", prop.major, prop.minor);
+        return fail(nullptr, MG_ENODEV, buf);
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return fail(nullptr, MG_ECUDA, "cudaSetDevice failed");
+    mg_process* p = new mg_process;
+    p->d = d; p->precision = precision; p->device = device;
+    int rc = upload_tables(p);
+    if (rc != MG_OK) { g_init_error = p->err; mg_destroy(p); return rc; }
+    for (int i = 0; i < 4; i++) cudaEventCreate(&p->ev_t[i]);
+    *out = p;
+    return MG_OK;
+}
+
+extern "C" void mg_destroy(mg_process* p)
+{
+    if (!p) return;
+    cudaSetDevice(p->device);
+    cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat);
+    cudaFree(p->d_mom_own); cudaFree(p->d_me_own); cudaFree(p->d_ws_own);
+    for (auto s : p->streams) cudaStreamDestroy(s);
+    for (auto e : p->ev_join) cudaEventDestroy(e);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    for (int i = 0; i < 4; i++) if (p->ev_t[i]) cudaEventDestroy(p->ev_t[i]);
+    delete p;
+}
+
+extern "C" int mg_process_info(const mg_process* p, int* npar, int* ncomb, int* ncolor, int* ndiagrams, int* ngroups)
+{
+    if (!p) return MG_EINVAL;
+    if (npar) *npar = p->d->npar;
+    if (ncomb) *ncomb = p->d->ncomb;
+    if (ncolor) *ncolor = p->d->ncolor;
+    if (ndiagrams) *ndiagrams = p->d->ndiagrams;
+    if (ngroups) *ngroups = p->d->ngroups;
+    return MG_OK;
+}
+
+extern "C" int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_flops)
+{
+    if (!p) return MG_EINVAL;
+    if (diagram_flops) *diagram_flops = p->d->flops;
+    if (color_flops) *color_flops = 4.0 * p->d->ncolor * p->d->ncolor + 4.0 * p->d->ncolor;
+    return MG_OK;
+}
+
+extern "C" int mg_set_parameters(mg_process* p, const char* const* keys, const double* values, int n)
+{
+    if (!p || (n > 0 && (!keys || !values))) return fail(p, MG_EINVAL, "bad arguments");
+    mg_process tmp;      // validate everything before changing anything
+    tmp.aEWM1 = p->aEWM1; tmp.mZ = p->mZ; tmp.wZ = p->wZ; tmp.mW = p->mW; tmp.mT = p->mT; tmp.wT = p->wT; tmp.aS = p->aS;
+    for (int i = 0; i < n; i++) {
+        const char* k = keys[i];
+        if (!k) return fail(p, MG_EINVAL, "NULL key");
+        if (!strcmp(k, "aEWM1")) tmp.aEWM1 = values[i];
+        else if (!strcmp(k, "mZ")) tmp.mZ = values[i];
+        else if (!strcmp(k, "wZ")) tmp.wZ = values[i];
+        else if (!strcmp(k, "mW")) tmp.mW = values[i];
+        else if (!strcmp(k, "mT")) tmp.mT = values[i];
+        else if (!strcmp(k, "wT")) tmp.wT = values[i];
+        else if (!strcmp(k, "aS")) tmp.aS = values[i];
+        else return fail(p, MG_EINVAL, std::string("unknown parameter ") + k);
+    }
+    if (!(tmp.aEWM1 > 0) || !(tmp.mZ > 0) || !(tmp.mW > 0) || !(tmp.mW < tmp.mZ) || !(tmp.mT >= 0) || !(tmp.aS > 0) ||
+        !(tmp.wZ >= 0) || !(tmp.wT >= 0))
+        return fail(p, MG_EINVAL, "parameter out of range");
+    p->aEWM1 = tmp.aEWM1; p->mZ = tmp.mZ; p->wZ = tmp.wZ; p->mW = tmp.mW; p->mT = tmp.mT; p->wT = tmp.wT; p->aS = tmp.aS;
+    return MG_OK;
+}
+
+extern "C" int mg_set_option(mg_process* p, const char* key, int value)
+{
+    if (!p || !key) return MG_EINVAL;
+    if (!strcmp(key, "color_sum")) {
+        if (value != MG_CS_FUSED && value != MG_CS_TENSOR) return fail(p, MG_EINVAL, "bad color_sum");
+        p->color_sum = value;
+    } else if (!strcmp(key, "schedule")) {
+        if (value != MG_SCHED_GRID && value != MG_SCHED_STREAMS) return fail(p, MG_EINVAL, "bad schedule");
+        p->schedule = value;
+    } else if (!strcmp(key, "block")) {
+        if (value < 32 || value > 256 || value % 32) return fail(p, MG_EINVAL, "bad block");
+        p->block = value;
+    } else if (!strcmp(key, "timing")) {
+        p->timing = value != 0;
+    } else if (!strcmp(key, "jamp_chunk_mib")) {
+        if (value < 1) return fail(p, MG_EINVAL, "bad jamp_chunk_mib");
+        p->jamp_chunk_bytes = (long)value << 20;
+    } else return fail(p, MG_EINVAL, std::string("unknown option ") + key);
+    return MG_OK;
+}
+
+// events per jamps chunk in MG_CS_TENSOR mode
+static int chunk_events(const mg_process* p, int nevt, int nhel)
+{
+    const size_t per_evt = (size_t)nhel * p->d->ncolor * 2 * cs_elem(p);
+    long ce = (long)(p->jamp_chunk_bytes / per_evt);
+    ce = (ce / 128) * 128;
+    if (ce < 128) ce = 128;
+    if (ce > nevt) ce = nevt;
+    return (int)ce;
+}
+
+static size_t ws_bytes_for(const mg_process* p, int nevt, int nhel)
+{
+    size_t b = align256((size_t)nhel * nevt * sizeof(double));
+    if (p->color_sum == MG_CS_TENSOR && nevt > 0) {
+        const int ce = chunk_events(p, nevt, nhel);
+        b += align256(color_sum_padded_rows((long)nhel * ce) * p->d->ncolor * 2 * cs_elem(p));
+    }
+    return b;
+}
+
+extern "C" size_t mg_workspace_bytes(const mg_process* p, int nevt)
+{
+    if (!p || nevt < 0) return 0;
+    const int nprobe = nevt < 1024 ? nevt : 1024;
+    size_t a = ws_bytes_for(p, nevt, p->good.empty() ? p->d->ncomb : (int)p->good.size());
+    size_t b = p->good.empty() ? align256((size_t)p->d->ncomb * nprobe * sizeof(double)) : 0;   // filter uses FUSED
+    return a > b ? a : b;
+}
+
+__global__ void helicity_sum_kernel(const double* __restrict__ meh, int nhel, int nevt, double* __restrict__ me)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nevt) return;
+    double s = 0.0;
+    for (int h = 0; h < nhel; h++) s += meh[(size_t)h * nevt + e];
+    me[e] = s;
+}
+
+static int set_good(mg_process* p, const std::vector<int>& good)
+{
+    p->good = good;
+    if (!good.empty())
+        CUDA_TRY(p, cudaMemcpy(p->d_good, good.data(), good.size() * sizeof(int), cudaMemcpyHostToDevice));
+    return MG_OK;
+}
+
+extern "C" int mg_set_good_helicities(mg_process* p, const unsigned char* h_mask)
+{
+    if (!p || !h_mask) return fail(p, MG_EINVAL, "bad arguments");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    std::vector<int> g;
+    for (int h = 0; h < p->d->ncomb; h++) if (h_mask[h]) g.push_back(h);
+    if (g.empty()) return fail(p, MG_EINVAL, "empty helicity mask");
+    return set_good(p, g);
+}
+
+static DiagLaunch base_launch(const mg_process* p, const double* d_mom, int nevt)
+{
+    DiagLaunch a;
+    memset(&a, 0, sizeof a);
+    a.mom = d_mom; a.nevt = nevt; a.evt_stride = nevt; a.evt_offset = 0;
+    a.ph = make_phys(p); a.norm = make_norm(p); a.d_cmat = p->d_cmat; a.block = p->block;
+    return a;
+}
+
+extern "C" int mg_helicity_filter(mg_process* p, const double* d_momenta, int nprobe, void* d_workspace, size_t ws_bytes,
+                                  void* cuda_stream, unsigned char* h_mask, int* ngood)
+{
+    if (!p || !d_momenta || nprobe <= 0 || !d_workspace) return fail(p, MG_EINVAL, "bad arguments");
+    const int ncomb = p->d->ncomb;
+    const size_t need = (size_t)ncomb * nprobe * sizeof(double);
+    if (ws_bytes < need) return fail(p, MG_EINVAL, "workspace too small for the helicity filter");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    DiagLaunch a = base_launch(p, d_momenta, nprobe);
+    a.d_hel = p->d_all; a.hel_base = 0; a.nhel = ncomb; a.d_meh = (double*)d_workspace; a.mode = MG_CS_FUSED;
+    CUDA_TRY(p, p->d->launch(p->precision, a, st));
+    std::vector<double> h(need / sizeof(double));
+    CUDA_TRY(p, cudaMemcpyAsync(h.data(), d_workspace, need, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(p, cudaStreamSynchronize(st));
+    std::vector<int> good;
+    std::vector<double> tot(nprobe, 0.0);
+    for (int hh = 0; hh < ncomb; hh++)
+        for (int e = 0; e < nprobe; e++) tot[e] += h[(size_t)hh * nprobe + e];
+    for (int hh = 0; hh < ncomb; hh++) {
+        bool ok = false;
+        for (int e = 0; e < nprobe && !ok; e++)
+            if (tot[e] > 0 && h[(size_t)hh * nprobe + e] > 1e-8 * tot[e]) ok = true;
+        if (h_mask) h_mask[hh] = ok ? 1 : 0;
+        if (ok) good.push_back(hh);
+    }
+    if (ngood) *ngood = (int)good.size();
+    if (good.empty()) return fail(p, MG_ESTATE, "helicity filter found no contributing helicity");
+    return set_good(p, good);
+}
+
+static int ensure_streams(mg_process* p, int n)
+{
+    while ((int)p->streams.size() < n) {
+        cudaStream_t s; cudaEvent_t e;
+        CUDA_TRY(p, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+        CUDA_TRY(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        p->streams.push_back(s); p->ev_join.push_back(e);
+    }
+    if (!p->ev_fork) CUDA_TRY(p, cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+    return MG_OK;
+}
+
+// diagram stage for events [e0, e0+ne) of the batch, all good helicities
+static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
+{
+    const int nhel = (int)p->good.size();
+    if (p->schedule == MG_SCHED_GRID) {
+        a.hel_base = 0; a.nhel = nhel;
+        CUDA_TRY(p, p->d->launch(p->precision, a, st));
+    } else {
+        int rc = ensure_streams(p, nhel);
+        if (rc != MG_OK) return rc;
+        CUDA_TRY(p, cudaEventRecord(p->ev_fork, st));
+        for (int h = 0; h < nhel; h++) {
+            CUDA_TRY(p, cudaStreamWaitEvent(p->streams[h], p->ev_fork, 0));
+            a.hel_base = h; a.nhel = 1;
+            CUDA_TRY(p, p->d->launch(p->precision, a, p->streams[h]));
+            CUDA_TRY(p, cudaEventRecord(p->ev_join[h], p->streams[h]));
+            CUDA_TRY(p, cudaStreamWaitEvent(st, p->ev_join[h], 0));
+        }
+    }
+    return MG_OK;
+}
+
+extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                              size_t ws_bytes, void* cuda_stream)
+{
+    if (!p || nevt < 0) return fail(p, MG_EINVAL, "bad arguments");
+    if (nevt == 0) return MG_OK;
+    if (!d_momenta || !d_me || !d_workspace) return fail(p, MG_EINVAL, "NULL buffer");
+    if (((size_t)d_workspace & 255) != 0) return fail(p, MG_EINVAL, "workspace must be 256-byte aligned");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (ws_bytes < mg_workspace_bytes(p, nevt)) return fail(p, MG_EINVAL, "workspace too small");
+    if (p->good.empty()) {
+        const int nprobe = nevt < 1024 ? nevt : 1024;
+        int rc = mg_helicity_filter(p, d_momenta, nprobe, d_workspace, ws_bytes, cuda_stream, nullptr, nullptr);
+        if (rc != MG_OK) return rc;
+        if (ws_bytes < mg_workspace_bytes(p, nevt)) return fail(p, MG_EINVAL, "workspace too small");
+    }
+    const int nhel = (int)p->good.size();
+    double* d_meh = (double*)d_workspace;
+    char* d_j = (char*)d_workspace + align256((size_t)nhel * nevt * sizeof(double));
+    p->timed = false;
+    if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[0], st));
+    if (p->color_sum == MG_CS_FUSED) {
+        DiagLaunch a = base_launch(p, d_momenta, nevt);
+        a.d_hel = p->d_good; a.d_meh = d_meh; a.mode = MG_CS_FUSED;
+        int rc = run_diagrams(p, a, st);
+        if (rc != MG_OK) return rc;
+        if (p->timing) { CUDA_TRY(p, cudaEventRecord(p->ev_t[1], st)); CUDA_TRY(p, cudaEventRecord(p->ev_t[2], st)); }
+    } else {
+        const int ce = chunk_events(p, nevt, nhel);
+        if (p->timing && ce < nevt) return fail(p, MG_EINVAL, "timing needs a single jamps chunk (raise jamp_chunk_mib)");
+        for (int e0 = 0; e0 < nevt; e0 += ce) {
+            const int ne = nevt - e0 < ce ? nevt - e0 : ce;
+            const long rows = (long)nhel * ne;
+            DiagLaunch a = base_launch(p, d_momenta + (size_t)e0 * p->d->npar * 4, ne);
+            a.d_hel = p->d_good; a.mode = MG_CS_TENSOR; a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows);
+            int rc = run_diagrams(p, a, st);
+            if (rc != MG_OK) return rc;
+            if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[1], st));
+            // rows are (helicity-major, event-minor); the contraction writes norm * J^T C J per row into me_h
+            cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_j, a.rows, rows, ne,
+                                               nevt, e0, make_norm(p), d_meh, st);
+            if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("color_sum_tensor: ") + cudaGetErrorString(ce_));
+            if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[2], st));
+        }
+    }
+    helicity_sum_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, d_me);
+    CUDA_TRY(p, cudaGetLastError());
+    if (p->timing) { CUDA_TRY(p, cudaEventRecord(p->ev_t[3], st)); p->timed = true; }
+    return MG_OK;
+}
+
+extern "C" int mg_last_stage_ms(mg_process* p, float ms[3])
+{
+    if (!p || !ms) return MG_EINVAL;
+    if (!p->timed) return fail(p, MG_ESTATE, "no timed batch (set option timing=1 first)");
+    CUDA_TRY(p, cudaEventSynchronize(p->ev_t[3]));
+    for (int i = 0; i < 3; i++) CUDA_TRY(p, cudaEventElapsedTime(&ms[i], p->ev_t[i], p->ev_t[i + 1]));
+    return MG_OK;
+}
+
+extern "C" int mg_last_helicity_terms(mg_process* p, int nevt, const void* d_workspace, double* d_out, void* cuda_stream)
+{
+    if (!p || !d_workspace || !d_out || nevt <= 0 || p->good.empty()) return fail(p, MG_EINVAL, "bad arguments");
+    CUDA_TRY(p, cudaMemcpyAsync(d_out, d_workspace, p->good.size() * (size_t)nevt * sizeof(double), cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)cuda_stream));
+    return MG_OK;
+}
+
+extern "C" int mg_sigma_batch_host(mg_process* p, const double* h_momenta, int nevt, double* h_me)
+{
+    if (!p || nevt < 0) return fail(p, MG_EINVAL, "bad arguments");
+    if (nevt == 0) return MG_OK;
+    if (!h_momenta || !h_me) return fail(p, MG_EINVAL, "NULL buffer");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    const size_t mom_bytes = (size_t)nevt * p->d->npar * 4 * sizeof(double);
+    if (nevt > p->own_nevt) {
+        cudaFree(p->d_mom_own); cudaFree(p->d_me_own); p->d_mom_own = nullptr; p->d_me_own = nullptr; p->own_nevt = 0;
+        CUDA_TRY(p, cudaMalloc(&p->d_mom_own, mom_bytes));
+        CUDA_TRY(p, cudaMalloc(&p->d_me_own, (size_t)nevt * sizeof(double)));
+        p->own_nevt = nevt;
+    }
+    size_t ws = mg_workspace_bytes(p, nevt);
+    size_t ws_all = ws_bytes_for(p, nevt, p->d->ncomb);      // enough for whatever the filter decides
+    if (ws_all > ws) ws = ws_all;
+    if (ws > p->own_ws) {
+        cudaFree(p->d_ws_own); p->d_ws_own = nullptr; p->own_ws = 0;
+        CUDA_TRY(p, cudaMalloc(&p->d_ws_own, ws));
+        p->own_ws = ws;
+    }
+    CUDA_TRY(p, cudaMemcpyAsync(p->d_mom_own, h_momenta, mom_bytes, cudaMemcpyHostToDevice, 0));
+    int rc = mg_sigma_batch(p, p->d_mom_own, nevt, p->d_me_own, p->d_ws_own, p->own_ws, nullptr);
+    if (rc != MG_OK) return rc;
+    CUDA_TRY(p, cudaMemcpyAsync(h_me, p->d_me_own, (size_t)nevt * sizeof(double), cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(p, cudaStreamSynchronize(0));
+    return MG_OK;
+}
+
+extern "C" int mg_color_matrix(const mg_process* p, int* h_numerators, int* denominator)
+{
+    if (!p) return MG_EINVAL;
+    if (h_numerators) memcpy(h_numerators, p->d->cmat, sizeof(int) * p->d->ncolor * p->d->ncolor);
+    if (denominator) *denominator = p->d->cden;
+    return MG_OK;
+}
+
+extern "C" int mg_color_sum(mg_process* p, int impl, const void* d_jamps, long nrows, double* d_out, void* cuda_stream)
+{
+    if (!p || !d_jamps || !d_out || nrows <= 0) return fail(p, MG_EINVAL, "bad arguments");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (impl == MG_CS_FUSED) e = color_sum_alu(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_jamps, nrows, d_out, st);
+    else if (impl == MG_CS_TENSOR) {
+        if (nrows != color_sum_padded_rows(nrows)) return fail(p, MG_EINVAL, "nrows must be a multiple of 128 for the tensor kernel");
+        e = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_jamps, nrows, nrows, (int)nrows, (int)nrows, 0,
+                             1.0, d_out, st);
+    } else return fail(p, MG_EINVAL, "bad impl");
+    if (e != cudaSuccess) return fail(p, MG_ECUDA, std::string("color sum: ") + cudaGetErrorString(e));
+    return MG_OK;
+}

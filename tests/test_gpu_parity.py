@@ -1,0 +1,192 @@
+"""GPU parity: the CUDA path through the C ABI against the CPU oracle, element by element, same seeded momenta.
+
+Tolerances (BASELINE.json north_star): fp64 relative 1e-10 per event; mixed/fp32 median 2e-4, max 1e-3;
+helicity mask exact.  Sizes span several thread blocks and a ragged tail.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2510_05392_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+SMALL = {"epem_mupmum": 1037, "gg_ttx": 1037, "gg_ttxg": 1037, "gg_ttxgg": 549, "gg_ttxggg": 293}
+EXPECTED_MASK = {"epem_mupmum": [5, 6, 9, 10]}
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2510_05392_b200 import binding
+    binding.load_library()
+    assert torch.cuda.is_available()
+    return binding
+
+
+def _oracle(process, mom, per_helicity=False):
+    return oracle.matrix_elements(process, mom, inputs.PARAMS, per_helicity=per_helicity)
+
+
+def _relerr(a, b):
+    return np.abs(a / b - 1)
+
+
+@pytest.mark.parametrize("process", list(SMALL))
+def test_fp64_parity_and_mask(B, process):
+    nevt = SMALL[process]
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, "fp64")
+    d_mom = torch.from_numpy(mom).cuda()
+    mask = proc.helicity_filter(d_mom)
+    ref, ref_h = _oracle(process, mom, per_helicity=True)
+    # mask: h good iff max_e me_h / sum_h me_h > 1e-8 on the probe events (reading A5), both sides
+    nprobe = min(nevt, 1024)
+    omask = (ref_h[:nprobe] / ref[:nprobe, None] > 1e-8).any(axis=0)
+    assert np.array_equal(mask.astype(bool), omask)
+    if process in EXPECTED_MASK:
+        assert list(np.nonzero(mask)[0]) == EXPECTED_MASK[process]
+    else:
+        assert mask.all()                              # PAPER.md:203 row (6)
+    me = proc.sigma_batch(d_mom).cpu().numpy()
+    assert _relerr(me, ref).max() < 1e-10
+    # per-helicity terms too
+    meh = proc.last_helicity_terms(nevt).cpu().numpy()
+    good = np.nonzero(mask)[0]
+    scale = ref[None, :]
+    assert np.abs(meh - ref_h[:, good].T).max() / 1.0 < np.inf
+    assert (np.abs(meh - ref_h[:, good].T) / scale).max() < 1e-10
+    proc.close()
+
+
+@pytest.mark.parametrize("process", list(SMALL))
+@pytest.mark.parametrize("precision", ["mixed", "fp32"])
+def test_reduced_precision_parity(B, process, precision):
+    if process == "gg_ttxggg" and precision == "fp32":
+        pytest.skip("all-fp32 instantiation of the 1240-diagram kernel is not built by default (compile time)")
+    nevt = SMALL[process]
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, precision)
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    ref = _oracle(process, mom)
+    err = _relerr(me, ref)
+    assert np.median(err) < 2e-4 and err.max() < 1e-3, (np.median(err), err.max())
+    proc.close()
+
+
+@pytest.mark.parametrize("process", ["gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg"])
+def test_scheduling_variants_agree(B, process):
+    """helicity streams vs helicity-in-grid, fused vs tensor-core colour sum: same me[] (PAPER.md:500 'basic validation')"""
+    nevt = 391 if process != "gg_ttxggg" else 131
+    mom = inputs.momenta(process, nevt, seed=2)
+    d_mom = torch.from_numpy(mom).cuda()
+    base = None
+    for opts in ({}, {"schedule": 1}, {"color_sum": 1}, {"color_sum": 1, "schedule": 1}, {"block": 64}):
+        proc = B.init_process(process, "fp64")
+        for k, v in opts.items():
+            proc.set_option(k, v)
+        me = proc.sigma_batch(d_mom).cpu().numpy()
+        if base is None:
+            base = me
+        else:
+            assert _relerr(me, base).max() < 1e-12, opts
+        proc.close()
+
+
+def test_tensor_color_sum_chunked(B):
+    """jamps buffer smaller than the batch: several chunks, ragged last chunk"""
+    process, nevt = "gg_ttxgg", 700
+    mom = inputs.momenta(process, nevt, seed=4)
+    d_mom = torch.from_numpy(mom).cuda()
+    proc = B.init_process(process, "fp64")
+    ref = proc.sigma_batch(d_mom).cpu().numpy()
+    proc.close()
+    proc = B.init_process(process, "fp64")
+    proc.set_option("color_sum", 1)
+    proc.set_option("jamp_chunk_mib", 1)     # 1 MiB -> 128-event chunks (floor)
+    me = proc.sigma_batch(d_mom).cpu().numpy()
+    assert _relerr(me, ref).max() < 1e-12
+    proc.close()
+
+
+def test_standalone_color_sum_kernels(B):
+    """mg_color_sum on random jamps against numpy J^T C J (ALU and tensor kernels, fp64 and fp32)"""
+    rng = np.random.default_rng(0)
+    for process in ("gg_ttxgg", "gg_ttxggg"):
+        for prec, dt, tol in (("fp64", np.float64, 1e-12), ("mixed", np.float32, 2e-5)):
+            proc = B.init_process(process, prec)
+            C, den = proc.color_matrix()
+            nrows = 1024
+            J = rng.normal(size=(2, proc.ncolor, nrows)).astype(dt)
+            ref = np.einsum("pir,ij,pjr->r", J.astype(np.float64), C.astype(np.float64), J.astype(np.float64))
+            dJ = torch.from_numpy(J).cuda()
+            for impl in (0, 1):
+                out = proc.color_sum(dJ, impl).cpu().numpy()
+                assert np.abs(out / ref - 1).max() < tol, (process, prec, impl, np.abs(out / ref - 1).max())
+            proc.close()
+
+
+def test_edge_cases(B):
+    proc = B.init_process("gg_ttx", "fp64")
+    # empty batch
+    me = proc.sigma_batch(torch.empty((0, 4, 4), dtype=torch.float64, device="cuda"))
+    assert me.numel() == 0
+    # single event, and the library's implicit filter
+    mom = inputs.momenta("gg_ttx", 1)
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert _relerr(me, _oracle("gg_ttx", mom)).max() < 1e-10
+    # GOODHELICITIES=ALL: same answer
+    proc.set_good_helicities(np.ones(16, dtype=np.uint8))
+    me2 = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert _relerr(me2, me).max() < 1e-14
+    # parameters: zero width reproduces the analytic formula's oracle value
+    proc.set_parameters(wT=0.0)
+    me3 = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    ref3 = oracle.matrix_elements("gg_ttx", mom, dict(inputs.PARAMS, wT=0.0))
+    assert _relerr(me3, ref3).max() < 1e-10
+    with pytest.raises(B.MGError):
+        proc.set_parameters(bogus=1.0)
+    with pytest.raises(B.MGError):
+        proc.set_option("block", 100)
+    proc.close()
+    with pytest.raises(B.MGError):
+        B.init_process("gg_nothing", "fp64")
+
+
+def test_beam_swap_and_collinear_externals(B):
+    """external wavefunctions with pT = 0 along +z and -z, both beam assignments (reading A8)"""
+    mom = inputs.momenta("gg_ttxg", 64, seed=11)
+    swapped = mom.copy()
+    swapped[:, [0, 1]] = mom[:, [1, 0]]
+    proc = B.init_process("gg_ttxg", "fp64")
+    a = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    b = proc.sigma_batch(torch.from_numpy(swapped).cuda()).cpu().numpy()
+    assert _relerr(a, b).max() < 1e-11
+    assert _relerr(b, _oracle("gg_ttxg", swapped)).max() < 1e-10
+    proc.close()
+
+
+def test_host_buffer_entry_point(B):
+    mom = inputs.momenta("gg_ttxg", 777)
+    proc = B.init_process("gg_ttxg", "fp64")
+    a = proc.sigma_batch_host(mom)
+    b = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert np.array_equal(a, b)
+    proc.close()
+
+
+@pytest.mark.parametrize("process", list(SMALL))
+def test_full_size_sampled(B, process):
+    """BASELINE.json's full batch in the launch configuration bench.py times; oracle on sampled events"""
+    nevt = inputs.PROCESSES[process]["nevt"]
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, "fp64")
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert np.isfinite(me).all() and (me > 0).all()
+    ns = 64 if process == "gg_ttxggg" else 256
+    rng = np.random.default_rng(1)
+    idx = np.unique(np.concatenate([np.arange(ns), np.arange(nevt - ns, nevt), rng.integers(0, nevt, ns)]))
+    ref = _oracle(process, mom[idx])
+    assert _relerr(me[idx], ref).max() < 1e-10
+    proc.close()
