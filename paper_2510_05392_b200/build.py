@@ -29,19 +29,27 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 EXTRA = {"proc_gg_ttxggg.cu": ["-DMG_NO_FP32"] if os.environ.get("MG_FP32_ALL", "0") != "1" else []}
 
 
-def _newest_header_mtime():
-    hs = glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + \
-        glob.glob(os.path.join(HERE, "..", "include", "*.h"))
-    return max(os.path.getmtime(h) for h in hs)
+import re
+
+_INC = re.compile(r'^\s*#\s*include\s+"([^"]+)"', re.M)
+
+
+def _deps(path, seen=None):
+    """the file and every header it includes with "..." (recursively)"""
+    seen = set() if seen is None else seen
+    path = os.path.normpath(path)
+    if path in seen or not os.path.exists(path):
+        return seen
+    seen.add(path)
+    for inc in _INC.findall(open(path).read()):
+        _deps(os.path.join(os.path.dirname(path), inc), seen)
+    return seen
 
 
 def _compile(src, verbose):
     base = os.path.basename(src)
     obj = os.path.join(OBJ, base.replace(".cu", ".o"))
-    dep_m = max(os.path.getmtime(src), _newest_header_mtime())
-    gen_h = glob.glob(os.path.join(GEN, base.replace("proc_", "").replace(".cu", "") + "_*"))
-    for g in gen_h:
-        dep_m = max(dep_m, os.path.getmtime(g))
+    dep_m = max(os.path.getmtime(d) for d in _deps(src))
     if os.path.exists(obj) and os.path.getmtime(obj) >= dep_m:
         return obj, 0.0, ""
     t = time.time()

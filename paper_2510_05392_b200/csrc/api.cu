@@ -35,6 +35,7 @@ struct mg_process {
     int* d_good = nullptr;     // DEVICE [ncomb]
     int* d_all = nullptr;      // DEVICE [ncomb] = 0..ncomb-1
     void* d_cmat = nullptr;    // DEVICE [ncolor^2] numerators as the colour-sum type
+    double* d_chol = nullptr;  // DEVICE [ncp^2] Cholesky factor of the numerators (MG_FP64 tensor colour sum)
     // helicity streams
     std::vector<cudaStream_t> streams;
     cudaEvent_t ev_fork = nullptr;
@@ -98,6 +99,12 @@ static int upload_tables(mg_process* p)
         for (int i = 0; i < n2; i++) h[i] = (float)d->cmat[i];
         CUDA_TRY(p, cudaMemcpy(p->d_cmat, h.data(), n2 * sizeof(float), cudaMemcpyHostToDevice));
     }
+    if (p->precision == MG_FP64) {
+        std::vector<double> lp; int ncp = 0;
+        if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
+        CUDA_TRY(p, cudaMalloc(&p->d_chol, lp.size() * sizeof(double)));
+        CUDA_TRY(p, cudaMemcpy(p->d_chol, lp.data(), lp.size() * sizeof(double), cudaMemcpyHostToDevice));
+    }
     std::vector<int> all(d->ncomb);
     for (int i = 0; i < d->ncomb; i++) all[i] = i;
     CUDA_TRY(p, cudaMalloc(&p->d_all, d->ncomb * sizeof(int)));
@@ -146,7 +153,7 @@ extern "C" void mg_destroy(mg_process* p)
 {
     if (!p) return;
     cudaSetDevice(p->device);
-    cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat);
+    cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat); cudaFree(p->d_chol);
     cudaFree(p->d_mom_own); cudaFree(p->d_me_own); cudaFree(p->d_ws_own);
     for (auto s : p->streams) cudaStreamDestroy(s);
     for (auto e : p->ev_join) cudaEventDestroy(e);
@@ -389,7 +396,7 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             if (rc != MG_OK) return rc;
             if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[1], st));
             // rows are (helicity-major, event-minor); the contraction writes norm * J^T C J per row into me_h
-            cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_j, a.rows, rows, ne,
+            cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, rows, ne,
                                                nevt, e0, make_norm(p), d_meh, st);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("color_sum_tensor: ") + cudaGetErrorString(ce_));
             if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[2], st));
@@ -464,7 +471,7 @@ extern "C" int mg_color_sum(mg_process* p, int impl, const void* d_jamps, long n
     if (impl == MG_CS_FUSED) e = color_sum_alu(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_jamps, nrows, d_out, st);
     else if (impl == MG_CS_TENSOR) {
         if (nrows != color_sum_padded_rows(nrows)) return fail(p, MG_EINVAL, "nrows must be a multiple of 128 for the tensor kernel");
-        e = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_jamps, nrows, nrows, (int)nrows, (int)nrows, 0,
+        e = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_jamps, nrows, nrows, (int)nrows, (int)nrows, 0,
                              1.0, d_out, st);
     } else return fail(p, MG_EINVAL, "bad impl");
     if (e != cudaSuccess) return fail(p, MG_ECUDA, std::string("color sum: ") + cudaGetErrorString(e));

@@ -12,8 +12,6 @@
 #include <math.h>
 #include <stdint.h>
 
-#include <map>
-#include <mutex>
 #include <vector>
 
 #include "color_sum.cuh"
@@ -118,57 +116,42 @@ __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __res
     }
 }
 
-// Cholesky factors, one per (device matrix pointer): computed on the host in long double from the integer matrix
-struct CholEntry { double* d_L; int ncp; };
-static std::map<const void*, CholEntry> g_chol;
-static std::mutex g_chol_mutex;
-
-static cudaError_t get_cholesky(int ncolor, const void* d_cmat, CholEntry* out)
+// Cholesky factor of the integer colour matrix, computed on the host in long double and zero-padded to a
+// multiple of 8 columns; the caller (api.cu) uploads it once per handle.  Returns false if C is not
+// positive definite.
+bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out)
 {
-    std::lock_guard<std::mutex> lock(g_chol_mutex);
-    auto it = g_chol.find(d_cmat);
-    if (it != g_chol.end()) { *out = it->second; return cudaSuccess; }
-    std::vector<double> c((size_t)ncolor * ncolor);
-    cudaError_t e = cudaMemcpy(c.data(), d_cmat, c.size() * sizeof(double), cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) return e;
     const int ncp = (ncolor + 7) / 8 * 8;
     std::vector<long double> l((size_t)ncolor * ncolor, 0.0L);
     for (int i = 0; i < ncolor; i++)
         for (int j = 0; j <= i; j++) {
-            long double s = c[(size_t)i * ncolor + j];
+            long double s = cmat[(size_t)i * ncolor + j];
             for (int k = 0; k < j; k++) s -= l[(size_t)i * ncolor + k] * l[(size_t)j * ncolor + k];
-            if (i == j) { if (s <= 0) return cudaErrorInvalidValue; l[(size_t)i * ncolor + i] = sqrtl(s); }
+            if (i == j) { if (s <= 0) return false; l[(size_t)i * ncolor + i] = sqrtl(s); }
             else l[(size_t)i * ncolor + j] = s / l[(size_t)j * ncolor + j];
         }
-    std::vector<double> lp((size_t)ncp * ncp, 0.0);
+    lp.assign((size_t)ncp * ncp, 0.0);
     for (int i = 0; i < ncolor; i++)
         for (int j = 0; j <= i; j++) lp[(size_t)i * ncp + j] = (double)l[(size_t)i * ncolor + j];
-    CholEntry ce; ce.ncp = ncp;
-    e = cudaMalloc(&ce.d_L, lp.size() * sizeof(double));
-    if (e != cudaSuccess) return e;
-    e = cudaMemcpy(ce.d_L, lp.data(), lp.size() * sizeof(double), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) return e;
-    g_chol[d_cmat] = ce;
-    *out = ce;
-    return cudaSuccess;
+    *ncp_out = ncp;
+    return true;
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded, long rows_valid, int ne,
                            int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st);
 
-cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded,
-                             long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st)
+cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
+                             long rows_padded, long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st)
 {
     if (!is_fp64) return color_sum_tf32(ncolor, d_cmat, d_jamps, rows_padded, rows_valid, ne, evt_stride, e0, norm, d_meh, st);
-    CholEntry ce;
-    cudaError_t e = get_cholesky(ncolor, d_cmat, &ce);
-    if (e != cudaSuccess) return e;
+    if (!d_chol) return cudaErrorInvalidValue;
+    const int ncp = (ncolor + 7) / 8 * 8;
     const int warps = 4;
     const unsigned grid = (unsigned)((rows_padded / 8 + warps - 1) / warps);
     const double* X = (const double*)d_jamps;
-#define LAUNCH(NT) color_sum_dmma_kernel<NT><<<grid, warps * 32, 0, st>>>(ce.d_L, X, ncolor, rows_padded, rows_valid, ne, \
+#define LAUNCH(NT) color_sum_dmma_kernel<NT><<<grid, warps * 32, 0, st>>>(d_chol, X, ncolor, rows_padded, rows_valid, ne, \
                                                                            evt_stride, e0, norm, d_meh)
-    switch (ce.ncp / 8) {
+    switch (ncp / 8) {
         case 1: LAUNCH(1); break;
         case 3: LAUNCH(3); break;
         case 15: LAUNCH(15); break;

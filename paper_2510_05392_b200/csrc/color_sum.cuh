@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <vector>
+
 namespace mg {
 
 // rows of the jamps buffer are padded to the tensor kernels' row tile
@@ -16,8 +18,12 @@ cudaError_t color_sum_alu(bool is_fp64, int ncolor, const void* d_cmat, const vo
 // events per helicity; row (ih, el) goes to d_meh[ih * evt_stride + e0 + el] = norm * J^T C J.
 //   fp64: DMMA (mma.sync m8n8k4 f64) on Z = X L with C = L L^T (Cholesky, lower-triangular: upper k-tiles skipped)
 //   fp32: tcgen05.mma kind::tf32, exact integer C, J split in two TF32 terms, fp32 accumulation in TMEM
-cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded,
-                             long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st);
+//   d_chol: DEVICE [ncp][ncp] padded Cholesky factor (fp64 only; see color_cholesky_padded)
+cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
+                             long rows_padded, long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st);
+
+// host: L with C = L L^T (lower-triangular, row-major, zero-padded to ncp = 8*ceil(ncolor/8) columns)
+bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out);
 
 // peak probes (mg_measure_peak)
 cudaError_t measure_peak(int kind, double* tflops);
