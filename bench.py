@@ -155,8 +155,7 @@ def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world,
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
         dist.barrier()
-    launches_per_step = (1 if not opts or opts.get("schedule", 0) == 0 else int(mask.sum())) + 1 + \
-        (1 if opts and opts.get("color_sum", 0) == 1 else 0)
+    launches_per_step = proc.last_launch_count()
     res = {"proc": proc, "ms_total": ms, "ms_per_step": ms / steps, "value": world * nevt * steps / (ms * 1e-3),
            "stage_ms": (stage / steps).tolist(), "ngood": int(mask.sum()), "launches": launches_per_step * steps,
            "d_mom": d_mom, "d_me": d_me, "mom_h": mom_h}
@@ -174,6 +173,9 @@ def main():
     ap.add_argument("--nevt", type=int, default=None)
     ap.add_argument("--color-sum", type=int, default=None, help="0 fused ALU, 1 tensor-core kernel")
     ap.add_argument("--schedule", type=int, default=0, help="0 helicity in the grid, 1 helicity streams")
+    ap.add_argument("--diagrams", type=int, default=None, help="0 thread per (event, helicity), 1 helicity-shared CTA per event")
+    ap.add_argument("--hs-split", type=int, default=None)
+    ap.add_argument("--chunk-mib", type=int, default=None, help="jamps buffer size inside the workspace")
     ap.add_argument("--no-extras", action="store_true", help="skip per-process table, e2e and cpu baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -200,6 +202,12 @@ def main():
     opts = {"schedule": args.schedule}
     if args.color_sum is not None:
         opts["color_sum"] = args.color_sum
+    if args.diagrams is not None:
+        opts["diagrams"] = args.diagrams
+    if args.hs_split is not None:
+        opts["hs_split"] = args.hs_split
+    if args.chunk_mib is not None:
+        opts["jamp_chunk_mib"] = args.chunk_mib
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")
 
     peaks, peak_src = read_peaks()
@@ -214,11 +222,12 @@ def main():
 
     # roofline of the dominant kernel (the diagram kernel): plain FP64 ALU bound
     diag_ms = r["stage_ms"][0]
+    shared = proc.get_option("diagrams") == 1
     alg_flop = proc.diagram_flops * nevt * r["ngood"]
-    if opts.get("color_sum", 0) == 0:
+    if not shared and proc.get_option("color_sum") == 0:
         alg_flop += (2.0 * proc.ncolor * (proc.ncolor + 1) + 4.0 * proc.ncolor) * nevt * r["ngood"]   # fused triangular colour sum
     achieved = alg_flop / (diag_ms * 1e-3) * 1e-12
-    roofline = {"bound": "alu", "kernel": "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": "hs_diagrams_kernel" if shared else "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak if fp64_peak else None, "traffic": None,
                 "peak_source": "fp64 FMA probe kernel measured in this run (mg_measure_peak, burst); "
                                "MEASURED_PEAKS.json holds no fp64 figure",
@@ -231,8 +240,11 @@ def main():
            "data": "synthetic",
            "config": {"workload": f"{process}: {nevt} events/batch/GPU, flat RAMBO sqrt(s)=1500 GeV seed 1 (BASELINE.json config)",
                       "process": process, "precision": args.precision, "nevt_per_gpu": nevt, "good_helicities": r["ngood"],
-                      "schedule": "helicity streams" if args.schedule else "helicity = grid.y",
-                      "color_sum": "tensor" if opts.get("color_sum", 0) == 1 else "fused ALU",
+                      "diagrams": "helicity-shared (CTA = event, thread = helicity)" if shared else "thread = (event, helicity)",
+                      "schedule": "helicity streams" if args.schedule else ("helicity = thread index" if shared else "helicity = grid.y"),
+                      "color_sum": ("tensor" if (shared and args.precision in ("fp64", "d")) or proc.get_option("color_sum") == 1
+                                    else ("ALU kernel" if shared else "fused ALU")),
+                      "jamp_chunk_mib": proc.get_option("jamp_chunk_mib"),
                       "l2": "256 MiB device memset between timed steps (outside the per-step event pairs)"},
            "gpu_launches": r["launches"], "stage_ms": {"diagrams": r["stage_ms"][0], "color_sum": r["stage_ms"][1],
                                                          "helicity_sum": r["stage_ms"][2]},

@@ -50,6 +50,13 @@ enum { MG_CS_FUSED = 0, MG_CS_TENSOR = 1 };
  *                      joined back into the caller's stream with events */
 enum { MG_SCHED_GRID = 0, MG_SCHED_STREAMS = 1 };
 
+/* diagram stage:
+ *   MG_DIAG_THREAD : one thread per (event, helicity), the paper's layout
+ *   MG_DIAG_SHARED : one CTA per event, one thread per helicity; wavefunctions shared between helicities in shared
+ *                    memory, jamps written to the workspace and contracted by the colour-sum kernel (gg processes,
+ *                    MG_FP64 / MG_MIXED; default for >= 4 gluons) */
+enum { MG_DIAG_THREAD = 0, MG_DIAG_SHARED = 1 };
+
 /* Create a process.  name: "epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg" (BASELINE.json configs;
  * Table 2).  Parameters start at the BASELINE.json card.  *out is NULL on failure. */
 int mg_init_process(const char* name, int precision, int device, mg_process** out);
@@ -66,9 +73,13 @@ int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_f
  * Derived couplings are recomputed on the host.  Unknown key -> MG_EINVAL, nothing changed. */
 int mg_set_parameters(mg_process* p, const char* const* keys, const double* values, int n);
 
-/* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "block" (threads per block of the diagram kernel,
- * multiple of 32, <= 256).  Unknown key or bad value -> MG_EINVAL. */
+/* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
+ * MG_DIAG_THREAD kernel, multiple of 32, <= 256), "hs_split" (threads per helicity of the MG_DIAG_SHARED kernel: 1, 2, 4),
+ * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1).
+ * Unknown key or bad value -> MG_EINVAL. */
 int mg_set_option(mg_process* p, const char* key, int value);
+/* Current value of an option (same keys).  Unknown key -> MG_EINVAL. */
+int mg_get_option(const mg_process* p, const char* key, int* value);
 
 /* Bytes of DEVICE workspace needed by mg_sigma_batch / mg_helicity_filter for batches of up to nevt events
  * with the current options and good-helicity list (all ncomb helicities if none is set yet).
@@ -104,6 +115,9 @@ int mg_last_helicity_terms(mg_process* p, int nevt, const void* d_workspace, dou
 /* Device time (ms, CUDA events on the caller's stream) of the stages of the last mg_sigma_batch when option
  * "timing" = 1: [0] diagram kernels, [1] colour sum (0 when fused), [2] helicity sum.  Synchronises. */
 int mg_last_stage_ms(mg_process* p, float ms[3]);
+
+/* Number of kernels the last mg_sigma_batch launched (diagram + colour-sum + helicity-sum kernels). */
+int mg_last_launch_count(const mg_process* p, int* launches);
 
 /* Stand-alone colour sum over rows of jamps already in DEVICE memory, layout [2][ncolor][nrows] (re block,
  * im block) of the precision's colour-sum type (fp64 for MG_FP64, fp32 otherwise):

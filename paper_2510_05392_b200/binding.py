@@ -21,9 +21,9 @@ PRECISIONS = {"fp64": MG_FP64, "d": MG_FP64, "mixed": MG_MIXED, "m": MG_MIXED, "
 
 _ERR = {-1: "MG_EINVAL", -2: "MG_ENODEV", -3: "MG_ENOMEM", -4: "MG_ECUDA", -5: "MG_ESTATE"}
 
-EXPORTS = ["mg_init_process", "mg_process_info", "mg_process_flops", "mg_set_parameters", "mg_set_option",
+EXPORTS = ["mg_init_process", "mg_process_info", "mg_process_flops", "mg_set_parameters", "mg_set_option", "mg_get_option",
            "mg_workspace_bytes", "mg_helicity_filter", "mg_set_good_helicities", "mg_sigma_batch",
-           "mg_sigma_batch_host", "mg_last_helicity_terms", "mg_last_stage_ms", "mg_color_sum", "mg_color_matrix",
+           "mg_sigma_batch_host", "mg_last_helicity_terms", "mg_last_stage_ms", "mg_last_launch_count", "mg_color_sum", "mg_color_matrix",
            "mg_measure_peak", "mg_last_error", "mg_destroy"]
 
 _lib = None
@@ -48,6 +48,7 @@ def load_library() -> ctypes.CDLL:
     lib.mg_process_flops.argtypes = [vp, dp, dp]
     lib.mg_set_parameters.argtypes = [vp, ctypes.POINTER(ctypes.c_char_p), dp, ctypes.c_int]
     lib.mg_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
+    lib.mg_get_option.argtypes = [vp, ctypes.c_char_p, ip]
     lib.mg_workspace_bytes.argtypes = [vp, ctypes.c_int]
     lib.mg_workspace_bytes.restype = ctypes.c_size_t
     lib.mg_helicity_filter.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_size_t, vp, ctypes.POINTER(ctypes.c_ubyte), ip]
@@ -56,6 +57,7 @@ def load_library() -> ctypes.CDLL:
     lib.mg_sigma_batch_host.argtypes = [vp, vp, ctypes.c_int, vp]
     lib.mg_last_helicity_terms.argtypes = [vp, ctypes.c_int, vp, vp, vp]
     lib.mg_last_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    lib.mg_last_launch_count.argtypes = [vp, ip]
     lib.mg_color_sum.argtypes = [vp, ctypes.c_int, vp, ctypes.c_long, vp, vp]
     lib.mg_color_matrix.argtypes = [vp, ip, ip]
     lib.mg_measure_peak.argtypes = [ctypes.c_int, ctypes.c_int, dp]
@@ -95,11 +97,14 @@ class Process:
         v = [ctypes.c_int() for _ in range(5)]
         self._check(self.lib.mg_process_info(self.h, *[ctypes.byref(x) for x in v]))
         self.npar, self.ncomb, self.ncolor, self.ndiagrams, self.ngroups = [x.value for x in v]
+        self._read_flops()
+        self._ws = None
+        self.ngood = None
+
+    def _read_flops(self):
         a, b = ctypes.c_double(), ctypes.c_double()
         self._check(self.lib.mg_process_flops(self.h, ctypes.byref(a), ctypes.byref(b)))
         self.diagram_flops, self.color_flops = a.value, b.value
-        self._ws = None
-        self.ngood = None
 
     # -- plumbing -----------------------------------------------------------------------------------
     def _check(self, rc):
@@ -134,7 +139,13 @@ class Process:
 
     def set_option(self, key: str, value: int):
         self._check(self.lib.mg_set_option(self.h, key.encode(), int(value)))
+        self._read_flops()
         self._ws = None
+
+    def get_option(self, key: str) -> int:
+        v = ctypes.c_int()
+        self._check(self.lib.mg_get_option(self.h, key.encode(), ctypes.byref(v)))
+        return v.value
 
     def helicity_filter(self, d_momenta, nprobe=None):
         nevt = d_momenta.shape[0]
@@ -189,6 +200,11 @@ class Process:
         ms = (ctypes.c_float * 3)()
         self._check(self.lib.mg_last_stage_ms(self.h, ms))
         return [ms[0], ms[1], ms[2]]
+
+    def last_launch_count(self):
+        n = ctypes.c_int()
+        self._check(self.lib.mg_last_launch_count(self.h, ctypes.byref(n)))
+        return n.value
 
     def color_sum(self, d_jamps, impl=MG_CS_TENSOR):
         """d_jamps: cuda tensor [2][ncolor][nrows] (fp64 for MG_FP64, fp32 otherwise) -> cuda fp64 [nrows] (numerators only)"""

@@ -15,6 +15,7 @@
 
 #include "../../include/mg5_b200.h"
 #include "color_sum.cuh"
+#include "hs_kernel.cuh"
 #include "mg_internal.cuh"
 
 using namespace mg;
@@ -29,6 +30,9 @@ struct mg_process {
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
+    int diagrams = MG_DIAG_THREAD, hs_split = 1;
+    HsContext* hs = nullptr;   // helicity-shared program (gg processes)
+    int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 1L << 30;
     // good helicities
     std::vector<int> good;
@@ -44,8 +48,11 @@ struct mg_process {
     double* d_mom_own = nullptr; double* d_me_own = nullptr; void* d_ws_own = nullptr;
     int own_nevt = 0; size_t own_ws = 0;
     // timing
-    cudaEvent_t ev_t[4] = { nullptr, nullptr, nullptr, nullptr };
+    std::vector<cudaEvent_t> ev_pool;     // timing marks of the last batch: mark k closes stage ev_stage[k]
+    std::vector<int> ev_stage;
+    int ev_n = 0;
     bool timed = false;
+    int launches = 0;          // kernels launched by the last mg_sigma_batch
     std::string err;
 };
 
@@ -109,6 +116,7 @@ static int upload_tables(mg_process* p)
     for (int i = 0; i < d->ncomb; i++) all[i] = i;
     CUDA_TRY(p, cudaMalloc(&p->d_all, d->ncomb * sizeof(int)));
     CUDA_TRY(p, cudaMalloc(&p->d_good, d->ncomb * sizeof(int)));
+    CUDA_TRY(p, cudaMalloc(&p->d_pos, d->ncomb * sizeof(int)));
     CUDA_TRY(p, cudaMemcpy(p->d_all, all.data(), d->ncomb * sizeof(int), cudaMemcpyHostToDevice));
     return MG_OK;
 }
@@ -144,7 +152,11 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     p->d = d; p->precision = precision; p->device = device;
     int rc = upload_tables(p);
     if (rc != MG_OK) { g_init_error = p->err; mg_destroy(p); return rc; }
-    for (int i = 0; i < 4; i++) cudaEventCreate(&p->ev_t[i]);
+    if (d->ngluon >= 2 && precision != MG_FP32) {
+        cudaError_t e = hs_create(d->ngluon, &p->hs);
+        if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
+        if (d->ngluon >= 4) p->diagrams = MG_DIAG_SHARED;     // measured default, see DESIGN.md
+    }
     *out = p;
     return MG_OK;
 }
@@ -153,12 +165,14 @@ extern "C" void mg_destroy(mg_process* p)
 {
     if (!p) return;
     cudaSetDevice(p->device);
+    hs_destroy(p->hs);
+    cudaFree(p->d_pos);
     cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat); cudaFree(p->d_chol);
     cudaFree(p->d_mom_own); cudaFree(p->d_me_own); cudaFree(p->d_ws_own);
     for (auto s : p->streams) cudaStreamDestroy(s);
     for (auto e : p->ev_join) cudaEventDestroy(e);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
-    for (int i = 0; i < 4; i++) if (p->ev_t[i]) cudaEventDestroy(p->ev_t[i]);
+    for (auto e : p->ev_pool) cudaEventDestroy(e);
     delete p;
 }
 
@@ -176,7 +190,13 @@ extern "C" int mg_process_info(const mg_process* p, int* npar, int* ncomb, int* 
 extern "C" int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_flops)
 {
     if (!p) return MG_EINVAL;
-    if (diagram_flops) *diagram_flops = p->d->flops;
+    if (diagram_flops) {
+        *diagram_flops = p->d->flops;
+        if (p->diagrams == MG_DIAG_SHARED && p->hs) {
+            const HsTables* t = hs_host_tables(p->hs);
+            *diagram_flops = (t->flops_p1 + t->flops_p2) / p->d->ncomb + t->flops_p3;
+        }
+    }
     if (color_flops) *color_flops = 4.0 * p->d->ncolor * p->d->ncolor + 4.0 * p->d->ncolor;
     return MG_OK;
 }
@@ -217,12 +237,34 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
     } else if (!strcmp(key, "block")) {
         if (value < 32 || value > 256 || value % 32) return fail(p, MG_EINVAL, "bad block");
         p->block = value;
+    } else if (!strcmp(key, "diagrams")) {
+        if (value != MG_DIAG_THREAD && value != MG_DIAG_SHARED) return fail(p, MG_EINVAL, "bad diagrams");
+        if (value == MG_DIAG_SHARED && !p->hs) return fail(p, MG_EINVAL, "this process/precision has no helicity-shared program");
+        p->diagrams = value;
+    } else if (!strcmp(key, "hs_split")) {
+        if (value != 1 && value != 2 && value != 4) return fail(p, MG_EINVAL, "bad hs_split");
+        if (value * p->d->ncomb > 256) return fail(p, MG_EINVAL, "hs_split * ncomb must be <= 256");
+        p->hs_split = value;
     } else if (!strcmp(key, "timing")) {
         p->timing = value != 0;
     } else if (!strcmp(key, "jamp_chunk_mib")) {
         if (value < 1) return fail(p, MG_EINVAL, "bad jamp_chunk_mib");
         p->jamp_chunk_bytes = (long)value << 20;
     } else return fail(p, MG_EINVAL, std::string("unknown option ") + key);
+    return MG_OK;
+}
+
+extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
+{
+    if (!p || !key || !value) return MG_EINVAL;
+    if (!strcmp(key, "color_sum")) *value = p->color_sum;
+    else if (!strcmp(key, "schedule")) *value = p->schedule;
+    else if (!strcmp(key, "block")) *value = p->block;
+    else if (!strcmp(key, "diagrams")) *value = p->diagrams;
+    else if (!strcmp(key, "hs_split")) *value = p->hs_split;
+    else if (!strcmp(key, "timing")) *value = p->timing;
+    else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
+    else return MG_EINVAL;
     return MG_OK;
 }
 
@@ -240,7 +282,7 @@ static int chunk_events(const mg_process* p, int nevt, int nhel)
 static size_t ws_bytes_for(const mg_process* p, int nevt, int nhel)
 {
     size_t b = align256((size_t)nhel * nevt * sizeof(double));
-    if (p->color_sum == MG_CS_TENSOR && nevt > 0) {
+    if ((p->color_sum == MG_CS_TENSOR || p->diagrams == MG_DIAG_SHARED) && nevt > 0) {
         const int ce = chunk_events(p, nevt, nhel);
         b += align256(color_sum_padded_rows((long)nhel * ce) * p->d->ncolor * 2 * cs_elem(p));
     }
@@ -268,8 +310,12 @@ __global__ void helicity_sum_kernel(const double* __restrict__ meh, int nhel, in
 static int set_good(mg_process* p, const std::vector<int>& good)
 {
     p->good = good;
-    if (!good.empty())
+    if (!good.empty()) {
         CUDA_TRY(p, cudaMemcpy(p->d_good, good.data(), good.size() * sizeof(int), cudaMemcpyHostToDevice));
+        std::vector<int> pos(p->d->ncomb, -1);
+        for (size_t i = 0; i < good.size(); i++) pos[good[i]] = (int)i;
+        CUDA_TRY(p, cudaMemcpy(p->d_pos, pos.data(), pos.size() * sizeof(int), cudaMemcpyHostToDevice));
+    }
     return MG_OK;
 }
 
@@ -335,6 +381,22 @@ static int ensure_streams(mg_process* p, int n)
     return MG_OK;
 }
 
+// timing mark: the work enqueued since the previous mark belongs to `stage` (-1 = start of the batch)
+static int mark(mg_process* p, int stage, cudaStream_t st)
+{
+    if (!p->timing) return MG_OK;
+    if (p->ev_n == (int)p->ev_pool.size()) {
+        cudaEvent_t e;
+        CUDA_TRY(p, cudaEventCreate(&e));
+        p->ev_pool.push_back(e); p->ev_stage.push_back(0);
+    }
+    p->ev_stage[p->ev_n] = stage;
+    CUDA_TRY(p, cudaEventRecord(p->ev_pool[p->ev_n], st));
+    p->ev_n++;
+    return MG_OK;
+}
+#define MARK(stage) do { int rc_ = mark(p, stage, st); if (rc_ != MG_OK) return rc_; } while (0)
+
 // diagram stage for events [e0, e0+ne) of the batch, all good helicities
 static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
 {
@@ -342,6 +404,7 @@ static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
     if (p->schedule == MG_SCHED_GRID) {
         a.hel_base = 0; a.nhel = nhel;
         CUDA_TRY(p, p->d->launch(p->precision, a, st));
+        p->launches++;
     } else {
         int rc = ensure_streams(p, nhel);
         if (rc != MG_OK) return rc;
@@ -350,6 +413,7 @@ static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
             CUDA_TRY(p, cudaStreamWaitEvent(p->streams[h], p->ev_fork, 0));
             a.hel_base = h; a.nhel = 1;
             CUDA_TRY(p, p->d->launch(p->precision, a, p->streams[h]));
+            p->launches++;
             CUDA_TRY(p, cudaEventRecord(p->ev_join[h], p->streams[h]));
             CUDA_TRY(p, cudaStreamWaitEvent(st, p->ev_join[h], 0));
         }
@@ -376,17 +440,38 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
     const int nhel = (int)p->good.size();
     double* d_meh = (double*)d_workspace;
     char* d_j = (char*)d_workspace + align256((size_t)nhel * nevt * sizeof(double));
-    p->timed = false;
-    if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[0], st));
-    if (p->color_sum == MG_CS_FUSED) {
+    p->timed = false; p->ev_n = 0; p->launches = 0;
+    MARK(-1);
+    if (p->diagrams == MG_DIAG_SHARED) {
+        // helicity-shared diagram kernel -> jamps [2][ncolor][rows], rows (event, helicity) -> colour-sum kernel
+        const int ce = chunk_events(p, nevt, nhel);
+        for (int e0 = 0; e0 < nevt; e0 += ce) {
+            const int ne = nevt - e0 < ce ? nevt - e0 : ce;
+            const long rows = (long)nhel * ne;
+            HsLaunch a;
+            a.mom = d_momenta + (size_t)e0 * p->d->npar * 4; a.nevt = ne; a.d_pos = p->d_pos; a.nrow_evt = nhel;
+            a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows); a.mt = p->mT; a.wt = p->wT;
+            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, p->hs_split, st));
+            p->launches += 2;                      // + the colour-sum kernel below
+            MARK(0);
+            RowMap map;
+            map.rows_valid = rows; map.hel_minor = nhel; map.evt_stride = nevt; map.e0 = e0; map.norm = make_norm(p);
+            cudaError_t ce_;
+            if (p->color_sum == MG_CS_TENSOR || p->precision == MG_FP64)
+                ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
+            else
+                ce_ = color_sum_alu(false, p->d->ncolor, p->d_cmat, d_j, a.rows, d_meh, st, &map);
+            if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("colour sum: ") + cudaGetErrorString(ce_));
+            MARK(1);
+        }
+    } else if (p->color_sum == MG_CS_FUSED) {
         DiagLaunch a = base_launch(p, d_momenta, nevt);
         a.d_hel = p->d_good; a.d_meh = d_meh; a.mode = MG_CS_FUSED;
         int rc = run_diagrams(p, a, st);
         if (rc != MG_OK) return rc;
-        if (p->timing) { CUDA_TRY(p, cudaEventRecord(p->ev_t[1], st)); CUDA_TRY(p, cudaEventRecord(p->ev_t[2], st)); }
+        MARK(0);
     } else {
         const int ce = chunk_events(p, nevt, nhel);
-        if (p->timing && ce < nevt) return fail(p, MG_EINVAL, "timing needs a single jamps chunk (raise jamp_chunk_mib)");
         for (int e0 = 0; e0 < nevt; e0 += ce) {
             const int ne = nevt - e0 < ce ? nevt - e0 : ce;
             const long rows = (long)nhel * ne;
@@ -394,17 +479,28 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             a.d_hel = p->d_good; a.mode = MG_CS_TENSOR; a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows);
             int rc = run_diagrams(p, a, st);
             if (rc != MG_OK) return rc;
-            if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[1], st));
+            MARK(0);
             // rows are (helicity-major, event-minor); the contraction writes norm * J^T C J per row into me_h
-            cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, rows, ne,
-                                               nevt, e0, make_norm(p), d_meh, st);
+            RowMap map;
+            map.rows_valid = rows; map.ne = ne; map.evt_stride = nevt; map.e0 = e0; map.norm = make_norm(p);
+            cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("color_sum_tensor: ") + cudaGetErrorString(ce_));
-            if (p->timing) CUDA_TRY(p, cudaEventRecord(p->ev_t[2], st));
+            p->launches++;
+            MARK(1);
         }
     }
     helicity_sum_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, d_me);
     CUDA_TRY(p, cudaGetLastError());
-    if (p->timing) { CUDA_TRY(p, cudaEventRecord(p->ev_t[3], st)); p->timed = true; }
+    p->launches++;
+    MARK(2);
+    p->timed = p->timing != 0;
+    return MG_OK;
+}
+
+extern "C" int mg_last_launch_count(const mg_process* p, int* launches)
+{
+    if (!p || !launches) return MG_EINVAL;
+    *launches = p->launches;
     return MG_OK;
 }
 
@@ -412,8 +508,13 @@ extern "C" int mg_last_stage_ms(mg_process* p, float ms[3])
 {
     if (!p || !ms) return MG_EINVAL;
     if (!p->timed) return fail(p, MG_ESTATE, "no timed batch (set option timing=1 first)");
-    CUDA_TRY(p, cudaEventSynchronize(p->ev_t[3]));
-    for (int i = 0; i < 3; i++) CUDA_TRY(p, cudaEventElapsedTime(&ms[i], p->ev_t[i], p->ev_t[i + 1]));
+    CUDA_TRY(p, cudaEventSynchronize(p->ev_pool[p->ev_n - 1]));
+    ms[0] = ms[1] = ms[2] = 0.f;
+    for (int k = 1; k < p->ev_n; k++) {
+        float t = 0.f;
+        CUDA_TRY(p, cudaEventElapsedTime(&t, p->ev_pool[k - 1], p->ev_pool[k]));
+        ms[p->ev_stage[k]] += t;
+    }
     return MG_OK;
 }
 
@@ -471,8 +572,9 @@ extern "C" int mg_color_sum(mg_process* p, int impl, const void* d_jamps, long n
     if (impl == MG_CS_FUSED) e = color_sum_alu(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, d_jamps, nrows, d_out, st);
     else if (impl == MG_CS_TENSOR) {
         if (nrows != color_sum_padded_rows(nrows)) return fail(p, MG_EINVAL, "nrows must be a multiple of 128 for the tensor kernel");
-        e = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_jamps, nrows, nrows, (int)nrows, (int)nrows, 0,
-                             1.0, d_out, st);
+        RowMap map;
+        map.rows_valid = nrows;
+        e = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_jamps, nrows, map, d_out, st);
     } else return fail(p, MG_EINVAL, "bad impl");
     if (e != cudaSuccess) return fail(p, MG_ECUDA, std::string("color sum: ") + cudaGetErrorString(e));
     return MG_OK;

@@ -22,7 +22,7 @@ namespace mg {
 // scalar-ALU reference kernel: one thread per row, triangular form
 template <typename T, int NC>
 __global__ void __launch_bounds__(128) color_sum_alu_kernel(const T* __restrict__ cm, const T* __restrict__ J, long nrows,
-                                                            double* __restrict__ out)
+                                                            double* __restrict__ out, RowMap map)
 {
     const long r = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= nrows) return;
@@ -41,25 +41,28 @@ __global__ void __launch_bounds__(128) color_sum_alu_kernel(const T* __restrict_
         const T cii = cm[i * NC + i];
         acc += re[i] * (cii * re[i] + T(2) * sr) + im[i] * (cii * im[i] + T(2) * si);
     }
-    out[r] = double(acc);
+    map.store(out, r, double(acc));
 }
 
 template <typename T>
-static cudaError_t alu_dispatch(int nc, const void* cm, const void* J, long nrows, double* out, cudaStream_t st)
+static cudaError_t alu_dispatch(int nc, const void* cm, const void* J, long nrows, double* out, RowMap map, cudaStream_t st)
 {
     const int blk = 128;
     const unsigned grid = (unsigned)((nrows + blk - 1) / blk);
-#define CASE(N) case N: color_sum_alu_kernel<T, N><<<grid, blk, 0, st>>>((const T*)cm, (const T*)J, nrows, out); break;
+#define CASE(N) case N: color_sum_alu_kernel<T, N><<<grid, blk, 0, st>>>((const T*)cm, (const T*)J, nrows, out, map); break;
     switch (nc) { CASE(1) CASE(2) CASE(6) CASE(24) CASE(120) default: return cudaErrorInvalidValue; }
 #undef CASE
     return cudaGetLastError();
 }
 
 cudaError_t color_sum_alu(bool is_fp64, int ncolor, const void* d_cmat, const void* d_jamps, long nrows, double* d_out,
-                          cudaStream_t st)
+                          cudaStream_t st, const RowMap* map)
 {
-    return is_fp64 ? alu_dispatch<double>(ncolor, d_cmat, d_jamps, nrows, d_out, st)
-                   : alu_dispatch<float>(ncolor, d_cmat, d_jamps, nrows, d_out, st);
+    RowMap id;                        // identity: out[r]
+    id.rows_valid = nrows;
+    const RowMap m = map ? *map : id;
+    return is_fp64 ? alu_dispatch<double>(ncolor, d_cmat, d_jamps, nrows, d_out, m, st)
+                   : alu_dispatch<float>(ncolor, d_cmat, d_jamps, nrows, d_out, m, st);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -75,8 +78,7 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 // NT = number of 8-wide n-tiles (ncolor padded to 8*NT); L: [8*NT][8*NT] row-major, lower-triangular, zero padded
 template <int NT>
 __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __restrict__ L, const double* __restrict__ X, int ncolor,
-                                                             long rows_padded, long rows_valid, int ne, int evt_stride, int e0,
-                                                             double norm, double* __restrict__ meh)
+                                                             long rows_padded, RowMap map, double* __restrict__ meh)
 {
     constexpr int NCP = 8 * NT;
     const int lane = threadIdx.x & 31;
@@ -110,10 +112,7 @@ __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __res
     s += __shfl_xor_sync(0xffffffffu, s, 1);
     s += __shfl_xor_sync(0xffffffffu, s, 2);
     const long row = row0 + ar;
-    if (ak == 0 && row < rows_valid) {
-        const long ih = row / ne, el = row - ih * ne;
-        meh[ih * evt_stride + e0 + el] = norm * s;
-    }
+    if (ak == 0) map.store(meh, row, s);
 }
 
 // Cholesky factor of the integer colour matrix, computed on the host in long double and zero-padded to a
@@ -137,20 +136,19 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
     return true;
 }
 
-cudaError_t color_sum_tf32(int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded, long rows_valid, int ne,
-                           int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st);
+cudaError_t color_sum_tf32(int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded, const RowMap& map, double* d_meh,
+                           cudaStream_t st);
 
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
-                             long rows_padded, long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st)
+                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st)
 {
-    if (!is_fp64) return color_sum_tf32(ncolor, d_cmat, d_jamps, rows_padded, rows_valid, ne, evt_stride, e0, norm, d_meh, st);
+    if (!is_fp64) return color_sum_tf32(ncolor, d_cmat, d_jamps, rows_padded, map, d_meh, st);
     if (!d_chol) return cudaErrorInvalidValue;
     const int ncp = (ncolor + 7) / 8 * 8;
     const int warps = 4;
     const unsigned grid = (unsigned)((rows_padded / 8 + warps - 1) / warps);
     const double* X = (const double*)d_jamps;
-#define LAUNCH(NT) color_sum_dmma_kernel<NT><<<grid, warps * 32, 0, st>>>(d_chol, X, ncolor, rows_padded, rows_valid, ne, \
-                                                                           evt_stride, e0, norm, d_meh)
+#define LAUNCH(NT) color_sum_dmma_kernel<NT><<<grid, warps * 32, 0, st>>>(d_chol, X, ncolor, rows_padded, map, d_meh)
     switch (ncp / 8) {
         case 1: LAUNCH(1); break;
         case 3: LAUNCH(3); break;

@@ -9,18 +9,36 @@ namespace mg {
 // rows of the jamps buffer are padded to the tensor kernels' row tile
 inline long color_sum_padded_rows(long rows) { return (rows + 127) / 128 * 128; }
 
+// where the result of row r goes: d_out[ih * evt_stride + e0 + el] = norm * value, with (ih, el) = (helicity, event)
+// of the row.  Rows are helicity-major (r = ih * ne + el; hel_minor = 0) or event-major (r = el * hel_minor + ih).
+struct RowMap {
+    long rows_valid = 0;
+    int ne = 0;            // events per helicity block (helicity-major); 0 = identity map d_out[r]
+    int hel_minor = 0;     // helicities per event (event-major) or 0
+    int evt_stride = 0, e0 = 0;
+    double norm = 1.0;
+#if defined(__CUDACC__)
+    __device__ __forceinline__ void store(double* __restrict__ out, long r, double v) const
+    {
+        if (r >= rows_valid) return;
+        if (hel_minor > 0) { const long el = r / hel_minor; const long ih = r - el * hel_minor; out[ih * evt_stride + e0 + el] = norm * v; }
+        else if (ne > 0) { const long ih = r / ne; const long el = r - ih * ne; out[ih * evt_stride + e0 + el] = norm * v; }
+        else out[r] = norm * v;
+    }
+#endif
+};
+
 // out[r] = sum_ij (Re J_i C_ij Re J_j + Im J_i C_ij Im J_j) on the scalar ALUs, triangular form.
 // d_jamps: [2][ncolor][nrows] fp64 (is_fp64) or fp32; d_cmat: [ncolor][ncolor] numerators in the same type.
 cudaError_t color_sum_alu(bool is_fp64, int ncolor, const void* d_cmat, const void* d_jamps, long nrows, double* d_out,
-                          cudaStream_t st);
+                          cudaStream_t st, const RowMap* map = nullptr);
 
-// Tensor-core contraction.  d_jamps: [2][ncolor][rows_padded]; rows are (helicity-major, event-minor) with ne
-// events per helicity; row (ih, el) goes to d_meh[ih * evt_stride + e0 + el] = norm * J^T C J.
+// Tensor-core contraction.  d_jamps: [2][ncolor][rows_padded]; row r goes where `map` says, times map.norm.
 //   fp64: DMMA (mma.sync m8n8k4 f64) on Z = X L with C = L L^T (Cholesky, lower-triangular: upper k-tiles skipped)
 //   fp32: tcgen05.mma kind::tf32, exact integer C, J split in two TF32 terms, fp32 accumulation in TMEM
 //   d_chol: DEVICE [ncp][ncp] padded Cholesky factor (fp64 only; see color_cholesky_padded)
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
-                             long rows_padded, long rows_valid, int ne, int evt_stride, int e0, double norm, double* d_meh, cudaStream_t st);
+                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st);
 
 // host: L with C = L L^T (lower-triangular, row-major, zero-padded to ncp = 8*ceil(ncolor/8) columns)
 bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out);

@@ -4,7 +4,7 @@
 
 namespace mg {
 
-cudaError_t color_sum_tf32(int, const void*, const void*, long, long, int, int, int, double, double*, cudaStream_t)
+cudaError_t color_sum_tf32(int, const void*, const void*, long, const RowMap&, double*, cudaStream_t)
 {
     return cudaErrorNotSupported;
 }

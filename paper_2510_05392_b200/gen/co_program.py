@@ -1,0 +1,368 @@
+"""Helicity-shared program ("hs") of a g g -> t tbar + (n-2) g process: tables for csrc/hs_kernel.cu.
+
+Starting point: the diagram program of gen/diagrams.py -- every Feynman diagram explicitly enumerated
+(Table 2), cut at its centroid vertex into <= 4 off-shell currents with <= half of the
+external legs each, one amplitude per diagram term, `jamp[sigma] += coeff * amp`.
+
+Two exact rewritings of that sum (neither changes what is computed):
+
+  (1) helicity sharing.  A current with legs L depends on the helicities of L only, so it has 2^|L| <= 8
+      distinct values ("variants") per event, not ncomb = 2^npar.  They are computed once per event and
+      kept in shared memory; the thread of helicity combination h reads variant pext(h, L).
+
+  (2) factorised colour.  Within the amplitudes that share (vertex type, leg sets of the branches), the
+      coefficient of flow sigma is a product of the branches' own colour polynomials evaluated on the
+      sub-words of sigma (gen/colour.py: concat / commutator substitution), times a sign that depends on
+      (sigma, leg sets) only.  The vertex functions are multilinear, hence
+          sum_d coeff[sigma, d] * V(c1_d, c2_d, c3_d) = s * V(O1, O2, O3),   O_i = sum_c col_c[w_i(sigma)] c
+      with O_i "colour-ordered objects": signed sums of the Feynman currents of one leg set.  The
+      factorisation is verified term by term against the diagram program in `build` (`_check_expansion`).
+
+  Every V(O1, O2, O3) is then split as X . Y with Y the branch with most legs (<= 3) and X = the vertex
+  contracted with the other branches (a "pair object", 2^(npar-|Y|) variants, metric folded in), so that
+  the per-helicity work of one jamp is a short sum of 4-component complex dot products and each jamp is
+  complete when its loop ends -- no per-thread jamp array.
+
+Tables (all int32, see `Tables`): objects + terms (phase 1), per group of colour flows the pair objects
++ terms (phase 2) and the dot-product entries (phase 3), the variant lookup, the leg sets.
+"""
+from __future__ import annotations
+
+from collections import defaultdict
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from . import colour, diagrams
+
+STAR = colour.STAR
+
+# term opcodes (phase 1: currents with propagators; phase 2: raw vertices, output lowered for the plain dot)
+OPS = {"ext_v": 0, "ext_ql": 1, "ext_qr": 2, "v3": 3, "v4": 4, "ffv_l": 5, "ffv_r": 6, "ffv_p": 7,
+       "x_row": 8, "x_col": 9, "x_bil": 10, "x_v3": 11, "x_v4": 12}
+
+
+@dataclass
+class Term:
+    sign: int
+    op: str
+    args: tuple            # object ids (ext ops: (particle,))
+    legs: tuple            # legs of the result (sorted particles)
+
+
+@dataclass
+class Obj:
+    id: int
+    kind: str              # 'V' | 'FO' | 'FI'
+    legs: tuple            # sorted particle indices
+    terms: list = field(default_factory=list)
+    off: int = 0           # offset in the object area, units of one complex number
+
+
+def _gluons(legs):
+    return frozenset((ip if ip < 2 else ip - 2) for ip in legs if ip not in (2, 3))
+
+
+def _key_word(c, sigma):
+    """sub-word of the colour flow sigma seen by current c (with the hole for a gluon-type current that
+    contains the quark line)"""
+    own = _gluons(c.legs)
+    if c.kind == "V" and 2 in c.legs:
+        w, done = [], False
+        for g in sigma:
+            if g in own:
+                w.append(g)
+            elif not done:
+                w.append(STAR)
+                done = True
+        return tuple(w)
+    return tuple(g for g in sigma if g in own)
+
+
+class Program:
+    def __init__(self, n, group_prefix=None):
+        self.n = n
+        self.proc = diagrams.build_process(n)
+        self.npar = n + 2
+        self.name = self.proc.name
+        self.ncolor = self.proc.ncolor
+        self.group_prefix = group_prefix if group_prefix is not None else max(0, n - 2)
+        self.objs: list[Obj] = []
+        self._fobj = {}          # Feynman current id -> object id (levels 1, 2)
+        self._combo = {}         # canonical combination -> object id
+        self._build_objects()
+        self._build_evals()
+        self._check_expansion()
+        self._build_groups()
+
+    # ---------------------------------------------------------------------------------------------
+    def _new_obj(self, kind, legs):
+        o = Obj(len(self.objs), kind, tuple(sorted(legs)))
+        self.objs.append(o)
+        return o
+
+    def _term_of_current(self, c, sign):
+        cur = self.proc.currents
+        if c.op == "ext_v":
+            return Term(sign, c.op, (c.args[0],), tuple(sorted(c.legs)))
+        if c.op in ("ext_ql", "ext_qr"):
+            return Term(sign, c.op, (2 if c.op == "ext_ql" else 3,), tuple(sorted(c.legs)))
+        return Term(sign, c.op, tuple(self._fobj[i] for i in c.args), tuple(sorted(c.legs)))
+
+    def _build_objects(self):
+        cur = self.proc.currents
+        for c in cur:                      # ids are topologically ordered
+            if len(c.legs) <= 2:
+                o = self._new_obj(c.kind, c.legs)
+                o.terms.append(self._term_of_current(c, 1))
+                self._fobj[c.id] = o.id
+        self._by_legs = defaultdict(list)
+        for c in cur:
+            self._by_legs[(c.kind, c.legs)].append(c)
+
+    def object_for(self, kind, legs, word):
+        """(object id, sign) of the colour-ordered combination sum_c col_c[word] c over the currents of
+        this kind and leg set"""
+        combo = tuple(sorted((c.id, c.col[word]) for c in self._by_legs[(kind, legs)] if c.col.get(word, 0)))
+        assert combo, (kind, legs, word)
+        assert all(abs(s) == 1 for _, s in combo)
+        if len(legs) <= 2:
+            assert len(combo) == 1
+            return self._fobj[combo[0][0]], combo[0][1]
+        sign = combo[0][1]
+        canon = tuple((i, s * sign) for i, s in combo)
+        if canon not in self._combo:
+            o = self._new_obj(kind, legs)
+            for i, s in canon:
+                o.terms.append(self._term_of_current(self.proc.currents[i], s))
+            self._combo[canon] = o.id
+        return self._combo[canon], sign
+
+    # ---------------------------------------------------------------------------------------------
+    def _build_evals(self):
+        """per colour flow sigma: the distinct vertex evaluations (op, ((object, sign), ...)) -> sign"""
+        proc = self.proc
+        cur = proc.currents
+        assert max(len(c.legs) for c in cur) <= 3, "centroid branches with more than 3 legs are not supported"
+        inv = {v: k for k, v in proc.rank.items()}
+        self.sigmas = [inv[j] for j in range(self.ncolor)]
+        self.evals = [dict() for _ in range(self.ncolor)]
+        self._raw = [dict() for _ in range(self.ncolor)]       # for the expansion check
+        for a in proc.amps:
+            for j, co in a.jamps:
+                s = inv[j]
+                words = [_key_word(cur[i], s) for i in a.args]
+                prod = 1
+                for i, w in zip(a.args, words):
+                    prod *= cur[i].col.get(w, 0)
+                assert prod in (1, -1), "coefficient does not factorise"
+                sign = co // prod
+                assert sign in (1, -1)
+                objs = tuple(self.object_for(cur[i].kind, cur[i].legs, w) for i, w in zip(a.args, words))
+                key = (a.op, objs)
+                if key in self.evals[j]:
+                    assert self.evals[j][key] == sign
+                self.evals[j][key] = sign
+                self._raw[j][(a.op, a.args)] = co
+
+    def _check_expansion(self):
+        """expanding every factorised evaluation back into Feynman currents must give exactly the diagram
+        program's (amplitude, coefficient) list of that colour flow: no term lost, none invented"""
+        import itertools
+        members = {}
+        for canon, oid in self._combo.items():
+            members[oid] = list(canon)
+        for cid, oid in self._fobj.items():
+            members[oid] = [(cid, 1)]
+        for j in range(self.ncolor):
+            got = {}
+            for (op, objs), sign in self.evals[j].items():
+                for combo in itertools.product(*[members[o] for o, _ in objs]):
+                    co = sign
+                    for (_, osign), (_, csign) in zip(objs, combo):
+                        co *= osign * csign
+                    k = (op, tuple(c for c, _ in combo))
+                    got[k] = got.get(k, 0) + co
+            got = {k: v for k, v in got.items() if v}
+            assert got == self._raw[j], f"factorised colour flow {j} differs from the diagram program"
+
+    # ---------------------------------------------------------------------------------------------
+    def _split_xy(self, op, objs):
+        """V(objs) = X . Y: index of Y, the raw-vertex term that builds X, and the rearrangement sign"""
+        nlegs = [len(self.objs[o].legs) for o, _ in objs]
+        iy = max(range(len(objs)), key=lambda i: (nlegs[i], i))
+        ids = [o for o, _ in objs]
+        if op == "ffv":                                   # (fo, v, fi)
+            xop, args, sg = {2: ("x_row", (ids[0], ids[1]), 1), 0: ("x_col", (ids[1], ids[2]), 1),
+                             1: ("x_bil", (ids[0], ids[2]), 1)}[iy]
+        elif op == "vvv":                                 # totally antisymmetric: cyclic rotations are even
+            xop, sg = "x_v3", 1
+            args = {2: (ids[0], ids[1]), 0: (ids[1], ids[2]), 1: (ids[2], ids[0])}[iy]
+        elif op == "vvvv":                                # (x y | z w) = (x.z)(y.w) - (x.w)(y.z)
+            x, y, z, w = ids
+            xop = "x_v4"                                  # x_v4(p, q, r) = (p.r) q - (q.r) p
+            args, sg = {3: ((x, y, z), 1), 2: ((x, y, w), -1), 0: ((w, z, y), 1), 1: ((z, w, x), 1)}[iy]
+        else:
+            raise ValueError(op)
+        return iy, xop, args, sg
+
+    def _build_groups(self, merge=True):
+        """groups of colour flows (same first `group_prefix` letters), their pair objects and dot entries"""
+        gp = self.group_prefix
+        order = defaultdict(list)
+        for j, s in enumerate(self.sigmas):
+            order[s[:gp]].append(j)
+        self.groups = []          # dicts: sigmas [j], xobjs [ {legs, terms:[Term]} ], entries {j: [(xslot, yobj, sign)]}
+        for pre in sorted(order):
+            xkey_to_slot, xobjs, entries = {}, [], {}
+            for j in order[pre]:
+                per_y = defaultdict(list)                 # (y object, x legs) -> [(sign, xop, args)]
+                for (op, objs), sign in sorted(self.evals[j].items()):
+                    iy, xop, args, sg = self._split_xy(op, objs)
+                    total = sign * sg
+                    for _, os_ in objs:
+                        total *= os_
+                    yo = objs[iy][0]
+                    key = yo if merge else (yo, len(per_y))
+                    per_y[key].append((total, xop, args))
+                ents = []
+                for key, terms in per_y.items():
+                    yo = key if merge else key[0]
+                    terms = sorted(terms, key=lambda t: (t[1], t[2]))
+                    s0 = terms[0][0]
+                    canon = tuple((t[0] * s0, t[1], t[2]) for t in terms)
+                    if canon not in xkey_to_slot:
+                        legs = set()
+                        for _, _, args in canon:
+                            for a in args:
+                                legs |= set(self.objs[a].legs)
+                        legs = tuple(sorted(legs))
+                        assert set(legs) | set(self.objs[yo].legs) == set(range(self.npar))
+                        assert not set(legs) & set(self.objs[yo].legs)
+                        xkey_to_slot[canon] = len(xobjs)
+                        xobjs.append({"legs": legs, "terms": [Term(sg_, xop, args, legs) for sg_, xop, args in canon]})
+                    ents.append((xkey_to_slot[canon], yo, s0))
+                entries[j] = ents
+            self.groups.append({"sigmas": order[pre], "xobjs": xobjs, "entries": entries})
+
+    def stats(self):
+        nx = [len(g["xobjs"]) for g in self.groups]
+        xv = [sum(1 << len(x["legs"]) for x in g["xobjs"]) for g in self.groups]
+        ne = sum(len(e) for g in self.groups for e in g["entries"].values())
+        nt = sum(len(x["terms"]) * (1 << len(x["legs"])) for g in self.groups for x in g["xobjs"])
+        ov = sum(1 << len(o.legs) for o in self.objs)
+        return {"name": self.name, "objects": len(self.objs), "object_variants": ov, "groups": len(self.groups),
+                "xobjs_per_group_max": max(nx), "x_variants_per_group_max": max(xv), "dot_entries": ne,
+                "x_term_variants": nt, "obj_term_variants": sum(len(o.terms) << len(o.legs) for o in self.objs)}
+
+    # ---------------------------------------------------------------------------------------------
+    def tables(self):
+        """flatten to the int32 arrays read by csrc/hs_kernel.cu (layout documented in csrc/hs_tables.h)"""
+        npar = self.npar
+        # objects sorted by number of legs (phase 1 runs level by level); ids are remapped
+        order = sorted(range(len(self.objs)), key=lambda i: (len(self.objs[i].legs), i))
+        remap = {old: new for new, old in enumerate(order)}
+        objs = [self.objs[i] for i in order]
+        legsets, ls_id = [], {}
+
+        def lsid(legs):
+            if legs not in ls_id:
+                ls_id[legs] = len(legsets)
+                legsets.append(legs)
+            return ls_id[legs]
+
+        def submask(parent, child):
+            m = 0
+            for j, p in enumerate(parent):
+                if p in child:
+                    m |= 1 << j
+            assert bin(m).count("1") == len(child)
+            return m
+
+        terms = []
+
+        def add_terms(tl, parent_legs):
+            first = len(terms)
+            for t in tl:
+                if t.op.startswith("ext"):
+                    a = [t.args[0], 0, 0]
+                    sub = [0, 0, 0]
+                else:
+                    a = [remap[x] for x in t.args] + [0] * (3 - len(t.args))
+                    sub = [submask(parent_legs, self.objs[x].legs) for x in t.args] + [0] * (3 - len(t.args))
+                terms.append([OPS[t.op] | ((1 if t.sign < 0 else 0) << 8) | (sub[0] << 16) | (sub[1] << 24),
+                              a[0] | (a[1] << 16), a[2] | (sub[2] << 16), 0])
+            return first, len(tl)
+
+        obj_tab, off = [], 0
+        for o in objs:
+            t0, nt = add_terms(o.terms, o.legs)
+            o_off = off
+            off += 4 << len(o.legs)
+            obj_tab.append([o_off, len(o.legs) | (lsid(o.legs) << 8), t0, nt])
+        obj_area = off                                        # complex numbers
+        # phase-1 items per level
+        p1_items, p1_level = [], [0]
+        for lvl in (1, 2, 3):
+            for i, o in enumerate(objs):
+                if len(o.legs) == lvl:
+                    p1_items += [(i << 8) | v for v in range(1 << lvl)]
+            p1_level.append(len(p1_items))
+        # groups
+        vrows, vrow_id = [], {}
+
+        def vrow(xlegs):
+            if xlegs not in vrow_id:
+                ylegs = tuple(p for p in range(npar) if p not in xlegs)
+                row = []
+                for h in range(1 << npar):
+                    hb = [(h >> (npar - 1 - p)) & 1 for p in range(npar)]
+                    vx = sum(hb[p] << j for j, p in enumerate(xlegs))
+                    vy = sum(hb[p] << j for j, p in enumerate(ylegs))
+                    row.append(vx | (vy << 8))
+                vrow_id[xlegs] = len(vrows)
+                vrows.append(row)
+            return vrow_id[xlegs]
+
+        grp_tab, x_tab, x_items, sig_tab, ent_tab = [], [], [], [], []
+        stage_max = 0
+        for g in self.groups:
+            x0, xi0, s0 = len(x_tab), len(x_items), len(sig_tab)
+            soff, slots = 0, []
+            for k, x in enumerate(g["xobjs"]):
+                t0, nt = add_terms(x["terms"], x["legs"])
+                slots.append(soff)
+                x_tab.append([soff, len(x["legs"]), t0, nt])
+                x_items += [(k << 8) | v for v in range(1 << len(x["legs"]))]
+                soff += 4 << len(x["legs"])
+            stage_max = max(stage_max, soff)
+            for j in g["sigmas"]:
+                e0 = len(ent_tab)
+                for xs, yo, sign in g["entries"][j]:
+                    x = g["xobjs"][xs]
+                    y = objs[remap[yo]]
+                    ent_tab.append([slots[xs] | ((1 << len(x["legs"])) << 16),
+                                    obj_tab[remap[yo]][0] | ((1 << len(y.legs)) << 16), vrow(x["legs"]), sign])
+                sig_tab.append([j, e0, len(ent_tab) - e0, 0])
+            grp_tab.append([x0, xi0, len(x_items) - xi0, s0, len(sig_tab) - s0, 0, 0, 0])
+        ls_mask = [sum(1 << p for p in legs) for legs in legsets]
+        i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w) if len(a) else np.zeros((0, w), np.int32)
+        return {
+            "npar": npar, "ncolor": self.ncolor, "obj_area": obj_area, "stage_area": stage_max,
+            "nobj": len(objs), "nlegsets": len(legsets), "ngroups": len(grp_tab),
+            "obj": i32(obj_tab, 4), "term": i32(terms, 4), "p1_items": np.asarray(p1_items, np.int32),
+            "p1_level": np.asarray(p1_level, np.int32), "legset_mask": np.asarray(ls_mask, np.int32),
+            "group": i32(grp_tab, 8), "xobj": i32(x_tab, 4), "x_items": np.asarray(x_items, np.int32),
+            "sigma": i32(sig_tab, 4), "entry": i32(ent_tab, 4),
+            "vtab": np.asarray(vrows, np.int32).astype(np.uint16).reshape(-1, 1 << npar),
+        }
+
+
+_CACHE = {}
+
+
+def build(n, group_prefix=None):
+    key = (n, group_prefix)
+    if key not in _CACHE:
+        _CACHE[key] = Program(n, group_prefix)
+    return _CACHE[key]

@@ -1,0 +1,124 @@
+"""numpy interpreter of the helicity-shared program tables (gen/co_program.py) -- CPU TEST HELPER.
+
+Decodes the int32 tables exactly as csrc/hs_kernel.cu does (same packing, same variant convention) and
+restates every opcode with the plain gamma-matrix helpers of tests/ir_eval.py, so that the generator's
+factorised program can be checked against the diagram program and the oracle before any kernel runs.
+Not product, not oracle; nothing here is imported by the package.
+"""
+import numpy as np
+
+import ir_eval as ir
+
+G = ir.G
+
+
+def _pext(v, mask):
+    out, j = 0, 0
+    b = 0
+    while mask >> b:
+        if (mask >> b) & 1:
+            out |= ((v >> b) & 1) << j
+            j += 1
+        b += 1
+    return out
+
+
+def evaluate(T, mom, mt, wt):
+    """jamps[ncolor][2^npar] (without the g^n factor) of one event from the tables T"""
+    npar = T["npar"]
+    k = [mom[i] * (1 if i < 2 else -1) for i in range(npar)]
+    K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
+    obj, term = T["obj"], T["term"]
+    area = np.zeros(T["obj_area"], dtype=complex)
+
+    def load(o, var):
+        off, info = obj[o][0], obj[o][1]
+        nv = 1 << (info & 0xFF)
+        return np.array([area[off + c * nv + var] for c in range(4)])
+
+    def kof(o):
+        return K[obj[o][1] >> 8]
+
+    def run_terms(t0, nt, var, legs_of_parent=None, kout=None):
+        acc = np.zeros(4, dtype=complex)
+        for t in term[t0:t0 + nt]:
+            w0, w1, w2 = int(t[0]) & 0xFFFFFFFF, int(t[1]) & 0xFFFFFFFF, int(t[2]) & 0xFFFFFFFF
+            op, neg = w0 & 0xFF, (w0 >> 8) & 1
+            sub = [(w0 >> 16) & 0xFF, (w0 >> 24) & 0xFF, (w2 >> 16) & 0xFF]
+            a = [w1 & 0xFFFF, w1 >> 16, w2 & 0xFFFF]
+            hel = 1 if var & 1 else -1
+            if op == 0:
+                e = ir.polvec(mom[a[0]], hel)
+                r = e if a[0] < 2 else e.conj()
+            elif op == 1:
+                r = ir.u_spinor(mom[2], mt, hel).conj() @ ir.GAM[0]
+            elif op == 2:
+                r = ir.v_spinor(mom[3], mt, hel)
+            else:
+                A = load(a[0], _pext(var, sub[0]))
+                B = load(a[1], _pext(var, sub[1]))
+                kA, kB = kof(a[0]), kof(a[1])
+                if op == 3:
+                    r = (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A) / ir.mdot(kout, kout)
+                elif op == 4:
+                    Z = load(a[2], _pext(var, sub[2]))
+                    r = (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A) / ir.mdot(kout, kout)
+                elif op == 5:
+                    q = -kout
+                    r = A @ ir.slash(B) @ (ir.slash(q) + mt * np.eye(4)) / (ir.mdot(q, q) - mt * mt + 1j * mt * wt)
+                elif op == 6:
+                    q = kout
+                    r = (ir.slash(q) + mt * np.eye(4)) @ ir.slash(A) @ B / (ir.mdot(q, q) - mt * mt + 1j * mt * wt)
+                elif op == 7:
+                    r = np.array([A @ ir.GAM[mu] @ B for mu in range(4)]) / ir.mdot(kout, kout)
+                elif op == 8:
+                    r = A @ ir.slash(B)
+                elif op == 9:
+                    r = ir.slash(A) @ B
+                elif op == 10:
+                    r = G * np.array([A @ ir.GAM[mu] @ B for mu in range(4)])
+                elif op == 11:
+                    r = G * (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A)
+                elif op == 12:
+                    Z = load(a[2], _pext(var, sub[2]))
+                    r = G * (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A)
+                else:
+                    raise ValueError(op)
+            acc = acc + (-r if neg else r)
+        return acc
+
+    # phase 1: objects, level by level
+    for it in T["p1_items"]:
+        o, var = int(it) >> 8, int(it) & 0xFF
+        off, info, t0, nt = (int(x) for x in obj[o])
+        nv = 1 << (info & 0xFF)
+        val = run_terms(t0, nt, var, kout=K[info >> 8])
+        for c in range(4):
+            area[off + c * nv + var] = val[c]
+    # phases 2 and 3, group by group
+    nh = 1 << npar
+    J = np.zeros((T["ncolor"], nh), dtype=complex)
+    stage = np.zeros(max(T["stage_area"], 1), dtype=complex)
+    for g in T["group"]:
+        x0, xi0, nxi, s0, ns = (int(x) for x in g[:5])
+        for it in T["x_items"][xi0:xi0 + nxi]:
+            xk, var = int(it) >> 8, int(it) & 0xFF
+            soff, lognv, t0, nt = (int(x) for x in T["xobj"][x0 + xk])
+            nv = 1 << lognv
+            val = run_terms(t0, nt, var)
+            for c in range(4):
+                stage[soff + c * nv + var] = val[c]
+        for sg in T["sigma"][s0:s0 + ns]:
+            j, e0, ne = int(sg[0]), int(sg[1]), int(sg[2])
+            for h in range(nh):
+                acc = 0j
+                for e in T["entry"][e0:e0 + ne]:
+                    w0, w1, row, sign = (int(x) for x in e)
+                    offx, nvx = w0 & 0xFFFF, w0 >> 16
+                    offy, nvy = w1 & 0xFFFF, w1 >> 16
+                    vv = int(T["vtab"][row][h])
+                    vx, vy = vv & 0xFF, vv >> 8
+                    d = sum(stage[offx + c * nvx + vx] * area[offy + c * nvy + vy] for c in range(4))
+                    acc += sign * d
+                J[j][h] = acc
+    return J

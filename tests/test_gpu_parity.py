@@ -82,7 +82,9 @@ def test_scheduling_variants_agree(B, process):
     mom = inputs.momenta(process, nevt, seed=2)
     d_mom = torch.from_numpy(mom).cuda()
     base = None
-    for opts in ({}, {"schedule": 1}, {"color_sum": 1}, {"color_sum": 1, "schedule": 1}, {"block": 64}):
+    for opts in ({"diagrams": 0}, {"diagrams": 0, "schedule": 1}, {"diagrams": 0, "color_sum": 1},
+                 {"diagrams": 0, "color_sum": 1, "schedule": 1}, {"diagrams": 0, "block": 64},
+                 {"diagrams": 1}, {"diagrams": 1, "hs_split": 2}, {"diagrams": 1, "jamp_chunk_mib": 1}):
         proc = B.init_process(process, "fp64")
         for k, v in opts.items():
             proc.set_option(k, v)
@@ -90,7 +92,8 @@ def test_scheduling_variants_agree(B, process):
         if base is None:
             base = me
         else:
-            assert _relerr(me, base).max() < 1e-12, opts
+            # the helicity-shared kernel sums the same diagram terms in another order: rounding-level differences
+            assert _relerr(me, base).max() < (1e-10 if opts.get("diagrams") else 1e-12), opts
         proc.close()
 
 
@@ -132,8 +135,12 @@ def test_edge_cases(B):
     # empty batch
     me = proc.sigma_batch(torch.empty((0, 4, 4), dtype=torch.float64, device="cuda"))
     assert me.numel() == 0
-    # single event, and the library's implicit filter
-    mom = inputs.momenta("gg_ttx", 1)
+    # the library's implicit filter on a small first batch (a single-event probe would drop helicities that are
+    # below 1e-8 on that one event: reading A5), then a single event
+    mom = inputs.momenta("gg_ttx", 64)
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert _relerr(me, _oracle("gg_ttx", mom)).max() < 1e-10
+    mom = mom[:1].copy()
     me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
     assert _relerr(me, _oracle("gg_ttx", mom)).max() < 1e-10
     # GOODHELICITIES=ALL: same answer
