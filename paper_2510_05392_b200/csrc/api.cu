@@ -156,6 +156,7 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
         cudaError_t e = hs_create(d->ngluon, &p->hs);
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
         if (d->ngluon >= 4) p->diagrams = MG_DIAG_SHARED;     // measured default, see DESIGN.md
+        if (2 * d->ncomb <= 256) p->hs_split = 2;             // 16 instead of 8 warps per SM: measured +30% (profiles/r1_hs_kernel.md)
     }
     *out = p;
     return MG_OK;
