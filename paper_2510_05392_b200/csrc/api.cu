@@ -39,7 +39,7 @@ struct mg_process {
     int* d_good = nullptr;     // DEVICE [ncomb]
     int* d_all = nullptr;      // DEVICE [ncomb] = 0..ncomb-1
     void* d_cmat = nullptr;    // DEVICE [ncolor^2] numerators as the colour-sum type
-    double* d_chol = nullptr;  // DEVICE [ncp^2] Cholesky factor of the numerators (MG_FP64 tensor colour sum)
+    void* d_chol = nullptr;    // DEVICE Cholesky factor of the numerators for the tensor colour sum: fp64 [ncp^2] (MG_FP64) or its TF32 image
     // helicity streams
     std::vector<cudaStream_t> streams;
     cudaEvent_t ev_fork = nullptr;
@@ -111,6 +111,11 @@ static int upload_tables(mg_process* p)
         if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
         CUDA_TRY(p, cudaMalloc(&p->d_chol, lp.size() * sizeof(double)));
         CUDA_TRY(p, cudaMemcpy(p->d_chol, lp.data(), lp.size() * sizeof(double), cudaMemcpyHostToDevice));
+    } else {
+        std::vector<float> img;
+        if (!tf32_build_factor_image(d->ncolor, d->cmat, img)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
+        CUDA_TRY(p, cudaMalloc(&p->d_chol, img.size() * sizeof(float)));
+        CUDA_TRY(p, cudaMemcpy(p->d_chol, img.data(), img.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     std::vector<int> all(d->ncomb);
     for (int i = 0; i < d->ncomb; i++) all[i] = i;

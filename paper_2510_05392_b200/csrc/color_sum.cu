@@ -136,14 +136,15 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
     return true;
 }
 
-cudaError_t color_sum_tf32(int ncolor, const void* d_cmat, const void* d_jamps, long rows_padded, const RowMap& map, double* d_meh,
-                           cudaStream_t st);
+cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
+                           double* d_meh, cudaStream_t st);
 
-cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
+cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
                              long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st)
 {
-    if (!is_fp64) return color_sum_tf32(ncolor, d_cmat, d_jamps, rows_padded, map, d_meh, st);
-    if (!d_chol) return cudaErrorInvalidValue;
+    if (!is_fp64) return color_sum_tf32(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st);
+    if (!d_factor) return cudaErrorInvalidValue;
+    const double* d_chol = (const double*)d_factor;
     const int ncp = (ncolor + 7) / 8 * 8;
     const int warps = 4;
     const unsigned grid = (unsigned)((rows_padded / 8 + warps - 1) / warps);

@@ -35,13 +35,17 @@ cudaError_t color_sum_alu(bool is_fp64, int ncolor, const void* d_cmat, const vo
 
 // Tensor-core contraction.  d_jamps: [2][ncolor][rows_padded]; row r goes where `map` says, times map.norm.
 //   fp64: DMMA (mma.sync m8n8k4 f64) on Z = X L with C = L L^T (Cholesky, lower-triangular: upper k-tiles skipped)
-//   fp32: tcgen05.mma kind::tf32, exact integer C, J split in two TF32 terms, fp32 accumulation in TMEM
-//   d_chol: DEVICE [ncp][ncp] padded Cholesky factor (fp64 only; see color_cholesky_padded)
-cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const double* d_chol, const void* d_jamps,
+//   fp32: tcgen05.mma kind::tf32 on Z = X L, X and L split in two TF32 terms (3 products), fp32 accumulation in TMEM
+//   d_factor: DEVICE Cholesky factor of C: fp64 [ncp][ncp] padded (color_cholesky_padded), or the two-term TF32
+//             image of it (tf32_build_factor_image) for fp32
+cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
                              long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st);
 
 // host: L with C = L L^T (lower-triangular, row-major, zero-padded to ncp = 8*ceil(ncolor/8) columns)
 bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out);
+
+// host: two-term TF32 image [hi | lo] of the Cholesky factor in the tcgen05 shared-memory layout (color_sum_tf32.cu)
+bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img);
 
 // peak probes (mg_measure_peak)
 cudaError_t measure_peak(int kind, double* tflops);
