@@ -30,7 +30,7 @@ struct mg_process {
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
-    int diagrams = MG_DIAG_THREAD, hs_split = 1;
+    int diagrams = MG_DIAG_THREAD, hs_split = 1, hs_phase3 = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 1L << 30;
@@ -161,6 +161,7 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
         cudaError_t e = hs_create(d->ngluon, &p->hs);
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
         if (d->ngluon >= 4) p->diagrams = MG_DIAG_SHARED;     // measured default, see DESIGN.md
+        if (d->npar >= 6) p->hs_phase3 = 1;                   // jamp dot products on the FP64 tensor path (DMMA)
         if (2 * d->ncomb <= 256) p->hs_split = 2;             // 16 instead of 8 warps per SM: measured +30% (profiles/r1_hs_kernel.md)
     }
     *out = p;
@@ -251,6 +252,10 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         if (value != 1 && value != 2 && value != 4) return fail(p, MG_EINVAL, "bad hs_split");
         if (value * p->d->ncomb > 256) return fail(p, MG_EINVAL, "hs_split * ncomb must be <= 256");
         p->hs_split = value;
+    } else if (!strcmp(key, "hs_phase3")) {
+        if (value != 0 && value != 1) return fail(p, MG_EINVAL, "bad hs_phase3");
+        if (value == 1 && p->d->npar < 6) return fail(p, MG_EINVAL, "hs_phase3 = 1 needs >= 6 external particles");
+        p->hs_phase3 = value;
     } else if (!strcmp(key, "timing")) {
         p->timing = value != 0;
     } else if (!strcmp(key, "jamp_chunk_mib")) {
@@ -268,6 +273,7 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "block")) *value = p->block;
     else if (!strcmp(key, "diagrams")) *value = p->diagrams;
     else if (!strcmp(key, "hs_split")) *value = p->hs_split;
+    else if (!strcmp(key, "hs_phase3")) *value = p->hs_phase3;
     else if (!strcmp(key, "timing")) *value = p->timing;
     else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
     else return MG_EINVAL;
@@ -457,7 +463,7 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             HsLaunch a;
             a.mom = d_momenta + (size_t)e0 * p->d->npar * 4; a.nevt = ne; a.d_pos = p->d_pos; a.nrow_evt = nhel;
             a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows); a.mt = p->mT; a.wt = p->wT;
-            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, p->hs_split, st));
+            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, p->hs_split, p->hs_phase3, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
             RowMap map;

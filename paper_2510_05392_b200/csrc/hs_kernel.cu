@@ -18,7 +18,9 @@ namespace mg {
 struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask; const int4* group;
     const int4* xobj; const int* x_items; const int4* sigma; const int4* entry; const unsigned short* vtab;
+    const unsigned char* hdep;
     int npar, ncolor, ngroups, obj_area, stage_area, nlegsets;
+    int nw3;               // warps with a jamp accumulator (phase 3 on the FP64 tensor path); 0 = scalar phase 3
     int p1_level[4];
 };
 
@@ -32,11 +34,24 @@ __device__ __forceinline__ int pext8(int v, int mask)
     return out;
 }
 
-__device__ __forceinline__ void load_obj(const double2* __restrict__ area, int off, int nv, int var, wf<double>& w)
+// Shared-memory layout of an object: [variant][component], 16 bytes per complex number, the component index
+// XOR-swizzled with bits 1-2 of the variant: slot(var, c) = 4 var + (c ^ ((var >> 1) & 3)).  Eight consecutive
+// variants of one component (phases 1, 2: lane <-> variant) and the 2 variants x 4 components of a DMMA fragment
+// quarter-warp (phase 3) both fall into eight different 16-byte bank groups.
+__device__ __forceinline__ int slot(int var, int c) { return 4 * var + (c ^ ((var >> 1) & 3)); }
+
+__device__ __forceinline__ void load_obj(const double2* __restrict__ area, int off, int var, wf<double>& w)
 {
-    const double2* p = area + off + var;
+    const double2* p = area + off;
 #pragma unroll
-    for (int c = 0; c < 4; c++) { const double2 v = p[c * nv]; w.c[c].re = v.x; w.c[c].im = v.y; }
+    for (int c = 0; c < 4; c++) { const double2 v = p[slot(var, c)]; w.c[c].re = v.x; w.c[c].im = v.y; }
+}
+
+__device__ __forceinline__ void store_obj(double2* __restrict__ area, int off, int var, const wf<double>& w)
+{
+    double2* p = area + off;
+#pragma unroll
+    for (int c = 0; c < 4; c++) p[slot(var, c)] = make_double2(w.c[c].re, w.c[c].im);
 }
 
 __device__ __forceinline__ p4<double> load_k(const double* __restrict__ Ks, int ls)
@@ -72,15 +87,15 @@ __device__ __noinline__ void run_terms(const HsDev& d, const double2* __restrict
         } else {
             const int4 oa = __ldg(d.obj + a0), ob = __ldg(d.obj + a1);
             wf<double> A, B;
-            load_obj(area, oa.x, 1 << (oa.y & 0xFF), pext8(var, (w.x >> 16) & 0xFF), A);
-            load_obj(area, ob.x, 1 << (ob.y & 0xFF), pext8(var, (w.x >> 24) & 0xFF), B);
+            load_obj(area, oa.x, pext8(var, (w.x >> 16) & 0xFF), A);
+            load_obj(area, ob.x, pext8(var, (w.x >> 24) & 0xFF), B);
             switch (op) {
                 case 3: v3_off(A, load_k(Ks, oa.y >> 8), B, load_k(Ks, ob.y >> 8), 1.0 / m2(load_k(Ks, ls_out)), r); break;
                 case 11: v3_off(A, load_k(Ks, oa.y >> 8), B, load_k(Ks, ob.y >> 8), 1.0, r); lower(r); break;
                 case 4: case 12: {
                     const int4 oc = __ldg(d.obj + a2);
                     wf<double> Z;
-                    load_obj(area, oc.x, 1 << (oc.y & 0xFF), pext8(var, (w.z >> 16) & 0xFF), Z);
+                    load_obj(area, oc.x, pext8(var, (w.z >> 16) & 0xFF), Z);
                     v4_off(A, B, Z, op == 4 ? 1.0 / m2(load_k(Ks, ls_out)) : 1.0, r);
                     if (op == 12) lower(r);
                     break;
@@ -98,6 +113,91 @@ __device__ __noinline__ void run_terms(const HsDev& d, const double2* __restrict
     }
 }
 
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// accumulator slot of helicity combination h (gen/co_program.py acc_swizzle)
+__device__ __forceinline__ int acc_swizzle(int h)
+{
+    const int hi = h >> 3;
+    return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7));
+}
+
+// Phase 3 on the FP64 tensor path (DMMA, mma.sync.m8n8k4.f64): ONE warp evaluates one dot entry for all 2^npar
+// helicity combinations.  With hx/hy the variants of X/Y, the entry is the complex product sum
+//     out[hx][hy] = sum_c X_c[hx] * Y_c[hy]      (c = 4 components)
+// i.e. a real GEMM  [nvx x 8] . [8 x 2 nvy]:  A = [Re X | Im X],  B = [Re Y, Im Y ; -Im Y, Re Y]  (columns (hy, re/im)).
+// A-fragment lane (row r = lane/4, k = lane%4) reads X_k[8 mt + r] once (16 bytes: the k-step 0 and k-step 1 values),
+// B-fragment lane (k = lane%4, col = lane/4) reads Y_k[4 nt + col/2]; the C fragment of a lane is the complex number
+// (hx = 8 mt + lane/4, hy = 4 nt + lane%4).  Operand traffic per entry: <= 6 LDS.128 per lane instead of 8 per
+// helicity.  Entries of one colour flow have different leg partitions, so the fragments are added into a per-warp
+// accumulator in shared memory indexed by the helicity combination (swizzled; tables hdep) and the finished jamp is
+// written once, coalesced over helicities.
+template <typename T2>
+__device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, const double2* __restrict__ area,
+                                            const double2* __restrict__ stage, double2* __restrict__ acc, int e, const int4 g0,
+                                            const int4 g1, int warp, int lane)
+{
+    const int nh = 1 << d.npar;
+    const int r = lane >> 2, c = lane & 3;
+    for (int s = warp; s < g1.x; s += d.nw3) {
+        const int4 sg = __ldg(d.sigma + g0.w + s);
+        for (int k = 0; k < sg.z; k++) {
+            const int4 en = __ldg(d.entry + sg.y + k);
+            const int nvx = en.x >> 16, nvy = en.y >> 16;
+            const double2* __restrict__ X = stage + (en.x & 0xFFFF);
+            const double2* __restrict__ Y = area + (en.y & 0xFFFF);
+            const unsigned char* __restrict__ hd = d.hdep + en.z * 40;
+            const int MT = nvx >> 3, NT = nvy >> 2;          // (MT, NT) in {(1,2), (2,1), (2,2), (4,1)}
+            double2 xa[4], yb[2];
+            double b0[2], b1[2];
+#pragma unroll
+            for (int mt = 0; mt < 4; mt++) if (mt < MT) xa[mt] = X[slot(8 * mt + r, c)];
+#pragma unroll
+            for (int nt = 0; nt < 2; nt++)
+                if (nt < NT) {
+                    yb[nt] = Y[slot(4 * nt + (r >> 1), c)];
+                    b0[nt] = (r & 1) ? yb[nt].y : yb[nt].x;          // k-step 0: A = Re X
+                    b1[nt] = (r & 1) ? yb[nt].x : -yb[nt].y;         // k-step 1: A = Im X
+                }
+            const double sgn = (double)en.w;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                if (t < MT * NT) {
+                    const int mt = NT == 2 ? (t >> 1) : t, nt = NT == 2 ? (t & 1) : 0;
+                    const double2 xv = NT == 2 ? xa[t >> 1] : xa[t];
+                    const double p0 = (NT == 2 && (t & 1)) ? b0[1] : b0[0];
+                    const double p1 = (NT == 2 && (t & 1)) ? b1[1] : b1[0];
+                    double c0 = 0.0, c1 = 0.0;
+                    dmma884(c0, c1, xv.x, p0);
+                    dmma884(c0, c1, xv.y, p1);
+                    const int idx = hd[8 * mt + r] ^ hd[32 + 4 * nt + c];
+                    double2 v = make_double2(0.0, 0.0);
+                    if (k > 0) v = acc[idx];
+                    v.x = fma(sgn, c0, v.x); v.y = fma(sgn, c1, v.y);
+                    acc[idx] = v;
+                }
+            }
+            __syncwarp();
+        }
+        // the finished jamp of this colour flow, all helicity combinations
+        T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
+        for (int h = lane; h < nh; h += 32) {
+            const int pos = a.d_pos[h];
+            if (pos >= 0) {
+                const double2 v = acc[acc_swizzle(h)];
+                const size_t row = (size_t)e * a.nrow_evt + pos;
+                out[(size_t)sg.x * a.rows + row] = T2(v.x);
+                out[(size_t)(d.ncolor + sg.x) * a.rows + row] = T2(v.y);
+            }
+        }
+        __syncwarp();
+    }
+}
+
 // T2 = type of the jamps buffer (double: MG_FP64, float: MG_MIXED -- PAPER.md:122 "FPTYPE=m")
 // blockDim.x = 2^npar * nsplit: thread = (sigma split s, helicity combination h)
 template <typename T2>
@@ -106,7 +206,8 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
     extern __shared__ double2 sm[];
     double2* __restrict__ area = sm;
     double2* __restrict__ stage = sm + d.obj_area;
-    double* __restrict__ Ks = reinterpret_cast<double*>(stage + d.stage_area);
+    double2* __restrict__ accs = stage + d.stage_area;
+    double* __restrict__ Ks = reinterpret_cast<double*>(accs + (d.nw3 << d.npar));
     double* __restrict__ pm = Ks + 4 * d.nlegsets;
     const int tid = threadIdx.x, nth = blockDim.x;
     const int nh = 1 << d.npar;
@@ -132,12 +233,10 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
             for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += nth) {
                 const int it = __ldg(d.p1_items + i);
                 const int4 o = __ldg(d.obj + (it >> 8));
-                const int var = it & 0xFF, nv = 1 << (o.y & 0xFF);
+                const int var = it & 0xFF;
                 wf<double> acc;
                 run_terms(d, area, Ks, pm, o.z, o.w, var, o.y >> 8, a.mt, a.wt, acc);
-                double2* out = area + o.x + var;
-#pragma unroll
-                for (int c = 0; c < 4; c++) out[c * nv] = make_double2(acc.c[c].re, acc.c[c].im);
+                store_obj(area, o.x, var, acc);
             }
             __syncthreads();
         }
@@ -148,16 +247,17 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
             for (int i = tid; i < g0.z; i += nth) {
                 const int it = __ldg(d.x_items + g0.y + i);
                 const int4 x = __ldg(d.xobj + g0.x + (it >> 8));
-                const int var = it & 0xFF, nv = 1 << x.y;
+                const int var = it & 0xFF;
                 wf<double> acc;
                 run_terms(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc);
-                double2* out = stage + x.x + var;
-#pragma unroll
-                for (int c = 0; c < 4; c++) out[c * nv] = make_double2(acc.c[c].re, acc.c[c].im);
+                store_obj(stage, x.x, var, acc);
             }
             __syncthreads();
             // phase 3: the jamps of this group, one colour flow at a time
-            if (pos >= 0) {
+            if (d.nw3 > 0) {
+                const int warp = tid >> 5;
+                if (warp < d.nw3) phase3_dmma<T2>(d, a, area, stage, accs + (warp << d.npar), e, g0, g1, warp, tid & 31);
+            } else if (pos >= 0) {
                 for (int s = split; s < g1.x; s += nsplit) {
                     const int4 sg = __ldg(d.sigma + g0.w + s);
                     double re = 0.0, im = 0.0;
@@ -165,13 +265,13 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                     for (int k = 0; k < sg.z; k++) {
                         const int4 en = __ldg(d.entry + sg.y + k);
                         const int vv = __ldg(d.vtab + en.z * nh + h);
-                        const int nvx = en.x >> 16, nvy = en.y >> 16;
-                        const double2* __restrict__ X = stage + (en.x & 0xFFFF) + (vv & 0xFF);
-                        const double2* __restrict__ Y = area + (en.y & 0xFFFF) + (vv >> 8);
+                        const int vx = vv & 0xFF, vy = vv >> 8;
+                        const double2* __restrict__ X = stage + (en.x & 0xFFFF);
+                        const double2* __restrict__ Y = area + (en.y & 0xFFFF);
                         double tr = 0.0, ti = 0.0;
 #pragma unroll
                         for (int c = 0; c < 4; c++) {
-                            const double2 x = X[c * nvx], y = Y[c * nvy];
+                            const double2 x = X[slot(vx, c)], y = Y[slot(vy, c)];
                             tr = fma(x.x, y.x, tr); tr = fma(-x.y, y.y, tr);
                             ti = fma(x.x, y.y, ti); ti = fma(x.y, y.x, ti);
                         }
@@ -195,6 +295,7 @@ struct HsContext {
     void* blob = nullptr;
     size_t smem = 0;
     int sms = 148;
+    int max_sigma = 0;
 };
 
 const HsTables* hs_host_tables(const HsContext* c) { return c->t; }
@@ -210,11 +311,12 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     // one device blob, every table 16-byte aligned
     struct Part { const void* src; size_t bytes; size_t off; };
     const int nh = 1 << t->npar;
-    Part parts[10] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
+    Part parts[11] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
                        { t->p1_items, sizeof(int) * t->np1, 0 }, { t->legset_mask, sizeof(int) * t->nlegsets, 0 },
                        { t->group, sizeof(int) * 8 * t->ngroups, 0 }, { t->xobj, sizeof(int) * 4 * t->nxobj, 0 },
                        { t->x_items, sizeof(int) * t->nxitems, 0 }, { t->sigma, sizeof(int) * 4 * t->nsigma, 0 },
-                       { t->entry, sizeof(int) * 4 * t->nentry, 0 }, { t->vtab, sizeof(unsigned short) * nh * t->nvrow, 0 } };
+                       { t->entry, sizeof(int) * 4 * t->nentry, 0 }, { t->vtab, sizeof(unsigned short) * nh * t->nvrow, 0 },
+                       { t->hdep, (size_t)40 * t->nvrow, 0 } };
     size_t total = 0;
     for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
     cudaError_t e = cudaMalloc(&c->blob, total ? total : 256);
@@ -231,12 +333,16 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     d.group = (const int4*)(b + parts[4].off); d.xobj = (const int4*)(b + parts[5].off);
     d.x_items = (const int*)(b + parts[6].off); d.sigma = (const int4*)(b + parts[7].off);
     d.entry = (const int4*)(b + parts[8].off); d.vtab = (const unsigned short*)(b + parts[9].off);
+    d.hdep = (const unsigned char*)(b + parts[10].off); d.nw3 = 0;
     d.npar = t->npar; d.ncolor = t->ncolor; d.ngroups = t->ngroups; d.obj_area = t->obj_area; d.stage_area = t->stage_area;
     d.nlegsets = t->nlegsets;
     for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
     c->smem = sizeof(double2) * ((size_t)t->obj_area + t->stage_area) + sizeof(double) * 4 * (t->nlegsets + t->npar);
-    e = cudaFuncSetAttribute(hs_diagrams_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(hs_diagrams_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    // colour flows per group (phase-3 tasks): at most that many warps get a jamp accumulator
+    for (int g = 0; g < t->ngroups; g++) if (t->group[8 * g + 4] > c->max_sigma) c->max_sigma = t->group[8 * g + 4];
+    const size_t smem_max = c->smem + sizeof(double2) * ((size_t)8 << t->npar);
+    e = cudaFuncSetAttribute(hs_diagrams_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hs_diagrams_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     if (e != cudaSuccess) { cudaFree(c->blob); delete c; return e; }
     int dev = 0;
     cudaGetDevice(&dev);
@@ -252,14 +358,22 @@ void hs_destroy(HsContext* c)
     delete c;
 }
 
-cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, int nsplit, cudaStream_t st)
+cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, int nsplit, int phase3, cudaStream_t st)
 {
     if (a.nevt <= 0) return cudaSuccess;
     const int threads = (1 << c->t->npar) * nsplit;
     if (nsplit < 1 || threads > 256) return cudaErrorInvalidValue;
+    HsDev d = c->d;
+    size_t smem = c->smem;
+    if (phase3 == 1) {                               // FP64 tensor path: needs the 8 x 4 fragment shapes (>= 3 legs on the X side)
+        if (c->t->npar < 6) return cudaErrorInvalidValue;
+        const int warps = threads / 32;
+        d.nw3 = warps < c->max_sigma ? warps : c->max_sigma;
+        smem += sizeof(double2) * ((size_t)d.nw3 << d.npar);
+    }
     const int grid = a.nevt;                         // one CTA per event; the hardware scheduler keeps every SM full
-    if (jamps_fp64) hs_diagrams_kernel<double><<<grid, threads, c->smem, st>>>(c->d, a);
-    else hs_diagrams_kernel<float><<<grid, threads, c->smem, st>>>(c->d, a);
+    if (jamps_fp64) hs_diagrams_kernel<double><<<grid, threads, smem, st>>>(d, a);
+    else hs_diagrams_kernel<float><<<grid, threads, smem, st>>>(d, a);
     return cudaGetLastError();
 }
 

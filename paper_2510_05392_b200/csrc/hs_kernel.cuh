@@ -23,6 +23,7 @@ void hs_destroy(HsContext* c);
 const HsTables* hs_host_tables(const HsContext* c);
 size_t hs_smem_bytes(const HsContext* c);
 // nsplit = threads per helicity combination (1, 2 or 4; blockDim = 2^npar * nsplit <= 256)
-cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, int nsplit, cudaStream_t st);
+// phase3 = 0: dot products on the scalar FP64 ALUs (thread = helicity); 1: on the FP64 tensor path (DMMA, warp = colour flow)
+cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, int nsplit, int phase3, cudaStream_t st);
 
 }  // namespace mg

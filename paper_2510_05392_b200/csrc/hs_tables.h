@@ -21,6 +21,8 @@
 //   sigma[s]  = { jamp index, first entry, number of entries, 0 }
 //   entry[e]  = { x offset | x variants<<16, y offset | y variants<<16, vtab row, sign }
 //   vtab[row][h] (uint16) = x variant | y variant<<8 for helicity combination h (particle 0 = most significant bit)
+//   hdep[row][v] (uint8)  = acc_swizzle(helicity bits of x variant v) for v < 32, of y variant v - 32 for v >= 32
+//                           (phase 3 on the FP64 tensor path: accumulator slot of (vx, vy) = hdep[vx] ^ hdep[32 + vy])
 #pragma once
 
 namespace mg {
@@ -39,6 +41,7 @@ struct HsTables {
     const int* sigma;
     const int* entry;
     const unsigned short* vtab;
+    const unsigned char* hdep;                // [nvrow][40]: swizzled accumulator index parts, x variants 0..31 then y variants 0..7
     double flops_p1, flops_p2, flops_p3;      // per event (phases 1, 2) and per (event, helicity) (phase 3)
 };
 

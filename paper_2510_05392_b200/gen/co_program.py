@@ -42,6 +42,15 @@ OPS = {"ext_v": 0, "ext_ql": 1, "ext_qr": 2, "v3": 3, "v4": 4, "ffv_l": 5, "ffv_
        "x_row": 8, "x_col": 9, "x_bil": 10, "x_v3": 11, "x_v4": 12}
 
 
+def acc_swizzle(h):
+    """index of helicity combination h in the per-warp jamp accumulator of csrc/hs_kernel.cu (phase 3): a GF(2)-linear
+    map that XORs the bank-group bits (h & 7) with distinct non-zero 3-bit codes of the higher bits, so that the 8
+    lanes of a quarter-warp (3 varying helicity bits) mostly hit 8 different 16-byte bank groups"""
+    hi = h >> 3
+    t = ((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7)
+    return h ^ t
+
+
 @dataclass
 class Term:
     sign: int
@@ -309,11 +318,15 @@ class Program:
                     p1_items += [(i << 8) | v for v in range(1 << lvl)]
             p1_level.append(len(p1_items))
         # groups
-        vrows, vrow_id = [], {}
+        vrows, vrow_id, hdep = [], {}, []
 
         def vrow(xlegs):
             if xlegs not in vrow_id:
                 ylegs = tuple(p for p in range(npar) if p not in xlegs)
+                # phase 3 on the FP64 tensor path: swizzled accumulator index of (x variant, y variant) = hdep_x ^ hdep_y
+                dep = lambda v, legs: sum(((v >> j) & 1) << (npar - 1 - p) for j, p in enumerate(legs))
+                hdep.append([acc_swizzle(dep(v, xlegs)) if v < (1 << len(xlegs)) else 0 for v in range(32)] +
+                            [acc_swizzle(dep(v, ylegs)) if v < (1 << len(ylegs)) else 0 for v in range(8)])
                 row = []
                 for h in range(1 << npar):
                     hb = [(h >> (npar - 1 - p)) & 1 for p in range(npar)]
@@ -355,6 +368,7 @@ class Program:
             "group": i32(grp_tab, 8), "xobj": i32(x_tab, 4), "x_items": np.asarray(x_items, np.int32),
             "sigma": i32(sig_tab, 4), "entry": i32(ent_tab, 4),
             "vtab": np.asarray(vrows, np.int32).astype(np.uint16).reshape(-1, 1 << npar),
+            "hdep": np.asarray(hdep, np.int32).astype(np.uint8).reshape(-1, 40),
         }
 
 
