@@ -20,18 +20,14 @@ struct HsDev {
     const int4* xobj; const int* x_items; const int4* sigma; const int4* entry; const unsigned short* vtab;
     const unsigned char* hdep;
     int npar, ncolor, ngroups, obj_area, stage_area, nlegsets;
-    int nw3;               // warps with a jamp accumulator (phase 3 on the FP64 tensor path); 0 = scalar phase 3
+    int nw3;               // jamp accumulators = colour flows per group (phase 3 on the FP64 tensor path); 0 = scalar phase 3
     int p1_level[4];
 };
 
-__device__ __forceinline__ int pext8(int v, int mask)
+// variant of an argument object: bit j = bit ((code >> 3j) & 7) of the parent's variant (7 = none; variants are < 128)
+__device__ __forceinline__ int sub_variant(int var, int code)
 {
-    int out = 0, j = 0;
-#pragma unroll
-    for (int b = 0; b < 5; b++) {
-        if ((mask >> b) & 1) { out |= ((v >> b) & 1) << j; j++; }
-    }
-    return out;
+    return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2);
 }
 
 // Shared-memory layout of an object: [variant][component], 16 bytes per complex number, the component index
@@ -66,36 +62,42 @@ __device__ __forceinline__ void lower(wf<double>& w)
     for (int c = 1; c < 4; c++) { w.c[c].re = -w.c[c].re; w.c[c].im = -w.c[c].im; }
 }
 
-// sum of the terms [t0, t0+nt) for helicity variant `var` of an object whose leg set has total momentum kout
-__device__ __noinline__ void run_terms(const HsDev& d, const double2* __restrict__ area, const double* __restrict__ Ks,
-                                       const double* __restrict__ pm, int t0, int nt, int var, int ls_out, double mt,
-                                       double wt, wf<double>& acc)
+// argument of a term: word = offset in the area (16 bits) | sub-variant code (9 bits) << 16
+__device__ __forceinline__ void load_arg(const double2* __restrict__ area, int word, int var, wf<double>& w)
+{
+    load_obj(area, word & 0xFFFF, sub_variant(var, (word >> 16) & 0x1FF), w);
+}
+
+// Sum of the terms [t0, t0 + nt) for helicity variant `var` of an object whose leg set has total momentum K(ls_out).
+// Inlined at its two call sites (phases 1 and 2) so that the accumulator stays in registers; the next term's table
+// word is fetched while the current one is evaluated.
+__device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restrict__ area, const double* __restrict__ Ks,
+                                          const double* __restrict__ pm, int t0, int nt, int var, int ls_out, double mt,
+                                          double wt, wf<double>& acc)
 {
 #pragma unroll
     for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
-    for (int t = t0; t < t0 + nt; t++) {
-        const int4 w = __ldg(d.term + t);
+    int4 w = __ldg(d.term + t0);
+    for (int t = 0; t < nt; t++) {
+        const int4 wn = __ldg(d.term + t0 + (t + 1 < nt ? t + 1 : t));
         const int op = w.x & 0xFF, neg = (w.x >> 8) & 1;
-        const int a0 = w.y & 0xFFFF, a1 = (w.y >> 16) & 0xFFFF, a2 = w.z & 0xFFFF;
         wf<double> r;
         if (op <= 2) {
             const int hel = (var & 1) ? 1 : -1;
-            const double* p = pm + 4 * a0;
-            if (op == 0) ext_eps(p, hel, a0 >= 2, r);
+            const double* p = pm + 4 * w.y;
+            if (op == 0) ext_eps(p, hel, w.y >= 2, r);
             else if (op == 1) ext_ubar(p, mt, hel, r);
             else ext_v(p, mt, hel, r);
         } else {
-            const int4 oa = __ldg(d.obj + a0), ob = __ldg(d.obj + a1);
             wf<double> A, B;
-            load_obj(area, oa.x, pext8(var, (w.x >> 16) & 0xFF), A);
-            load_obj(area, ob.x, pext8(var, (w.x >> 24) & 0xFF), B);
+            load_arg(area, w.y, var, A);
+            load_arg(area, w.z, var, B);
             switch (op) {
-                case 3: v3_off(A, load_k(Ks, oa.y >> 8), B, load_k(Ks, ob.y >> 8), 1.0 / m2(load_k(Ks, ls_out)), r); break;
-                case 11: v3_off(A, load_k(Ks, oa.y >> 8), B, load_k(Ks, ob.y >> 8), 1.0, r); lower(r); break;
+                case 3: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0 / m2(load_k(Ks, ls_out)), r); break;
+                case 11: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0, r); lower(r); break;
                 case 4: case 12: {
-                    const int4 oc = __ldg(d.obj + a2);
                     wf<double> Z;
-                    load_obj(area, oc.x, pext8(var, (w.z >> 16) & 0xFF), Z);
+                    load_arg(area, w.w, var, Z);
                     v4_off(A, B, Z, op == 4 ? 1.0 / m2(load_k(Ks, ls_out)) : 1.0, r);
                     if (op == 12) lower(r);
                     break;
@@ -108,8 +110,10 @@ __device__ __noinline__ void run_terms(const HsDev& d, const double2* __restrict
                 default: ffv_p(A, B, 1.0, r); lower(r); break;       // 10: x_bil
             }
         }
-        if (neg) { for (int c = 0; c < 4; c++) acc.c[c] -= r.c[c]; }
-        else { for (int c = 0; c < 4; c++) acc.c[c] += r.c[c]; }
+        const double sg = neg ? -1.0 : 1.0;
+#pragma unroll
+        for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
+        w = wn;
     }
 }
 
@@ -138,12 +142,18 @@ __device__ __forceinline__ int acc_swizzle(int h)
 // written once, coalesced over helicities.
 template <typename T2>
 __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, const double2* __restrict__ area,
-                                            const double2* __restrict__ stage, double2* __restrict__ acc, int e, const int4 g0,
-                                            const int4 g1, int warp, int lane)
+                                            const double2* __restrict__ stage, double2* __restrict__ accs, int e, const int4 g0,
+                                            const int4 g1, int* ctr, int lane)
 {
     const int nh = 1 << d.npar;
     const int r = lane >> 2, c = lane & 3;
-    for (int s = warp; s < g1.x; s += d.nw3) {
+    while (true) {
+        // colour flows of the group are handed to the warps dynamically; flow s owns accumulator s (g1.x <= nw3)
+        int s = 0;
+        if (lane == 0) s = atomicAdd(ctr, 1);
+        s = __shfl_sync(0xffffffffu, s, 0);
+        if (s >= g1.x) break;
+        double2* __restrict__ acc = accs + (s << d.npar);
         const int4 sg = __ldg(d.sigma + g0.w + s);
         for (int k = 0; k < sg.z; k++) {
             const int4 en = __ldg(d.entry + sg.y + k);
@@ -204,6 +214,8 @@ template <typename T2>
 __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const HsLaunch a)
 {
     extern __shared__ double2 sm[];
+    __shared__ int ctr[2];                            // work-unit counters of phases 2 and 3
+    if (threadIdx.x < 2) ctr[threadIdx.x] = 0;
     double2* __restrict__ area = sm;
     double2* __restrict__ stage = sm + d.obj_area;
     double2* __restrict__ accs = stage + d.stage_area;
@@ -243,20 +255,31 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
         const size_t row = (size_t)e * a.nrow_evt + pos;
         for (int g = 0; g < d.ngroups; g++) {
             const int4 g0 = __ldg(d.group + 2 * g), g1 = __ldg(d.group + 2 * g + 1);
-            // phase 2: pair objects of this group
-            for (int i = tid; i < g0.z; i += nth) {
-                const int it = __ldg(d.x_items + g0.y + i);
-                const int4 x = __ldg(d.xobj + g0.x + (it >> 8));
-                const int var = it & 0xFF;
-                wf<double> acc;
-                run_terms(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc);
-                store_obj(stage, x.x, var, acc);
+            // phase 2: pair objects of this group; work units of 32 (pair object, variant) items with the same term
+            // shape are handed to the warps dynamically, most expensive first (gen/co_program.py)
+            {
+                const int lane = tid & 31, nunits = g0.z >> 5;
+                while (true) {
+                    int u = 0;
+                    if (lane == 0) u = atomicAdd(&ctr[0], 1);
+                    u = __shfl_sync(0xffffffffu, u, 0);
+                    if (u >= nunits) break;
+                    const int it = __ldg(d.x_items + g0.y + 32 * u + lane);
+                    if (it >= 0) {
+                        const int4 x = __ldg(d.xobj + g0.x + (it >> 8));
+                        const int var = it & 0xFF;
+                        wf<double> acc;
+                        run_terms(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc);
+                        store_obj(stage, x.x, var, acc);
+                    }
+                    __syncwarp();
+                }
             }
             __syncthreads();
+            if (tid == 0) ctr[0] = 0;                 // every warp has left the loop above; next use is after the barrier below
             // phase 3: the jamps of this group, one colour flow at a time
             if (d.nw3 > 0) {
-                const int warp = tid >> 5;
-                if (warp < d.nw3) phase3_dmma<T2>(d, a, area, stage, accs + (warp << d.npar), e, g0, g1, warp, tid & 31);
+                phase3_dmma<T2>(d, a, area, stage, accs, e, g0, g1, &ctr[1], tid & 31);
             } else if (pos >= 0) {
                 for (int s = split; s < g1.x; s += nsplit) {
                     const int4 sg = __ldg(d.sigma + g0.w + s);
@@ -284,6 +307,7 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                 }
             }
             __syncthreads();
+            if (tid == 0) ctr[1] = 0;
         }
     }
 }
@@ -367,8 +391,7 @@ cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, in
     size_t smem = c->smem;
     if (phase3 == 1) {                               // FP64 tensor path: needs the 8 x 4 fragment shapes (>= 3 legs on the X side)
         if (c->t->npar < 6) return cudaErrorInvalidValue;
-        const int warps = threads / 32;
-        d.nw3 = warps < c->max_sigma ? warps : c->max_sigma;
+        d.nw3 = c->max_sigma;                        // one accumulator per colour flow of a group
         smem += sizeof(double2) * ((size_t)d.nw3 << d.npar);
     }
     const int grid = a.nevt;                         // one CTA per event; the hardware scheduler keeps every SM full

@@ -280,27 +280,30 @@ class Program:
                 legsets.append(legs)
             return ls_id[legs]
 
-        def submask(parent, child):
-            m = 0
-            for j, p in enumerate(parent):
-                if p in child:
-                    m |= 1 << j
-            assert bin(m).count("1") == len(child)
-            return m
+        def subpos(parent, child):
+            """9-bit code p0 | p1<<3 | p2<<6: position in the parent's variant index of the j-th leg of the child
+            (7 = none: the parent variant has no such bit, so it reads as 0)"""
+            pos = [parent.index(p) for p in child]
+            assert len(pos) <= 3 and all(q < 7 for q in pos)
+            pos += [7] * (3 - len(pos))
+            return pos[0] | (pos[1] << 3) | (pos[2] << 6)
 
         terms = []
+        pending = []          # (term index, argument slot, object id before remapping): offsets are filled in below
 
         def add_terms(tl, parent_legs):
             first = len(terms)
             for t in tl:
                 if t.op.startswith("ext"):
-                    a = [t.args[0], 0, 0]
-                    sub = [0, 0, 0]
-                else:
-                    a = [remap[x] for x in t.args] + [0] * (3 - len(t.args))
-                    sub = [submask(parent_legs, self.objs[x].legs) for x in t.args] + [0] * (3 - len(t.args))
-                terms.append([OPS[t.op] | ((1 if t.sign < 0 else 0) << 8) | (sub[0] << 16) | (sub[1] << 24),
-                              a[0] | (a[1] << 16), a[2] | (sub[2] << 16), 0])
+                    terms.append([OPS[t.op] | ((1 if t.sign < 0 else 0) << 8), t.args[0], 0, 0])
+                    continue
+                ls = [lsid(self.objs[x].legs) for x in t.args]
+                assert all(l < 256 for l in ls)
+                w = [OPS[t.op] | ((1 if t.sign < 0 else 0) << 8) | (ls[0] << 16) | (ls[1] << 24), 0, 0, 0]
+                for k, x in enumerate(t.args):
+                    w[1 + k] = subpos(parent_legs, self.objs[x].legs) << 16
+                    pending.append((len(terms), 1 + k, x))
+                terms.append(w)
             return first, len(tl)
 
         obj_tab, off = [], 0
@@ -310,6 +313,7 @@ class Program:
             off += 4 << len(o.legs)
             obj_tab.append([o_off, len(o.legs) | (lsid(o.legs) << 8), t0, nt])
         obj_area = off                                        # complex numbers
+        obj_off = {o.id: obj_tab[i][0] for i, o in enumerate(objs)}
         # phase-1 items per level
         p1_items, p1_level = [], [0]
         for lvl in (1, 2, 3):
@@ -346,9 +350,18 @@ class Program:
                 t0, nt = add_terms(x["terms"], x["legs"])
                 slots.append(soff)
                 x_tab.append([soff, len(x["legs"]), t0, nt])
-                x_items += [(k << 8) | v for v in range(1 << len(x["legs"]))]
                 soff += 4 << len(x["legs"])
             stage_max = max(stage_max, soff)
+            # phase-2 work units: 32 lanes = 32 (pair object, variant) items whose term lists have the same shape, so
+            # that a warp runs them in lockstep; units are handed out dynamically, most expensive first
+            sig = lambda x: (-(1 << len(x["legs"])), -len(x["terms"]), tuple(t.op for t in x["terms"]))
+            flat = []
+            for k in sorted(range(len(g["xobjs"])), key=lambda k: sig(g["xobjs"][k])):
+                flat += [((k << 8) | v, len(g["xobjs"][k]["terms"])) for v in range(1 << len(g["xobjs"][k]["legs"]))]
+            units = [flat[i:i + 32] for i in range(0, len(flat), 32)]
+            units.sort(key=lambda u: -max(c for _, c in u))
+            for u in units:
+                x_items += [it for it, _ in u] + [-1] * (32 - len(u))
             for j in g["sigmas"]:
                 e0 = len(ent_tab)
                 for xs, yo, sign in g["entries"][j]:
@@ -358,6 +371,8 @@ class Program:
                                     obj_tab[remap[yo]][0] | ((1 << len(y.legs)) << 16), vrow(x["legs"]), sign])
                 sig_tab.append([j, e0, len(ent_tab) - e0, 0])
             grp_tab.append([x0, xi0, len(x_items) - xi0, s0, len(sig_tab) - s0, 0, 0, 0])
+        for ti, slot_, x in pending:                          # argument offsets inside the object area
+            terms[ti][slot_] |= obj_off[x]
         ls_mask = [sum(1 << p for p in legs) for legs in legsets]
         i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w) if len(a) else np.zeros((0, w), np.int32)
         return {

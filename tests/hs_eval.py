@@ -12,15 +12,9 @@ import ir_eval as ir
 G = ir.G
 
 
-def _pext(v, mask):
-    out, j = 0, 0
-    b = 0
-    while mask >> b:
-        if (mask >> b) & 1:
-            out |= ((v >> b) & 1) << j
-            j += 1
-        b += 1
-    return out
+def _sub(v, code):
+    """variant of an argument: bit j = bit (code >> 3j) & 7 of the parent's variant (7 = none)"""
+    return sum(((v >> ((code >> (3 * j)) & 7)) & 1) << j for j in range(3))
 
 
 def evaluate(T, mom, mt, wt):
@@ -30,22 +24,18 @@ def evaluate(T, mom, mt, wt):
     K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
     obj, term = T["obj"], T["term"]
     area = np.zeros(T["obj_area"], dtype=complex)
+    # this interpreter keeps an object as [variant][component]; the kernel's bank swizzle is not modelled
 
-    def load(o, var):
-        off, info = obj[o][0], obj[o][1]
-        nv = 1 << (info & 0xFF)
-        return np.array([area[off + c * nv + var] for c in range(4)])
-
-    def kof(o):
-        return K[obj[o][1] >> 8]
+    def load(w, var):
+        off, code = w & 0xFFFF, (w >> 16) & 0x1FF
+        return area[off + 4 * _sub(var, code):off + 4 * _sub(var, code) + 4].copy()
 
     def run_terms(t0, nt, var, legs_of_parent=None, kout=None):
         acc = np.zeros(4, dtype=complex)
         for t in term[t0:t0 + nt]:
-            w0, w1, w2 = int(t[0]) & 0xFFFFFFFF, int(t[1]) & 0xFFFFFFFF, int(t[2]) & 0xFFFFFFFF
+            w0, w1, w2, w3 = (int(x) & 0xFFFFFFFF for x in t)
             op, neg = w0 & 0xFF, (w0 >> 8) & 1
-            sub = [(w0 >> 16) & 0xFF, (w0 >> 24) & 0xFF, (w2 >> 16) & 0xFF]
-            a = [w1 & 0xFFFF, w1 >> 16, w2 & 0xFFFF]
+            a = [w1]
             hel = 1 if var & 1 else -1
             if op == 0:
                 e = ir.polvec(mom[a[0]], hel)
@@ -55,13 +45,13 @@ def evaluate(T, mom, mt, wt):
             elif op == 2:
                 r = ir.v_spinor(mom[3], mt, hel)
             else:
-                A = load(a[0], _pext(var, sub[0]))
-                B = load(a[1], _pext(var, sub[1]))
-                kA, kB = kof(a[0]), kof(a[1])
+                A = load(w1, var)
+                B = load(w2, var)
+                kA, kB = K[(w0 >> 16) & 0xFF], K[(w0 >> 24) & 0xFF]
                 if op == 3:
                     r = (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A) / ir.mdot(kout, kout)
                 elif op == 4:
-                    Z = load(a[2], _pext(var, sub[2]))
+                    Z = load(w3, var)
                     r = (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A) / ir.mdot(kout, kout)
                 elif op == 5:
                     q = -kout
@@ -80,7 +70,7 @@ def evaluate(T, mom, mt, wt):
                 elif op == 11:
                     r = G * (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A)
                 elif op == 12:
-                    Z = load(a[2], _pext(var, sub[2]))
+                    Z = load(w3, var)
                     r = G * (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A)
                 else:
                     raise ValueError(op)
@@ -91,10 +81,8 @@ def evaluate(T, mom, mt, wt):
     for it in T["p1_items"]:
         o, var = int(it) >> 8, int(it) & 0xFF
         off, info, t0, nt = (int(x) for x in obj[o])
-        nv = 1 << (info & 0xFF)
         val = run_terms(t0, nt, var, kout=K[info >> 8])
-        for c in range(4):
-            area[off + c * nv + var] = val[c]
+        area[off + 4 * var:off + 4 * var + 4] = val
     # phases 2 and 3, group by group
     nh = 1 << npar
     J = np.zeros((T["ncolor"], nh), dtype=complex)
@@ -102,12 +90,11 @@ def evaluate(T, mom, mt, wt):
     for g in T["group"]:
         x0, xi0, nxi, s0, ns = (int(x) for x in g[:5])
         for it in T["x_items"][xi0:xi0 + nxi]:
+            if int(it) < 0:                                   # padding of the last work unit
+                continue
             xk, var = int(it) >> 8, int(it) & 0xFF
             soff, lognv, t0, nt = (int(x) for x in T["xobj"][x0 + xk])
-            nv = 1 << lognv
-            val = run_terms(t0, nt, var)
-            for c in range(4):
-                stage[soff + c * nv + var] = val[c]
+            stage[soff + 4 * var:soff + 4 * var + 4] = run_terms(t0, nt, var)
         for sg in T["sigma"][s0:s0 + ns]:
             j, e0, ne = int(sg[0]), int(sg[1]), int(sg[2])
             for h in range(nh):
@@ -118,7 +105,7 @@ def evaluate(T, mom, mt, wt):
                     offy, nvy = w1 & 0xFFFF, w1 >> 16
                     vv = int(T["vtab"][row][h])
                     vx, vy = vv & 0xFF, vv >> 8
-                    d = sum(stage[offx + c * nvx + vx] * area[offy + c * nvy + vy] for c in range(4))
+                    d = sum(stage[offx + 4 * vx + c] * area[offy + 4 * vy + c] for c in range(4))
                     acc += sign * d
                 J[j][h] = acc
     return J
