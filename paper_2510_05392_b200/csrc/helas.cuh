@@ -49,6 +49,12 @@ template <typename T> MG_HD cx<T> cfma(cx<T> b, cx<T> c, cx<T> a)
     return mk<T>(a.re + b.re * c.re - b.im * c.im, a.im + b.re * c.im + b.im * c.re);
 }
 
+// a - b*c  (4 FMAs)
+template <typename T> MG_HD cx<T> cfms(cx<T> b, cx<T> c, cx<T> a)
+{
+    return mk<T>(a.re - b.re * c.re + b.im * c.im, a.im - b.re * c.im - b.im * c.re);
+}
+
 template <typename T>
 struct p4 {            // real four-vector (E, x, y, z)
     T e, x, y, z;
@@ -66,7 +72,7 @@ struct wf {            // wavefunction: 4 complex components
 // Minkowski products (no complex conjugation)
 template <typename T> MG_HD cx<T> dot(const wf<T>& a, const wf<T>& b)
 {
-    return a.c[0] * b.c[0] - a.c[1] * b.c[1] - a.c[2] * b.c[2] - a.c[3] * b.c[3];
+    return cfms(a.c[3], b.c[3], cfms(a.c[2], b.c[2], cfms(a.c[1], b.c[1], a.c[0] * b.c[0])));     // FMA chain
 }
 template <typename T> MG_HD cx<T> dot(p4<T> k, const wf<T>& a)
 {
@@ -178,18 +184,18 @@ template <typename T> MG_HD slashed<T> make_slashed(const wf<T>& v)
 // row spinor times Vslash
 template <typename T> MG_HD void row_slash(const wf<T>& a, const slashed<T>& s, wf<T>& r)
 {
-    r.c[0] = a.c[2] * s.vp + a.c[3] * s.vr;
-    r.c[1] = a.c[2] * s.vl + a.c[3] * s.vm;
-    r.c[2] = a.c[0] * s.vm - a.c[1] * s.vr;
-    r.c[3] = a.c[1] * s.vp - a.c[0] * s.vl;
+    r.c[0] = cfma(a.c[3], s.vr, a.c[2] * s.vp);
+    r.c[1] = cfma(a.c[3], s.vm, a.c[2] * s.vl);
+    r.c[2] = cfms(a.c[1], s.vr, a.c[0] * s.vm);
+    r.c[3] = cfms(a.c[0], s.vl, a.c[1] * s.vp);
 }
 // Vslash times column spinor
 template <typename T> MG_HD void slash_col(const slashed<T>& s, const wf<T>& b, wf<T>& w)
 {
-    w.c[0] = s.vm * b.c[2] - s.vl * b.c[3];
-    w.c[1] = s.vp * b.c[3] - s.vr * b.c[2];
-    w.c[2] = s.vp * b.c[0] + s.vl * b.c[1];
-    w.c[3] = s.vr * b.c[0] + s.vm * b.c[1];
+    w.c[0] = cfms(s.vl, b.c[3], s.vm * b.c[2]);
+    w.c[1] = cfms(s.vr, b.c[2], s.vp * b.c[3]);
+    w.c[2] = cfma(s.vl, b.c[1], s.vp * b.c[0]);
+    w.c[3] = cfma(s.vm, b.c[1], s.vr * b.c[0]);
 }
 
 // FFV1_0: amplitude  psibar Vslash psi
@@ -250,9 +256,31 @@ template <typename T> MG_HD void ffv_p(const wf<T>& a, const wf<T>& b, T invk2, 
     out.c[3] = invk2 * (t02 - t13 - t20 + t31);
 }
 
+// psibar gamma^mu psi without the propagator factor (raw vertex), FMA chains
+template <typename T> MG_HD void ffv_p_raw(const wf<T>& a, const wf<T>& b, wf<T>& out)
+{
+    const cx<T> u = cfma(a.c[3], b.c[1], a.c[0] * b.c[2]);      // t02 + t31
+    const cx<T> v = cfma(a.c[2], b.c[0], a.c[1] * b.c[3]);      // t13 + t20
+    out.c[0] = u + v;
+    out.c[1] = cfms(a.c[3], b.c[0], cfms(a.c[2], b.c[1], cfma(a.c[1], b.c[2], a.c[0] * b.c[3])));            // t03 + t12 - t21 - t30
+    out.c[2] = times_i(cfms(a.c[3], b.c[0], cfms(a.c[0], b.c[3], cfma(a.c[2], b.c[1], a.c[1] * b.c[2]))));   // i (t12 + t21 - t03 - t30)
+    out.c[3] = u - v;
+}
+
 // VVV1P0_1-like: off-shell gluon from two gluon currents, all momenta incoming:
 //   J = [ (A.B)(kA-kB) + ((2kB+kA).A) B - ((2kA+kB).B) A ] / K^2,  K = kA + kB
 template <typename T> MG_HD void v3_off(const wf<T>& A, p4<T> kA, const wf<T>& B, p4<T> kB, T invk2, wf<T>& out)
+{
+    const cx<T> ab = invk2 * dot(A, B);                 // 1/K^2 folded into the three scalar factors
+    p4<T> ea = { T(2) * kB.e + kA.e, T(2) * kB.x + kA.x, T(2) * kB.y + kA.y, T(2) * kB.z + kA.z };
+    p4<T> eb = { T(2) * kA.e + kB.e, T(2) * kA.x + kB.x, T(2) * kA.y + kB.y, T(2) * kA.z + kB.z };
+    const cx<T> xa = invk2 * dot(ea, A), xb = invk2 * dot(eb, B);
+    const p4<T> d = kA - kB;
+    const T dd[4] = { d.e, d.x, d.y, d.z };
+    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(xb, A.c[mu], cfma(xa, B.c[mu], dd[mu] * ab));
+}
+// the same without the propagator factor (raw vertex)
+template <typename T> MG_HD void v3_raw(const wf<T>& A, p4<T> kA, const wf<T>& B, p4<T> kB, wf<T>& out)
 {
     const cx<T> ab = dot(A, B);
     p4<T> ea = { T(2) * kB.e + kA.e, T(2) * kB.x + kA.x, T(2) * kB.y + kA.y, T(2) * kB.z + kA.z };
@@ -260,20 +288,20 @@ template <typename T> MG_HD void v3_off(const wf<T>& A, p4<T> kA, const wf<T>& B
     const cx<T> xa = dot(ea, A), xb = dot(eb, B);
     const p4<T> d = kA - kB;
     const T dd[4] = { d.e, d.x, d.y, d.z };
-    for (int mu = 0; mu < 4; mu++) {
-        cx<T> t = dd[mu] * ab;
-        t = cfma(xa, B.c[mu], t);
-        t = t - xb * A.c[mu];
-        out.c[mu] = invk2 * t;
-    }
+    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(xb, A.c[mu], cfma(xa, B.c[mu], dd[mu] * ab));
 }
 
 // VVVV1/3/4P0_1-like: one colour/Lorentz term of the four-gluon vertex, (x y | z out):
 //   J = [ (X.Z) Y - (Y.Z) X ] / K^2
 template <typename T> MG_HD void v4_off(const wf<T>& X, const wf<T>& Y, const wf<T>& Z, T invk2, wf<T>& out)
 {
+    const cx<T> xz = invk2 * dot(X, Z), yz = invk2 * dot(Y, Z);
+    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(yz, X.c[mu], xz * Y.c[mu]);
+}
+template <typename T> MG_HD void v4_raw(const wf<T>& X, const wf<T>& Y, const wf<T>& Z, wf<T>& out)
+{
     const cx<T> xz = dot(X, Z), yz = dot(Y, Z);
-    for (int mu = 0; mu < 4; mu++) out.c[mu] = invk2 * (xz * Y.c[mu] - yz * X.c[mu]);
+    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(yz, X.c[mu], xz * Y.c[mu]);
 }
 
 // VVV1_0: (A.B)((kA-kB).C) + (B.C)((kB-kC).A) + (C.A)((kC-kA).B), all momenta incoming

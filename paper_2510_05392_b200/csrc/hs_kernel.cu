@@ -94,12 +94,12 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
             load_arg(area, w.z, var, B);
             switch (op) {
                 case 3: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0 / m2(load_k(Ks, ls_out)), r); break;
-                case 11: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0, r); lower(r); break;
+                case 11: v3_raw(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), r); lower(r); break;
                 case 4: case 12: {
                     wf<double> Z;
                     load_arg(area, w.w, var, Z);
-                    v4_off(A, B, Z, op == 4 ? 1.0 / m2(load_k(Ks, ls_out)) : 1.0, r);
-                    if (op == 12) lower(r);
+                    if (op == 4) v4_off(A, B, Z, 1.0 / m2(load_k(Ks, ls_out)), r);
+                    else { v4_raw(A, B, Z, r); lower(r); }
                     break;
                 }
                 case 5: { const p4<double> K = load_k(Ks, ls_out); ffv_l(A, B, -K, mt, inv_prop(m2(K), mt, wt), r); break; }
@@ -107,7 +107,7 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
                 case 7: ffv_p(A, B, 1.0 / m2(load_k(Ks, ls_out)), r); break;
                 case 8: row_slash(A, make_slashed(B), r); break;
                 case 9: slash_col(make_slashed(A), B, r); break;
-                default: ffv_p(A, B, 1.0, r); lower(r); break;       // 10: x_bil
+                default: ffv_p_raw(A, B, r); lower(r); break;       // 10: x_bil
             }
         }
         const double sg = neg ? -1.0 : 1.0;
@@ -140,6 +140,45 @@ __device__ __forceinline__ int acc_swizzle(int h)
 // helicity.  Entries of one colour flow have different leg partitions, so the fragments are added into a per-warp
 // accumulator in shared memory indexed by the helicity combination (swizzled; tables hdep) and the finished jamp is
 // written once, coalesced over helicities.
+// one dot entry, fragment shape fixed at compile time: MT m-tiles of 8 X variants, NT n-tiles of 4 Y variants
+template <int MT, int NT>
+__device__ __forceinline__ void p3_entry(const double2* __restrict__ X, const double2* __restrict__ Y,
+                                         const unsigned char* __restrict__ hd, double2* __restrict__ acc, double sgn, bool first,
+                                         int r, int c)
+{
+    double2 xa[MT];
+    double b0[NT], b1[NT];
+    int hx[MT], hy[NT];
+#pragma unroll
+    for (int mt = 0; mt < MT; mt++) { xa[mt] = X[slot(8 * mt + r, c)]; hx[mt] = hd[8 * mt + r]; }
+#pragma unroll
+    for (int nt = 0; nt < NT; nt++) {
+        const double2 y = Y[slot(4 * nt + (r >> 1), c)];
+        b0[nt] = (r & 1) ? y.y : y.x;            // k-step 0: A = Re X
+        b1[nt] = (r & 1) ? y.x : -y.y;           // k-step 1: A = Im X
+        hy[nt] = hd[32 + 4 * nt + c];
+    }
+    double c0[MT][NT], c1[MT][NT];
+#pragma unroll
+    for (int mt = 0; mt < MT; mt++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) { c0[mt][nt] = 0.0; c1[mt][nt] = 0.0; dmma884(c0[mt][nt], c1[mt][nt], xa[mt].x, b0[nt]); }
+#pragma unroll
+    for (int mt = 0; mt < MT; mt++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) dmma884(c0[mt][nt], c1[mt][nt], xa[mt].y, b1[nt]);
+#pragma unroll
+    for (int mt = 0; mt < MT; mt++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+            const int idx = hx[mt] ^ hy[nt];
+            double2 v = make_double2(0.0, 0.0);
+            if (!first) v = acc[idx];
+            v.x = fma(sgn, c0[mt][nt], v.x); v.y = fma(sgn, c1[mt][nt], v.y);
+            acc[idx] = v;
+        }
+}
+
 template <typename T2>
 __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, const double2* __restrict__ area,
                                             const double2* __restrict__ stage, double2* __restrict__ accs, int e, const int4 g0,
@@ -155,43 +194,20 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
         if (s >= g1.x) break;
         double2* __restrict__ acc = accs + (s << d.npar);
         const int4 sg = __ldg(d.sigma + g0.w + s);
+        int4 en = __ldg(d.entry + sg.y);
         for (int k = 0; k < sg.z; k++) {
-            const int4 en = __ldg(d.entry + sg.y + k);
+            const int4 enn = __ldg(d.entry + sg.y + (k + 1 < sg.z ? k + 1 : k));       // next entry, fetched early
             const int nvx = en.x >> 16, nvy = en.y >> 16;
             const double2* __restrict__ X = stage + (en.x & 0xFFFF);
             const double2* __restrict__ Y = area + (en.y & 0xFFFF);
             const unsigned char* __restrict__ hd = d.hdep + en.z * 40;
-            const int MT = nvx >> 3, NT = nvy >> 2;          // (MT, NT) in {(1,2), (2,1), (2,2), (4,1)}
-            double2 xa[4], yb[2];
-            double b0[2], b1[2];
-#pragma unroll
-            for (int mt = 0; mt < 4; mt++) if (mt < MT) xa[mt] = X[slot(8 * mt + r, c)];
-#pragma unroll
-            for (int nt = 0; nt < 2; nt++)
-                if (nt < NT) {
-                    yb[nt] = Y[slot(4 * nt + (r >> 1), c)];
-                    b0[nt] = (r & 1) ? yb[nt].y : yb[nt].x;          // k-step 0: A = Re X
-                    b1[nt] = (r & 1) ? yb[nt].x : -yb[nt].y;         // k-step 1: A = Im X
-                }
             const double sgn = (double)en.w;
-#pragma unroll
-            for (int t = 0; t < 4; t++) {
-                if (t < MT * NT) {
-                    const int mt = NT == 2 ? (t >> 1) : t, nt = NT == 2 ? (t & 1) : 0;
-                    const double2 xv = NT == 2 ? xa[t >> 1] : xa[t];
-                    const double p0 = (NT == 2 && (t & 1)) ? b0[1] : b0[0];
-                    const double p1 = (NT == 2 && (t & 1)) ? b1[1] : b1[0];
-                    double c0 = 0.0, c1 = 0.0;
-                    dmma884(c0, c1, xv.x, p0);
-                    dmma884(c0, c1, xv.y, p1);
-                    const int idx = hd[8 * mt + r] ^ hd[32 + 4 * nt + c];
-                    double2 v = make_double2(0.0, 0.0);
-                    if (k > 0) v = acc[idx];
-                    v.x = fma(sgn, c0, v.x); v.y = fma(sgn, c1, v.y);
-                    acc[idx] = v;
-                }
-            }
+            if (nvx == 32) p3_entry<4, 1>(X, Y, hd, acc, sgn, k == 0, r, c);
+            else if (nvx == 16 && nvy == 8) p3_entry<2, 2>(X, Y, hd, acc, sgn, k == 0, r, c);
+            else if (nvx == 16) p3_entry<2, 1>(X, Y, hd, acc, sgn, k == 0, r, c);
+            else p3_entry<1, 2>(X, Y, hd, acc, sgn, k == 0, r, c);
             __syncwarp();
+            en = enn;
         }
         // the finished jamp of this colour flow, all helicity combinations
         T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
