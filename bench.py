@@ -245,8 +245,9 @@ def main():
                       "process": process, "precision": args.precision, "nevt_per_gpu": nevt, "good_helicities": r["ngood"],
                       "diagrams": "helicity-shared (CTA = event, thread = helicity)" if shared else "thread = (event, helicity)",
                       "schedule": "helicity streams" if args.schedule else ("helicity = thread index" if shared else "helicity = grid.y"),
-                      "color_sum": ("tensor" if (shared and args.precision in ("fp64", "d")) or proc.get_option("color_sum") == 1
-                                    else ("ALU kernel" if shared else "fused ALU")),
+                      "color_sum": (("DMMA (mma.sync f64), Cholesky form" if args.precision in ("fp64", "d") else
+                                     ("ALU kernel" if proc.get_option("hs_color_alu") else "tcgen05 kind::tf32, split, Cholesky form"))
+                                    if shared else ("tensor" if proc.get_option("color_sum") == 1 else "fused ALU")),
                       "jamp_chunk_mib": proc.get_option("jamp_chunk_mib"),
                       "l2": "256 MiB device memset between timed steps (outside the per-step event pairs)"},
            "gpu_launches": r["launches"], "stage_ms": {"diagrams": r["stage_ms"][0], "color_sum": r["stage_ms"][1],

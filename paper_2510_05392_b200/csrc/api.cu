@@ -30,7 +30,7 @@ struct mg_process {
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
-    int diagrams = MG_DIAG_THREAD, hs_split = 1, hs_phase3 = 0;
+    int diagrams = MG_DIAG_THREAD, hs_split = 1, hs_phase3 = 0, hs_color_alu = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 1L << 30;
@@ -256,6 +256,8 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         if (value != 0 && value != 1) return fail(p, MG_EINVAL, "bad hs_phase3");
         if (value == 1 && p->d->npar < 6) return fail(p, MG_EINVAL, "hs_phase3 = 1 needs >= 6 external particles");
         p->hs_phase3 = value;
+    } else if (!strcmp(key, "hs_color_alu")) {
+        p->hs_color_alu = value != 0;
     } else if (!strcmp(key, "timing")) {
         p->timing = value != 0;
     } else if (!strcmp(key, "jamp_chunk_mib")) {
@@ -274,6 +276,7 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "diagrams")) *value = p->diagrams;
     else if (!strcmp(key, "hs_split")) *value = p->hs_split;
     else if (!strcmp(key, "hs_phase3")) *value = p->hs_phase3;
+    else if (!strcmp(key, "hs_color_alu")) *value = p->hs_color_alu;
     else if (!strcmp(key, "timing")) *value = p->timing;
     else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
     else return MG_EINVAL;
@@ -469,10 +472,11 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             RowMap map;
             map.rows_valid = rows; map.hel_minor = nhel; map.evt_stride = nevt; map.e0 = e0; map.norm = make_norm(p);
             cudaError_t ce_;
-            if (p->color_sum == MG_CS_TENSOR || p->precision == MG_FP64)
-                ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
-            else
+            // tensor-core contraction (DMMA in MG_FP64, tcgen05 kind::tf32 otherwise) unless the ALU kernel is asked for
+            if (p->hs_color_alu && p->precision != MG_FP64)
                 ce_ = color_sum_alu(false, p->d->ncolor, p->d_cmat, d_j, a.rows, d_meh, st, &map);
+            else
+                ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("colour sum: ") + cudaGetErrorString(ce_));
             MARK(1);
         }
