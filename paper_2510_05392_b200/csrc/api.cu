@@ -162,6 +162,7 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
         if (d->ngluon >= 4) p->diagrams = MG_DIAG_SHARED;     // measured default, see DESIGN.md
         if (d->npar >= 7) p->hs_phase3 = 1;                   // jamp dot products on the FP64 tensor path (DMMA): measured faster for 2->5 only
+        if (d->ncolor < 120) p->hs_color_alu = 1;             // 24 x 24: the fp32 ALU kernel beats the 128-row tcgen05 tiles (measured)
         if (2 * d->ncomb <= 256) p->hs_split = 2;             // 16 instead of 8 warps per SM: measured +30% (profiles/r1_hs_kernel.md)
     }
     *out = p;
