@@ -10,6 +10,8 @@
 // with rows ordered (event, helicity).
 #include <stdint.h>
 
+#include <vector>
+
 #include "helas.cuh"
 #include "hs_kernel.cuh"
 
@@ -19,6 +21,7 @@ struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask; const int4* group;
     const int4* xobj; const int* x_items; const int4* sigma; const int4* entry; const unsigned short* vtab;
     const unsigned char* hdep;
+    const uint2* argtab; const int* ubase;       // phase-2 argument table and its per-unit base (built in hs_create)
     int npar, ncolor, ngroups, obj_area, stage_area, nlegsets;
     int nw3;               // jamp accumulators = colour flows per group (phase 3 on the FP64 tensor path); 0 = scalar phase 3
     int p1_level[4];
@@ -30,24 +33,38 @@ __device__ __forceinline__ int sub_variant(int var, int code)
     return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2);
 }
 
-// Shared-memory layout of an object: [variant][component], 16 bytes per complex number, the component index
-// XOR-swizzled with bits 1-2 of the variant: slot(var, c) = 4 var + (c ^ ((var >> 1) & 3)).  Eight consecutive
-// variants of one component (phases 1, 2: lane <-> variant) and the 2 variants x 4 components of a DMMA fragment
-// quarter-warp (phase 3) both fall into eight different 16-byte bank groups.
-__device__ __forceinline__ int slot(int var, int c) { return 4 * var + (c ^ ((var >> 1) & 3)); }
+// Shared-memory layout of an area: 64-byte blocks, block b = (object offset / 4 + variant) holds the 4 components of one
+// variant as 16-byte complex numbers, the component index XOR-swizzled with bits 1-2 of the BLOCK index:
+//     slot(off, var, c) = 4 b + (c ^ ((b >> 1) & 3)),   b = off / 4 + var      (offsets are multiples of 8 slots)
+// Eight consecutive variants of one component (phases 1, 2: lane <-> variant) and the 2 variants x 4 components of a
+// DMMA fragment quarter-warp (phase 3) both fall into eight different 16-byte bank groups.  Using the block index
+// (not the variant) lets a precomputed block number address an argument without knowing its object (argument table).
+__device__ __forceinline__ int slot(int off, int var, int c)
+{
+    const int b = (off >> 2) + var;
+    return 4 * b + (c ^ ((b >> 1) & 3));
+}
+
+__device__ __forceinline__ void load_blk(const double2* __restrict__ area, int b, wf<double>& w)
+{
+    const char* p = reinterpret_cast<const char*>(area) + b * 64;
+    const int sw = (b & 6) << 3;
+#pragma unroll
+    for (int c = 0; c < 4; c++) {
+        const double2 v = *reinterpret_cast<const double2*>(p + ((c * 16) ^ sw));
+        w.c[c].re = v.x; w.c[c].im = v.y;
+    }
+}
 
 __device__ __forceinline__ void load_obj(const double2* __restrict__ area, int off, int var, wf<double>& w)
 {
-    const double2* p = area + off;
-#pragma unroll
-    for (int c = 0; c < 4; c++) { const double2 v = p[slot(var, c)]; w.c[c].re = v.x; w.c[c].im = v.y; }
+    load_blk(area, (off >> 2) + var, w);
 }
 
 __device__ __forceinline__ void store_obj(double2* __restrict__ area, int off, int var, const wf<double>& w)
 {
-    double2* p = area + off;
 #pragma unroll
-    for (int c = 0; c < 4; c++) p[slot(var, c)] = make_double2(w.c[c].re, w.c[c].im);
+    for (int c = 0; c < 4; c++) area[slot(off, var, c)] = make_double2(w.c[c].re, w.c[c].im);
 }
 
 __device__ __forceinline__ p4<double> load_k(const double* __restrict__ Ks, int ls)
@@ -71,15 +88,23 @@ __device__ __forceinline__ void load_arg(const double2* __restrict__ area, int w
 // Sum of the terms [t0, t0 + nt) for helicity variant `var` of an object whose leg set has total momentum K(ls_out).
 // Inlined at its two call sites (phases 1 and 2) so that the accumulator stays in registers; the next term's table
 // word is fetched while the current one is evaluated.
+// PRE (phase 2): the block numbers of the three arguments of (this lane's item, term t) come precomputed from the
+// argument table `at` (entry t * 32; built on the host in hs_create), which removes the per-lane variant gather.
+template <bool PRE>
 __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restrict__ area, const double* __restrict__ Ks,
                                           const double* __restrict__ pm, int t0, int nt, int var, int ls_out, double mt,
-                                          double wt, wf<double>& acc)
+                                          double wt, wf<double>& acc, const uint2* __restrict__ at = nullptr)
 {
 #pragma unroll
     for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
     int4 w = __ldg(d.term + t0);
+    uint2 aw = make_uint2(0u, 0u);
+    if (PRE) aw = __ldg(at);
     for (int t = 0; t < nt; t++) {
-        const int4 wn = __ldg(d.term + t0 + (t + 1 < nt ? t + 1 : t));
+        const int tn = t + 1 < nt ? t + 1 : t;
+        const int4 wn = __ldg(d.term + t0 + tn);
+        uint2 awn = make_uint2(0u, 0u);
+        if (PRE) awn = __ldg(at + 32 * tn);
         const int op = w.x & 0xFF, neg = (w.x >> 8) & 1;
         wf<double> r;
         if (op <= 2) {
@@ -90,14 +115,15 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
             else ext_v(p, mt, hel, r);
         } else {
             wf<double> A, B;
-            load_arg(area, w.y, var, A);
-            load_arg(area, w.z, var, B);
+            if (PRE) { load_blk(area, aw.x & 0xFFFF, A); load_blk(area, aw.x >> 16, B); }
+            else { load_arg(area, w.y, var, A); load_arg(area, w.z, var, B); }
             switch (op) {
                 case 3: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0 / m2(load_k(Ks, ls_out)), r); break;
                 case 11: v3_raw(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), r); lower(r); break;
                 case 4: case 12: {
                     wf<double> Z;
-                    load_arg(area, w.w, var, Z);
+                    if (PRE) load_blk(area, aw.y, Z);
+                    else load_arg(area, w.w, var, Z);
                     if (op == 4) v4_off(A, B, Z, 1.0 / m2(load_k(Ks, ls_out)), r);
                     else { v4_raw(A, B, Z, r); lower(r); }
                     break;
@@ -114,6 +140,7 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
 #pragma unroll
         for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
         w = wn;
+        aw = awn;
     }
 }
 
@@ -142,7 +169,7 @@ __device__ __forceinline__ int acc_swizzle(int h)
 // written once, coalesced over helicities.
 // one dot entry, fragment shape fixed at compile time: MT m-tiles of 8 X variants, NT n-tiles of 4 Y variants
 template <int MT, int NT>
-__device__ __forceinline__ void p3_entry(const double2* __restrict__ X, const double2* __restrict__ Y,
+__device__ __forceinline__ void p3_entry(const double2* __restrict__ X, int xoff, const double2* __restrict__ Y, int yoff,
                                          const unsigned char* __restrict__ hd, double2* __restrict__ acc, double sgn, bool first,
                                          int r, int c)
 {
@@ -150,10 +177,10 @@ __device__ __forceinline__ void p3_entry(const double2* __restrict__ X, const do
     double b0[NT], b1[NT];
     int hx[MT], hy[NT];
 #pragma unroll
-    for (int mt = 0; mt < MT; mt++) { xa[mt] = X[slot(8 * mt + r, c)]; hx[mt] = hd[8 * mt + r]; }
+    for (int mt = 0; mt < MT; mt++) { xa[mt] = X[slot(xoff, 8 * mt + r, c)]; hx[mt] = hd[8 * mt + r]; }
 #pragma unroll
     for (int nt = 0; nt < NT; nt++) {
-        const double2 y = Y[slot(4 * nt + (r >> 1), c)];
+        const double2 y = Y[slot(yoff, 4 * nt + (r >> 1), c)];
         b0[nt] = (r & 1) ? y.y : y.x;            // k-step 0: A = Re X
         b1[nt] = (r & 1) ? y.x : -y.y;           // k-step 1: A = Im X
         hy[nt] = hd[32 + 4 * nt + c];
@@ -198,14 +225,13 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
         for (int k = 0; k < sg.z; k++) {
             const int4 enn = __ldg(d.entry + sg.y + (k + 1 < sg.z ? k + 1 : k));       // next entry, fetched early
             const int nvx = en.x >> 16, nvy = en.y >> 16;
-            const double2* __restrict__ X = stage + (en.x & 0xFFFF);
-            const double2* __restrict__ Y = area + (en.y & 0xFFFF);
+            const int xoff = en.x & 0xFFFF, yoff = en.y & 0xFFFF;
             const unsigned char* __restrict__ hd = d.hdep + en.z * 40;
             const double sgn = (double)en.w;
-            if (nvx == 32) p3_entry<4, 1>(X, Y, hd, acc, sgn, k == 0, r, c);
-            else if (nvx == 16 && nvy == 8) p3_entry<2, 2>(X, Y, hd, acc, sgn, k == 0, r, c);
-            else if (nvx == 16) p3_entry<2, 1>(X, Y, hd, acc, sgn, k == 0, r, c);
-            else p3_entry<1, 2>(X, Y, hd, acc, sgn, k == 0, r, c);
+            if (nvx == 32) p3_entry<4, 1>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
+            else if (nvx == 16 && nvy == 8) p3_entry<2, 2>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
+            else if (nvx == 16) p3_entry<2, 1>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
+            else p3_entry<1, 2>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
             __syncwarp();
             en = enn;
         }
@@ -263,7 +289,7 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                 const int4 o = __ldg(d.obj + (it >> 8));
                 const int var = it & 0xFF;
                 wf<double> acc;
-                run_terms(d, area, Ks, pm, o.z, o.w, var, o.y >> 8, a.mt, a.wt, acc);
+                run_terms<false>(d, area, Ks, pm, o.z, o.w, var, o.y >> 8, a.mt, a.wt, acc);
                 store_obj(area, o.x, var, acc);
             }
             __syncthreads();
@@ -285,7 +311,8 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                         const int4 x = __ldg(d.xobj + g0.x + (it >> 8));
                         const int var = it & 0xFF;
                         wf<double> acc;
-                        run_terms(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc);
+                        run_terms<true>(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc,
+                                        d.argtab + __ldg(d.ubase + (g0.y >> 5) + u) + lane);
                         store_obj(stage, x.x, var, acc);
                     }
                     __syncwarp();
@@ -305,12 +332,11 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                         const int4 en = __ldg(d.entry + sg.y + k);
                         const int vv = __ldg(d.vtab + en.z * nh + h);
                         const int vx = vv & 0xFF, vy = vv >> 8;
-                        const double2* __restrict__ X = stage + (en.x & 0xFFFF);
-                        const double2* __restrict__ Y = area + (en.y & 0xFFFF);
+                        const int xoff = en.x & 0xFFFF, yoff = en.y & 0xFFFF;
                         double tr = 0.0, ti = 0.0;
 #pragma unroll
                         for (int c = 0; c < 4; c++) {
-                            const double2 x = X[slot(vx, c)], y = Y[slot(vy, c)];
+                            const double2 x = stage[slot(xoff, vx, c)], y = area[slot(yoff, vy, c)];
                             tr = fma(x.x, y.x, tr); tr = fma(-x.y, y.y, tr);
                             ti = fma(x.x, y.y, ti); ti = fma(x.y, y.x, ti);
                         }
@@ -333,6 +359,8 @@ struct HsContext {
     const HsTables* t = nullptr;
     HsDev d;
     void* blob = nullptr;
+    void* argtab = nullptr;
+    void* ubase = nullptr;
     size_t smem = 0;
     int sms = 148;
     int max_sigma = 0;
@@ -374,6 +402,50 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     d.x_items = (const int*)(b + parts[6].off); d.sigma = (const int4*)(b + parts[7].off);
     d.entry = (const int4*)(b + parts[8].off); d.vtab = (const unsigned short*)(b + parts[9].off);
     d.hdep = (const unsigned char*)(b + parts[10].off); d.nw3 = 0;
+    // phase-2 argument table: for every work unit (32 items), term k and lane the shared-memory block numbers of the
+    // term's arguments, [unit][k][lane] (coalesced); block = offset / 4 + variant of the argument
+    {
+        std::vector<int> ubase;
+        std::vector<uint2> tab;
+        auto subv = [](int var, int code) {
+            return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2);
+        };
+        for (int g = 0; g < t->ngroups; g++) {
+            const int* G = t->group + 8 * g;
+            for (int u = 0; u < G[2] / 32; u++) {
+                int maxnt = 0;
+                for (int l = 0; l < 32; l++) {
+                    const int it = t->x_items[G[1] + 32 * u + l];
+                    if (it >= 0 && t->xobj[4 * (G[0] + (it >> 8)) + 3] > maxnt) maxnt = t->xobj[4 * (G[0] + (it >> 8)) + 3];
+                }
+                ubase.push_back((int)tab.size());
+                tab.resize(tab.size() + (size_t)32 * maxnt, make_uint2(0u, 0u));
+                for (int l = 0; l < 32; l++) {
+                    const int it = t->x_items[G[1] + 32 * u + l];
+                    if (it < 0) continue;
+                    const int* X = t->xobj + 4 * (G[0] + (it >> 8));
+                    const int var = it & 0xFF;
+                    for (int k = 0; k < X[3]; k++) {
+                        const int* w = t->term + 4 * (X[2] + k);
+                        unsigned blk[3] = { 0, 0, 0 };
+                        for (int j = 0; j < 3; j++) {
+                            const unsigned word = (unsigned)w[1 + j];
+                            blk[j] = ((word & 0xFFFF) >> 2) + subv(var, (word >> 16) & 0x1FF);
+                        }
+                        tab[ubase.back() + 32 * k + l] = make_uint2(blk[0] | (blk[1] << 16), blk[2]);
+                    }
+                }
+            }
+        }
+        if (tab.empty()) tab.push_back(make_uint2(0u, 0u));
+        if (ubase.empty()) ubase.push_back(0);
+        e = cudaMalloc(&c->argtab, tab.size() * sizeof(uint2));
+        if (e == cudaSuccess) e = cudaMalloc(&c->ubase, ubase.size() * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemcpy(c->argtab, tab.data(), tab.size() * sizeof(uint2), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(c->ubase, ubase.data(), ubase.size() * sizeof(int), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { cudaFree(c->argtab); cudaFree(c->ubase); cudaFree(c->blob); delete c; return e; }
+        d.argtab = (const uint2*)c->argtab; d.ubase = (const int*)c->ubase;
+    }
     d.npar = t->npar; d.ncolor = t->ncolor; d.ngroups = t->ngroups; d.obj_area = t->obj_area; d.stage_area = t->stage_area;
     d.nlegsets = t->nlegsets;
     for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
@@ -394,7 +466,7 @@ cudaError_t hs_create(int ngluon, HsContext** out)
 void hs_destroy(HsContext* c)
 {
     if (!c) return;
-    cudaFree(c->blob);
+    cudaFree(c->blob); cudaFree(c->argtab); cudaFree(c->ubase);
     delete c;
 }
 
