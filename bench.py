@@ -91,7 +91,8 @@ def oracle_rate(process, nevt_sample, seed=1):
     return nevt_sample / dt, os.cpu_count(), dt
 
 
-ORACLE_SAMPLE = {"epem_mupmum": 16384, "gg_ttx": 16384, "gg_ttxg": 8192, "gg_ttxgg": 2048, "gg_ttxggg": 1024}
+# sized for about 10-30 s of oracle time on the 16 host cores of the GPU box (854 MEs/s measured for gg_ttxggg)
+ORACLE_SAMPLE = {"epem_mupmum": 16384, "gg_ttx": 65536, "gg_ttxg": 65536, "gg_ttxgg": 32768, "gg_ttxggg": 12288}
 
 
 def run_reference(args):

@@ -21,7 +21,8 @@ struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask; const int4* group;
     const int4* xobj; const int* x_items; const int4* sigma; const int4* entry; const unsigned short* vtab;
     const unsigned char* hdep;
-    const uint2* argtab; const int* ubase;       // phase-2 argument table and its per-unit base (built in hs_create)
+    const uint4* p3tab; int maxe;                // phase-3 stream: [colour flow][entry k < maxe][lane] records
+    const uint4* p2tab; int maxt;                // phase-2 stream: [unit][term k < maxt][lane] records (built in hs_create)
     int npar, ncolor, ngroups, obj_area, stage_area, nlegsets;
     int nw3;               // jamp accumulators = colour flows per group (phase 3 on the FP64 tensor path); 0 = scalar phase 3
     int p1_level[4];
@@ -144,6 +145,33 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
     }
 }
 
+// Phase-2 record of (work unit, term k, lane), built on the host from the tables (hs_create):
+//   x = block of argument A | block of argument B << 16      (shared-memory block = offset / 4 + variant)
+//   y = block of argument C | block of the item's own result in the staging area << 16
+//   z = opcode | negative << 8 | leg set of A << 16 | leg set of B << 24;  opcode 0xFF = this lane has no term k
+//   w = number of terms of the unit (largest over its lanes)
+// The address depends on the unit number only, so the next unit's first record is fetched while this one is evaluated.
+__device__ __forceinline__ void eval_x_term(const double2* __restrict__ area, const double* __restrict__ Ks, const uint4 e,
+                                            wf<double>& acc)
+{
+    const int op = e.z & 0xFF;
+    if (op == 0xFF) return;
+    wf<double> A, B, r;
+    load_blk(area, e.x & 0xFFFF, A);
+    load_blk(area, e.x >> 16, B);
+    switch (op) {
+        case 11: v3_raw(A, load_k(Ks, (e.z >> 16) & 0xFF), B, load_k(Ks, (e.z >> 24) & 0xFF), r); break;
+        case 12: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4_raw(A, B, Z, r); break; }
+        case 8: row_slash(A, make_slashed(B), r); break;
+        case 9: slash_col(make_slashed(A), B, r); break;
+        default: ffv_p_raw(A, B, r); break;                 // 10: x_bil
+    }
+    if (op >= 10) lower(r);
+    const double sg = ((e.z >> 8) & 1) ? -1.0 : 1.0;
+#pragma unroll
+    for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
+}
+
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
 {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -167,23 +195,28 @@ __device__ __forceinline__ int acc_swizzle(int h)
 // helicity.  Entries of one colour flow have different leg partitions, so the fragments are added into a per-warp
 // accumulator in shared memory indexed by the helicity combination (swizzled; tables hdep) and the finished jamp is
 // written once, coalesced over helicities.
+// Phase-3 record of (colour flow, entry k, lane), built on the host (hs_create):
+//   x = block of X variant (lane / 4) | block of Y variant (lane / 8) << 16     (m-tile mt adds 8, n-tile nt adds 4 blocks)
+//   y = accumulator index parts of the X variants 8 mt + lane / 4, one byte per m-tile (tables hdep)
+//   z = accumulator index parts of the Y variants 4 nt + lane % 4 (bytes 0, 1) | shape << 16 | negative << 18 |
+//       number of entries of the flow << 24;  shape 0: (MT, NT) = (4, 1), 1: (2, 2), 2: (2, 1), 3: (1, 2)
+//   w = jamp index of the flow
 // one dot entry, fragment shape fixed at compile time: MT m-tiles of 8 X variants, NT n-tiles of 4 Y variants
 template <int MT, int NT>
-__device__ __forceinline__ void p3_entry(const double2* __restrict__ X, int xoff, const double2* __restrict__ Y, int yoff,
-                                         const unsigned char* __restrict__ hd, double2* __restrict__ acc, double sgn, bool first,
-                                         int r, int c)
+__device__ __forceinline__ void p3_entry(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
+                                         double2* __restrict__ acc, bool first, int r, int c)
 {
     double2 xa[MT];
     double b0[NT], b1[NT];
-    int hx[MT], hy[NT];
+    const int xb = e.x & 0xFFFF, yb = e.x >> 16;
 #pragma unroll
-    for (int mt = 0; mt < MT; mt++) { xa[mt] = X[slot(xoff, 8 * mt + r, c)]; hx[mt] = hd[8 * mt + r]; }
+    for (int mt = 0; mt < MT; mt++) { const int b = xb + 8 * mt; xa[mt] = stage[4 * b + (c ^ ((b >> 1) & 3))]; }
 #pragma unroll
     for (int nt = 0; nt < NT; nt++) {
-        const double2 y = Y[slot(yoff, 4 * nt + (r >> 1), c)];
+        const int b = yb + 4 * nt;
+        const double2 y = area[4 * b + (c ^ ((b >> 1) & 3))];
         b0[nt] = (r & 1) ? y.y : y.x;            // k-step 0: A = Re X
         b1[nt] = (r & 1) ? y.x : -y.y;           // k-step 1: A = Im X
-        hy[nt] = hd[32 + 4 * nt + c];
     }
     double c0[MT][NT], c1[MT][NT];
 #pragma unroll
@@ -194,11 +227,12 @@ __device__ __forceinline__ void p3_entry(const double2* __restrict__ X, int xoff
     for (int mt = 0; mt < MT; mt++)
 #pragma unroll
         for (int nt = 0; nt < NT; nt++) dmma884(c0[mt][nt], c1[mt][nt], xa[mt].y, b1[nt]);
+    const double sgn = ((e.z >> 18) & 1) ? -1.0 : 1.0;
 #pragma unroll
     for (int mt = 0; mt < MT; mt++)
 #pragma unroll
         for (int nt = 0; nt < NT; nt++) {
-            const int idx = hx[mt] ^ hy[nt];
+            const int idx = ((e.y >> (8 * mt)) & 0xFF) ^ ((e.z >> (8 * nt)) & 0xFF);
             double2 v = make_double2(0.0, 0.0);
             if (!first) v = acc[idx];
             v.x = fma(sgn, c0[mt][nt], v.x); v.y = fma(sgn, c1[mt][nt], v.y);
@@ -213,25 +247,32 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
 {
     const int nh = 1 << d.npar;
     const int r = lane >> 2, c = lane & 3;
-    while (true) {
-        // colour flows of the group are handed to the warps dynamically; flow s owns accumulator s (g1.x <= nw3)
-        int s = 0;
-        if (lane == 0) s = atomicAdd(ctr, 1);
-        s = __shfl_sync(0xffffffffu, s, 0);
-        if (s >= g1.x) break;
+    const size_t sstride = (size_t)d.maxe * 32;
+    const uint4* __restrict__ tab = d.p3tab + (size_t)g0.w * sstride + lane;
+    // colour flows of the group are handed to the warps dynamically; flow s owns accumulator s (g1.x <= nw3)
+    int s = 0;
+    if (lane == 0) s = atomicAdd(ctr, 1);
+    s = __shfl_sync(0xffffffffu, s, 0);
+    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+    if (s < g1.x) cur = __ldg(tab + s * sstride);
+    while (s < g1.x) {
+        int sn = 0;                                         // next flow and its first record, fetched early
+        if (lane == 0) sn = atomicAdd(ctr, 1);
+        sn = __shfl_sync(0xffffffffu, sn, 0);
+        uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
+        if (sn < g1.x) nxt = __ldg(tab + sn * sstride);
         double2* __restrict__ acc = accs + (s << d.npar);
-        const int4 sg = __ldg(d.sigma + g0.w + s);
-        int4 en = __ldg(d.entry + sg.y);
-        for (int k = 0; k < sg.z; k++) {
-            const int4 enn = __ldg(d.entry + sg.y + (k + 1 < sg.z ? k + 1 : k));       // next entry, fetched early
-            const int nvx = en.x >> 16, nvy = en.y >> 16;
-            const int xoff = en.x & 0xFFFF, yoff = en.y & 0xFFFF;
-            const unsigned char* __restrict__ hd = d.hdep + en.z * 40;
-            const double sgn = (double)en.w;
-            if (nvx == 32) p3_entry<4, 1>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
-            else if (nvx == 16 && nvy == 8) p3_entry<2, 2>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
-            else if (nvx == 16) p3_entry<2, 1>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
-            else p3_entry<1, 2>(stage, xoff, area, yoff, hd, acc, sgn, k == 0, r, c);
+        const uint4* __restrict__ p = tab + s * sstride;
+        const int nent = (int)(cur.z >> 24), jamp = (int)cur.w;
+        uint4 en = cur;
+        for (int k = 0; k < nent; k++) {
+            const uint4 enn = __ldg(p + 32 * (k + 1 < nent ? k + 1 : k));
+            switch ((en.z >> 16) & 3) {
+                case 0: p3_entry<4, 1>(stage, area, en, acc, k == 0, r, c); break;
+                case 1: p3_entry<2, 2>(stage, area, en, acc, k == 0, r, c); break;
+                case 2: p3_entry<2, 1>(stage, area, en, acc, k == 0, r, c); break;
+                default: p3_entry<1, 2>(stage, area, en, acc, k == 0, r, c); break;
+            }
             __syncwarp();
             en = enn;
         }
@@ -242,11 +283,12 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
             if (pos >= 0) {
                 const double2 v = acc[acc_swizzle(h)];
                 const size_t row = (size_t)e * a.nrow_evt + pos;
-                out[(size_t)sg.x * a.rows + row] = T2(v.x);
-                out[(size_t)(d.ncolor + sg.x) * a.rows + row] = T2(v.y);
+                out[(size_t)jamp * a.rows + row] = T2(v.x);
+                out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
             }
         }
         __syncwarp();
+        s = sn; cur = nxt;
     }
 }
 
@@ -301,21 +343,37 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
             // shape are handed to the warps dynamically, most expensive first (gen/co_program.py)
             {
                 const int lane = tid & 31, nunits = g0.z >> 5;
-                while (true) {
-                    int u = 0;
-                    if (lane == 0) u = atomicAdd(&ctr[0], 1);
-                    u = __shfl_sync(0xffffffffu, u, 0);
-                    if (u >= nunits) break;
-                    const int it = __ldg(d.x_items + g0.y + 32 * u + lane);
-                    if (it >= 0) {
-                        const int4 x = __ldg(d.xobj + g0.x + (it >> 8));
-                        const int var = it & 0xFF;
-                        wf<double> acc;
-                        run_terms<true>(d, area, Ks, pm, x.z, x.w, var, 0, a.mt, a.wt, acc,
-                                        d.argtab + __ldg(d.ubase + (g0.y >> 5) + u) + lane);
-                        store_obj(stage, x.x, var, acc);
+                const size_t ustride = (size_t)d.maxt * 32;
+                const uint4* __restrict__ tab = d.p2tab + (size_t)(g0.y >> 5) * ustride + lane;
+                int u = 0;
+                if (lane == 0) u = atomicAdd(&ctr[0], 1);
+                u = __shfl_sync(0xffffffffu, u, 0);
+                uint4 cur = make_uint4(0u, 0u, 0xFFu, 0u);
+                if (u < nunits) cur = __ldg(tab + u * ustride);
+                while (u < nunits) {
+                    int un = 0;                                 // next unit and its first record, fetched early
+                    if (lane == 0) un = atomicAdd(&ctr[0], 1);
+                    un = __shfl_sync(0xffffffffu, un, 0);
+                    uint4 nxt = make_uint4(0u, 0u, 0xFFu, 0u);
+                    if (un < nunits) nxt = __ldg(tab + un * ustride);
+                    const uint4* __restrict__ p = tab + u * ustride;
+                    const int ntm = (int)cur.w;
+                    wf<double> acc;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
+                    uint4 en = cur;
+                    for (int k = 0; k < ntm; k++) {
+                        const uint4 enn = __ldg(p + 32 * (k + 1 < ntm ? k + 1 : k));
+                        eval_x_term(area, Ks, en, acc);
+                        en = enn;
                     }
-                    __syncwarp();
+                    if ((cur.z & 0xFF) != 0xFF) {
+                        const int bs = (int)(cur.y >> 16);
+                        const int sw = (bs >> 1) & 3;
+#pragma unroll
+                        for (int c = 0; c < 4; c++) stage[4 * bs + (c ^ sw)] = make_double2(acc.c[c].re, acc.c[c].im);
+                    }
+                    u = un; cur = nxt;
                 }
             }
             __syncthreads();
@@ -359,8 +417,8 @@ struct HsContext {
     const HsTables* t = nullptr;
     HsDev d;
     void* blob = nullptr;
-    void* argtab = nullptr;
-    void* ubase = nullptr;
+    void* p2tab = nullptr;
+    void* p3tab = nullptr;
     size_t smem = 0;
     int sms = 148;
     int max_sigma = 0;
@@ -402,29 +460,31 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     d.x_items = (const int*)(b + parts[6].off); d.sigma = (const int4*)(b + parts[7].off);
     d.entry = (const int4*)(b + parts[8].off); d.vtab = (const unsigned short*)(b + parts[9].off);
     d.hdep = (const unsigned char*)(b + parts[10].off); d.nw3 = 0;
-    // phase-2 argument table: for every work unit (32 items), term k and lane the shared-memory block numbers of the
-    // term's arguments, [unit][k][lane] (coalesced); block = offset / 4 + variant of the argument
+    // phase-2 stream: fixed-size records [unit][term k < maxt][lane] (see eval_x_term)
     {
-        std::vector<int> ubase;
-        std::vector<uint2> tab;
+        int maxt = 1;
+        for (int i = 0; i < t->nxobj; i++) if (t->xobj[4 * i + 3] > maxt) maxt = t->xobj[4 * i + 3];
         auto subv = [](int var, int code) {
             return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2);
         };
+        const size_t nunits = (size_t)t->nxitems / 32;
+        std::vector<uint4> tab(nunits * maxt * 32 + 1, make_uint4(0u, 0u, 0xFFu, 0u));
         for (int g = 0; g < t->ngroups; g++) {
             const int* G = t->group + 8 * g;
             for (int u = 0; u < G[2] / 32; u++) {
-                int maxnt = 0;
+                const size_t base = ((size_t)(G[1] / 32 + u) * maxt) * 32;
+                unsigned ntm = 0;
                 for (int l = 0; l < 32; l++) {
                     const int it = t->x_items[G[1] + 32 * u + l];
-                    if (it >= 0 && t->xobj[4 * (G[0] + (it >> 8)) + 3] > maxnt) maxnt = t->xobj[4 * (G[0] + (it >> 8)) + 3];
+                    if (it >= 0 && (unsigned)t->xobj[4 * (G[0] + (it >> 8)) + 3] > ntm) ntm = t->xobj[4 * (G[0] + (it >> 8)) + 3];
                 }
-                ubase.push_back((int)tab.size());
-                tab.resize(tab.size() + (size_t)32 * maxnt, make_uint2(0u, 0u));
                 for (int l = 0; l < 32; l++) {
                     const int it = t->x_items[G[1] + 32 * u + l];
+                    for (int k = 0; k < maxt; k++) tab[base + 32 * k + l].w = ntm;
                     if (it < 0) continue;
                     const int* X = t->xobj + 4 * (G[0] + (it >> 8));
                     const int var = it & 0xFF;
+                    const unsigned sblk = (unsigned)(X[0] >> 2) + var;
                     for (int k = 0; k < X[3]; k++) {
                         const int* w = t->term + 4 * (X[2] + k);
                         unsigned blk[3] = { 0, 0, 0 };
@@ -432,20 +492,54 @@ cudaError_t hs_create(int ngluon, HsContext** out)
                             const unsigned word = (unsigned)w[1 + j];
                             blk[j] = ((word & 0xFFFF) >> 2) + subv(var, (word >> 16) & 0x1FF);
                         }
-                        tab[ubase.back() + 32 * k + l] = make_uint2(blk[0] | (blk[1] << 16), blk[2]);
+                        uint4& r = tab[base + 32 * k + l];
+                        r.x = blk[0] | (blk[1] << 16); r.y = blk[2] | (sblk << 16); r.z = (unsigned)w[0];
                     }
+                    tab[base + l].y |= sblk << 16;          // the store block is read from record 0
                 }
             }
         }
-        if (tab.empty()) tab.push_back(make_uint2(0u, 0u));
-        if (ubase.empty()) ubase.push_back(0);
-        e = cudaMalloc(&c->argtab, tab.size() * sizeof(uint2));
-        if (e == cudaSuccess) e = cudaMalloc(&c->ubase, ubase.size() * sizeof(int));
-        if (e == cudaSuccess) e = cudaMemcpy(c->argtab, tab.data(), tab.size() * sizeof(uint2), cudaMemcpyHostToDevice);
-        if (e == cudaSuccess) e = cudaMemcpy(c->ubase, ubase.data(), ubase.size() * sizeof(int), cudaMemcpyHostToDevice);
-        if (e != cudaSuccess) { cudaFree(c->argtab); cudaFree(c->ubase); cudaFree(c->blob); delete c; return e; }
-        d.argtab = (const uint2*)c->argtab; d.ubase = (const int*)c->ubase;
+        e = cudaMalloc(&c->p2tab, tab.size() * sizeof(uint4));
+        if (e == cudaSuccess) e = cudaMemcpy(c->p2tab, tab.data(), tab.size() * sizeof(uint4), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { cudaFree(c->p2tab); cudaFree(c->blob); delete c; return e; }
+        d.p2tab = (const uint4*)c->p2tab; d.maxt = maxt;
     }
+    // phase-3 stream (FP64 tensor path): fixed-size records [colour flow][entry k < maxe][lane] (see p3_entry)
+    if (t->npar >= 6) {
+        int maxe = 1;
+        for (int i = 0; i < t->nsigma; i++) if (t->sigma[4 * i + 2] > maxe) maxe = t->sigma[4 * i + 2];
+        std::vector<uint4> tab((size_t)t->nsigma * maxe * 32 + 1, make_uint4(0u, 0u, 0u, 0u));
+        for (int sgi = 0; sgi < t->nsigma; sgi++) {
+            const int* S = t->sigma + 4 * sgi;
+            for (int k = 0; k < S[2]; k++) {
+                const int* E = t->entry + 4 * (S[1] + k);
+                const int xoff = E[0] & 0xFFFF, nvx = E[0] >> 16, yoff = E[1] & 0xFFFF, nvy = E[1] >> 16;
+                const unsigned char* hd = t->hdep + 40 * E[2];
+                unsigned shape;
+                if (nvx == 32 && nvy == 4) shape = 0;
+                else if (nvx == 16 && nvy == 8) shape = 1;
+                else if (nvx == 16 && nvy == 4) shape = 2;
+                else if (nvx == 8 && nvy == 8) shape = 3;
+                else { cudaFree(c->p2tab); cudaFree(c->blob); delete c; return cudaErrorInvalidValue; }
+                const int MT = nvx / 8, NT = nvy / 4;
+                for (int l = 0; l < 32; l++) {
+                    const int r = l >> 2, cc = l & 3;
+                    uint4& rec = tab[((size_t)sgi * maxe + k) * 32 + l];
+                    rec.x = (unsigned)((xoff >> 2) + r) | ((unsigned)((yoff >> 2) + (r >> 1)) << 16);
+                    rec.y = 0;
+                    for (int mt = 0; mt < MT; mt++) rec.y |= (unsigned)hd[8 * mt + r] << (8 * mt);
+                    rec.z = 0;
+                    for (int nt = 0; nt < NT; nt++) rec.z |= (unsigned)hd[32 + 4 * nt + cc] << (8 * nt);
+                    rec.z |= (shape << 16) | ((E[3] < 0 ? 1u : 0u) << 18) | ((unsigned)S[2] << 24);
+                    rec.w = (unsigned)S[0];
+                }
+            }
+        }
+        e = cudaMalloc(&c->p3tab, tab.size() * sizeof(uint4));
+        if (e == cudaSuccess) e = cudaMemcpy(c->p3tab, tab.data(), tab.size() * sizeof(uint4), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { cudaFree(c->p3tab); cudaFree(c->p2tab); cudaFree(c->blob); delete c; return e; }
+        d.p3tab = (const uint4*)c->p3tab; d.maxe = maxe;
+    } else { d.p3tab = nullptr; d.maxe = 0; }
     d.npar = t->npar; d.ncolor = t->ncolor; d.ngroups = t->ngroups; d.obj_area = t->obj_area; d.stage_area = t->stage_area;
     d.nlegsets = t->nlegsets;
     for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
@@ -466,7 +560,7 @@ cudaError_t hs_create(int ngluon, HsContext** out)
 void hs_destroy(HsContext* c)
 {
     if (!c) return;
-    cudaFree(c->blob); cudaFree(c->argtab); cudaFree(c->ubase);
+    cudaFree(c->blob); cudaFree(c->p2tab); cudaFree(c->p3tab);
     delete c;
 }
 
