@@ -11,13 +11,16 @@
 // both operands are split in two TF32 terms, X = Xh + Xl and L = Lh + Ll, and three products are accumulated
 // (Xh Lh + Xl Lh + Xh Ll; the dropped Xl Ll is 2^-22 relative): fp32-level accuracy on the tensor pipe.
 //
-// Kernel (v1, not warp-specialised): one persistent CTA per SM, 256 threads, tiles of 128 rows.
-//   smem: L image (hi, lo) resident; ring of A stages, each 128 rows x KC colours (hi, lo), K-major core matrices (no swizzle)
-//   per chunk of KC colours: all threads load four colours of one row (coalesced across rows), split, store 16 B per term; one thread
-//   issues the tcgen05.mma's and commits them to the stage's "empty" mbarrier; chunks run from the last colour
-//   down so that the first MMA of a tile (accumulate = 0) has the full width and earlier chunks can use the
-//   narrower N that the triangular L allows.  Accumulators: re part and im part, double-buffered across tiles
-//   (4 x NP TMEM columns).  Epilogue: warps 0-3 read the re part, warps 4-7 the im part (tcgen05.ld 32x32b).
+// Kernel: one persistent CTA per SM, warp-specialised, tiles of 128 rows, chunks of KC colours.
+//   warp 0      TMA producer: one cp.async.bulk (512 B = 128 rows of one colour) per colour of a chunk into a ring of
+//               raw fp32 stages, completion counted on the stage's "raw full" mbarrier
+//   warp 1      MMA issuer: per chunk 3 x KC/8 tcgen05.mma (M = 128, N = the width the triangular L needs for this
+//               chunk), tcgen05.commit to the A stage's "empty" barrier and, after a tile's last chunk, to "acc full"
+//   warp 2      TMEM allocation / release
+//   warps 4-7   epilogue: tcgen05.ld of the re and im accumulator rows, sum of squares, store (TMEM lane quarter = warp % 4)
+//   warps 8-11  converters: raw stage -> hi/lo TF32 terms in the K-major no-swizzle core-matrix layout of the A ring
+//   Chunks run from the last colour down: the first MMA of a tile (accumulate = 0) has the full width.
+//   Accumulators (re, im) are double-buffered across tiles (4 x NP TMEM columns).
 #include <math.h>
 #include <stdint.h>
 #include <string.h>
@@ -29,7 +32,7 @@
 
 namespace mg {
 
-struct Tf32Cfg { int nc, KP, NP, KC, nchunks, stages; };
+struct Tf32Cfg { int nc, KP, NP, KC, nchunks, raw_stages; };
 
 static bool tf32_cfg(int nc, Tf32Cfg* c)
 {
@@ -39,22 +42,35 @@ static bool tf32_cfg(int nc, Tf32Cfg* c)
     c->NP = (nc + 15) / 16 * 16;
     c->KC = c->KP % 24 == 0 ? 24 : 8;
     c->nchunks = c->KP / c->KC;
-    c->stages = c->nchunks >= 3 ? 3 : (c->nchunks == 2 ? 2 : 2);
+    c->raw_stages = 7;
     return true;
 }
 
-// byte offset of B element (n, k) inside one B image: K-major core matrices (8 n-rows x 16 bytes),
-// adjacent k-chunks 128 B apart (LBO), adjacent 8-row groups (KP/4)*128 B apart (SBO)
-static inline size_t b_off(int n, int k, int KP) { return (size_t)(n % 8) * 16 + (size_t)(n / 8) * (KP / 4) * 128 + (size_t)(k / 4) * 128 + (k % 4) * 4; }
+// width of the accumulator columns that chunk c (colours [c KC, (c+1) KC)) touches: L is lower triangular
+static inline int chunk_n(const Tf32Cfg& c, int chunk)
+{
+    int n = ((chunk + 1) * c.KC + 15) / 16 * 16;
+    return n > c.NP ? c.NP : n;
+}
+// float offset of chunk c inside one factor image: chunk c holds chunk_n rows x KC colours
+static inline size_t chunk_off(const Tf32Cfg& c, int chunk)
+{
+    size_t o = 0;
+    for (int i = 0; i < chunk; i++) o += (size_t)chunk_n(c, i) * c.KC;
+    return o;
+}
+// byte offset of element (n, kk) inside a chunk: K-major core matrices (8 n-rows x 16 bytes), adjacent k-quads 128 B
+// apart (LBO), adjacent 8-row groups (KC / 4) * 128 B apart (SBO)
+static inline size_t b_off(int n, int kk, int KC) { return (size_t)(n % 8) * 16 + (size_t)(n / 8) * (KC / 4) * 128 + (size_t)(kk / 4) * 128 + (kk % 4) * 4; }
 
-// host: the two-term TF32 image of L (C = L L^T), [hi | lo], each NP*KP floats in the layout of b_off
+// host: the two-term TF32 image of L (C = L L^T), [hi | lo], chunk by chunk, each chunk in the layout of b_off
 bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img)
 {
     Tf32Cfg c;
     if (!tf32_cfg(ncolor, &c)) return false;
     std::vector<double> lp; int ncp = 0;
     if (!color_cholesky_padded(ncolor, cmat, lp, &ncp)) return false;
-    const size_t per = (size_t)c.NP * c.KP;
+    const size_t per = chunk_off(c, c.nchunks);
     img.assign(2 * per, 0.0f);
     for (int k = 0; k < ncolor; k++)
         for (int n = 0; n <= k; n++) {
@@ -62,48 +78,51 @@ bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& im
             float hi = (float)l;
             uint32_t u; memcpy(&u, &hi, 4); u &= 0xFFFFE000u; memcpy(&hi, &u, 4);
             const float lo = (float)(l - (double)hi);
-            const size_t o = b_off(n, k, c.KP) / 4;
+            const int chunk = k / c.KC;
+            const size_t o = chunk_off(c, chunk) + b_off(n, k % c.KC, c.KC) / 4;
             img[o] = hi; img[per + o] = lo;
         }
     return true;
 }
 
-size_t tf32_factor_image_bytes(int ncolor)
-{
-    Tf32Cfg c;
-    return tf32_cfg(ncolor, &c) ? 2 * (size_t)c.NP * c.KP * sizeof(float) : 0;
-}
-
 struct Tf32Args {
     const float* X; const float* Bimg; double* out;
     long rows_padded;
-    int nc, KP, NP, KC, nchunks, stages;
+    int nc, KP, NP, KC, nchunks, raw_stages;
+    int b_floats;                  // floats of one factor image
+    int chunk_off[8], chunk_n[8];  // per chunk: float offset inside an image, accumulator width
     RowMap map;
 };
 
-__global__ void __launch_bounds__(256, 1) color_sum_tf32_kernel(const Tf32Args a)
+constexpr int TF32_THREADS = 384;
+constexpr int TF32_MAX_RAW = 8;
+
+__global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const Tf32Args a)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
-    __shared__ uint64_t bar_empty[4];
-    __shared__ uint64_t bar_acc[2];
+    __shared__ uint64_t raw_full[TF32_MAX_RAW], raw_empty[TF32_MAX_RAW];
+    __shared__ uint64_t a_full[2], a_empty[2], acc_full[2], acc_empty[2];
     __shared__ uint32_t tmem_slot;
-    __shared__ float im_part[128];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const size_t b_bytes = (size_t)a.NP * a.KP * 4;            // one B image
-    const size_t a_bytes = (size_t)a.KC * 128 * 4;             // one A term of one stage
+    const size_t b_bytes = (size_t)a.b_floats * 4;             // one factor image
+    const size_t a_bytes = (size_t)a.KC * 128 * 4;             // one A term of one stage = one raw stage
     float* Bs = reinterpret_cast<float*>(smem);
-    unsigned char* As = smem + 2 * b_bytes;
+    unsigned char* As = smem + 2 * b_bytes;                    // [2 stages][hi | lo]
+    unsigned char* Rs = As + 4 * a_bytes;                      // [raw_stages][KC][128] fp32
+    const int R = a.raw_stages;
     const uint32_t tcols = 4 * a.NP <= 32 ? 32 : (4 * a.NP <= 64 ? 64 : (4 * a.NP <= 128 ? 128 : (4 * a.NP <= 256 ? 256 : 512)));
 
     if (tid == 0) {
-        for (int s = 0; s < a.stages; s++) tc5::mbar_init(&bar_empty[s], 1);
-        tc5::mbar_init(&bar_acc[0], 1); tc5::mbar_init(&bar_acc[1], 1);
+        for (int s = 0; s < R; s++) { tc5::mbar_init(&raw_full[s], 1); tc5::mbar_init(&raw_empty[s], 4); }
+        for (int s = 0; s < 2; s++) {
+            tc5::mbar_init(&a_full[s], 4); tc5::mbar_init(&a_empty[s], 1);
+            tc5::mbar_init(&acc_full[s], 1); tc5::mbar_init(&acc_empty[s], 4);
+        }
         tc5::mbar_fence_init();
     }
-    if (warp == 0) tc5::tmem_alloc(&tmem_slot, tcols);
-    // resident factor image
-    {
+    if (warp == 2) tc5::tmem_alloc(&tmem_slot, tcols);
+    {   // resident factor image
         const float4* src = reinterpret_cast<const float4*>(a.Bimg);
         float4* dst = reinterpret_cast<float4*>(Bs);
         const int n4 = (int)(2 * b_bytes / 16);
@@ -114,76 +133,74 @@ __global__ void __launch_bounds__(256, 1) color_sum_tf32_kernel(const Tf32Args a
     __syncthreads();
     tc5::tc_fence_after();
     const uint32_t tmem = tmem_slot;
-    const uint32_t b_base = tc5::smem_u32(Bs), a_base = tc5::smem_u32(As);
-    const uint32_t sbo_b = (uint32_t)(a.KP / 4) * 128, sbo_a = (uint32_t)(a.KC / 4) * 128;
-
     const long ntiles = a.rows_padded / 128;
-    uint32_t it = 0;                 // chunk-stage uses so far (same sequence in every thread)
-    uint32_t tl = 0;                 // tiles done by this CTA
-    for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, tl++) {
-        const long row0 = tile * 128;
-        const uint32_t accbuf = tl & 1;
-        for (int part = 0; part < 2; part++) {
-            const uint32_t tm_d = tmem + accbuf * 2 * a.NP + part * a.NP;
-            for (int ci = 0; ci < a.nchunks; ci++, it++) {
-                const int c = a.nchunks - 1 - ci;                     // last colours first (full N, accumulate = 0)
+    const int cpt = 2 * a.nchunks;                             // chunks per tile (re part, then im part)
+
+    if (warp == 0) {
+        // ---- TMA producer: lane 0 waits for the stage and posts the byte count, then lane kk copies colour kk ----
+        uint32_t q = 0;
+        for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const long row0 = tile * 128;
+            for (int j = 0; j < cpt; j++, q++) {
+                const int part = j / a.nchunks, c = a.nchunks - 1 - j % a.nchunks;
                 const int k0 = c * a.KC;
-                const uint32_t s = it % a.stages, use = it / a.stages;
-                if (use > 0) tc5::mbar_wait(&bar_empty[s], (use - 1) & 1);        // MMAs that read this stage are done
-                unsigned char* st_hi = As + (size_t)s * 2 * a_bytes;
-                unsigned char* st_lo = st_hi + a_bytes;
-                // K-major core matrices (8 rows x 16 B): [row / 8][k / 4][row % 8][k % 4]; item = (k-quad, row): four
-                // coalesced loads (one colour each, 128 consecutive rows per warp-quad), one 16-byte store per term
-                const int items = (a.KC / 4) * 128;
-                for (int i = tid; i < items; i += blockDim.x) {
-                    const int m = i & 127, kc = i >> 7;
-                    float x[4];
-#pragma unroll
-                    for (int j = 0; j < 4; j++) {
-                        const int k = k0 + 4 * kc + j;
-                        x[j] = k < a.nc ? __ldg(a.X + ((size_t)part * a.nc + k) * a.rows_padded + row0 + m) : 0.f;
-                    }
-                    float4 h, l;
-                    h.x = __uint_as_float(__float_as_uint(x[0]) & 0xFFFFE000u); l.x = x[0] - h.x;
-                    h.y = __uint_as_float(__float_as_uint(x[1]) & 0xFFFFE000u); l.y = x[1] - h.y;
-                    h.z = __uint_as_float(__float_as_uint(x[2]) & 0xFFFFE000u); l.z = x[2] - h.z;
-                    h.w = __uint_as_float(__float_as_uint(x[3]) & 0xFFFFE000u); l.w = x[3] - h.w;
-                    const size_t o = (size_t)(m >> 3) * sbo_a + (size_t)kc * 128 + (m & 7) * 16;
-                    *reinterpret_cast<float4*>(st_hi + o) = h;
-                    *reinterpret_cast<float4*>(st_lo + o) = l;
+                const uint32_t s = q % R;
+                int nk = a.nc - k0;
+                if (nk > a.KC) nk = a.KC;
+                if (lane == 0) {
+                    tc5::mbar_wait(&raw_empty[s], ((q / R) & 1) ^ 1);
+                    tc5::mbar_arrive_expect_tx(&raw_full[s], (uint32_t)nk * 512u);
                 }
-                tc5::fence_async_smem();
-                tc5::tc_fence_before();
-                __syncthreads();
-                if (tid == 0) {
+                __syncwarp();
+                float* dst = reinterpret_cast<float*>(Rs + (size_t)s * a_bytes);
+                if (lane < nk)
+                    tc5::tma_load_1d(dst + lane * 128, a.X + ((size_t)part * a.nc + k0 + lane) * a.rows_padded + row0, 512u, &raw_full[s]);
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // ---- MMA issuer ----
+        if (lane == 0) {
+            const uint32_t b_base = tc5::smem_u32(Bs), a_base = tc5::smem_u32(As);
+            const uint32_t sbo = (uint32_t)(a.KC / 4) * 128;
+            uint32_t q = 0, tl = 0;
+            for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, tl++) {
+                const uint32_t buf = tl & 1;
+                tc5::mbar_wait(&acc_empty[buf], ((tl >> 1) & 1) ^ 1);
+                tc5::tc_fence_after();
+                for (int j = 0; j < cpt; j++, q++) {
+                    const int part = j / a.nchunks, ci = j % a.nchunks, c = a.nchunks - 1 - ci;
+                    const uint32_t sa = q & 1;
+                    tc5::mbar_wait(&a_full[sa], (q >> 1) & 1);
                     tc5::tc_fence_after();
-                    int n = (k0 + a.KC + 15) / 16 * 16;
-                    if (n > a.NP) n = a.NP;
-                    const uint32_t idesc = tc5::idesc_tf32(n, 0, 0);
-                    const uint32_t ah = a_base + (uint32_t)(s * 2 * a_bytes), al = ah + (uint32_t)a_bytes;
+                    const uint32_t tm_d = tmem + buf * 2 * a.NP + part * a.NP;
+                    const uint32_t idesc = tc5::idesc_tf32(a.chunk_n[c], 0, 0);
+                    const uint32_t ah = a_base + (uint32_t)(sa * 2 * a_bytes), al = ah + (uint32_t)a_bytes;
+                    const uint32_t bh = b_base + (uint32_t)a.chunk_off[c] * 4, bl = bh + (uint32_t)b_bytes;
                     for (int ks = 0; ks < a.KC / 8; ks++) {
-                        const uint64_t dah = tc5::smem_desc(ah + ks * 256, 128, sbo_a);
-                        const uint64_t dal = tc5::smem_desc(al + ks * 256, 128, sbo_a);
-                        const uint32_t bo = (uint32_t)((k0 / 4 + ks * 2) * 128);
-                        const uint64_t dbh = tc5::smem_desc(b_base + bo, 128, sbo_b);
-                        const uint64_t dbl = tc5::smem_desc(b_base + (uint32_t)b_bytes + bo, 128, sbo_b);
+                        const uint64_t dah = tc5::smem_desc(ah + ks * 256, 128, sbo), dal = tc5::smem_desc(al + ks * 256, 128, sbo);
+                        const uint64_t dbh = tc5::smem_desc(bh + ks * 256, 128, sbo), dbl = tc5::smem_desc(bl + ks * 256, 128, sbo);
                         tc5::mma_tf32(tm_d, dah, dbh, idesc, (ci | ks) != 0);
                         tc5::mma_tf32(tm_d, dal, dbh, idesc, 1);
                         tc5::mma_tf32(tm_d, dah, dbl, idesc, 1);
                     }
-                    tc5::mma_commit(&bar_empty[s]);
-                    if (part == 1 && ci == a.nchunks - 1) tc5::mma_commit(&bar_acc[accbuf]);
+                    tc5::mma_commit(&a_empty[sa]);
+                    if (j == cpt - 1) tc5::mma_commit(&acc_full[buf]);
                 }
             }
         }
-        // epilogue of this tile: sum of squares of the accumulator row
-        tc5::mbar_wait(&bar_acc[accbuf], (tl >> 1) & 1);
-        tc5::tc_fence_after();
-        {
-            const int part = warp >> 2;
-            const uint32_t taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + accbuf * 2 * a.NP + part * a.NP;
+        __syncwarp();
+    } else if (warp >= 4 && warp < 8) {
+        // ---- epilogue ----
+        uint32_t tl = 0;
+        const int r = (warp & 3) * 32 + lane;
+        for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, tl++) {
+            const uint32_t buf = tl & 1;
+            tc5::mbar_wait(&acc_full[buf], (tl >> 1) & 1);
+            tc5::tc_fence_after();
+            const uint32_t taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + buf * 2 * a.NP;
             float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-            for (int c0 = 0; c0 < a.NP; c0 += 16) {
+            for (int c0 = 0; c0 < 2 * a.NP; c0 += 16) {
                 float v[16];
                 tc5::tmem_ld16(taddr + c0, v);
 #pragma unroll
@@ -192,29 +209,60 @@ __global__ void __launch_bounds__(256, 1) color_sum_tf32_kernel(const Tf32Args a
                     s2 = fmaf(v[i + 2], v[i + 2], s2); s3 = fmaf(v[i + 3], v[i + 3], s3);
                 }
             }
-            const float sum = (s0 + s1) + (s2 + s3);
-            const int r = (warp & 3) * 32 + lane;
-            if (part == 1) im_part[r] = sum;
             tc5::tc_fence_before();
-            __syncthreads();
-            if (part == 0) a.map.store(a.out, row0 + r, (double)sum + (double)im_part[r]);
+            __syncwarp();
+            if (lane == 0) tc5::mbar_arrive(&acc_empty[buf]);
+            a.map.store(a.out, tile * 128 + r, (double)s0 + (double)s1 + ((double)s2 + (double)s3));
+        }
+    } else if (warp >= 8) {
+        // ---- converters: thread m = row m of the tile ----
+        const int m = tid - 256;
+        const uint32_t sbo = (uint32_t)(a.KC / 4) * 128;
+        uint32_t q = 0;
+        for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            for (int j = 0; j < cpt; j++, q++) {
+                const int c = a.nchunks - 1 - j % a.nchunks;
+                int nk = a.nc - c * a.KC;
+                if (nk > a.KC) nk = a.KC;
+                const uint32_t s = q % R, sa = q & 1;
+                tc5::mbar_wait(&raw_full[s], (q / R) & 1);
+                tc5::mbar_wait(&a_empty[sa], ((q >> 1) & 1) ^ 1);
+                const float* src = reinterpret_cast<const float*>(Rs + (size_t)s * a_bytes) + m;
+                unsigned char* st_hi = As + (size_t)sa * 2 * a_bytes + (size_t)(m >> 3) * sbo + (m & 7) * 16;
+                unsigned char* st_lo = st_hi + a_bytes;
+                for (int kc = 0; kc < a.KC / 4; kc++) {
+                    float x[4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) x[i] = 4 * kc + i < nk ? src[(4 * kc + i) * 128] : 0.f;
+                    float4 h, l;
+                    h.x = __uint_as_float(__float_as_uint(x[0]) & 0xFFFFE000u); l.x = x[0] - h.x;
+                    h.y = __uint_as_float(__float_as_uint(x[1]) & 0xFFFFE000u); l.y = x[1] - h.y;
+                    h.z = __uint_as_float(__float_as_uint(x[2]) & 0xFFFFE000u); l.z = x[2] - h.z;
+                    h.w = __uint_as_float(__float_as_uint(x[3]) & 0xFFFFE000u); l.w = x[3] - h.w;
+                    *reinterpret_cast<float4*>(st_hi + kc * 128) = h;
+                    *reinterpret_cast<float4*>(st_lo + kc * 128) = l;
+                }
+                tc5::fence_async_smem();
+                __syncwarp();
+                if (lane == 0) { tc5::mbar_arrive(&a_full[sa]); tc5::mbar_arrive(&raw_empty[s]); }
+            }
         }
     }
     tc5::tc_fence_before();
     __syncthreads();
-    if (warp == 0) tc5::tmem_free(tmem, tcols);
+    if (warp == 2) tc5::tmem_free(tmem, tcols);
 }
 
 static size_t tf32_smem_bytes(const Tf32Cfg& c)
 {
-    return 2 * (size_t)c.NP * c.KP * 4 + (size_t)c.stages * 2 * c.KC * 128 * 4 + 1024;
+    return 2 * chunk_off(c, c.nchunks) * 4 + (size_t)(4 + c.raw_stages) * c.KC * 128 * 4 + 1024;
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
                            double* d_meh, cudaStream_t st)
 {
     Tf32Cfg c;
-    if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128) return cudaErrorInvalidValue;
+    if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128 || c.nchunks > 8) return cudaErrorInvalidValue;
     static int sms = 0;
     static size_t smem_set = 0;
     if (!sms) {
@@ -230,11 +278,12 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     }
     Tf32Args a;
     a.X = (const float*)d_jamps; a.Bimg = (const float*)d_factor_img; a.out = d_meh; a.rows_padded = rows_padded;
-    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.stages = c.stages; a.map = map;
+    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.raw_stages = c.raw_stages; a.map = map;
+    a.b_floats = (int)chunk_off(c, c.nchunks);
+    for (int i = 0; i < 8; i++) { a.chunk_off[i] = i < c.nchunks ? (int)chunk_off(c, i) : 0; a.chunk_n[i] = i < c.nchunks ? chunk_n(c, i) : 0; }
     const long ntiles = rows_padded / 128;
-    // NP <= 32: several CTAs per SM would each need their TMEM columns; one per SM keeps the allocation uncontended
-    const int grid = (int)(ntiles < sms ? ntiles : sms);
-    color_sum_tf32_kernel<<<grid, 256, smem, st>>>(a);
+    const int grid = (int)(ntiles < sms ? ntiles : sms);      // one CTA per SM: each owns its TMEM columns
+    color_sum_tf32_kernel<<<grid, TF32_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
