@@ -467,6 +467,9 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             HsLaunch a;
             a.mom = d_momenta + (size_t)e0 * p->d->npar * 4; a.nevt = ne; a.d_pos = p->d_pos; a.nrow_evt = nhel;
             a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows); a.mt = p->mT; a.wt = p->wT;
+            // tcgen05 colour sum: one contiguous block per 128-row tile, so that a chunk of colours is ONE bulk copy
+            const bool tile_major = p->precision != MG_FP64 && !p->hs_color_alu;
+            a.tile_major = tile_major ? 1 : 0;
             CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, p->hs_split, p->hs_phase3, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
@@ -477,7 +480,7 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             if (p->hs_color_alu && p->precision != MG_FP64)
                 ce_ = color_sum_alu(false, p->d->ncolor, p->d_cmat, d_j, a.rows, d_meh, st, &map);
             else
-                ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
+                ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st, tile_major);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("colour sum: ") + cudaGetErrorString(ce_));
             MARK(1);
         }

@@ -137,12 +137,13 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
-                           double* d_meh, cudaStream_t st);
+                           double* d_meh, cudaStream_t st, bool tile_major);
 
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
-                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st)
+                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, bool tile_major)
 {
-    if (!is_fp64) return color_sum_tf32(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st);
+    if (!is_fp64) return color_sum_tf32(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st, tile_major);
+    if (tile_major) return cudaErrorInvalidValue;
     if (!d_factor) return cudaErrorInvalidValue;
     const double* d_chol = (const double*)d_factor;
     const int ncp = (ncolor + 7) / 8 * 8;

@@ -12,13 +12,14 @@
 // (Xh Lh + Xl Lh + Xh Ll; the dropped Xl Ll is 2^-22 relative): fp32-level accuracy on the tensor pipe.
 //
 // Kernel: one persistent CTA per SM, warp-specialised, tiles of 128 rows, chunks of KC colours.
-//   warp 0      TMA producer: one cp.async.bulk (512 B = 128 rows of one colour) per colour of a chunk into a ring of
-//               raw fp32 stages, completion counted on the stage's "raw full" mbarrier
+//   warp 0      TMA producer: cp.async.bulk into a ring of raw fp32 stages, completion counted on the stage's "raw full"
+//               mbarrier.  Tile-major jamps ([row / 128][2][nc][128], written so by the helicity-shared kernel): ONE
+//               bulk copy of KC x 512 B per chunk; plain [2][nc][rows] jamps (mg_color_sum): one 512-B copy per colour
 //   warp 1      MMA issuer: per chunk 3 x KC/8 tcgen05.mma (M = 128, N = the width the triangular L needs for this
 //               chunk), tcgen05.commit to the A stage's "empty" barrier and, after a tile's last chunk, to "acc full"
 //   warp 2      TMEM allocation / release
 //   warps 4-7   epilogue: tcgen05.ld of the re and im accumulator rows, sum of squares, store (TMEM lane quarter = warp % 4)
-//   warps 8-11  converters: raw stage -> hi/lo TF32 terms in the K-major no-swizzle core-matrix layout of the A ring
+//   warps 8-15  converters: raw stage -> hi/lo TF32 terms in the K-major no-swizzle core-matrix layout of the A ring
 //   Chunks run from the last colour down: the first MMA of a tile (accumulate = 0) has the full width.
 //   Accumulators (re, im) are double-buffered across tiles (4 x NP TMEM columns).
 #include <math.h>
@@ -32,7 +33,7 @@
 
 namespace mg {
 
-struct Tf32Cfg { int nc, KP, NP, KC, nchunks, raw_stages; };
+struct Tf32Cfg { int nc, KP, NP, KC, nchunks, raw_stages, a_stages; };
 
 static bool tf32_cfg(int nc, Tf32Cfg* c)
 {
@@ -42,7 +43,7 @@ static bool tf32_cfg(int nc, Tf32Cfg* c)
     c->NP = (nc + 15) / 16 * 16;
     c->KC = c->KP % 24 == 0 ? 24 : 8;
     c->nchunks = c->KP / c->KC;
-    c->raw_stages = 7;
+    c->raw_stages = 5; c->a_stages = 3;
     return true;
 }
 
@@ -88,37 +89,36 @@ bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& im
 struct Tf32Args {
     const float* X; const float* Bimg; double* out;
     long rows_padded;
-    int nc, KP, NP, KC, nchunks, raw_stages;
+    int nc, KP, NP, KC, nchunks, raw_stages, a_stages;
+    int tile_major;                // jamps as [row / 128][2][nc][128]: one bulk copy per chunk
     int b_floats;                  // floats of one factor image
     int chunk_off[8], chunk_n[8];  // per chunk: float offset inside an image, accumulator width
     RowMap map;
 };
 
-constexpr int TF32_THREADS = 384;
+constexpr int TF32_THREADS = 512;
 constexpr int TF32_MAX_RAW = 8;
 
 __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const Tf32Args a)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ uint64_t raw_full[TF32_MAX_RAW], raw_empty[TF32_MAX_RAW];
-    __shared__ uint64_t a_full[2], a_empty[2], acc_full[2], acc_empty[2];
+    __shared__ uint64_t a_full[4], a_empty[4], acc_full[2], acc_empty[2];
     __shared__ uint32_t tmem_slot;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const size_t b_bytes = (size_t)a.b_floats * 4;             // one factor image
     const size_t a_bytes = (size_t)a.KC * 128 * 4;             // one A term of one stage = one raw stage
     float* Bs = reinterpret_cast<float*>(smem);
-    unsigned char* As = smem + 2 * b_bytes;                    // [2 stages][hi | lo]
-    unsigned char* Rs = As + 4 * a_bytes;                      // [raw_stages][KC][128] fp32
-    const int R = a.raw_stages;
+    unsigned char* As = smem + 2 * b_bytes;                    // [a_stages][hi | lo]
+    const int R = a.raw_stages, NA = a.a_stages;
+    unsigned char* Rs = As + (size_t)2 * NA * a_bytes;         // [raw_stages][KC][128] fp32
     const uint32_t tcols = 4 * a.NP <= 32 ? 32 : (4 * a.NP <= 64 ? 64 : (4 * a.NP <= 128 ? 128 : (4 * a.NP <= 256 ? 256 : 512)));
 
     if (tid == 0) {
-        for (int s = 0; s < R; s++) { tc5::mbar_init(&raw_full[s], 1); tc5::mbar_init(&raw_empty[s], 4); }
-        for (int s = 0; s < 2; s++) {
-            tc5::mbar_init(&a_full[s], 4); tc5::mbar_init(&a_empty[s], 1);
-            tc5::mbar_init(&acc_full[s], 1); tc5::mbar_init(&acc_empty[s], 4);
-        }
+        for (int s = 0; s < R; s++) { tc5::mbar_init(&raw_full[s], 1); tc5::mbar_init(&raw_empty[s], 8); }
+        for (int s = 0; s < NA; s++) { tc5::mbar_init(&a_full[s], 8); tc5::mbar_init(&a_empty[s], 1); }
+        for (int s = 0; s < 2; s++) { tc5::mbar_init(&acc_full[s], 1); tc5::mbar_init(&acc_empty[s], 4); }
         tc5::mbar_fence_init();
     }
     if (warp == 2) tc5::tmem_alloc(&tmem_slot, tcols);
@@ -153,7 +153,10 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
                 }
                 __syncwarp();
                 float* dst = reinterpret_cast<float*>(Rs + (size_t)s * a_bytes);
-                if (lane < nk)
+                if (a.tile_major) {
+                    if (lane == 0)
+                        tc5::tma_load_1d(dst, a.X + (size_t)tile * (256 * a.nc) + ((size_t)part * a.nc + k0) * 128, (uint32_t)nk * 512u, &raw_full[s]);
+                } else if (lane < nk)
                     tc5::tma_load_1d(dst + lane * 128, a.X + ((size_t)part * a.nc + k0 + lane) * a.rows_padded + row0, 512u, &raw_full[s]);
             }
         }
@@ -170,8 +173,8 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
                 tc5::tc_fence_after();
                 for (int j = 0; j < cpt; j++, q++) {
                     const int part = j / a.nchunks, ci = j % a.nchunks, c = a.nchunks - 1 - ci;
-                    const uint32_t sa = q & 1;
-                    tc5::mbar_wait(&a_full[sa], (q >> 1) & 1);
+                    const uint32_t sa = q % NA;
+                    tc5::mbar_wait(&a_full[sa], (q / NA) & 1);
                     tc5::tc_fence_after();
                     const uint32_t tm_d = tmem + buf * 2 * a.NP + part * a.NP;
                     const uint32_t idesc = tc5::idesc_tf32(a.chunk_n[c], 0, 0);
@@ -215,8 +218,9 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
             a.map.store(a.out, tile * 128 + r, (double)s0 + (double)s1 + ((double)s2 + (double)s3));
         }
     } else if (warp >= 8) {
-        // ---- converters: thread m = row m of the tile ----
-        const int m = tid - 256;
+        // ---- converters: 8 warps; thread = (row m of the tile, half of the chunk's colour quads) ----
+        const int m = (tid - 256) & 127, half = (tid - 256) >> 7;
+        const int nq = a.KC / 4, q0 = half * nq / 2, q1 = (half + 1) * nq / 2;
         const uint32_t sbo = (uint32_t)(a.KC / 4) * 128;
         uint32_t q = 0;
         for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -224,13 +228,13 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
                 const int c = a.nchunks - 1 - j % a.nchunks;
                 int nk = a.nc - c * a.KC;
                 if (nk > a.KC) nk = a.KC;
-                const uint32_t s = q % R, sa = q & 1;
+                const uint32_t s = q % R, sa = q % NA;
                 tc5::mbar_wait(&raw_full[s], (q / R) & 1);
-                tc5::mbar_wait(&a_empty[sa], ((q >> 1) & 1) ^ 1);
+                tc5::mbar_wait(&a_empty[sa], ((q / NA) & 1) ^ 1);
                 const float* src = reinterpret_cast<const float*>(Rs + (size_t)s * a_bytes) + m;
                 unsigned char* st_hi = As + (size_t)sa * 2 * a_bytes + (size_t)(m >> 3) * sbo + (m & 7) * 16;
                 unsigned char* st_lo = st_hi + a_bytes;
-                for (int kc = 0; kc < a.KC / 4; kc++) {
+                for (int kc = q0; kc < q1; kc++) {
                     float x[4];
 #pragma unroll
                     for (int i = 0; i < 4; i++) x[i] = 4 * kc + i < nk ? src[(4 * kc + i) * 128] : 0.f;
@@ -255,14 +259,15 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
 
 static size_t tf32_smem_bytes(const Tf32Cfg& c)
 {
-    return 2 * chunk_off(c, c.nchunks) * 4 + (size_t)(4 + c.raw_stages) * c.KC * 128 * 4 + 1024;
+    return 2 * chunk_off(c, c.nchunks) * 4 + (size_t)(2 * c.a_stages + c.raw_stages) * c.KC * 128 * 4 + 1024;
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
-                           double* d_meh, cudaStream_t st)
+                           double* d_meh, cudaStream_t st, bool tile_major)
 {
     Tf32Cfg c;
-    if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128 || c.nchunks > 8) return cudaErrorInvalidValue;
+    if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128 || c.nchunks > 8 || c.a_stages > 4 || c.raw_stages > TF32_MAX_RAW)
+        return cudaErrorInvalidValue;
     static int sms = 0;
     static size_t smem_set = 0;
     if (!sms) {
@@ -278,7 +283,7 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     }
     Tf32Args a;
     a.X = (const float*)d_jamps; a.Bimg = (const float*)d_factor_img; a.out = d_meh; a.rows_padded = rows_padded;
-    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.raw_stages = c.raw_stages; a.map = map;
+    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.raw_stages = c.raw_stages; a.a_stages = c.a_stages; a.map = map; a.tile_major = tile_major ? 1 : 0;
     a.b_floats = (int)chunk_off(c, c.nchunks);
     for (int i = 0; i < 8; i++) { a.chunk_off[i] = i < c.nchunks ? (int)chunk_off(c, i) : 0; a.chunk_n[i] = i < c.nchunks ? chunk_n(c, i) : 0; }
     const long ntiles = rows_padded / 128;

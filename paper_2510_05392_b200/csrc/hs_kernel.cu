@@ -283,8 +283,13 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
             if (pos >= 0) {
                 const double2 v = acc[acc_swizzle(h)];
                 const size_t row = (size_t)e * a.nrow_evt + pos;
-                out[(size_t)jamp * a.rows + row] = T2(v.x);
-                out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
+                if (a.tile_major) {
+                    T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)jamp * 128 + (row & 127);
+                    o[0] = T2(v.x); o[(size_t)d.ncolor * 128] = T2(v.y);
+                } else {
+                    out[(size_t)jamp * a.rows + row] = T2(v.x);
+                    out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
+                }
             }
         }
         __syncwarp();
@@ -402,8 +407,13 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                         re = fma(sgn, tr, re); im = fma(sgn, ti, im);
                     }
                     T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
-                    out[(size_t)sg.x * a.rows + row] = T2(re);
-                    out[(size_t)(d.ncolor + sg.x) * a.rows + row] = T2(im);
+                    if (a.tile_major) {
+                        T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)sg.x * 128 + (row & 127);
+                        o[0] = T2(re); o[(size_t)d.ncolor * 128] = T2(im);
+                    } else {
+                        out[(size_t)sg.x * a.rows + row] = T2(re);
+                        out[(size_t)(d.ncolor + sg.x) * a.rows + row] = T2(im);
+                    }
                 }
             }
             __syncthreads();

@@ -13,6 +13,7 @@ struct HsLaunch {
     int nrow_evt;          // rows per event (= number of good helicities)
     void* d_jamps;         // DEVICE [2][ncolor][rows] fp64 or fp32; row = event * nrow_evt + pos[h]
     long rows;             // row stride of the jamps buffer
+    int tile_major;        // 1: [row / 128][2][ncolor][128] (one contiguous block per 128-row tile: TMA-friendly) instead
     double mt, wt;
 };
 
