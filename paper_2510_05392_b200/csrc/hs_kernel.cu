@@ -80,6 +80,16 @@ __device__ __forceinline__ void lower(wf<double>& w)
     for (int c = 1; c < 4; c++) { w.c[c].re = -w.c[c].re; w.c[c].im = -w.c[c].im; }
 }
 
+// both orderings of the four-gluon vertex that share the middle leg: (x y | z out) + (z y | x out)
+//   J = 2 (X.Z) Y - (Y.Z) X - (Y.X) Z      (raw vertex, no propagator factor)
+template <typename T> __device__ __forceinline__ void v4s_raw(const wf<T>& X, const wf<T>& Y, const wf<T>& Z, wf<T>& out)
+{
+    cx<T> xz = dot(X, Z);
+    xz = xz + xz;
+    const cx<T> yz = dot(Y, Z), yx = dot(Y, X);
+    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(yx, Z.c[mu], cfms(yz, X.c[mu], xz * Y.c[mu]));
+}
+
 // argument of a term: word = offset in the area (16 bits) | sub-variant code (9 bits) << 16
 __device__ __forceinline__ void load_arg(const double2* __restrict__ area, int word, int var, wf<double>& w)
 {
@@ -121,6 +131,7 @@ __device__ __forceinline__ void run_terms(const HsDev& d, const double2* __restr
             switch (op) {
                 case 3: v3_off(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), 1.0 / m2(load_k(Ks, ls_out)), r); break;
                 case 11: v3_raw(A, load_k(Ks, (w.x >> 16) & 0xFF), B, load_k(Ks, (w.x >> 24) & 0xFF), r); lower(r); break;
+                case 13: { wf<double> Z; load_arg(area, w.w, var, Z); v4s_raw(A, B, Z, r); lower(r); break; }
                 case 4: case 12: {
                     wf<double> Z;
                     if (PRE) load_blk(area, aw.y, Z);
@@ -162,6 +173,7 @@ __device__ __forceinline__ void eval_x_term(const double2* __restrict__ area, co
     switch (op) {
         case 11: v3_raw(A, load_k(Ks, (e.z >> 16) & 0xFF), B, load_k(Ks, (e.z >> 24) & 0xFF), r); break;
         case 12: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4_raw(A, B, Z, r); break; }
+        case 13: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4s_raw(A, B, Z, r); break; }
         case 8: row_slash(A, make_slashed(B), r); break;
         case 9: slash_col(make_slashed(A), B, r); break;
         default: ffv_p_raw(A, B, r); break;                 // 10: x_bil

@@ -39,7 +39,38 @@ STAR = colour.STAR
 
 # term opcodes (phase 1: currents with propagators; phase 2: raw vertices, output lowered for the plain dot)
 OPS = {"ext_v": 0, "ext_ql": 1, "ext_qr": 2, "v3": 3, "v4": 4, "ffv_l": 5, "ffv_r": 6, "ffv_p": 7,
-       "x_row": 8, "x_col": 9, "x_bil": 10, "x_v3": 11, "x_v4": 12}
+       "x_row": 8, "x_col": 9, "x_bil": 10, "x_v3": 11, "x_v4": 12, "x_v4s": 13}
+
+
+def merge_v4_pairs(terms):
+    """With x_v4(p, q, r) = (p.r) q - (q.r) p and S(m; a, b) = 2 (a.b) m - (m.b) a - (m.a) b =: x_v4s(a, m, b):
+         x_v4(p, q, r) + x_v4(r, q, p) =  S(q; p, r)
+         x_v4(p, q, r) - x_v4(q, r, p) =  S(q; p, r)
+         x_v4(p, q, r) + x_v4(p, r, q) = -S(p; q, r)
+    The two orderings of the four-gluon vertex that a colour-ordered amplitude takes together share their dot
+    products: 3 dots + 12 complex multiply-adds instead of 4 + 16, and one pass over the arguments instead of two."""
+    out, used = [], set()
+    for i, t in enumerate(terms):
+        if i in used:
+            continue
+        merged = None
+        if t.op == "x_v4":
+            p_, q_, r_ = t.args
+            for j in range(i + 1, len(terms)):
+                u = terms[j]
+                if j in used or u.op != "x_v4":
+                    continue
+                if u.args == (r_, q_, p_) and u.sign == t.sign:
+                    merged = Term(t.sign, "x_v4s", (p_, q_, r_), t.legs)
+                elif u.args == (q_, r_, p_) and u.sign == -t.sign:
+                    merged = Term(t.sign, "x_v4s", (p_, q_, r_), t.legs)
+                elif u.args == (p_, r_, q_) and u.sign == t.sign:
+                    merged = Term(-t.sign, "x_v4s", (q_, p_, r_), t.legs)
+                if merged is not None:
+                    used.add(j)
+                    break
+        out.append(merged if merged is not None else t)
+    return out
 
 
 def acc_swizzle(h):
@@ -249,7 +280,8 @@ class Program:
                         assert set(legs) | set(self.objs[yo].legs) == set(range(self.npar))
                         assert not set(legs) & set(self.objs[yo].legs)
                         xkey_to_slot[canon] = len(xobjs)
-                        xobjs.append({"legs": legs, "terms": [Term(sg_, xop, args, legs) for sg_, xop, args in canon]})
+                        xobjs.append({"legs": legs,
+                                      "terms": merge_v4_pairs([Term(sg_, xop, args, legs) for sg_, xop, args in canon])})
                     ents.append((xkey_to_slot[canon], yo, s0))
                 entries[j] = ents
             self.groups.append({"sigmas": order[pre], "xobjs": xobjs, "entries": entries})

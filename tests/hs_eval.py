@@ -72,6 +72,9 @@ def evaluate(T, mom, mt, wt):
                 elif op == 12:
                     Z = load(w3, var)
                     r = G * (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A)
+                elif op == 13:
+                    Z = load(w3, var)
+                    r = G * (2 * ir.mdot(A, Z) * B - ir.mdot(B, Z) * A - ir.mdot(A, B) * Z)
                 else:
                     raise ValueError(op)
             acc = acc + (-r if neg else r)
