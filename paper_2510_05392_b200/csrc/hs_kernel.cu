@@ -9,6 +9,8 @@
 // jamp is finished in registers and written once, coalesced, to the jamps buffer [2][ncolor][rows]
 // with rows ordered (event, helicity).
 #include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
 
 #include <vector>
 
@@ -214,9 +216,12 @@ __device__ __forceinline__ int acc_swizzle(int h)
 //       number of entries of the flow << 24;  shape 0: (MT, NT) = (4, 1), 1: (2, 2), 2: (2, 1), 3: (1, 2)
 //   w = jamp index of the flow
 // one dot entry, fragment shape fixed at compile time: MT m-tiles of 8 X variants, NT n-tiles of 4 Y variants
+// The FP64 MMA has a dependent-issue latency of ~200 cycles on B200 (measured; a DFMA has ~10), so the two k-steps of a
+// tile go to SEPARATE accumulators: 8 independent DMMAs per entry, one latency instead of two.
+// f[4 t + {0,1,2,3}] = {re, im of k-step 0, re, im of k-step 1} of tile t = mt * NT + nt
 template <int MT, int NT>
-__device__ __forceinline__ void p3_entry(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
-                                         double2* __restrict__ acc, bool first, int r, int c)
+__device__ __forceinline__ void p3_issue(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
+                                         int r, int c, double (&f)[16])
 {
     double2 xa[MT];
     double b0[NT], b1[NT];
@@ -230,25 +235,51 @@ __device__ __forceinline__ void p3_entry(const double2* __restrict__ stage, cons
         b0[nt] = (r & 1) ? y.y : y.x;            // k-step 0: A = Re X
         b1[nt] = (r & 1) ? y.x : -y.y;           // k-step 1: A = Im X
     }
-    double c0[MT][NT], c1[MT][NT];
 #pragma unroll
-    for (int mt = 0; mt < MT; mt++)
-#pragma unroll
-        for (int nt = 0; nt < NT; nt++) { c0[mt][nt] = 0.0; c1[mt][nt] = 0.0; dmma884(c0[mt][nt], c1[mt][nt], xa[mt].x, b0[nt]); }
-#pragma unroll
-    for (int mt = 0; mt < MT; mt++)
-#pragma unroll
-        for (int nt = 0; nt < NT; nt++) dmma884(c0[mt][nt], c1[mt][nt], xa[mt].y, b1[nt]);
-    const double sgn = ((e.z >> 18) & 1) ? -1.0 : 1.0;
+    for (int i = 0; i < 16; i++) f[i] = 0.0;
 #pragma unroll
     for (int mt = 0; mt < MT; mt++)
 #pragma unroll
         for (int nt = 0; nt < NT; nt++) {
-            const int idx = ((e.y >> (8 * mt)) & 0xFF) ^ ((e.z >> (8 * nt)) & 0xFF);
-            double2 v = make_double2(0.0, 0.0);
-            if (!first) v = acc[idx];
-            v.x = fma(sgn, c0[mt][nt], v.x); v.y = fma(sgn, c1[mt][nt], v.y);
-            acc[idx] = v;
+            const int t = mt * NT + nt;
+            dmma884(f[4 * t], f[4 * t + 1], xa[mt].x, b0[nt]);
+            dmma884(f[4 * t + 2], f[4 * t + 3], xa[mt].y, b1[nt]);
+        }
+}
+
+__device__ __forceinline__ void p3_issue_any(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
+                                             int r, int c, double (&f)[16])
+{
+    switch ((e.z >> 16) & 3) {
+        case 0: p3_issue<4, 1>(stage, area, e, r, c, f); break;
+        case 1: p3_issue<2, 2>(stage, area, e, r, c, f); break;
+        case 2: p3_issue<2, 1>(stage, area, e, r, c, f); break;
+        default: p3_issue<1, 2>(stage, area, e, r, c, f); break;
+    }
+}
+
+// add the fragments of one entry into the flow's accumulator (all loads first: the slots of one entry are distinct)
+__device__ __forceinline__ void p3_update(const uint4 e, const double (&f)[16], double2* __restrict__ acc, bool first)
+{
+    const int shape = (e.z >> 16) & 3;
+    const bool nt2 = shape & 1;                  // shapes (2,2) and (1,2) have two n-tiles
+    const int ntile = shape < 2 ? 4 : 2;
+    const double sgn = ((e.z >> 18) & 1) ? -1.0 : 1.0;
+    int idx[4];
+    double2 v[4];
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+        const int mt = nt2 ? (t >> 1) : t, nt = nt2 ? (t & 1) : 0;
+        idx[t] = ((e.y >> (8 * mt)) & 0xFF) ^ ((e.z >> (8 * nt)) & 0xFF);
+        v[t] = make_double2(0.0, 0.0);
+        if (!first && t < ntile) v[t] = acc[idx[t]];
+    }
+#pragma unroll
+    for (int t = 0; t < 4; t++)
+        if (t < ntile) {
+            v[t].x = fma(sgn, f[4 * t] + f[4 * t + 2], v[t].x);
+            v[t].y = fma(sgn, f[4 * t + 1] + f[4 * t + 3], v[t].y);
+            acc[idx[t]] = v[t];
         }
 }
 
@@ -276,22 +307,29 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
         double2* __restrict__ acc = accs + (s << d.npar);
         const uint4* __restrict__ p = tab + s * sstride;
         const int nent = (int)(cur.z >> 24), jamp = (int)cur.w;
+        const long long tp0 = a.prof ? clock64() : 0;
+        int posr[4];                                        // rows of this lane's helicity combinations (write-out below)
+#pragma unroll
+        for (int j = 0; j < 4; j++) posr[j] = lane + 32 * j < nh ? a.d_pos[lane + 32 * j] : -1;
+        // records are fetched three entries ahead: the L2 latency of the record stream under load (~1000+ cycles,
+        // measured with MG_HS_PROFILE) is several entry times
         uint4 en = cur;
+        uint4 enn = __ldg(p + 32 * (nent > 1 ? 1 : 0));
+        uint4 en2 = __ldg(p + 32 * (nent > 2 ? 2 : nent - 1));
         for (int k = 0; k < nent; k++) {
-            const uint4 enn = __ldg(p + 32 * (k + 1 < nent ? k + 1 : k));
-            switch ((en.z >> 16) & 3) {
-                case 0: p3_entry<4, 1>(stage, area, en, acc, k == 0, r, c); break;
-                case 1: p3_entry<2, 2>(stage, area, en, acc, k == 0, r, c); break;
-                case 2: p3_entry<2, 1>(stage, area, en, acc, k == 0, r, c); break;
-                default: p3_entry<1, 2>(stage, area, en, acc, k == 0, r, c); break;
-            }
+            const uint4 en3 = __ldg(p + 32 * (k + 3 < nent ? k + 3 : nent - 1));
+            double f[16];
+            p3_issue_any(stage, area, en, r, c, f);
+            p3_update(en, f, acc, k == 0);
             __syncwarp();
-            en = enn;
+            en = enn; enn = en2; en2 = en3;
         }
+        const long long tp1 = a.prof ? clock64() : 0;
         // the finished jamp of this colour flow, all helicity combinations
         T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
-        for (int h = lane; h < nh; h += 32) {
-            const int pos = a.d_pos[h];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int h = lane + 32 * j, pos = posr[j];
             if (pos >= 0) {
                 const double2 v = acc[acc_swizzle(h)];
                 const size_t row = (size_t)e * a.nrow_evt + pos;
@@ -305,6 +343,7 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
             }
         }
         __syncwarp();
+        if (a.prof && lane == 0) { atomicAdd(a.prof + 6, (unsigned long long)(tp1 - tp0)); atomicAdd(a.prof + 7, (unsigned long long)(clock64() - tp1)); }
         s = sn; cur = nxt;
     }
 }
@@ -326,6 +365,8 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
     const int nh = 1 << d.npar;
     const int h = tid & (nh - 1), split = tid >> d.npar, nsplit = nth >> d.npar;
     const int pos = a.d_pos[h];                       // row of this helicity inside the event, -1 = not a good helicity
+    long long tprof = a.prof ? clock64() : 0;
+#define HS_PROF(i) do { if (a.prof && tid == 0) { const long long t_ = clock64(); atomicAdd(a.prof + (i), (unsigned long long)(t_ - tprof)); tprof = t_; } } while (0)
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
         // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
         for (int i = tid; i < 4 * d.npar; i += nth) pm[i] = a.mom[(size_t)e * (4 * d.npar) + i];
@@ -341,6 +382,7 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
             Ks[4 * s] = k0; Ks[4 * s + 1] = k1; Ks[4 * s + 2] = k2; Ks[4 * s + 3] = k3;
         }
         __syncthreads();
+        HS_PROF(0);
         // phase 1: objects, level by level
         for (int lvl = 0; lvl < 3; lvl++) {
             for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += nth) {
@@ -353,6 +395,7 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
             }
             __syncthreads();
         }
+        HS_PROF(1);
         const size_t row = (size_t)e * a.nrow_evt + pos;
         for (int g = 0; g < d.ngroups; g++) {
             const int4 g0 = __ldg(d.group + 2 * g), g1 = __ldg(d.group + 2 * g + 1);
@@ -378,11 +421,13 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                     wf<double> acc;
 #pragma unroll
                     for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
-                    uint4 en = cur;
+                    uint4 en = cur;                             // records are fetched three terms ahead (L2 latency under load)
+                    uint4 enn = __ldg(p + 32 * (ntm > 1 ? 1 : 0));
+                    uint4 en2 = __ldg(p + 32 * (ntm > 2 ? 2 : ntm - 1));
                     for (int k = 0; k < ntm; k++) {
-                        const uint4 enn = __ldg(p + 32 * (k + 1 < ntm ? k + 1 : k));
+                        const uint4 en3 = __ldg(p + 32 * (k + 3 < ntm ? k + 3 : ntm - 1));
                         eval_x_term(area, Ks, en, acc);
-                        en = enn;
+                        en = enn; enn = en2; en2 = en3;
                     }
                     if ((cur.z & 0xFF) != 0xFF) {
                         const int bs = (int)(cur.y >> 16);
@@ -393,7 +438,9 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                     u = un; cur = nxt;
                 }
             }
+            HS_PROF(2);
             __syncthreads();
+            HS_PROF(3);
             if (tid == 0) ctr[0] = 0;                 // every warp has left the loop above; next use is after the barrier below
             // phase 3: the jamps of this group, one colour flow at a time
             if (d.nw3 > 0) {
@@ -428,7 +475,9 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
                     }
                 }
             }
+            HS_PROF(4);
             __syncthreads();
+            HS_PROF(5);
             if (tid == 0) ctr[1] = 0;
         }
     }
@@ -599,8 +648,29 @@ cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, in
         smem += sizeof(double2) * ((size_t)d.nw3 << d.npar);
     }
     const int grid = a.nevt;                         // one CTA per event; the hardware scheduler keeps every SM full
-    if (jamps_fp64) hs_diagrams_kernel<double><<<grid, threads, smem, st>>>(d, a);
-    else hs_diagrams_kernel<float><<<grid, threads, smem, st>>>(d, a);
+    // diagnostics: MG_HS_PROFILE=1 prints the share of each phase as seen by thread 0 of every CTA (synchronises)
+    static const bool profile = getenv("MG_HS_PROFILE") != nullptr;
+    HsLaunch al = a;
+    al.prof = nullptr;
+    if (profile) {
+        static unsigned long long* buf = nullptr;
+        if (!buf) cudaMallocManaged(&buf, 8 * sizeof(unsigned long long));
+        cudaDeviceSynchronize();
+        for (int i = 0; i < 8; i++) buf[i] = 0;
+        al.prof = buf;
+    }
+    if (jamps_fp64) hs_diagrams_kernel<double><<<grid, threads, smem, st>>>(d, al);
+    else hs_diagrams_kernel<float><<<grid, threads, smem, st>>>(d, al);
+    if (profile) {
+        cudaDeviceSynchronize();
+        double tot = 0;
+        for (int i = 0; i < 6; i++) tot += (double)al.prof[i];
+        fprintf(stderr, "[hs profile] setup %.1f%% | phase 1 %.1f%% | phase 2 work %.1f%% wait %.1f%% | phase 3 work %.1f%% wait %.1f%% | %.0f cycles/event\n",
+                100 * al.prof[0] / tot, 100 * al.prof[1] / tot, 100 * al.prof[2] / tot, 100 * al.prof[3] / tot, 100 * al.prof[4] / tot,
+                100 * al.prof[5] / tot, tot / a.nevt);
+        fprintf(stderr, "[hs profile] per colour flow: entries %.0f cycles, write-out %.0f cycles\n",
+                (double)al.prof[6] / ((double)a.nevt * c->t->ncolor), (double)al.prof[7] / ((double)a.nevt * c->t->ncolor));
+    }
     return cudaGetLastError();
 }
 

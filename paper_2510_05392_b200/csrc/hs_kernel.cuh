@@ -15,6 +15,7 @@ struct HsLaunch {
     long rows;             // row stride of the jamps buffer
     int tile_major;        // 1: [row / 128][2][ncolor][128] (one contiguous block per 128-row tile: TMA-friendly) instead
     double mt, wt;
+    unsigned long long* prof;   // DEVICE [8] or NULL: clock64 sums per phase as seen by thread 0 of every CTA (diagnostics)
 };
 
 struct HsContext;          // device copies of the tables
