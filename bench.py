@@ -26,6 +26,10 @@ sys.path.insert(0, ROOT)
 
 from paper_2510_05392_b200 import inputs  # noqa: E402
 
+# DRAM bytes per event of the diagram kernel from the committed ncu --set full capture (profiles/r1_summary.md:
+# dram__bytes_read.sum + dram__bytes_write.sum = 3.3 MB + 948.0 MB for 4096 events); algorithmic = the jamps, 245 760 B
+NCU_DRAM_BYTES_PER_EVENT = {("gg_ttxggg", "fp64"): (3.335168e6 + 947.964928e6) / 4096}
+
 HEADLINE = "gg_ttxggg"      # BASELINE.json configs[4]: the process the north star's roofline targets are set on
 METRIC = "matrix elements/sec"
 
@@ -232,7 +236,10 @@ def main():
         alg_flop += (2.0 * proc.ncolor * (proc.ncolor + 1) + 4.0 * proc.ncolor) * nevt * r["ngood"]   # fused triangular colour sum
     achieved = alg_flop / (diag_ms * 1e-3) * 1e-12
     roofline = {"bound": "alu", "kernel": "hs_diagrams_kernel" if shared else "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                "frac": achieved / fp64_peak if fp64_peak else None, "traffic": None,
+                "frac": achieved / fp64_peak if fp64_peak else None,
+                "traffic": (NCU_DRAM_BYTES_PER_EVENT[(process, args.precision)] * nevt
+                            if shared and (process, args.precision) in NCU_DRAM_BYTES_PER_EVENT else None),
+                "traffic_source": "ncu capture at 4096 events (profiles/r1_summary.md), scaled to this launch by the event count",
                 "peak_source": "fp64 FMA probe kernel measured in this run (mg_measure_peak, burst); "
                                "MEASURED_PEAKS.json holds no fp64 figure",
                 "flop_per_event_helicity": proc.diagram_flops, "kernel_ms": diag_ms,
