@@ -201,3 +201,42 @@ def test_full_size_sampled(B, process):
     ref = _oracle(process, mom[idx])
     assert _relerr(me[idx], ref).max() < 1e-10
     proc.close()
+
+
+@pytest.mark.parametrize("process", ["gg_ttxgg", "gg_ttxggg"])
+def test_full_size_sampled_mixed(B, process):
+    """mixed precision at BASELINE.json's full batch in bench.py's launch configuration (helicity-shared kernel, tile-major
+    jamps + tcgen05 colour sum for gg_ttxggg, ALU colour sum for gg_ttxgg); oracle on sampled events; ragged chunks too"""
+    nevt = inputs.PROCESSES[process]["nevt"]
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, "mixed")
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    assert np.isfinite(me).all() and (me > 0).all()
+    ns = 48 if process == "gg_ttxggg" else 256
+    rng = np.random.default_rng(2)
+    idx = np.unique(np.concatenate([np.arange(ns), np.arange(nevt - ns, nevt), rng.integers(0, nevt, ns)]))
+    err = _relerr(me[idx], _oracle(process, mom[idx]))
+    assert np.median(err) < 2e-4 and err.max() < 1e-3, (np.median(err), err.max())
+    # a jamps buffer smaller than the batch and a batch that is not a multiple of the chunk: same numbers
+    proc.set_option("jamp_chunk_mib", 64)
+    me2 = proc.sigma_batch(torch.from_numpy(mom[:5000 + 77]).cuda()).cpu().numpy()
+    assert _relerr(me2, me[:5077]).max() < 1e-12
+    proc.close()
+
+
+def test_mixed_color_sum_variants_agree(B):
+    """gg_ttxggg, mixed: tcgen05 split-TF32 colour sum (tile-major jamps) against the fp32 ALU kernel, and both phase-3
+    variants of the helicity-shared kernel"""
+    mom = inputs.momenta("gg_ttxggg", 203, seed=5)
+    d_mom = torch.from_numpy(mom).cuda()
+    ref = None
+    for opts in ({}, {"hs_color_alu": 1}, {"hs_phase3": 0}, {"hs_phase3": 0, "hs_color_alu": 1, "hs_split": 1}):
+        proc = B.init_process("gg_ttxggg", "mixed")
+        for k, v in opts.items():
+            proc.set_option(k, v)
+        me = proc.sigma_batch(d_mom).cpu().numpy()
+        if ref is None:
+            ref = me
+        else:
+            assert _relerr(me, ref).max() < 2e-5, opts
+        proc.close()
