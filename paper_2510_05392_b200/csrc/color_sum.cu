@@ -90,12 +90,19 @@ __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __res
     for (int j = 0; j < NT; j++) { cre[j][0] = cre[j][1] = cim[j][0] = cim[j][1] = 0.0; }
     const double* xre = X + row0 + ar;
     const double* xim = X + (long)ncolor * rows_padded + row0 + ar;
+    // the A fragments (jamps, streamed from HBM) are fetched two k-steps ahead; L stays in L1/L2
+    auto load_a = [&](int k0, double& are, double& aim) {
+        const int k = k0 + ak;
+        are = 0.0; aim = 0.0;
+        if (k < ncolor) { are = __ldg(xre + (long)k * rows_padded); aim = __ldg(xim + (long)k * rows_padded); }
+    };
+    double a_re, a_im, n_re, n_im, m_re, m_im;
+    load_a(0, a_re, a_im);
+    load_a(4, n_re, n_im);
 #pragma unroll 1
     for (int k0 = 0; k0 < NCP; k0 += 4) {
-        const int k = k0 + ak;
-        double a_re = 0.0, a_im = 0.0;
-        if (k < ncolor) { a_re = __ldg(xre + (long)k * rows_padded); a_im = __ldg(xim + (long)k * rows_padded); }
-        const double* lrow = L + (long)k * NCP + ar;      // b = L[k0 + lane%4][8j + lane/4]
+        load_a(k0 + 8, m_re, m_im);
+        const double* lrow = L + (long)(k0 + ak) * NCP + ar;      // b = L[k0 + lane%4][8j + lane/4]
 #pragma unroll
         for (int j = 0; j < NT; j++) {
             if (8 * j <= k0 + 3) {                            // lower-triangular: columns 8j.. need k >= 8j
@@ -104,6 +111,7 @@ __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __res
                 dmma(cim[j][0], cim[j][1], a_im, b);
             }
         }
+        a_re = n_re; a_im = n_im; n_re = m_re; n_im = m_im;
     }
     double s = 0.0;
 #pragma unroll
