@@ -209,31 +209,32 @@ __device__ __forceinline__ int acc_swizzle(int h)
 // helicity.  Entries of one colour flow have different leg partitions, so the fragments are added into a per-warp
 // accumulator in shared memory indexed by the helicity combination (swizzled; tables hdep) and the finished jamp is
 // written once, coalesced over helicities.
-// Phase-3 record of (colour flow, entry k, lane), built on the host (hs_create):
-//   x = block of X variant (lane / 4) | block of Y variant (lane / 8) << 16     (m-tile mt adds 8, n-tile nt adds 4 blocks)
-//   y = accumulator index parts of the X variants 8 mt + lane / 4, one byte per m-tile (tables hdep)
-//   z = accumulator index parts of the Y variants 4 nt + lane % 4 (bytes 0, 1) | shape << 16 | negative << 18 |
-//       number of entries of the flow << 24;  shape 0: (MT, NT) = (4, 1), 1: (2, 2), 2: (2, 1), 3: (1, 2)
+// Phase-3 record of (colour flow, entry k, lane), built on the host (hs_create); everything a lane needs is
+// precomputed so that an entry costs few integer instructions (a warp with phase-3 work runs almost alone on its
+// scheduler, so its time is instructions x dependent latency):
+//   x = 16-byte slot of X variant (lane / 4), component (lane % 4), m-tile 0 (m-tile mt adds 32 slots: same swizzle)
+//       | slot of Y variant (lane / 8), n-tile 0 << 16
+//   y = slot of Y, n-tile 1 | shape << 16 | negative << 18 | number of entries of the flow << 24
+//       shape 0: (MT, NT) = (4, 1), 1: (2, 2), 2: (2, 1), 3: (1, 2)
+//   z = accumulator slots of this lane's complex number in tiles 0..3, one byte each (tile t = mt * NT + nt)
 //   w = jamp index of the flow
-// one dot entry, fragment shape fixed at compile time: MT m-tiles of 8 X variants, NT n-tiles of 4 Y variants
-// The FP64 MMA has a dependent-issue latency of ~200 cycles on B200 (measured; a DFMA has ~10), so the two k-steps of a
-// tile go to SEPARATE accumulators: 8 independent DMMAs per entry, one latency instead of two.
-// f[4 t + {0,1,2,3}] = {re, im of k-step 0, re, im of k-step 1} of tile t = mt * NT + nt
+// The FP64 MMA has a dependent-issue latency of ~200 cycles on B200 (measured; a DFMA has ~10), so the two k-steps of
+// a tile go to SEPARATE accumulators: f[4 t + {0,1}] = sum_c Re X (Re Y | Im Y), f[4 t + {2,3}] = sum_c Im X (Im Y | Re Y),
+// re = f[4t] - f[4t+2], im = f[4t+1] + f[4t+3]  (no negated operand, no select: a lane loads its 8-byte halves directly).
 template <int MT, int NT>
 __device__ __forceinline__ void p3_issue(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
-                                         int r, int c, double (&f)[16])
+                                         int o0, double (&f)[16])
 {
+    const double2* __restrict__ xp = stage + (e.x & 0xFFFF);
     double2 xa[MT];
     double b0[NT], b1[NT];
-    const int xb = e.x & 0xFFFF, yb = e.x >> 16;
 #pragma unroll
-    for (int mt = 0; mt < MT; mt++) { const int b = xb + 8 * mt; xa[mt] = stage[4 * b + (c ^ ((b >> 1) & 3))]; }
+    for (int mt = 0; mt < MT; mt++) xa[mt] = xp[32 * mt];
 #pragma unroll
     for (int nt = 0; nt < NT; nt++) {
-        const int b = yb + 4 * nt;
-        const double2 y = area[4 * b + (c ^ ((b >> 1) & 3))];
-        b0[nt] = (r & 1) ? y.y : y.x;            // k-step 0: A = Re X
-        b1[nt] = (r & 1) ? y.x : -y.y;           // k-step 1: A = Im X
+        const char* yp = reinterpret_cast<const char*>(area + (nt == 0 ? (e.x >> 16) : (e.y & 0xFFFF)));
+        b0[nt] = *reinterpret_cast<const double*>(yp + o0);           // odd column (im out): Im Y, even: Re Y
+        b1[nt] = *reinterpret_cast<const double*>(yp + (8 - o0));     // odd column: Re Y, even: Im Y
     }
 #pragma unroll
     for (int i = 0; i < 16; i++) f[i] = 0.0;
@@ -247,40 +248,35 @@ __device__ __forceinline__ void p3_issue(const double2* __restrict__ stage, cons
         }
 }
 
-__device__ __forceinline__ void p3_issue_any(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
-                                             int r, int c, double (&f)[16])
+// add the fragments of one entry into the flow's accumulator (all loads first: the slots of one entry are distinct)
+template <int NTILE>
+__device__ __forceinline__ void p3_update(const uint4 e, const double (&f)[16], double2* __restrict__ acc, bool first)
 {
-    switch ((e.z >> 16) & 3) {
-        case 0: p3_issue<4, 1>(stage, area, e, r, c, f); break;
-        case 1: p3_issue<2, 2>(stage, area, e, r, c, f); break;
-        case 2: p3_issue<2, 1>(stage, area, e, r, c, f); break;
-        default: p3_issue<1, 2>(stage, area, e, r, c, f); break;
+    const double sgn = ((e.y >> 18) & 1) ? -1.0 : 1.0;
+    double2 v[NTILE];
+#pragma unroll
+    for (int t = 0; t < NTILE; t++) {
+        v[t] = make_double2(0.0, 0.0);
+        if (!first) v[t] = acc[(e.z >> (8 * t)) & 0xFF];
+    }
+#pragma unroll
+    for (int t = 0; t < NTILE; t++) {
+        v[t].x = fma(sgn, f[4 * t] - f[4 * t + 2], v[t].x);
+        v[t].y = fma(sgn, f[4 * t + 1] + f[4 * t + 3], v[t].y);
+        acc[(e.z >> (8 * t)) & 0xFF] = v[t];
     }
 }
 
-// add the fragments of one entry into the flow's accumulator (all loads first: the slots of one entry are distinct)
-__device__ __forceinline__ void p3_update(const uint4 e, const double (&f)[16], double2* __restrict__ acc, bool first)
+__device__ __forceinline__ void p3_entry(const double2* __restrict__ stage, const double2* __restrict__ area, const uint4 e,
+                                         int o0, double2* __restrict__ acc, bool first)
 {
-    const int shape = (e.z >> 16) & 3;
-    const bool nt2 = shape & 1;                  // shapes (2,2) and (1,2) have two n-tiles
-    const int ntile = shape < 2 ? 4 : 2;
-    const double sgn = ((e.z >> 18) & 1) ? -1.0 : 1.0;
-    int idx[4];
-    double2 v[4];
-#pragma unroll
-    for (int t = 0; t < 4; t++) {
-        const int mt = nt2 ? (t >> 1) : t, nt = nt2 ? (t & 1) : 0;
-        idx[t] = ((e.y >> (8 * mt)) & 0xFF) ^ ((e.z >> (8 * nt)) & 0xFF);
-        v[t] = make_double2(0.0, 0.0);
-        if (!first && t < ntile) v[t] = acc[idx[t]];
+    double f[16];
+    switch ((e.y >> 16) & 3) {
+        case 0: p3_issue<4, 1>(stage, area, e, o0, f); p3_update<4>(e, f, acc, first); break;
+        case 1: p3_issue<2, 2>(stage, area, e, o0, f); p3_update<4>(e, f, acc, first); break;
+        case 2: p3_issue<2, 1>(stage, area, e, o0, f); p3_update<2>(e, f, acc, first); break;
+        default: p3_issue<1, 2>(stage, area, e, o0, f); p3_update<2>(e, f, acc, first); break;
     }
-#pragma unroll
-    for (int t = 0; t < 4; t++)
-        if (t < ntile) {
-            v[t].x = fma(sgn, f[4 * t] + f[4 * t + 2], v[t].x);
-            v[t].y = fma(sgn, f[4 * t + 1] + f[4 * t + 3], v[t].y);
-            acc[idx[t]] = v[t];
-        }
 }
 
 template <typename T2>
@@ -289,7 +285,7 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
                                             const int4 g1, int* ctr, int lane)
 {
     const int nh = 1 << d.npar;
-    const int r = lane >> 2, c = lane & 3;
+    const int o0 = ((lane >> 2) & 1) * 8;                  // B-fragment column parity: which 8-byte half of Y is k-step 0
     const size_t sstride = (size_t)d.maxe * 32;
     const uint4* __restrict__ tab = d.p3tab + (size_t)g0.w * sstride + lane;
     // colour flows of the group are handed to the warps dynamically; flow s owns accumulator s (g1.x <= nw3)
@@ -306,7 +302,7 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
         if (sn < g1.x) nxt = __ldg(tab + sn * sstride);
         double2* __restrict__ acc = accs + (s << d.npar);
         const uint4* __restrict__ p = tab + s * sstride;
-        const int nent = (int)(cur.z >> 24), jamp = (int)cur.w;
+        const int nent = (int)(cur.y >> 24), jamp = (int)cur.w;
         const long long tp0 = a.prof ? clock64() : 0;
         int posr[4];                                        // rows of this lane's helicity combinations (write-out below)
 #pragma unroll
@@ -318,9 +314,7 @@ __device__ __forceinline__ void phase3_dmma(const HsDev& d, const HsLaunch& a, c
         uint4 en2 = __ldg(p + 32 * (nent > 2 ? 2 : nent - 1));
         for (int k = 0; k < nent; k++) {
             const uint4 en3 = __ldg(p + 32 * (k + 3 < nent ? k + 3 : nent - 1));
-            double f[16];
-            p3_issue_any(stage, area, en, r, c, f);
-            p3_update(en, f, acc, k == 0);
+            p3_entry(stage, area, en, o0, acc, k == 0);
             __syncwarp();
             en = enn; enn = en2; en2 = en3;
         }
@@ -593,15 +587,17 @@ cudaError_t hs_create(int ngluon, HsContext** out)
                 else if (nvx == 8 && nvy == 8) shape = 3;
                 else { cudaFree(c->p2tab); cudaFree(c->blob); delete c; return cudaErrorInvalidValue; }
                 const int MT = nvx / 8, NT = nvy / 4;
+                auto slot_of = [](int off, int var, int comp) { const int bb = (off >> 2) + var; return 4 * bb + (comp ^ ((bb >> 1) & 3)); };
                 for (int l = 0; l < 32; l++) {
                     const int r = l >> 2, cc = l & 3;
                     uint4& rec = tab[((size_t)sgi * maxe + k) * 32 + l];
-                    rec.x = (unsigned)((xoff >> 2) + r) | ((unsigned)((yoff >> 2) + (r >> 1)) << 16);
-                    rec.y = 0;
-                    for (int mt = 0; mt < MT; mt++) rec.y |= (unsigned)hd[8 * mt + r] << (8 * mt);
+                    const unsigned ys1 = NT == 2 ? (unsigned)slot_of(yoff, 4 + (r >> 1), cc) : 0u;
+                    rec.x = (unsigned)slot_of(xoff, r, cc) | ((unsigned)slot_of(yoff, r >> 1, cc) << 16);
+                    rec.y = ys1 | (shape << 16) | ((E[3] < 0 ? 1u : 0u) << 18) | ((unsigned)S[2] << 24);
                     rec.z = 0;
-                    for (int nt = 0; nt < NT; nt++) rec.z |= (unsigned)hd[32 + 4 * nt + cc] << (8 * nt);
-                    rec.z |= (shape << 16) | ((E[3] < 0 ? 1u : 0u) << 18) | ((unsigned)S[2] << 24);
+                    for (int mt = 0; mt < MT; mt++)
+                        for (int nt = 0; nt < NT; nt++)
+                            rec.z |= (unsigned)(hd[8 * mt + r] ^ hd[32 + 4 * nt + cc]) << (8 * (mt * NT + nt));
                     rec.w = (unsigned)S[0];
                 }
             }
