@@ -169,21 +169,25 @@ __device__ __forceinline__ void eval_x_term(const double2* __restrict__ area, co
 {
     const int op = e.z & 0xFF;
     if (op == 0xFF) return;
+    const double sg = ((e.z >> 8) & 1) ? -1.0 : 1.0;
+    // the accumulation is repeated in every case (no merge of the per-case result registers), and the index lowering of
+    // the raw vertices (components 1-3 negated) is folded into its sign
+    auto add = [&](const wf<double>& r, double s123) {
+        acc.c[0].re = fma(sg, r.c[0].re, acc.c[0].re); acc.c[0].im = fma(sg, r.c[0].im, acc.c[0].im);
+#pragma unroll
+        for (int c = 1; c < 4; c++) { acc.c[c].re = fma(s123, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(s123, r.c[c].im, acc.c[c].im); }
+    };
     wf<double> A, B, r;
     load_blk(area, e.x & 0xFFFF, A);
     load_blk(area, e.x >> 16, B);
     switch (op) {
-        case 11: v3_raw(A, load_k(Ks, (e.z >> 16) & 0xFF), B, load_k(Ks, (e.z >> 24) & 0xFF), r); break;
-        case 12: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4_raw(A, B, Z, r); break; }
-        case 13: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4s_raw(A, B, Z, r); break; }
-        case 8: row_slash(A, make_slashed(B), r); break;
-        case 9: slash_col(make_slashed(A), B, r); break;
-        default: ffv_p_raw(A, B, r); break;                 // 10: x_bil
+        case 11: v3_raw(A, load_k(Ks, (e.z >> 16) & 0xFF), B, load_k(Ks, (e.z >> 24) & 0xFF), r); add(r, -sg); break;
+        case 12: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4_raw(A, B, Z, r); add(r, -sg); break; }
+        case 13: { wf<double> Z; load_blk(area, e.y & 0xFFFF, Z); v4s_raw(A, B, Z, r); add(r, -sg); break; }
+        case 8: row_slash(A, make_slashed(B), r); add(r, sg); break;
+        case 9: slash_col(make_slashed(A), B, r); add(r, sg); break;
+        default: ffv_p_raw(A, B, r); add(r, -sg); break;                 // 10: x_bil
     }
-    if (op >= 10) lower(r);
-    const double sg = ((e.z >> 8) & 1) ? -1.0 : 1.0;
-#pragma unroll
-    for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
 }
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
