@@ -27,8 +27,8 @@ sys.path.insert(0, ROOT)
 from paper_2510_05392_b200 import inputs  # noqa: E402
 
 # DRAM bytes per event of the diagram kernel from the committed ncu --set full capture (profiles/r1_summary.md:
-# dram__bytes_read.sum + dram__bytes_write.sum = 3.3 MB + 948.0 MB for 4096 events); algorithmic = the jamps, 245 760 B
-NCU_DRAM_BYTES_PER_EVENT = {("gg_ttxggg", "fp64"): (3.335168e6 + 947.964928e6) / 4096}
+# dram__bytes_read.sum + dram__bytes_write.sum = 3.3 MB + 948.3 MB for 4096 events); algorithmic = the jamps, 245 760 B
+NCU_DRAM_BYTES_PER_EVENT = {("gg_ttxggg", "fp64"): (3.291648e6 + 948.265216e6) / 4096}
 
 HEADLINE = "gg_ttxggg"      # BASELINE.json configs[4]: the process the north star's roofline targets are set on
 METRIC = "matrix elements/sec"
