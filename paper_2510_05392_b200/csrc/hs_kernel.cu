@@ -1,13 +1,13 @@
-// hs_kernel.cu -- helicity-shared diagram kernel: one CTA = one event, one thread =
-// one helicity combination; interprets the tables of gen/co_program.py (layout: hs_tables.h).
+// hs_kernel.cu -- helicity-shared diagram kernel: one CTA = one event; interprets the tables of
+// gen/co_program.py (layout: hs_tables.h) and the record streams hs_create builds from them.
 //
-// Why this shape on B200: the paper keeps one thread per (event, helicity) and lets
-// every helicity recompute every wavefunction, with up to 121 wavefunctions + 120 jamps of per-thread state
-// -- 12 KB per thread, i.e. local-memory traffic.  Here the state that depends on
-// few helicities lives once per event in shared memory (<= 8 variants per object), the per-helicity work is a
-// stream of 4-component complex dot products whose operands are broadcast reads of shared memory, and every
-// jamp is finished in registers and written once, coalesced, to the jamps buffer [2][ncolor][rows]
-// with rows ordered (event, helicity).
+// Why this shape on B200: the paper keeps one thread per (event, helicity) and lets every helicity
+// recompute every wavefunction, with up to 121 wavefunctions + 120 jamps of per-thread state (PAPER.md:101-119, 141,
+// 187) -- 12 KB per thread, i.e. local-memory traffic.  Here the state that depends on few helicities lives once per
+// event in shared memory (<= 8 variants per object; phase 1), the vertices are contracted with all branches but the
+// largest once per variant (phase 2, work units handed to warps dynamically), and the per-helicity work is a stream of
+// 4-component complex dot products evaluated for all helicities at once on the FP64 tensor path (phase 3).  Every
+// jamp is finished on chip and written once, coalesced, to the jamps buffer, rows ordered (event, helicity).
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
