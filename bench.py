@@ -183,6 +183,8 @@ def main():
     ap.add_argument("--hs-phase3", type=int, default=None, help="helicity-shared kernel, jamp dot products: 0 scalar ALUs, 1 FP64 tensor path")
     ap.add_argument("--chunk-mib", type=int, default=None, help="jamps buffer size inside the workspace")
     ap.add_argument("--no-extras", action="store_true", help="skip per-process table, e2e and cpu baseline")
+    ap.add_argument("--ramp", action="store_true",
+                    help="also report MEs/s against the number of events per batch, 32 ... full (the paper's small-grid curves, PAPER.md:174, 225)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
     if args.impl == "reference":
@@ -262,6 +264,14 @@ def main():
                                                          "helicity_sum": r["stage_ms"][2]},
            "roofline": roofline, "clocks": clocks}
 
+    if rank == 0 and args.ramp:
+        ramp, n = {}, 32
+        while n <= nevt:
+            q = time_process(torch, B, process, args.precision, n, 5, 3, 0, 1, flush, opts)
+            ramp[str(n)] = q["value"]
+            q["proc"].close()
+            n *= 4
+        out["ramp_MEs_per_s"] = ramp
     if rank == 0 and not args.no_extras:
         # end to end through the host-buffer entry point: pinned host momenta -> device -> me -> host, every step
         hm = torch.from_numpy(r["mom_h"]).pin_memory()
