@@ -76,7 +76,8 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
 /* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
  * MG_DIAG_THREAD kernel, multiple of 32, <= 256), "hs_split" (threads per helicity of the MG_DIAG_SHARED kernel: 1, 2, 4),
  * "hs_color_alu" (MG_DIAG_SHARED in MG_MIXED: 1 = scalar-ALU fp32 colour-sum kernel instead of the tcgen05 one),
- * "hs_phase3" (jamp dot products of the MG_DIAG_SHARED kernel: 0 = scalar FP64 ALUs, 1 = FP64 tensor path, needs npar >= 6),
+ * "hs_phase3" (jamp dot products of the MG_DIAG_SHARED kernel: 0 = scalar FP64 ALUs, 1 = FP64 tensor path, 2 = FP64 tensor
+ * path with the jamps of one group of colour flows overlapped with the vertices of the next; 1 and 2 need npar >= 6),
  * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1).
  * Unknown key or bad value -> MG_EINVAL. */
 int mg_set_option(mg_process* p, const char* key, int value);

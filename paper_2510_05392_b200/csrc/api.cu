@@ -254,8 +254,8 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         if (value * p->d->ncomb > 256) return fail(p, MG_EINVAL, "hs_split * ncomb must be <= 256");
         p->hs_split = value;
     } else if (!strcmp(key, "hs_phase3")) {
-        if (value != 0 && value != 1) return fail(p, MG_EINVAL, "bad hs_phase3");
-        if (value == 1 && p->d->npar < 6) return fail(p, MG_EINVAL, "hs_phase3 = 1 needs >= 6 external particles");
+        if (value < 0 || value > 2) return fail(p, MG_EINVAL, "bad hs_phase3");
+        if (value >= 1 && p->d->npar < 6) return fail(p, MG_EINVAL, "hs_phase3 = 1, 2 need >= 6 external particles");
         p->hs_phase3 = value;
     } else if (!strcmp(key, "hs_color_alu")) {
         p->hs_color_alu = value != 0;

@@ -482,6 +482,145 @@ __global__ void __launch_bounds__(256) hs_diagrams_kernel(const HsDev d, const H
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Overlapped variant (hs_phase3 = 2): ONE 512-thread CTA per SM with a double-buffered staging area.  Phase 3 of group g
+// (few, long, latency-bound colour-flow units) and phase 2 of group g + 1 (many short units) are drawn from ONE work
+// queue, so that no warp idles while the colour flows of a group are finished; one barrier per group instead of two.
+__device__ __forceinline__ void p2_unit(const HsDev& d, const double2* __restrict__ area, double2* __restrict__ stagew,
+                                        const double* __restrict__ Ks, const int4 g0, int u, int lane)
+{
+    const size_t ustride = (size_t)d.maxt * 32;
+    const uint4* __restrict__ p = d.p2tab + ((size_t)(g0.y >> 5) + u) * ustride + lane;
+    const uint4 cur = __ldg(p);
+    const int ntm = (int)cur.w;
+    wf<double> acc;
+#pragma unroll
+    for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
+    uint4 en = cur;
+    uint4 enn = __ldg(p + 32 * (ntm > 1 ? 1 : 0));
+    uint4 en2 = __ldg(p + 32 * (ntm > 2 ? 2 : ntm - 1));
+    for (int k = 0; k < ntm; k++) {
+        const uint4 en3 = __ldg(p + 32 * (k + 3 < ntm ? k + 3 : ntm - 1));
+        eval_x_term(area, Ks, en, acc);
+        en = enn; enn = en2; en2 = en3;
+    }
+    if ((cur.z & 0xFF) != 0xFF) {
+        const int bs = (int)(cur.y >> 16);
+        const int sw = (bs >> 1) & 3;
+#pragma unroll
+        for (int c = 0; c < 4; c++) stagew[4 * bs + (c ^ sw)] = make_double2(acc.c[c].re, acc.c[c].im);
+    }
+}
+
+template <typename T2>
+__device__ __forceinline__ void p3_flow(const HsDev& d, const HsLaunch& a, const double2* __restrict__ area,
+                                        const double2* __restrict__ stager, double2* __restrict__ accs, int e, const int4 g0,
+                                        int s, int lane)
+{
+    const int nh = 1 << d.npar;
+    const int o0 = ((lane >> 2) & 1) * 8;
+    const uint4* __restrict__ p = d.p3tab + ((size_t)g0.w + s) * ((size_t)d.maxe * 32) + lane;
+    double2* __restrict__ acc = accs + (s << d.npar);
+    const uint4 cur = __ldg(p);
+    const int nent = (int)(cur.y >> 24), jamp = (int)cur.w;
+    int posr[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++) posr[j] = lane + 32 * j < nh ? a.d_pos[lane + 32 * j] : -1;
+    uint4 en = cur;
+    uint4 enn = __ldg(p + 32 * (nent > 1 ? 1 : 0));
+    uint4 en2 = __ldg(p + 32 * (nent > 2 ? 2 : nent - 1));
+    for (int k = 0; k < nent; k++) {
+        const uint4 en3 = __ldg(p + 32 * (k + 3 < nent ? k + 3 : nent - 1));
+        p3_entry(stager, area, en, o0, acc, k == 0);
+        __syncwarp();
+        en = enn; enn = en2; en2 = en3;
+    }
+    T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const int h = lane + 32 * j, pos = posr[j];
+        if (pos >= 0) {
+            const double2 v = acc[acc_swizzle(h)];
+            const size_t row = (size_t)e * a.nrow_evt + pos;
+            if (a.tile_major) {
+                T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)jamp * 128 + (row & 127);
+                o[0] = T2(v.x); o[(size_t)d.ncolor * 128] = T2(v.y);
+            } else {
+                out[(size_t)jamp * a.rows + row] = T2(v.x);
+                out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+template <typename T2>
+__global__ void __launch_bounds__(512, 1) hs_overlap_kernel(const HsDev d, const HsLaunch a)
+{
+    extern __shared__ double2 sm[];
+    __shared__ int ctr;
+    if (threadIdx.x == 0) ctr = 0;
+    double2* __restrict__ area = sm;
+    double2* __restrict__ stage0 = sm + d.obj_area;
+    double2* __restrict__ stage1 = stage0 + d.stage_area;
+    double2* __restrict__ accs = stage1 + d.stage_area;
+    double* __restrict__ Ks = reinterpret_cast<double*>(accs + (d.nw3 << d.npar));
+    double* __restrict__ pm = Ks + 4 * d.nlegsets;
+    const int tid = threadIdx.x, nth = blockDim.x, lane = tid & 31;
+    auto grab = [&]() { int u = 0; if (lane == 0) u = atomicAdd(&ctr, 1); return __shfl_sync(0xffffffffu, u, 0); };
+    for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
+        for (int i = tid; i < 4 * d.npar; i += nth) pm[i] = a.mom[(size_t)e * (4 * d.npar) + i];
+        __syncthreads();
+        for (int s = tid; s < d.nlegsets; s += nth) {
+            const int m = __ldg(d.legset_mask + s);
+            double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
+            for (int p = 0; p < d.npar; p++)
+                if ((m >> p) & 1) {
+                    const double sg = p < 2 ? 1.0 : -1.0;
+                    k0 += sg * pm[4 * p]; k1 += sg * pm[4 * p + 1]; k2 += sg * pm[4 * p + 2]; k3 += sg * pm[4 * p + 3];
+                }
+            Ks[4 * s] = k0; Ks[4 * s + 1] = k1; Ks[4 * s + 2] = k2; Ks[4 * s + 3] = k3;
+        }
+        __syncthreads();
+        for (int lvl = 0; lvl < 3; lvl++) {
+            for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += nth) {
+                const int it = __ldg(d.p1_items + i);
+                const int4 o = __ldg(d.obj + (it >> 8));
+                const int var = it & 0xFF;
+                wf<double> acc;
+                run_terms<false>(d, area, Ks, pm, o.z, o.w, var, o.y >> 8, a.mt, a.wt, acc);
+                store_obj(area, o.x, var, acc);
+            }
+            __syncthreads();
+        }
+        // prologue: pair objects of group 0
+        {
+            const int4 g0 = __ldg(d.group);
+            const int nu = g0.z >> 5;
+            for (int u = grab(); u < nu; u = grab()) p2_unit(d, area, stage0, Ks, g0, u, lane);
+        }
+        __syncthreads();
+        if (tid == 0) ctr = 0;
+        __syncthreads();
+        for (int g = 0; g < d.ngroups; g++) {
+            const int4 g0 = __ldg(d.group + 2 * g), g1 = __ldg(d.group + 2 * g + 1);
+            const double2* __restrict__ sr = (g & 1) ? stage1 : stage0;
+            double2* __restrict__ sw = (g & 1) ? stage0 : stage1;
+            int4 n0 = make_int4(0, 0, 0, 0);
+            if (g + 1 < d.ngroups) n0 = __ldg(d.group + 2 * (g + 1));
+            const int ns = g1.x, total = ns + (n0.z >> 5);
+            // colour flows first (long units), then the next group's pair objects
+            for (int u = grab(); u < total; u = grab()) {
+                if (u < ns) p3_flow<T2>(d, a, area, sr, accs, e, g0, u, lane);
+                else p2_unit(d, area, sw, Ks, n0, u - ns, lane);
+            }
+            __syncthreads();
+            if (tid == 0) ctr = 0;
+            __syncthreads();
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
 struct HsContext {
     const HsTables* t = nullptr;
     HsDev d;
@@ -491,6 +630,7 @@ struct HsContext {
     size_t smem = 0;
     int sms = 148;
     int max_sigma = 0;
+    size_t smem_overlap = 0;   // 0 = the overlapped variant does not fit / does not apply
 };
 
 const HsTables* hs_host_tables(const HsContext* c) { return c->t; }
@@ -621,6 +761,15 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     e = cudaFuncSetAttribute(hs_diagrams_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(hs_diagrams_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     if (e != cudaSuccess) { cudaFree(c->blob); delete c; return e; }
+    {
+        const size_t smem_ov = c->smem + sizeof(double2) * ((size_t)t->stage_area + ((size_t)c->max_sigma << t->npar));
+        if (t->npar >= 6 && smem_ov <= 226 * 1024) {
+            e = cudaFuncSetAttribute(hs_overlap_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ov);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(hs_overlap_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ov);
+            if (e != cudaSuccess) { cudaFree(c->blob); delete c; return e; }
+            c->smem_overlap = smem_ov;
+        }
+    }
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
@@ -642,6 +791,15 @@ cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, in
     if (nsplit < 1 || threads > 256) return cudaErrorInvalidValue;
     HsDev d = c->d;
     size_t smem = c->smem;
+    if (phase3 == 2) {                               // overlapped variant: one 512-thread CTA per SM
+        if (!c->smem_overlap) return cudaErrorInvalidValue;
+        d.nw3 = c->max_sigma;
+        HsLaunch al2 = a;
+        al2.prof = nullptr;
+        if (jamps_fp64) hs_overlap_kernel<double><<<a.nevt, 512, c->smem_overlap, st>>>(d, al2);
+        else hs_overlap_kernel<float><<<a.nevt, 512, c->smem_overlap, st>>>(d, al2);
+        return cudaGetLastError();
+    }
     if (phase3 == 1) {                               // FP64 tensor path: needs the 8 x 4 fragment shapes (>= 3 legs on the X side)
         if (c->t->npar < 6) return cudaErrorInvalidValue;
         d.nw3 = c->max_sigma;                        // one accumulator per colour flow of a group

@@ -86,8 +86,8 @@ def test_scheduling_variants_agree(B, process):
                  {"diagrams": 0, "color_sum": 1, "schedule": 1}, {"diagrams": 0, "block": 64},
                  {"diagrams": 1}, {"diagrams": 1, "hs_split": 2}, {"diagrams": 1, "jamp_chunk_mib": 1},
                  {"diagrams": 1, "hs_phase3": 0, "hs_split": 1}, {"diagrams": 1, "hs_phase3": 1, "hs_split": 1},
-                 {"diagrams": 1, "hs_phase3": 1, "hs_split": 2}):
-        if opts.get("hs_phase3") == 1 and process in ("gg_ttx", "gg_ttxg"):
+                 {"diagrams": 1, "hs_phase3": 1, "hs_split": 2}, {"diagrams": 1, "hs_phase3": 2}):
+        if opts.get("hs_phase3", 0) >= 1 and process in ("gg_ttx", "gg_ttxg"):
             continue                                   # the FP64 tensor path of phase 3 needs >= 6 external particles
         proc = B.init_process(process, "fp64")
         for k, v in opts.items():
