@@ -126,6 +126,47 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+def shard_first_event(rank, nevt_per_rank):
+    """weak scaling (events are independent): rank r evaluates the contiguous event
+    range [r * nevt, (r + 1) * nevt) of the seeded stream; no collective on the data path"""
+    return rank * nevt_per_rank
+
+
+def reduce_max_ms(ms, dist, device="cpu"):
+    """device time of the slowest rank (the one all-reduce of the run: a scalar, for the timing only)"""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def masks_agree(mask, dist, device="cpu"):
+    """the helicity mask is a property of the process (SURVEY.md §8(e)): every rank derives it from its own probe events;
+    True iff all ranks found the same one"""
+    if dist is None:
+        return True
+    import torch
+    m = torch.as_tensor(np.asarray(mask, dtype=np.int32), device=device)
+    lo, hi = m.clone(), m.clone()
+    dist.all_reduce(lo, op=dist.ReduceOp.MIN)
+    dist.all_reduce(hi, op=dist.ReduceOp.MAX)
+    return bool((lo == hi).all().item())
+
+
+def spawn_ranks(argv, gpus):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script under torch.distributed.run (one process
+    per GPU, rendezvous on 127.0.0.1) and hand their output through"""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd)
+
+
 def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world, flush, opts=None, dist=None):
     """returns dict with device-timed throughput of `steps` batches"""
     dev = torch.cuda.current_device()
@@ -133,9 +174,11 @@ def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world,
     for k, v in (opts or {}).items():
         proc.set_option(k, v)
     proc.set_option("timing", 1)
-    mom_h = inputs.momenta(process, nevt, seed=1, first_event=rank * nevt)
+    mom_h = inputs.momenta(process, nevt, seed=1, first_event=shard_first_event(rank, nevt))
     d_mom = torch.from_numpy(mom_h).to(f"cuda:{dev}")
     mask = proc.helicity_filter(d_mom)
+    if not masks_agree(mask, dist, f"cuda:{dev}"):
+        raise SystemExit("ranks disagree on the good-helicity mask")
     d_me = torch.empty(nevt, dtype=torch.float64, device=f"cuda:{dev}")
     for _ in range(warmup):
         proc.sigma_batch(d_mom, d_me)
@@ -155,10 +198,8 @@ def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world,
         stage += np.array(proc.last_stage_ms())
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in ev)
+    ms = reduce_max_ms(ms, dist, f"cuda:{dev}")
     if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{dev}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
         dist.barrier()
     launches_per_step = proc.last_launch_count()
     res = {"proc": proc, "ms_total": ms, "ms_per_step": ms / steps, "value": world * nevt * steps / (ms * 1e-3),
@@ -187,6 +228,12 @@ def main():
                     help="also report MEs/s against the number of events per batch, 32 ... full (the paper's small-grid curves, PAPER.md:174, 225)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        raise SystemExit(spawn_ranks(sys.argv[1:], args.gpus))
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE')}: launch one rank per GPU")
     if args.impl == "reference":
         return run_reference(args)
 
@@ -201,6 +248,8 @@ def main():
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")             # rank/transport lines (NVLink, NVLS) for whoever reads the log
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")  # stdout carries the JSON line only
         import torch.distributed as dist_
         dist_.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
         dist = dist_

@@ -100,22 +100,33 @@ def test_emitted_code_on_host_matches_ir(host_jamps, name, n):
 
 
 def test_two_rank_sharding_gloo(tmp_path):
-    """N > 1 path of bench.py on CPU: gloo, world_size 2: disjoint event shards, max-over-ranks reduction"""
+    """N > 1 path of bench.py on CPU (gloo, world_size 2), calling bench.py's own functions: disjoint contiguous event
+    shards, the max-over-ranks reduction of the device time, and the agreement check of the helicity masks.  The masks
+    themselves come from the oracle's per-helicity terms on each rank's own probe events with the 1e-8 rule of reading A5:
+    a property of the process, the same on every shard."""
     script = tmp_path / "w.py"
     script.write_text(f"""
 import os, sys
 sys.path.insert(0, {ROOT!r})
 import numpy as np, torch, torch.distributed as dist
+import bench, oracle
 from paper_2510_05392_b200 import inputs
 dist.init_process_group('gloo')
 rank, world = dist.get_rank(), dist.get_world_size()
 nevt = 64
-mom = inputs.momenta('gg_ttx', nevt, seed=1, first_event=rank * nevt)      # weak scaling: each rank its own events
+first = bench.shard_first_event(rank, nevt)
+assert first == rank * nevt
+mom = inputs.momenta('gg_ttx', nevt, seed=1, first_event=first)            # weak scaling: each rank its own events
 full = inputs.momenta('gg_ttx', nevt * world, seed=1)
 assert np.array_equal(mom, full[rank * nevt:(rank + 1) * nevt])
-t = torch.tensor([10.0 + rank], dtype=torch.float64)
-dist.all_reduce(t, op=dist.ReduceOp.MAX)
-assert t.item() == 10.0 + world - 1
+assert bench.reduce_max_ms(10.0 + rank, dist) == 10.0 + world - 1
+for process in ('epem_mupmum', 'gg_ttxg'):
+    m = inputs.momenta(process, nevt, seed=1, first_event=first)
+    me, meh = oracle.matrix_elements(process, m, inputs.PARAMS, per_helicity=True)
+    mask = (meh / me[:, None] > 1e-8).any(axis=0)
+    assert bench.masks_agree(mask, dist), process
+    bad = mask.copy(); bad[0] ^= (rank == 1)
+    assert not bench.masks_agree(bad, dist)
 dist.barrier()
 if rank == 0:
     print('OK', world)
@@ -126,3 +137,19 @@ dist.destroy_process_group()
                        capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stderr[-2000:]
     assert "OK 2" in r.stdout
+
+
+def test_bench_gpus_flag_spawns_ranks_and_fails_loudly_without_gpu():
+    """`python bench.py --gpus 2` starts two ranks itself; on a CPU box every rank refuses to run (no fallback)"""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"], capture_output=True,
+                       text=True, timeout=300, env=env)
+    assert r.returncode != 0
+    assert (r.stdout + r.stderr).count("no CPU fallback") >= 2
+    # a world size that contradicts --gpus is an error, not a silent single-GPU run
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4"], capture_output=True, text=True,
+                       timeout=120, env=dict(env, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0"))
+    assert r.returncode != 0 and "WORLD_SIZE" in (r.stdout + r.stderr)
