@@ -220,8 +220,6 @@ def main():
     ap.add_argument("--color-sum", type=int, default=None, help="0 fused ALU, 1 tensor-core kernel")
     ap.add_argument("--schedule", type=int, default=0, help="0 helicity in the grid, 1 helicity streams")
     ap.add_argument("--diagrams", type=int, default=None, help="0 thread per (event, helicity), 1 helicity-shared CTA per event")
-    ap.add_argument("--hs-split", type=int, default=None)
-    ap.add_argument("--hs-phase3", type=int, default=None, help="helicity-shared kernel, jamp dot products: 0 scalar ALUs, 1 FP64 tensor path")
     ap.add_argument("--chunk-mib", type=int, default=None, help="jamps buffer size inside the workspace")
     ap.add_argument("--no-extras", action="store_true", help="skip per-process table, e2e and cpu baseline")
     ap.add_argument("--ramp", action="store_true",
@@ -256,15 +254,13 @@ def main():
 
     process = args.process or HEADLINE
     nevt = args.nevt or inputs.PROCESSES[process]["nevt"]
-    opts = {"schedule": args.schedule}
+    opts = {}
+    if args.diagrams is not None:
+        opts["diagrams"] = args.diagrams           # before "schedule": streams exist for the thread kernel only
+    if args.schedule:
+        opts["schedule"] = args.schedule
     if args.color_sum is not None:
         opts["color_sum"] = args.color_sum
-    if args.diagrams is not None:
-        opts["diagrams"] = args.diagrams
-    if args.hs_split is not None:
-        opts["hs_split"] = args.hs_split
-    if args.hs_phase3 is not None:
-        opts["hs_phase3"] = args.hs_phase3
     if args.chunk_mib is not None:
         opts["jamp_chunk_mib"] = args.chunk_mib
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")

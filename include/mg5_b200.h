@@ -52,9 +52,9 @@ enum { MG_SCHED_GRID = 0, MG_SCHED_STREAMS = 1 };
 
 /* diagram stage:
  *   MG_DIAG_THREAD : one thread per (event, helicity), the paper's layout
- *   MG_DIAG_SHARED : one CTA per event, one thread per helicity; wavefunctions shared between helicities in shared
- *                    memory, jamps written to the workspace and contracted by the colour-sum kernel (gg processes,
- *                    MG_FP64 / MG_MIXED; default for >= 4 gluons) */
+ *   MG_DIAG_SHARED : one CTA per event, all helicities at once; wavefunctions shared between helicities in shared
+ *                    memory, jamps written to the workspace and contracted by the colour-sum kernel (g g -> t tbar +
+ *                    2 or 3 gluons, MG_FP64 / MG_MIXED; the default there) */
 enum { MG_DIAG_THREAD = 0, MG_DIAG_SHARED = 1 };
 
 /* Create a process.  name: "epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg" (BASELINE.json configs;
@@ -74,12 +74,11 @@ int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_f
 int mg_set_parameters(mg_process* p, const char* const* keys, const double* values, int n);
 
 /* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
- * MG_DIAG_THREAD kernel, multiple of 32, <= 256), "hs_split" (threads per helicity of the MG_DIAG_SHARED kernel: 1, 2, 4),
+ * MG_DIAG_THREAD kernel, multiple of 32, <= 256),
  * "hs_color_alu" (MG_DIAG_SHARED in MG_MIXED: 1 = scalar-ALU fp32 colour-sum kernel instead of the tcgen05 one),
- * "hs_phase3" (jamp dot products of the MG_DIAG_SHARED kernel: 0 = scalar FP64 ALUs, 1 = FP64 tensor path, 2 = FP64 tensor
- * path with the jamps of one group of colour flows overlapped with the vertices of the next; 1 and 2 need npar >= 6),
  * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1).
- * Unknown key or bad value -> MG_EINVAL. */
+ * Unknown key, bad value, or a combination that cannot run (helicity streams with the MG_DIAG_SHARED kernel, which has
+ * no per-helicity launches) -> MG_EINVAL, nothing changed. */
 int mg_set_option(mg_process* p, const char* key, int value);
 /* Current value of an option (same keys).  Unknown key -> MG_EINVAL. */
 int mg_get_option(const mg_process* p, const char* key, int* value);

@@ -30,7 +30,7 @@ struct mg_process {
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
-    int diagrams = MG_DIAG_THREAD, hs_split = 1, hs_phase3 = 0, hs_color_alu = 0;
+    int diagrams = MG_DIAG_THREAD, hs_color_alu = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 1L << 30;
@@ -39,6 +39,7 @@ struct mg_process {
     int* d_good = nullptr;     // DEVICE [ncomb]
     int* d_all = nullptr;      // DEVICE [ncomb] = 0..ncomb-1
     void* d_cmat = nullptr;    // DEVICE [ncolor^2] numerators as the colour-sum type
+    void* d_cmat64 = nullptr;  // DEVICE [ncolor^2] numerators in fp64 (helicity filter; = d_cmat in MG_FP64)
     void* d_chol = nullptr;    // DEVICE Cholesky factor of the numerators for the tensor colour sum: fp64 [ncp^2] (MG_FP64) or its TF32 image
     // helicity streams
     std::vector<cudaStream_t> streams;
@@ -105,7 +106,12 @@ static int upload_tables(mg_process* p)
         std::vector<float> h(n2);
         for (int i = 0; i < n2; i++) h[i] = (float)d->cmat[i];
         CUDA_TRY(p, cudaMemcpy(p->d_cmat, h.data(), n2 * sizeof(float), cudaMemcpyHostToDevice));
+        std::vector<double> h64(n2);
+        for (int i = 0; i < n2; i++) h64[i] = d->cmat[i];
+        CUDA_TRY(p, cudaMalloc(&p->d_cmat64, (size_t)n2 * sizeof(double)));
+        CUDA_TRY(p, cudaMemcpy(p->d_cmat64, h64.data(), n2 * sizeof(double), cudaMemcpyHostToDevice));
     }
+    if (p->precision == MG_FP64) p->d_cmat64 = p->d_cmat;
     if (p->precision == MG_FP64) {
         std::vector<double> lp; int ncp = 0;
         if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
@@ -139,9 +145,8 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     else if (!strcmp(name, "gg_ttxgg")) d = desc_gg_ttxgg();
     else if (!strcmp(name, "gg_ttxggg")) d = desc_gg_ttxggg();
     else return fail(nullptr, MG_EINVAL, std::string("unknown process ") + name);
-#ifdef MG_NO_FP32
-    if (precision == MG_FP32) return fail(nullptr, MG_EINVAL, "library built without MG_FP32");
-#endif
+    if (precision == MG_FP32 && !d->has_fp32)
+        return fail(nullptr, MG_EINVAL, std::string("library built without the MG_FP32 instantiation of ") + name);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
         return fail(nullptr, MG_ENODEV, "no such CUDA device");
@@ -157,13 +162,11 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     p->d = d; p->precision = precision; p->device = device;
     int rc = upload_tables(p);
     if (rc != MG_OK) { g_init_error = p->err; mg_destroy(p); return rc; }
-    if (d->ngluon >= 2 && precision != MG_FP32) {
+    if (hs_tables(d->ngluon) && precision != MG_FP32) {       // helicity-shared program: g g -> t tbar + >= 2 g
         cudaError_t e = hs_create(d->ngluon, &p->hs);
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
-        if (d->ngluon >= 4) p->diagrams = MG_DIAG_SHARED;     // measured default, see DESIGN.md
-        if (d->npar >= 7) p->hs_phase3 = 1;                   // jamp dot products on the FP64 tensor path (DMMA): measured faster for 2->5 only
+        p->diagrams = MG_DIAG_SHARED;                         // measured default, see DESIGN.md
         if (d->ncolor < 120) p->hs_color_alu = 1;             // 24 x 24: the fp32 ALU kernel beats the 128-row tcgen05 tiles (measured)
-        if (2 * d->ncomb <= 256) p->hs_split = 2;             // 16 instead of 8 warps per SM: measured +30% (profiles/r1_hs_kernel.md)
     }
     *out = p;
     return MG_OK;
@@ -175,6 +178,7 @@ extern "C" void mg_destroy(mg_process* p)
     cudaSetDevice(p->device);
     hs_destroy(p->hs);
     cudaFree(p->d_pos);
+    if (p->d_cmat64 != p->d_cmat) cudaFree(p->d_cmat64);
     cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat); cudaFree(p->d_chol);
     cudaFree(p->d_mom_own); cudaFree(p->d_me_own); cudaFree(p->d_ws_own);
     for (auto s : p->streams) cudaStreamDestroy(s);
@@ -241,6 +245,8 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         p->color_sum = value;
     } else if (!strcmp(key, "schedule")) {
         if (value != MG_SCHED_GRID && value != MG_SCHED_STREAMS) return fail(p, MG_EINVAL, "bad schedule");
+        if (value == MG_SCHED_STREAMS && p->diagrams == MG_DIAG_SHARED)
+            return fail(p, MG_EINVAL, "helicity streams apply to the MG_DIAG_THREAD kernel only (set diagrams = 0 first)");
         p->schedule = value;
     } else if (!strcmp(key, "block")) {
         if (value < 32 || value > 256 || value % 32) return fail(p, MG_EINVAL, "bad block");
@@ -248,15 +254,9 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
     } else if (!strcmp(key, "diagrams")) {
         if (value != MG_DIAG_THREAD && value != MG_DIAG_SHARED) return fail(p, MG_EINVAL, "bad diagrams");
         if (value == MG_DIAG_SHARED && !p->hs) return fail(p, MG_EINVAL, "this process/precision has no helicity-shared program");
+        if (value == MG_DIAG_SHARED && p->schedule == MG_SCHED_STREAMS)
+            return fail(p, MG_EINVAL, "the helicity-shared kernel has no helicity streams (set schedule = 0 first)");
         p->diagrams = value;
-    } else if (!strcmp(key, "hs_split")) {
-        if (value != 1 && value != 2 && value != 4) return fail(p, MG_EINVAL, "bad hs_split");
-        if (value * p->d->ncomb > 256) return fail(p, MG_EINVAL, "hs_split * ncomb must be <= 256");
-        p->hs_split = value;
-    } else if (!strcmp(key, "hs_phase3")) {
-        if (value < 0 || value > 2) return fail(p, MG_EINVAL, "bad hs_phase3");
-        if (value >= 1 && p->d->npar < 6) return fail(p, MG_EINVAL, "hs_phase3 = 1, 2 need >= 6 external particles");
-        p->hs_phase3 = value;
     } else if (!strcmp(key, "hs_color_alu")) {
         p->hs_color_alu = value != 0;
     } else if (!strcmp(key, "timing")) {
@@ -275,8 +275,6 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "schedule")) *value = p->schedule;
     else if (!strcmp(key, "block")) *value = p->block;
     else if (!strcmp(key, "diagrams")) *value = p->diagrams;
-    else if (!strcmp(key, "hs_split")) *value = p->hs_split;
-    else if (!strcmp(key, "hs_phase3")) *value = p->hs_phase3;
     else if (!strcmp(key, "hs_color_alu")) *value = p->hs_color_alu;
     else if (!strcmp(key, "timing")) *value = p->timing;
     else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
@@ -365,7 +363,8 @@ extern "C" int mg_helicity_filter(mg_process* p, const double* d_momenta, int np
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DiagLaunch a = base_launch(p, d_momenta, nprobe);
     a.d_hel = p->d_all; a.hel_base = 0; a.nhel = ncomb; a.d_meh = (double*)d_workspace; a.mode = MG_CS_FUSED;
-    CUDA_TRY(p, p->d->launch(p->precision, a, st));
+    a.d_cmat = p->d_cmat64;
+    CUDA_TRY(p, p->d->launch(MG_FP64, a, st));          // both sides decide in fp64 whatever the handle's precision (reading A5)
     std::vector<double> h(need / sizeof(double));
     CUDA_TRY(p, cudaMemcpyAsync(h.data(), d_workspace, need, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(p, cudaStreamSynchronize(st));
@@ -470,7 +469,7 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             // tcgen05 colour sum: one contiguous block per 128-row tile, so that a chunk of colours is ONE bulk copy
             const bool tile_major = p->precision != MG_FP64 && !p->hs_color_alu;
             a.tile_major = tile_major ? 1 : 0;
-            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, p->hs_split, p->hs_phase3, st));
+            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
             RowMap map;

@@ -54,7 +54,7 @@ const ProcessDesc* desc_epem_mupmum()
 {
     using namespace epem_mupmum;
     static const ProcessDesc d = { "epem_mupmum", NGLUON, NPAR, NCOMB, NCOLOR, NDIAGRAMS, NAMPS, NCURRENTS, 1,
-                                   DENOM, CDEN, CMAT, FLOPS_PER_EVENT_HELICITY, 0, &launch_any<P_epem_mupmum> };
+                                   DENOM, CDEN, CMAT, FLOPS_PER_EVENT_HELICITY, 0, true, &launch_any<P_epem_mupmum> };
     return &d;
 }
 }  // namespace mg

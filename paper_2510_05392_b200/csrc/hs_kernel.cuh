@@ -15,17 +15,15 @@ struct HsLaunch {
     long rows;             // row stride of the jamps buffer
     int tile_major;        // 1: [row / 128][2][ncolor][128] (one contiguous block per 128-row tile: TMA-friendly) instead
     double mt, wt;
-    unsigned long long* prof;   // DEVICE [8] or NULL: clock64 sums per phase as seen by thread 0 of every CTA (diagnostics)
 };
 
 struct HsContext;          // device copies of the tables
 
-cudaError_t hs_create(int ngluon, HsContext** out);      // cudaErrorInvalidValue if the process has no tables
+// tables go to the CURRENT device; cudaErrorInvalidValue if the process has no helicity-shared program
+cudaError_t hs_create(int ngluon, HsContext** out);
 void hs_destroy(HsContext* c);
 const HsTables* hs_host_tables(const HsContext* c);
 size_t hs_smem_bytes(const HsContext* c);
-// nsplit = threads per helicity combination (1, 2 or 4; blockDim = 2^npar * nsplit <= 256)
-// phase3 = 0: dot products on the scalar FP64 ALUs (thread = helicity); 1: on the FP64 tensor path (DMMA, warp = colour flow)
-cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, int nsplit, int phase3, cudaStream_t st);
+cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
 
 }  // namespace mg

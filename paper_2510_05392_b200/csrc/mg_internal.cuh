@@ -41,6 +41,7 @@ struct ProcessDesc {
     const int* cmat;       // HOST [ncolor*ncolor]
     double flops;          // diagram stage, per (event, helicity)
     int coupling_order;    // norm carries g^(2*coupling_order)
+    bool has_fp32;         // the all-fp32 instantiation (MG_FP32) was compiled in
     // precision: 0 = fp64 amplitudes + fp64 colour sum, 1 = fp64 + fp32, 2 = fp32 + fp32
     cudaError_t (*launch)(int precision, const DiagLaunch&, cudaStream_t);
 };

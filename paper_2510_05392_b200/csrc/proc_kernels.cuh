@@ -78,6 +78,12 @@ static cudaError_t launch_any(int precision, const DiagLaunch& a, cudaStream_t s
 
 }  // namespace mg
 
+#ifdef MG_NO_FP32
+#define MG_HAS_FP32 false
+#else
+#define MG_HAS_FP32 true
+#endif
+
 // Defines the traits struct and the descriptor of a generated process namespace NS.
 #define MG_DEFINE_GG_PROCESS(NS, NGROUPS)                                                                  \
     namespace mg {                                                                                         \
@@ -93,7 +99,7 @@ static cudaError_t launch_any(int precision, const DiagLaunch& a, cudaStream_t s
     {                                                                                                      \
         static const ProcessDesc d = { #NS, NS::NGLUON, NS::NPAR, NS::NCOMB, NS::NCOLOR, NS::NDIAGRAMS,    \
                                        NS::NAMPS, NS::NCURRENTS, NGROUPS, NS::DENOM, NS::CDEN, NS::CMAT,   \
-                                       NS::FLOPS_PER_EVENT_HELICITY, NS::NGLUON, &launch_any<P_##NS> };    \
+                                       NS::FLOPS_PER_EVENT_HELICITY, NS::NGLUON, MG_HAS_FP32, &launch_any<P_##NS> }; \
         return &d;                                                                                         \
     }                                                                                                      \
     }

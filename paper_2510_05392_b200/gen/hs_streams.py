@@ -1,0 +1,351 @@
+"""Device streams of the helicity-shared program (gen/co_program.py) in the form csrc/hs_kernel.cu reads them.
+
+co_program.Program holds the factorised diagram program of g g -> t tbar + (n-2) g (Table 2 at
+PAPER.md:180-187): colour-ordered objects (phase 1), per group of colour flows the pair objects X (phase 2) and the
+dot-product entries jamp[sigma][h] += sign * sum_c X_c[hx] * Y_c[hy] (phase 3).  This module lowers it to what one CTA
+(= one event, NW warps) executes, with every shared-memory address precomputed:
+
+  shared-memory layout (per event).  An area (objects; staging area of the group's pair objects) is four PLANES, one
+      per wavefunction component c; plane c holds one 16-byte complex number per SLOT:  byte(c, s) = c * PLANE + 16 s.
+      PLANE = 32 (mod 128) bytes.  Variant v of an object with first slot s0 lives in slot s0 + perm(v),
+      perm(v) = (v & ~1) | parity(v): flipping ANY one helicity bit of v changes the slot index by an odd number.
+      Consequences: lane <-> variant accesses of one component (phases 1, 2) touch distinct consecutive 16-byte bank
+      groups; the FP64 tensor-core fragments of phase 3 (two variants that differ in one helicity x four components)
+      touch all eight bank groups whatever helicity bit distinguishes the two rows; component c is a compile-time
+      immediate offset from ONE address register.
+
+  phase 2  "chunks": 32 lanes = 32 (pair object, variant) items whose next <= 3 terms have the same opcodes, so that a
+      chunk is straight-line code (csrc/hs_kernel.cu instantiates one function per chunk type listed here) and all
+      terms of a chunk are in flight together.  A chunk is four uint2 per lane:
+          rec0 = { byte offset of the item's slot in the staging plane | sign bits << 16,  type | first << 12 | last << 13 }
+                 (type = one hex digit (opcode - 7) per term)
+          rec1..3 (term k) = { offA | offB << 16,  offC | 0 }  or for x_v3  { offA | offB << 16,  32 lsA | (32 lsB) << 16 }
+      off* = byte offsets of the argument's slot in plane 0 of the object area; ls* = leg sets (momenta K_ls).
+      Chunks are dealt to the NW warps of the CTA at build time (longest processing time first), p2sched[group][warp].
+
+  phase 3  one warp = one colour flow.  The entries of a flow are sorted into CLASSES: a class fixes which three legs
+      index the 8 rows of the m8n8k4 FP64 MMA tile (R), which two legs its 4 complex columns (C) and which legs the tiles
+      (T), so that all entries of a class accumulate into the SAME register fragments; only when a class is finished are
+      the fragments added to the flow's accumulator in shared memory (slot = acc_swizzle(helicity)).  An entry fits a
+      class if R is inside X's legs and C inside Y's (rows from X) or R = Y's legs and C inside X's ("swapped": rows
+      from Y).  Records are per (entry, row = lane / 4): six 16-bit byte offsets (A fragments then B fragments; a lane
+      adds (lane % 4) * PLANE) and a flag word; per (class, lane) the accumulator offsets of the lane's tiles.
+
+Everything here is integer bookkeeping of an exact rewriting; tests/hs_eval.py interprets these very streams in numpy and
+tests/test_generator.py compares the resulting jamps with the oracle (CPU, no kernel involved).
+"""
+from __future__ import annotations
+
+import itertools
+from collections import defaultdict
+
+import numpy as np
+
+from . import co_program
+
+NW = 8                      # warps per CTA
+MAXCHUNK = 3                # terms per phase-2 chunk
+
+OPS = co_program.OPS
+# order of the phase-2 opcodes inside an item (chunks are cut from the sorted list)
+X_ORDER = ["x_v3", "x_v4s", "x_v4", "x_row", "x_col", "x_bil"]
+# relative cost of a term (flops of emit_hs.FLOPS + accumulation), for the static schedule
+X_COST = {"x_row": 72, "x_col": 72, "x_bil": 80, "x_v3": 134, "x_v4": 112, "x_v4s": 170}
+
+
+def chunk_code(ops):
+    """type of a phase-2 chunk: one hex digit (opcode - 7) per term, first term in the low digit"""
+    return sum((OPS[o] - 7) << (4 * j) for j, o in enumerate(ops))
+
+
+def perm(v):
+    return (v & ~1) | (bin(v).count("1") & 1)
+
+
+def plane_bytes(nslots):
+    b = 16 * nslots
+    while b % 128 != 32:
+        b += 16
+    return b
+
+
+def acc_swizzle(h):
+    return co_program.acc_swizzle(h)
+
+
+def _subpos(parent, child):
+    pos = [parent.index(p) for p in child]
+    assert len(pos) <= 3 and all(q < 7 for q in pos)
+    pos += [7] * (3 - len(pos))
+    return pos[0] | (pos[1] << 3) | (pos[2] << 6)
+
+
+def _subvar(v, parent, child):
+    """variant of `child` (legs, ascending) seen from variant v of `parent`"""
+    return sum(((v >> parent.index(p)) & 1) << j for j, p in enumerate(child))
+
+
+class Streams:
+    def __init__(self, prog: co_program.Program):
+        self.prog = prog
+        self.npar = prog.npar
+        self.ncolor = prog.ncolor
+        self.ntile = 1 << (self.npar - 5)
+        assert self.npar >= 6, "the streams need at least one tile leg (npar >= 6)"
+        self._objects()
+        self._phase2()
+        self._phase3()
+
+    # ---------------------------------------------------------------------------------------------
+    def _lsid(self, legs):
+        legs = tuple(sorted(legs))
+        if legs not in self._ls:
+            self._ls[legs] = len(self.legsets)
+            self.legsets.append(legs)
+        return self._ls[legs]
+
+    def _objects(self):
+        prog = self.prog
+        self._ls, self.legsets = {}, []
+        order = sorted(range(len(prog.objs)), key=lambda i: (len(prog.objs[i].legs), i))
+        self.obj_order = order
+        self.obj_slot = {}
+        slot = 0
+        for i in order:
+            self.obj_slot[i] = slot
+            slot += 1 << len(prog.objs[i].legs)
+        self.ns_obj = slot
+        self.obj_plane = plane_bytes(slot)
+        index_of = {old: new for new, old in enumerate(order)}
+        terms, obj_tab = [], []
+        for i in order:
+            o = prog.objs[i]
+            t0 = len(terms)
+            for t in o.terms:
+                neg = 1 if t.sign < 0 else 0
+                if t.op.startswith("ext"):
+                    terms.append([OPS[t.op] | (neg << 8), t.args[0], 0, 0])
+                    continue
+                ls = [self._lsid(prog.objs[x].legs) for x in t.args]
+                w = [OPS[t.op] | (neg << 8) | (ls[0] << 16) | (ls[1] << 24), 0, 0, 0]
+                for k, x in enumerate(t.args):
+                    w[1 + k] = self.obj_slot[x] | (_subpos(o.legs, prog.objs[x].legs) << 16)
+                terms.append(w)
+            obj_tab.append([self.obj_slot[i], len(o.legs) | (self._lsid(o.legs) << 8), t0, len(o.terms)])
+        p1_items, p1_level = [], [0]
+        for lvl in (1, 2, 3):
+            for new, i in enumerate(order):
+                if len(prog.objs[i].legs) == lvl:
+                    p1_items += [(new << 8) | v for v in range(1 << lvl)]
+            p1_level.append(len(p1_items))
+        assert max(len(o.legs) for o in prog.objs) <= 3
+        self.obj_tab, self.p1_terms, self.p1_items, self.p1_level = obj_tab, terms, p1_items, p1_level
+        self._index_of = index_of
+
+    def _obj_off(self, oid, var):
+        """byte offset (plane 0 of the object area) of variant `var` of object `oid`"""
+        return 16 * (self.obj_slot[oid] + perm(var))
+
+    # ---------------------------------------------------------------------------------------------
+    def _phase2(self):
+        prog = self.prog
+        chunk_types = {}          # tuple of opcodes -> id
+        recs, sched = [], []      # recs: [chunk][4][32][2] uint32
+        self.xslot = []           # per group: list of first staging slots of its pair objects
+        ns_stage = 0
+        for g in prog.groups:
+            slots, s = [], 0
+            for x in g["xobjs"]:
+                slots.append(s)
+                s += 1 << len(x["legs"])
+            self.xslot.append(slots)
+            ns_stage = max(ns_stage, s)
+        self.trash_slot = ns_stage                      # padding lanes store here
+        self.ns_stage = ns_stage + 2
+        self.stage_plane = plane_bytes(self.ns_stage)
+        assert 4 * self.stage_plane < 65536 and 4 * self.obj_plane < 65536, "16-bit byte offsets"
+        for gi, g in enumerate(prog.groups):
+            by_shape = defaultdict(list)
+            for k, x in enumerate(g["xobjs"]):
+                terms = sorted(x["terms"], key=lambda t: (X_ORDER.index(t.op), t.args))
+                shape = tuple(t.op for t in terms)
+                for v in range(1 << len(x["legs"])):
+                    by_shape[shape].append((k, v, terms))
+            units = []            # (cost, [chunk blocks])
+            for shape, items in sorted(by_shape.items()):
+                cuts = [shape[i:i + MAXCHUNK] for i in range(0, len(shape), MAXCHUNK)]
+                if len(shape) == 4:                       # 2 + 2 rather than 3 + 1
+                    cuts = [shape[:2], shape[2:]]
+                for i in range(0, len(items), 32):
+                    lanes = items[i:i + 32]
+                    blocks, t0 = [], 0
+                    for ci, ops in enumerate(cuts):
+                        ct = chunk_code(ops)
+                        chunk_types[ct] = tuple(OPS[o] for o in ops)
+                        blk = np.zeros((4, 32, 2), dtype=np.uint32)
+                        blk[0, :, 0] = 16 * self.trash_slot
+                        blk[0, :, 1] = ct | ((1 if ci == 0 else 0) << 12) | ((1 if ci == len(cuts) - 1 else 0) << 13)
+                        for l, (k, v, terms) in enumerate(lanes):
+                            x = g["xobjs"][k]
+                            signs = 0
+                            for j in range(len(ops)):
+                                t = terms[t0 + j]
+                                assert t.op == ops[j]
+                                if t.sign < 0:
+                                    signs |= 1 << j
+                                offs = [self._obj_off(a, _subvar(v, x["legs"], prog.objs[a].legs)) for a in t.args]
+                                if t.op == "x_v3":
+                                    ls = [self._lsid(prog.objs[a].legs) for a in t.args]
+                                    blk[1 + j, l] = (offs[0] | (offs[1] << 16), (32 * ls[0]) | ((32 * ls[1]) << 16))
+                                else:
+                                    blk[1 + j, l] = (offs[0] | (offs[1] << 16), offs[2] if len(offs) > 2 else 0)
+                            blk[0, l, 0] = (16 * (self.xslot[gi][k] + perm(v))) | (signs << 16)
+                        blocks.append(blk)
+                        t0 += len(ops)
+                    units.append((sum(X_COST[o] for o in shape), blocks))
+            # longest processing time first onto the NW warps
+            load = [0] * NW
+            per_warp = [[] for _ in range(NW)]
+            for cost, blocks in sorted(units, key=lambda u: -u[0]):
+                w = min(range(NW), key=lambda i: (load[i], i))
+                load[w] += cost
+                per_warp[w] += blocks
+            for w in range(NW):
+                sched.append((len(recs), len(per_warp[w])))
+                recs += per_warp[w]
+        self.chunk_types = dict(sorted(chunk_types.items()))      # code -> opcodes
+        self.p2rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 4, 32, 2)
+        self.p2sched = np.asarray(sched, dtype=np.int32).reshape(-1, 2)
+
+    # ---------------------------------------------------------------------------------------------
+    def _classes_for(self, ents):
+        """smallest set of classes (R, C, swapped-allowed) covering the entries [(X legs, Y legs)] of one colour flow"""
+        legs = range(self.npar)
+        cover = {}
+        for R in itertools.combinations(legs, 3):
+            Rs = frozenset(R)
+            rest = [l for l in legs if l not in Rs]
+            for C in itertools.combinations(rest, 2):
+                Cs = frozenset(C)
+                got = frozenset(i for i, (X, Y) in enumerate(ents)
+                                if (Rs <= X and Cs <= Y) or (Rs == Y and Cs <= X))
+                if got and got not in cover:
+                    cover[got] = (R, C)
+        sets = sorted(cover, key=lambda s: (-len(s), sorted(s)))
+        full = frozenset(range(len(ents)))
+        for k in range(1, 7):
+            for combo in itertools.combinations(sets, k):
+                if frozenset().union(*combo) == full:
+                    return [cover[c] for c in combo], [set(c) for c in combo]
+        raise AssertionError("no class cover")
+
+    def _phase3(self):
+        prog, npar = self.prog, self.npar
+        ntile = self.ntile
+        hbit = lambda p: npar - 1 - p
+        recs, cls_tab, flows, sched = [], [], [], []
+        self.max_flows = 0
+        shapes = set()
+        for gi, g in enumerate(prog.groups):
+            per_warp = [[] for _ in range(NW)]
+            for fi, j in enumerate(g["sigmas"]):
+                per_warp[fi % NW].append((fi, j))
+            self.max_flows = max(self.max_flows, min(NW, len(g["sigmas"])))
+            for w in range(NW):
+                sched.append((len(flows), len(per_warp[w])))
+                for fi, j in per_warp[w]:
+                    ents = [(frozenset(g["xobjs"][xs]["legs"]), frozenset(prog.objs[yo].legs), xs, yo, sign)
+                            for xs, yo, sign in g["entries"][j]]
+                    classes, covered = self._classes_for([(e[0], e[1]) for e in ents])
+                    # every entry goes to the compatible class with the fewest entries so far
+                    members = [[] for _ in classes]
+                    for i in sorted(range(len(ents)), key=lambda i: sum(i in c for c in covered)):
+                        k = min((k for k in range(len(classes)) if i in covered[k]), key=lambda k: len(members[k]))
+                        members[k].append(i)
+                    assert all(members)
+                    rec0, cls0 = len(recs), len(cls_tab)
+                    for (R, C), mem in zip(classes, members):
+                        T = tuple(l for l in range(npar) if l not in R and l not in C)
+                        # helicity of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
+                        ct = np.zeros((32, 4), dtype=np.uint32)
+                        for lane in range(32):
+                            row, c2 = lane >> 2, lane & 3
+                            for t in range(ntile):
+                                h = sum(((row >> b) & 1) << hbit(R[b]) for b in range(3))
+                                h |= sum(((c2 >> b) & 1) << hbit(C[b]) for b in range(2))
+                                h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
+                                ct[lane, t] = 16 * acc_swizzle(h)
+                        cls_tab.append(ct)
+                        for n_, i in enumerate(mem):
+                            X, Y, xs, yo, sign = ents[i]
+                            xl, yl = tuple(sorted(X)), tuple(sorted(Y))
+                            swapped = not (frozenset(R) <= X)
+                            al, bl = (yl, xl) if swapped else (xl, yl)          # legs of the A-side / B-side operand
+                            a_off = (lambda v: self._obj_off(yo, v)) if swapped else (lambda v: 16 * (self.xslot[gi][xs] + perm(v)))
+                            b_off = (lambda v: 16 * (self.xslot[gi][xs] + perm(v))) if swapped else (lambda v: self._obj_off(yo, v))
+                            assert set(R) <= set(al) and set(C) <= set(bl)
+                            mask = sum(1 << b for b in range(len(T)) if T[b] in al)     # tile bits that select the A fragment
+                            ta = [b for b in range(len(T)) if T[b] in al]
+                            tb = [b for b in range(len(T)) if T[b] not in al]
+                            na, nb = 1 << len(ta), 1 << len(tb)
+                            shape = (1 if swapped else 0) | (mask << 1)
+                            shapes.add((shape, na, nb))
+                            rec = np.zeros((8, 4), dtype=np.uint32)
+                            for row in range(8):
+                                offs = []
+                                for a in range(na):
+                                    v = sum(((row >> b) & 1) << al.index(R[b]) for b in range(3))
+                                    v |= sum(((a >> q) & 1) << al.index(T[ta[q]]) for q in range(len(ta)))
+                                    offs.append(a_off(v))
+                                aw = [0, 0]
+                                for q, o in enumerate(offs):
+                                    aw[q >> 1] |= o << (16 * (q & 1))
+                                offs = []
+                                c2, ri = row >> 1, row & 1
+                                for b_ in range(nb):
+                                    v = sum(((c2 >> b) & 1) << bl.index(C[b]) for b in range(2))
+                                    v |= sum(((b_ >> q) & 1) << bl.index(T[tb[q]]) for q in range(len(tb)))
+                                    offs.append(b_off(v) + 8 * ri)
+                                bw = [0, 0]
+                                for q, o in enumerate(offs):
+                                    bw[q >> 1] |= o << (16 * (q & 1))
+                                # word layout: A offsets fill x (, y); B offsets follow in the next free word(s)
+                                words = aw[: (na + 1) // 2] + bw[: (nb + 1) // 2]
+                                assert len(words) <= 3
+                                words += [0] * (3 - len(words))
+                                flags = shape | ((1 if n_ == len(mem) - 1 else 0) << 4) | ((1 if n_ == 0 else 0) << 5) | \
+                                        ((1 if sign < 0 else 0) << 31)
+                                rec[row] = words + [flags]
+                            recs.append(rec)
+                    flows.append((rec0, len(ents) | (len(classes) << 8) | ((fi % NW) << 16), cls0, j))
+        self.p3rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 8, 4)
+        self.p3cls = np.asarray(cls_tab, dtype=np.uint32).reshape(-1, 32, 4)
+        self.p3flow = np.asarray(flows, dtype=np.int32).reshape(-1, 4)
+        self.p3sched = np.asarray(sched, dtype=np.int32).reshape(-1, 2)
+        self.p3shapes = sorted(shapes)
+
+    # ---------------------------------------------------------------------------------------------
+    def tables(self):
+        i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w)
+        ncls = self.p3flow[:, 1] >> 8 & 0xFF
+        return {
+            "npar": self.npar, "ncolor": self.ncolor, "ngroups": len(self.prog.groups), "nw": NW, "ntile": self.ntile,
+            "ns_obj": self.ns_obj, "obj_plane": self.obj_plane, "ns_stage": self.ns_stage, "stage_plane": self.stage_plane,
+            "nlegsets": len(self.legsets), "max_flows": self.max_flows, "max_classes": int(ncls.max()),
+            "legset_mask": np.asarray([sum(1 << p for p in legs) for legs in self.legsets], np.int32),
+            "obj": i32(self.obj_tab, 4), "term": i32(self.p1_terms, 4), "p1_items": np.asarray(self.p1_items, np.int32),
+            "p1_level": np.asarray(self.p1_level, np.int32),
+            "p2rec": self.p2rec, "p2sched": self.p2sched, "chunk_types": self.chunk_types,
+            "p3rec": self.p3rec, "p3cls": self.p3cls, "p3flow": self.p3flow, "p3sched": self.p3sched,
+            "p3shapes": self.p3shapes,
+        }
+
+
+_CACHE = {}
+
+
+def build(n, group_prefix):
+    key = (n, group_prefix)
+    if key not in _CACHE:
+        _CACHE[key] = Streams(co_program.build(n, group_prefix))
+    return _CACHE[key]

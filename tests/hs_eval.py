@@ -1,9 +1,11 @@
-"""numpy interpreter of the helicity-shared program tables (gen/co_program.py) -- CPU TEST HELPER.
+"""numpy interpreter of the device streams of the helicity-shared program (gen/hs_streams.py) -- CPU TEST HELPER.
 
-Decodes the int32 tables exactly as csrc/hs_kernel.cu does (same packing, same variant convention) and
-restates every opcode with the plain gamma-matrix helpers of tests/ir_eval.py, so that the generator's
-factorised program can be checked against the diagram program and the oracle before any kernel runs.
-Not product, not oracle; nothing here is imported by the package.
+Executes, lane by lane, exactly what one CTA of csrc/hs_kernel.cu executes for one event: the same packed records, the
+same byte offsets into the shared-memory planes, the same fragment <-> (row, column, tile) conventions of the FP64
+tensor-core tiles and the same accumulator slots -- but every opcode is restated with the plain gamma-matrix helpers of
+tests/ir_eval.py.  So the generator's factorisation (merge_v4_pairs, the X.Y split and its signs, chunking, classes,
+packing) is checked against the oracle on CPU before any kernel runs.  Not product, not oracle; nothing here is imported
+by the package.
 """
 import numpy as np
 
@@ -12,46 +14,84 @@ import ir_eval as ir
 G = ir.G
 
 
+def _perm(v):
+    return (v & ~1) | (bin(v).count("1") & 1)
+
+
 def _sub(v, code):
-    """variant of an argument: bit j = bit (code >> 3j) & 7 of the parent's variant (7 = none)"""
     return sum(((v >> ((code >> (3 * j)) & 7)) & 1) << j for j in range(3))
 
 
+def _acc_swizzle(h):
+    hi = h >> 3
+    return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7))
+
+
+class _Planes:
+    """an area of four component planes; addressed by the byte offset inside plane 0 like the kernel does"""
+
+    def __init__(self, plane_bytes):
+        assert plane_bytes % 128 == 32
+        self.a = np.full((4, plane_bytes // 16), np.nan + 0j, dtype=complex)
+
+    def load(self, off):
+        assert off % 16 == 0
+        return self.a[:, off // 16].copy()
+
+    def store(self, off, val):
+        self.a[:, off // 16] = val
+
+
+def _x_term(op, A, B, Z, kA, kB):
+    if op == 8:
+        return A @ ir.slash(B)
+    if op == 9:
+        return ir.slash(A) @ B
+    if op == 10:
+        return G * np.array([A @ ir.GAM[mu] @ B for mu in range(4)])
+    if op == 11:
+        return G * (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A)
+    if op == 12:
+        return G * (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A)
+    if op == 13:
+        return G * (2 * ir.mdot(A, Z) * B - ir.mdot(B, Z) * A - ir.mdot(A, B) * Z)
+    raise ValueError(op)
+
+
 def evaluate(T, mom, mt, wt):
-    """jamps[ncolor][2^npar] (without the g^n factor) of one event from the tables T"""
-    npar = T["npar"]
+    """jamps[ncolor][2^npar] (without the g^n factor) of one event from the streams T = Streams.tables()"""
+    npar, nw, ntile = T["npar"], T["nw"], T["ntile"]
     k = [mom[i] * (1 if i < 2 else -1) for i in range(npar)]
     K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
-    obj, term = T["obj"], T["term"]
-    area = np.zeros(T["obj_area"], dtype=complex)
-    # this interpreter keeps an object as [variant][component]; the kernel's bank swizzle is not modelled
+    obj = _Planes(T["obj_plane"])
 
-    def load(w, var):
-        off, code = w & 0xFFFF, (w >> 16) & 0x1FF
-        return area[off + 4 * _sub(var, code):off + 4 * _sub(var, code) + 4].copy()
+    # phase 1: colour-ordered objects, level by level (term table interpreted directly)
+    def arg(w, var):
+        return obj.load(16 * ((w & 0xFFFF) + _perm(_sub(var, (w >> 16) & 0x1FF))))
 
-    def run_terms(t0, nt, var, legs_of_parent=None, kout=None):
+    for it in T["p1_items"]:
+        o, var = int(it) >> 8, int(it) & 0xFF
+        slot0, info, t0, nt = (int(x) for x in T["obj"][o])
+        kout = K[info >> 8]
         acc = np.zeros(4, dtype=complex)
-        for t in term[t0:t0 + nt]:
+        for t in T["term"][t0:t0 + nt]:
             w0, w1, w2, w3 = (int(x) & 0xFFFFFFFF for x in t)
             op, neg = w0 & 0xFF, (w0 >> 8) & 1
-            a = [w1]
             hel = 1 if var & 1 else -1
             if op == 0:
-                e = ir.polvec(mom[a[0]], hel)
-                r = e if a[0] < 2 else e.conj()
+                e = ir.polvec(mom[w1], hel)
+                r = e if w1 < 2 else e.conj()
             elif op == 1:
                 r = ir.u_spinor(mom[2], mt, hel).conj() @ ir.GAM[0]
             elif op == 2:
                 r = ir.v_spinor(mom[3], mt, hel)
             else:
-                A = load(w1, var)
-                B = load(w2, var)
+                A, B = arg(w1, var), arg(w2, var)
                 kA, kB = K[(w0 >> 16) & 0xFF], K[(w0 >> 24) & 0xFF]
                 if op == 3:
                     r = (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A) / ir.mdot(kout, kout)
                 elif op == 4:
-                    Z = load(w3, var)
+                    Z = arg(w3, var)
                     r = (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A) / ir.mdot(kout, kout)
                 elif op == 5:
                     q = -kout
@@ -61,54 +101,98 @@ def evaluate(T, mom, mt, wt):
                     r = (ir.slash(q) + mt * np.eye(4)) @ ir.slash(A) @ B / (ir.mdot(q, q) - mt * mt + 1j * mt * wt)
                 elif op == 7:
                     r = np.array([A @ ir.GAM[mu] @ B for mu in range(4)]) / ir.mdot(kout, kout)
-                elif op == 8:
-                    r = A @ ir.slash(B)
-                elif op == 9:
-                    r = ir.slash(A) @ B
-                elif op == 10:
-                    r = G * np.array([A @ ir.GAM[mu] @ B for mu in range(4)])
-                elif op == 11:
-                    r = G * (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A)
-                elif op == 12:
-                    Z = load(w3, var)
-                    r = G * (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A)
-                elif op == 13:
-                    Z = load(w3, var)
-                    r = G * (2 * ir.mdot(A, Z) * B - ir.mdot(B, Z) * A - ir.mdot(A, B) * Z)
                 else:
                     raise ValueError(op)
             acc = acc + (-r if neg else r)
-        return acc
+        obj.store(16 * (slot0 + _perm(var)), acc)
 
-    # phase 1: objects, level by level
-    for it in T["p1_items"]:
-        o, var = int(it) >> 8, int(it) & 0xFF
-        off, info, t0, nt = (int(x) for x in obj[o])
-        val = run_terms(t0, nt, var, kout=K[info >> 8])
-        area[off + 4 * var:off + 4 * var + 4] = val
-    # phases 2 and 3, group by group
     nh = 1 << npar
-    J = np.zeros((T["ncolor"], nh), dtype=complex)
-    stage = np.zeros(max(T["stage_area"], 1), dtype=complex)
-    for g in T["group"]:
-        x0, xi0, nxi, s0, ns = (int(x) for x in g[:5])
-        for it in T["x_items"][xi0:xi0 + nxi]:
-            if int(it) < 0:                                   # padding of the last work unit
-                continue
-            xk, var = int(it) >> 8, int(it) & 0xFF
-            soff, lognv, t0, nt = (int(x) for x in T["xobj"][x0 + xk])
-            stage[soff + 4 * var:soff + 4 * var + 4] = run_terms(t0, nt, var)
-        for sg in T["sigma"][s0:s0 + ns]:
-            j, e0, ne = int(sg[0]), int(sg[1]), int(sg[2])
-            for h in range(nh):
-                acc = 0j
-                for e in T["entry"][e0:e0 + ne]:
-                    w0, w1, row, sign = (int(x) for x in e)
-                    offx, nvx = w0 & 0xFFFF, w0 >> 16
-                    offy, nvy = w1 & 0xFFFF, w1 >> 16
-                    vv = int(T["vtab"][row][h])
-                    vx, vy = vv & 0xFF, vv >> 8
-                    d = sum(stage[offx + 4 * vx + c] * area[offy + 4 * vy + c] for c in range(4))
-                    acc += sign * d
-                J[j][h] = acc
+    J = np.full((T["ncolor"], nh), np.nan + 0j, dtype=complex)
+    for g in range(T["ngroups"]):
+        stage = _Planes(T["stage_plane"])
+        # phase 2: chunks of every warp
+        for w in range(nw):
+            c0, nc = (int(x) for x in T["p2sched"][g * nw + w])
+            acc = np.zeros((32, 4), dtype=complex)
+            for c in range(c0, c0 + nc):
+                blk = T["p2rec"][c]
+                for lane in range(32):
+                    r0x, r0y = int(blk[0, lane, 0]), int(blk[0, lane, 1])
+                    ctype, first, last = r0y & 0xFFF, (r0y >> 12) & 1, (r0y >> 13) & 1
+                    if first:
+                        acc[lane] = 0
+                    for j in range(3):
+                        op7 = (ctype >> (4 * j)) & 0xF
+                        if op7 == 0:
+                            break
+                        op = op7 + 7
+                        x, y = int(blk[1 + j, lane, 0]), int(blk[1 + j, lane, 1])
+                        A, B = obj.load(x & 0xFFFF), obj.load(x >> 16)
+                        Z = kA = kB = None
+                        if op == 11:
+                            assert (y & 0xFFFF) % 32 == 0 and (y >> 16) % 32 == 0
+                            kA, kB = K[(y & 0xFFFF) // 32], K[(y >> 16) // 32]
+                        elif op in (12, 13):
+                            Z = obj.load(y & 0xFFFF)
+                        r = _x_term(op, A, B, Z, kA, kB)
+                        acc[lane] += -r if (r0x >> (16 + j)) & 1 else r
+                    if last:
+                        stage.store(r0x & 0xFFFF, acc[lane])
+        # phase 3: colour flows of every warp
+        for w in range(nw):
+            f0, nf = (int(x) for x in T["p3sched"][g * nw + w])
+            for f in range(f0, f0 + nf):
+                rec0, info, cls0, jamp = (int(x) for x in T["p3flow"][f])
+                nent, ncls = info & 0xFF, (info >> 8) & 0xFF
+                accum = np.zeros(nh, dtype=complex)            # the flow's accumulator in shared memory, [slot]
+                written = np.zeros(nh, dtype=bool)
+                cls, frag = cls0, None
+                for e in range(rec0, rec0 + nent):
+                    rec = T["p3rec"][e]
+                    flags = int(rec[0, 3])
+                    shape, lastc, firstc, neg = flags & 0xF, (flags >> 4) & 1, (flags >> 5) & 1, (flags >> 31) & 1
+                    assert all(int(rec[r, 3]) == flags for r in range(8))
+                    swapped, mask = shape & 1, shape >> 1
+                    na = 1 << bin(mask).count("1")
+                    nb = ntile // na
+                    if firstc:
+                        frag = np.zeros((32, ntile), dtype=complex)
+                    aplanes, bplanes = (obj, stage) if swapped else (stage, obj)
+                    for lane in range(32):
+                        row, kk = lane >> 2, lane & 3
+                        words = [int(x) for x in rec[row, :3]]
+                        halves = [w_ >> (16 * q) & 0xFFFF for w_ in words for q in range(2)]
+                        a_offs = halves[:na]
+                        b_offs = halves[2 * ((na + 1) // 2):][:nb]
+                        # A fragment of this lane: component kk of the variant of row `row`; B fragment: component kk of
+                        # the variant of complex column row >> 1, real or imaginary half by row & 1
+                        for t in range(ntile):
+                            ai = sum(((t >> b) & 1) << i for i, b in enumerate([b for b in range(8) if (mask >> b) & 1]))
+                            bi = sum(((t >> b) & 1) << i for i, b in enumerate([b for b in range(ntile.bit_length() - 1) if not (mask >> b) & 1]))
+                            # the MMA sums over kk; emulate by letting lane (row, c2) gather all four components itself
+                            if True:
+                                r_, c2 = lane >> 2, lane & 3
+                                arow = [int(x) for x in rec[r_, :3]]
+                                ah = [w_ >> (16 * q) & 0xFFFF for w_ in arow for q in range(2)][:na]
+                                # column c2 is served by record rows 2 c2 (re half) and 2 c2 + 1 (im half): same slot, +8 bytes
+                                brow = [int(x) for x in rec[2 * c2, :3]]
+                                bh = [w_ >> (16 * q) & 0xFFFF for w_ in brow for q in range(2)][2 * ((na + 1) // 2):][:nb]
+                                brow1 = [int(x) for x in rec[2 * c2 + 1, :3]]
+                                bh1 = [w_ >> (16 * q) & 0xFFFF for w_ in brow1 for q in range(2)][2 * ((na + 1) // 2):][:nb]
+                                assert bh[bi] % 16 == 0 and bh1[bi] == bh[bi] + 8
+                                Xv, Yv = aplanes.load(ah[ai]), bplanes.load(bh[bi])
+                                val = np.sum(Xv * Yv)
+                                frag[lane, t] += -val if neg else val
+                    if lastc:
+                        for lane in range(32):
+                            for t in range(ntile):
+                                off = int(T["p3cls"][cls][lane, t])
+                                assert off % 16 == 0
+                                accum[off // 16] += frag[lane, t]
+                                written[off // 16] = True
+                        cls += 1
+                assert cls == cls0 + ncls and written.all()
+                for h in range(nh):
+                    J[jamp][h] = accum[_acc_swizzle(h)]
+    assert not np.isnan(J).any()
     return J

@@ -75,3 +75,21 @@ def test_program_matches_oracle_per_helicity(name, n, hels, params):
         j = ir_eval.evaluate(proc, p[1], hel, params["mT"], params["wT"])
         mh = (j.conj() @ C @ j).real * gs ** (2 * n) / oracle.DENOM[name]
         assert abs(mh / mh_o[1][h] - 1) < 1e-10, (h, mh, mh_o[1][h])
+
+
+@pytest.mark.parametrize("name,n,gp,nev", [("gg_ttxgg", 4, 0, 2), ("gg_ttxggg", 5, 2, 1)])
+def test_helicity_shared_streams_match_oracle(name, n, gp, nev, params):
+    """the device streams of the helicity-shared kernel (gen/hs_streams.py: merged four-gluon vertices, X.Y split, chunks,
+    classes, packed offsets), interpreted lane by lane by tests/hs_eval.py, give the oracle's per-helicity colour-summed
+    |M|^2 for EVERY helicity -- the program that is the default for these processes, checked without a GPU"""
+    import hs_eval
+    from paper_2510_05392_b200.gen import hs_streams
+    T = hs_streams.build(n, gp).tables()
+    C = np.array([[float(x) for x in r] for r in colour.colour_matrix(n)])
+    gs = math.sqrt(4 * math.pi * params["aS"])
+    p = inputs.momenta(name, nev, seed=7)
+    _, mh_o = oracle.matrix_elements(name, p, params, per_helicity=True)
+    for e in range(nev):
+        J = hs_eval.evaluate(T, p[e], params["mT"], params["wT"])
+        mh = np.einsum("ih,ij,jh->h", J.conj(), C, J).real * gs ** (2 * n) / oracle.DENOM[name]
+        assert np.abs(mh / mh_o[e] - 1).max() < 1e-10

@@ -83,11 +83,9 @@ def test_scheduling_variants_agree(B, process):
     base = None
     for opts in ({"diagrams": 0}, {"diagrams": 0, "schedule": 1}, {"diagrams": 0, "color_sum": 1},
                  {"diagrams": 0, "color_sum": 1, "schedule": 1}, {"diagrams": 0, "block": 64},
-                 {"diagrams": 1}, {"diagrams": 1, "hs_split": 2}, {"diagrams": 1, "jamp_chunk_mib": 1},
-                 {"diagrams": 1, "hs_phase3": 0, "hs_split": 1}, {"diagrams": 1, "hs_phase3": 1, "hs_split": 1},
-                 {"diagrams": 1, "hs_phase3": 1, "hs_split": 2}, {"diagrams": 1, "hs_phase3": 2}):
-        if opts.get("hs_phase3", 0) >= 1 and process in ("gg_ttx", "gg_ttxg"):
-            continue                                   # the FP64 tensor path of phase 3 needs >= 6 external particles
+                 {"diagrams": 1}, {"diagrams": 1, "jamp_chunk_mib": 1}):
+        if opts.get("diagrams") == 1 and process in ("gg_ttx", "gg_ttxg"):
+            continue                                   # the helicity-shared program exists for >= 2 final-state gluons
         proc = B.init_process(process, "fp64")
         for k, v in opts.items():
             proc.set_option(k, v)
@@ -250,12 +248,11 @@ def test_full_size_sampled_mixed(B, process):
 
 
 def test_mixed_color_sum_variants_agree(B):
-    """gg_ttxggg, mixed: tcgen05 split-TF32 colour sum (tile-major jamps) against the fp32 ALU kernel, and both phase-3
-    variants of the helicity-shared kernel"""
+    """gg_ttxggg, mixed: tcgen05 split-TF32 colour sum (tile-major jamps) against the fp32 ALU kernel, and the thread kernel"""
     mom = inputs.momenta("gg_ttxggg", 203, seed=5)
     d_mom = torch.from_numpy(mom).cuda()
     ref = None
-    for opts in ({}, {"hs_color_alu": 1}, {"hs_phase3": 0}, {"hs_phase3": 0, "hs_color_alu": 1, "hs_split": 1}):
+    for opts in ({}, {"hs_color_alu": 1}, {"diagrams": 0, "color_sum": 1}):
         proc = B.init_process("gg_ttxggg", "mixed")
         for k, v in opts.items():
             proc.set_option(k, v)
