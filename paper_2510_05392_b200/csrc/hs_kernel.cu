@@ -26,7 +26,7 @@ namespace mg {
 struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
     const uint2* p2rec; const int2* p2sched;
-    const uint4* p3rec; const uint2* p3cls; const int4* p3flow; const int2* p3sched;
+    const uint4* p3rec; const uint2* p3cls; const int* p3clsh; const int4* p3flow; const int2* p3sched;
     int ncolor;
     int p1_level[4];
 };
@@ -61,22 +61,6 @@ __device__ __forceinline__ p4<double> ld_k(const char* __restrict__ Ks, unsigned
     const double2 a = *reinterpret_cast<const double2*>(Ks + off), b = *reinterpret_cast<const double2*>(Ks + off + 16);
     p4<double> k = { a.x, a.y, b.x, b.y };
     return k;
-}
-
-__device__ __forceinline__ void lower(wf<double>& w)
-{
-#pragma unroll
-    for (int c = 1; c < 4; c++) { w.c[c].re = -w.c[c].re; w.c[c].im = -w.c[c].im; }
-}
-
-// both orderings of the four-gluon vertex that share the middle leg: (x y | z out) + (z y | x out)
-//   J = 2 (X.Z) Y - (Y.Z) X - (Y.X) Z      (raw vertex, no propagator factor)
-template <typename T> __device__ __forceinline__ void v4s_raw(const wf<T>& X, const wf<T>& Y, const wf<T>& Z, wf<T>& out)
-{
-    cx<T> xz = dot(X, Z);
-    xz = xz + xz;
-    const cx<T> yz = dot(Y, Z), yx = dot(Y, X);
-    for (int mu = 0; mu < 4; mu++) out.c[mu] = cfms(yx, Z.c[mu], cfms(yz, X.c[mu], xz * Y.c[mu]));
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -123,58 +107,81 @@ __device__ __forceinline__ void p1_terms(const HsDev& d, const char* __restrict_
 // ------------------------------------------------------------------------------------------------------------
 // phase 2: one term of a chunk; OP is a compile-time constant, the record holds the byte offsets of the arguments
 //   r.x = offA | offB << 16,  r.y = offC  (x_v3: 32 legset(A) | 32 legset(B) << 16)
+// The term's sign (smask = 0 or 0x80000000) goes onto the scalar coefficients of the vertex with integer XORs and the
+// vertex is accumulated straight into acc (no separate signed add); acc is kept contravariant, the index lowering for the
+// plain dot of phase 3 happens once per item at the store (p2_chunk).
+__device__ __forceinline__ double flip(double v, unsigned smask)
+{
+    return __hiloint2double(__double2hiint(v) ^ (int)smask, __double2loint(v));
+}
+__device__ __forceinline__ cx<double> flip(cx<double> v, unsigned smask) { return mk<double>(flip(v.re, smask), flip(v.im, smask)); }
+
 template <int OP, int OBJ_PLANE>
-__device__ __forceinline__ void x_term(const char* __restrict__ obj, const char* __restrict__ Ks, const uint2 r, const double sg,
+__device__ __forceinline__ void x_term(const char* __restrict__ obj, const char* __restrict__ Ks, const uint2 r, const unsigned smask,
                                        wf<double>& acc)
 {
-    // the index lowering of the raw vertices (components 1-3 negated, for the plain dot of phase 3) is folded into the sign
-    auto add = [&](const wf<double>& q, double s123) {
-        acc.c[0].re = fma(sg, q.c[0].re, acc.c[0].re); acc.c[0].im = fma(sg, q.c[0].im, acc.c[0].im);
-#pragma unroll
-        for (int c = 1; c < 4; c++) { acc.c[c].re = fma(s123, q.c[c].re, acc.c[c].re); acc.c[c].im = fma(s123, q.c[c].im, acc.c[c].im); }
-    };
-    wf<double> A, B, q;
+    wf<double> A, B;
     ld_wf<OBJ_PLANE>(obj, r.x & 0xFFFFu, A);
     ld_wf<OBJ_PLANE>(obj, r.x >> 16, B);
     if constexpr (OP == 11) {
-        v3_raw(A, ld_k(Ks, r.y & 0xFFFFu), B, ld_k(Ks, r.y >> 16), q);
-        add(q, -sg);
+        // (A.B)(kA - kB) + ((2 kB + kA).A) B - ((2 kA + kB).B) A
+        const p4<double> kA = ld_k(Ks, r.y & 0xFFFFu), kB = ld_k(Ks, r.y >> 16);
+        const p4<double> ea = { fma(2.0, kB.e, kA.e), fma(2.0, kB.x, kA.x), fma(2.0, kB.y, kA.y), fma(2.0, kB.z, kA.z) };
+        const p4<double> eb = { fma(2.0, kA.e, kB.e), fma(2.0, kA.x, kB.x), fma(2.0, kA.y, kB.y), fma(2.0, kA.z, kB.z) };
+        const cx<double> ab = flip(dot(A, B), smask), xa = flip(dot(ea, A), smask), xb = flip(dot(eb, B), smask);
+        const double dd[4] = { kA.e - kB.e, kA.x - kB.x, kA.y - kB.y, kA.z - kB.z };
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const cx<double> t = mk<double>(fma(dd[mu], ab.re, acc.c[mu].re), fma(dd[mu], ab.im, acc.c[mu].im));
+            acc.c[mu] = cfms(xb, A.c[mu], cfma(xa, B.c[mu], t));
+        }
     } else if constexpr (OP == 12) {
+        // (A.Z) B - (B.Z) A
         wf<double> Z; ld_wf<OBJ_PLANE>(obj, r.y & 0xFFFFu, Z);
-        v4_raw(A, B, Z, q);
-        add(q, -sg);
+        const cx<double> xz = flip(dot(A, Z), smask), yz = flip(dot(B, Z), smask);
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) acc.c[mu] = cfms(yz, A.c[mu], cfma(xz, B.c[mu], acc.c[mu]));
     } else if constexpr (OP == 13) {
+        // both orderings of the four-gluon vertex that share the middle leg: 2 (A.Z) B - (B.Z) A - (B.A) Z
         wf<double> Z; ld_wf<OBJ_PLANE>(obj, r.y & 0xFFFFu, Z);
-        v4s_raw(A, B, Z, q);
-        add(q, -sg);
-    } else if constexpr (OP == 8) {
-        row_slash(A, make_slashed(B), q);
-        add(q, sg);
-    } else if constexpr (OP == 9) {
-        slash_col(make_slashed(A), B, q);
-        add(q, sg);
+        cx<double> xz = dot(A, Z);
+        xz = flip(xz + xz, smask);
+        const cx<double> yz = flip(dot(B, Z), smask), yx = flip(dot(B, A), smask);
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) acc.c[mu] = cfms(yx, Z.c[mu], cfms(yz, A.c[mu], cfma(xz, B.c[mu], acc.c[mu])));
     } else {
-        static_assert(OP == 10, "unknown phase-2 opcode");
-        ffv_p_raw(A, B, q);
-        add(q, -sg);
+        wf<double> q;
+        if constexpr (OP == 8) row_slash(A, make_slashed(B), q);
+        else if constexpr (OP == 9) slash_col(make_slashed(A), B, q);
+        else {
+            static_assert(OP == 10, "unknown phase-2 opcode");
+            ffv_p_raw(A, B, q);
+        }
+        const double sg = flip(1.0, smask);
+#pragma unroll
+        for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, q.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, q.c[c].im, acc.c[c].im); }
     }
 }
 
-// +1.0 or -1.0 from bit `bit` of a word
-__device__ __forceinline__ double sign_of(unsigned word, int bit)
-{
-    return __hiloint2double((int)(0x3FF00000u | ((word << (31 - bit)) & 0x80000000u)), 0);
-}
-
-// a chunk = up to three terms of fixed opcodes for 32 items (CT: one hex digit (opcode - 7) per term)
-template <int CT, int OBJ_PLANE>
-__device__ __forceinline__ void p2_chunk(const char* __restrict__ obj, const char* __restrict__ Ks, const uint2 r0, const uint2 r1,
-                                         const uint2 r2, const uint2 r3, wf<double>& acc)
+// a chunk = up to three terms of fixed opcodes for 32 items (CT: one hex digit (opcode - 7) per term); sign of term j =
+// bit 16 + j of r0.x.  All terms of an item are of one kind: vector-valued (opcodes >= 10: the pair object is contracted
+// with a gluon-type Y, components 1-3 are negated at the store) or spinor-valued (8, 9).
+template <int CT, int OBJ_PLANE, int STG_PLANE>
+__device__ __forceinline__ void p2_chunk(const char* __restrict__ obj, const char* __restrict__ Ks, char* __restrict__ stage,
+                                         const uint2 r0, const uint2 r1, const uint2 r2, const uint2 r3, wf<double>& acc)
 {
     constexpr int O0 = CT & 0xF, O1 = (CT >> 4) & 0xF, O2 = (CT >> 8) & 0xF;
-    x_term<O0 + 7, OBJ_PLANE>(obj, Ks, r1, sign_of(r0.x, 16), acc);
-    if constexpr (O1 != 0) x_term<O1 + 7, OBJ_PLANE>(obj, Ks, r2, sign_of(r0.x, 17), acc);
-    if constexpr (O2 != 0) x_term<O2 + 7, OBJ_PLANE>(obj, Ks, r3, sign_of(r0.x, 18), acc);
+    x_term<O0 + 7, OBJ_PLANE>(obj, Ks, r1, (r0.x << 15) & 0x80000000u, acc);
+    if constexpr (O1 != 0) x_term<O1 + 7, OBJ_PLANE>(obj, Ks, r2, (r0.x << 14) & 0x80000000u, acc);
+    if constexpr (O2 != 0) x_term<O2 + 7, OBJ_PLANE>(obj, Ks, r3, (r0.x << 13) & 0x80000000u, acc);
+    if (r0.y & 0x2000u) {
+        wf<double> o = acc;
+        if constexpr (O0 + 7 >= 10) {
+#pragma unroll
+            for (int c = 1; c < 4; c++) o.c[c] = flip(o.c[c], 0x80000000u);
+        }
+        st_wf<STG_PLANE>(stage, r0.x & 0xFFFFu, o);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -190,11 +197,6 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-__device__ __forceinline__ double flip(double v, unsigned smask)
-{
-    return __hiloint2double(__double2hiint(v) ^ (int)smask, __double2loint(v));
 }
 
 __host__ __device__ constexpr int popc_c(int m)
@@ -252,6 +254,22 @@ __device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const c
     }
 }
 
+// the n entries of shape CODE (= swapped | mask << 1; < 0: shape not used by this process) of the current class
+template <int CODE, int NTILE>
+__device__ __forceinline__ void p3_run(int n, const uint4* __restrict__& rp, uint4& nxt, const char* __restrict__ obj,
+                                       const char* __restrict__ stage, unsigned kO2, unsigned kS2, double (&f)[4 * NTILE])
+{
+    if constexpr (CODE >= 0) {
+        for (int i = 0; i < n; i++) {
+            const uint4 en = nxt;
+            rp += 8;
+            nxt = __ldg(rp);
+            if constexpr (CODE & 1) p3_entry<1, (CODE >> 1), NTILE>(obj, stage, kO2, kS2, en, f);
+            else p3_entry<0, (CODE >> 1), NTILE>(stage, obj, kS2, kO2, en, f);
+        }
+    }
+}
+
 // add the fragments of a finished class to the flow's accumulator (first class: plain store)
 template <int NTILE>
 __device__ __forceinline__ void p3_flush(char* __restrict__ acc, const uint2 cl, const double (&f)[4 * NTILE], bool first)
@@ -297,6 +315,9 @@ __global__ void __launch_bounds__(32 * HS_NW, 2) hs_diagrams_kernel(const HsDev 
     constexpr int NTH = 32 * HS_NW;
     // lane constants of phase 3: (lane % 4) * plane in both 16-bit halves
     const unsigned kS2 = (unsigned)((lane & 3) * STG_PLANE) * 0x10001u, kO2 = (unsigned)((lane & 3) * OBJ_PLANE) * 0x10001u;
+    int posr[NH / 32];                                  // rows of this lane's helicity combinations (write-out of phase 3)
+#pragma unroll
+    for (int j = 0; j < NH / 32; j++) posr[j] = a.d_pos[lane + 32 * j];
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
         // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
         for (int i = tid; i < 4 * NPAR; i += NTH) pm[i] = a.mom[(size_t)e * (4 * NPAR) + i];
@@ -345,63 +366,40 @@ __global__ void __launch_bounds__(32 * HS_NW, 2) hs_diagrams_kernel(const HsDev 
                         for (int q = 0; q < 4; q++) acc.c[q] = mk<double>(0.0, 0.0);
                     }
                     switch (r0.y & 0xFFFu) {
-#define HS_CASE(CT) case CT: p2_chunk<CT, OBJ_PLANE>(obj, Ks, r0, r1, r2, r3, acc); break;
+#define HS_CASE(CT) case CT: p2_chunk<CT, OBJ_PLANE, STG_PLANE>(obj, Ks, stage, r0, r1, r2, r3, acc); break;
                         HS_CHUNK_TYPES(HS_CASE)
 #undef HS_CASE
                         default: break;
                     }
-                    if (r0.y & 0x2000u) st_wf<STG_PLANE>(stage, r0.x & 0xFFFFu, acc);
                 }
             }
             __syncthreads();
-            // phase 3: the jamps of this group; this warp's colour flows
+            // phase 3: the jamps of this group; this warp's colour flows, class by class, one run of entries per shape
             {
                 const int2 sc = __ldg(d.p3sched + g * HS_NW + warp);
                 for (int fl = sc.x; fl < sc.x + sc.y; fl++) {
                     const int4 fd = __ldg(d.p3flow + fl);
-                    const int nent = fd.y & 0xFF, jamp = fd.w;
+                    const int ncls = fd.y & 0xFF, jamp = fd.w;
                     char* __restrict__ acc = accs + (size_t)(fd.y >> 16) * (NH * 16);
                     const uint4* __restrict__ rp = d.p3rec + (size_t)fd.x * 8 + (lane >> 2);
                     const uint2* __restrict__ cp = d.p3cls + (size_t)fd.z * 32 + lane;
-                    int posr[NH / 32];                      // rows of this lane's helicity combinations (write-out below)
-#pragma unroll
-                    for (int j = 0; j < NH / 32; j++) posr[j] = a.d_pos[lane + 32 * j];
-                    double f[4 * NTILE];
-                    bool first_class = true;
-                    // records are fetched four entries ahead (L2 latency of the record stream under load)
-                    uint4 ring[4];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) ring[i] = __ldg(rp + 8 * (i < nent ? i : nent - 1));
+                    const int* __restrict__ hp = d.p3clsh + fd.z;
+                    uint4 nxt = __ldg(rp);                  // the record of the next entry is always in flight
+                    int hdr = __ldg(hp);
                     uint2 cl = __ldg(cp);
-                    for (int k0 = 0; k0 < nent; k0 += 4) {
+                    for (int c = 0; c < ncls; c++) {
+                        const int h_ = hdr;
+                        const uint2 cl_ = cl;
+                        hdr = __ldg(hp + c + 1);            // (one past the end: inside the blob)
+                        cl = __ldg(cp + 32 * (c + 1));
+                        double f[4 * NTILE];
 #pragma unroll
-                        for (int i = 0; i < 4; i++) {
-                            if (k0 + i < nent) {
-                                const uint4 en = ring[i];
-                                ring[i] = __ldg(rp + 8 * (k0 + i + 4 < nent ? k0 + i + 4 : nent - 1));
-                                if (en.w & 0x20u) {
-#pragma unroll
-                                    for (int q = 0; q < 4 * NTILE; q++) f[q] = 0.0;
-                                }
-                                const int swap = en.w & 1;
-                                if (swap) p3_entry<1, 0, NTILE>(obj, stage, kO2, kS2, en, f);
-                                else {
-                                    switch ((en.w >> 1) & 7) {
-                                        case 1: if constexpr (NTILE >= 2) p3_entry<0, 1, NTILE>(stage, obj, kS2, kO2, en, f); break;
-                                        case 2: if constexpr (NTILE >= 4) p3_entry<0, 2, NTILE>(stage, obj, kS2, kO2, en, f); break;
-                                        case 3: if constexpr (NTILE >= 4) p3_entry<0, 3, NTILE>(stage, obj, kS2, kO2, en, f); break;
-                                        default: p3_entry<0, 0, NTILE>(stage, obj, kS2, kO2, en, f); break;
-                                    }
-                                }
-                                if (en.w & 0x10u) {
-                                    __syncwarp();
-                                    p3_flush<NTILE>(acc, cl, f, first_class);
-                                    first_class = false;
-                                    cp += 32;
-                                    cl = __ldg(cp);
-                                }
-                            }
-                        }
+                        for (int q = 0; q < 4 * NTILE; q++) f[q] = 0.0;
+                        p3_run<Cfg::SHAPE0, NTILE>(h_ & 15, rp, nxt, obj, stage, kO2, kS2, f);
+                        p3_run<Cfg::SHAPE1, NTILE>((h_ >> 4) & 15, rp, nxt, obj, stage, kO2, kS2, f);
+                        p3_run<Cfg::SHAPE2, NTILE>((h_ >> 8) & 15, rp, nxt, obj, stage, kO2, kS2, f);
+                        p3_run<Cfg::SHAPE3, NTILE>((h_ >> 12) & 15, rp, nxt, obj, stage, kO2, kS2, f);
+                        p3_flush<NTILE>(acc, cl_, f, c == 0);
                     }
                     __syncwarp();
                     // the finished jamp of this colour flow, all helicity combinations
@@ -459,11 +457,12 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     c->t = t; c->ngluon = ngluon;
     // one device blob, every table 256-byte aligned
     struct Part { const void* src; size_t bytes; size_t off; };
-    Part parts[10] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
+    Part parts[11] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
                        { t->p1_items, sizeof(int) * t->np1, 0 }, { t->legset_mask, sizeof(int) * t->nlegsets, 0 },
                        { t->p2rec, sizeof(unsigned) * 256 * (size_t)t->nchunk, 0 }, { t->p2sched, sizeof(int) * 2 * HS_NW * t->ngroups, 0 },
                        { t->p3rec, sizeof(unsigned) * 32 * (size_t)t->nentry, 0 }, { t->p3cls, sizeof(unsigned) * 64 * (size_t)t->ncls, 0 },
-                       { t->p3flow, sizeof(int) * 4 * t->nflow, 0 }, { t->p3sched, sizeof(int) * 2 * HS_NW * t->ngroups, 0 } };
+                       { t->p3flow, sizeof(int) * 4 * t->nflow, 0 }, { t->p3sched, sizeof(int) * 2 * HS_NW * t->ngroups, 0 },
+                       { t->p3clsh, sizeof(int) * (size_t)t->ncls, 0 } };
     size_t total = 0;
     for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
     total += 4096;                                  // the record prefetch may run a few records past the end of a stream
@@ -480,6 +479,7 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     d.p2rec = (const uint2*)(b + parts[4].off); d.p2sched = (const int2*)(b + parts[5].off);
     d.p3rec = (const uint4*)(b + parts[6].off); d.p3cls = (const uint2*)(b + parts[7].off);
     d.p3flow = (const int4*)(b + parts[8].off); d.p3sched = (const int2*)(b + parts[9].off);
+    d.p3clsh = (const int*)(b + parts[10].off);
     d.ncolor = t->ncolor;
     for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
     c->smem = 4 * (size_t)t->obj_plane + 4 * (size_t)t->stage_plane + (size_t)t->max_flows * (16u << t->npar) +

@@ -29,10 +29,12 @@
 //               off* = byte offset of the argument's slot in object plane 0
 //   p2sched[group * NW + warp] = { first chunk, number of chunks }
 //   p3rec[entry][row = lane / 4] (uint4): x, y, z = 16-bit byte offsets of the A fragments (nA of them, whole words),
-//               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | last-of-class << 4 |
-//               first-of-class << 5 | negative << 31, shape = swapped | mask << 1 (mask: tile bits that select the A fragment)
+//               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | negative << 31,
+//               shape = swapped | mask << 1 (mask: tile bits that select the A fragment); the entries of a class are
+//               sorted by shape, in the order HsCfg<NG>::SHAPE0..3
 //   p3cls[class][lane] (uint2): 16-bit byte offsets into the flow's accumulator of this lane's complex number in tiles 0..3
-//   p3flow[f] = { first entry, entries | classes << 8 | accumulator << 16, first class, jamp index }
+//   p3clsh[class] = number of entries of shape k in bits 4k .. 4k+3
+//   p3flow[f] = { first entry, classes | entries << 8 | accumulator << 16, first class, jamp index }
 //   p3sched[group * NW + warp] = { first flow, number of flows }
 #pragma once
 
@@ -52,6 +54,7 @@ struct HsTables {
     const int* p2sched;
     const unsigned* p3rec;
     const unsigned* p3cls;
+    const int* p3clsh;
     const int* p3flow;
     const int* p3sched;
     double flops_p1, flops_p2, flops_p3;      // per event (phases 1, 2) and per (event, helicity) (phase 3)

@@ -121,6 +121,8 @@ def _key_word(c, sigma):
 
 class Program:
     def __init__(self, n, group_prefix=None):
+        """group_prefix: number of leading letters of sigma shared by a group of colour flows, or "file": the partition
+        of gen/flow_groups_n<n>.txt (gen/regroup.py)"""
         self.n = n
         self.proc = diagrams.build_process(n)
         self.npar = n + 2
@@ -247,11 +249,17 @@ class Program:
         return iy, xop, args, sg
 
     def _build_groups(self, merge=True):
-        """groups of colour flows (same first `group_prefix` letters), their pair objects and dot entries"""
+        """groups of colour flows (same first `group_prefix` letters, or the stored partition), their pair objects and
+        dot entries"""
         gp = self.group_prefix
         order = defaultdict(list)
-        for j, s in enumerate(self.sigmas):
-            order[s[:gp]].append(j)
+        if gp == "file":
+            from . import regroup
+            for k, members in enumerate(regroup.load(self.n, self.sigmas)):
+                order[k] = members
+        else:
+            for j, s in enumerate(self.sigmas):
+                order[s[:gp]].append(j)
         self.groups = []          # dicts: sigmas [j], xobjs [ {legs, terms:[Term]} ], entries {j: [(xslot, yobj, sign)]}
         for pre in sorted(order):
             xkey_to_slot, xobjs, entries = {}, [], {}

@@ -29,7 +29,10 @@ dot-product entries jamp[sigma][h] += sign * sum_c X_c[hx] * Y_c[hy] (phase 3). 
       the fragments added to the flow's accumulator in shared memory (slot = acc_swizzle(helicity)).  An entry fits a
       class if R is inside X's legs and C inside Y's (rows from X) or R = Y's legs and C inside X's ("swapped": rows
       from Y).  Records are per (entry, row = lane / 4): six 16-bit byte offsets (A fragments then B fragments; a lane
-      adds (lane % 4) * PLANE) and a flag word; per (class, lane) the accumulator offsets of the lane's tiles.
+      adds (lane % 4) * PLANE) and a flag word; per (class, lane) the accumulator offsets of the lane's tiles.  Inside a
+      class the entries are sorted by SHAPE (which operand gives the rows, which tile bits select the A fragment) and
+      the class header holds the number of entries of each shape, so that the kernel runs one tight loop per shape
+      with no per-entry dispatch.
 
 Everything here is integer bookkeeping of an exact rewriting; tests/hs_eval.py interprets these very streams in numpy and
 tests/test_generator.py compares the resulting jamps with the oracle (CPU, no kernel involved).
@@ -169,6 +172,8 @@ class Streams:
             for k, x in enumerate(g["xobjs"]):
                 terms = sorted(x["terms"], key=lambda t: (X_ORDER.index(t.op), t.args))
                 shape = tuple(t.op for t in terms)
+                # one kind per item: vector-valued (lowered at the store) or spinor-valued
+                assert len({OPS[o] >= 10 for o in shape}) == 1
                 for v in range(1 << len(x["legs"])):
                     by_shape[shape].append((k, v, terms))
             units = []            # (cost, [chunk blocks])
@@ -243,30 +248,79 @@ class Streams:
         prog, npar = self.prog, self.npar
         ntile = self.ntile
         hbit = lambda p: npar - 1 - p
-        recs, cls_tab, flows, sched = [], [], [], []
         self.max_flows = 0
+        flows_raw = []            # per flow: (group, warp, acc, jamp, [(R, C, T, [(shape, rec)])])
         shapes = set()
         for gi, g in enumerate(prog.groups):
-            per_warp = [[] for _ in range(NW)]
-            for fi, j in enumerate(g["sigmas"]):
-                per_warp[fi % NW].append((fi, j))
             self.max_flows = max(self.max_flows, min(NW, len(g["sigmas"])))
+            for fi, j in enumerate(g["sigmas"]):
+                ents = [(frozenset(g["xobjs"][xs]["legs"]), frozenset(prog.objs[yo].legs), xs, yo, sign)
+                        for xs, yo, sign in g["entries"][j]]
+                classes, covered = self._classes_for([(e[0], e[1]) for e in ents])
+                # every entry goes to the compatible class with the fewest entries so far
+                members = [[] for _ in classes]
+                for i in sorted(range(len(ents)), key=lambda i: sum(i in c for c in covered)):
+                    k = min((k for k in range(len(classes)) if i in covered[k]), key=lambda k: len(members[k]))
+                    members[k].append(i)
+                assert all(members)
+                cls_out = []
+                for (R, C), mem in zip(classes, members):
+                    T = tuple(l for l in range(npar) if l not in R and l not in C)
+                    recs_c = []
+                    for i in mem:
+                        X, Y, xs, yo, sign = ents[i]
+                        xl, yl = tuple(sorted(X)), tuple(sorted(Y))
+                        swapped = not (frozenset(R) <= X)
+                        al, bl = (yl, xl) if swapped else (xl, yl)          # legs of the A-side / B-side operand
+                        a_off = (lambda v: self._obj_off(yo, v)) if swapped else (lambda v: 16 * (self.xslot[gi][xs] + perm(v)))
+                        b_off = (lambda v: 16 * (self.xslot[gi][xs] + perm(v))) if swapped else (lambda v: self._obj_off(yo, v))
+                        assert set(R) <= set(al) and set(C) <= set(bl)
+                        mask = sum(1 << b for b in range(len(T)) if T[b] in al)     # tile bits that select the A fragment
+                        ta = [b for b in range(len(T)) if T[b] in al]
+                        tb = [b for b in range(len(T)) if T[b] not in al]
+                        na, nb = 1 << len(ta), 1 << len(tb)
+                        shape = (1 if swapped else 0) | (mask << 1)
+                        shapes.add((shape, na, nb))
+                        rec = np.zeros((8, 4), dtype=np.uint32)
+                        for row in range(8):
+                            offs = []
+                            for a in range(na):
+                                v = sum(((row >> b) & 1) << al.index(R[b]) for b in range(3))
+                                v |= sum(((a >> q) & 1) << al.index(T[ta[q]]) for q in range(len(ta)))
+                                offs.append(a_off(v))
+                            aw = [0, 0]
+                            for q, o in enumerate(offs):
+                                aw[q >> 1] |= o << (16 * (q & 1))
+                            offs = []
+                            c2, ri = row >> 1, row & 1
+                            for b_ in range(nb):
+                                v = sum(((c2 >> b) & 1) << bl.index(C[b]) for b in range(2))
+                                v |= sum(((b_ >> q) & 1) << bl.index(T[tb[q]]) for q in range(len(tb)))
+                                offs.append(b_off(v) + 8 * ri)
+                            bw = [0, 0]
+                            for q, o in enumerate(offs):
+                                bw[q >> 1] |= o << (16 * (q & 1))
+                            # word layout: A offsets fill x (, y); B offsets follow in the next free word(s)
+                            words = aw[: (na + 1) // 2] + bw[: (nb + 1) // 2]
+                            assert len(words) <= 3
+                            words += [0] * (3 - len(words))
+                            rec[row] = words + [shape | ((1 if sign < 0 else 0) << 31)]
+                        recs_c.append((shape, rec))
+                    cls_out.append((R, C, T, recs_c))
+                flows_raw.append((gi, fi % NW, fi % NW, j, cls_out))
+        self.p3shapes = sorted(shapes)
+        codes = [sh for sh, _, _ in self.p3shapes]
+        assert len(codes) <= 4, "the class header holds four shape counts"
+        self.p3shape_codes = codes
+        recs, cls_tab, cls_hdr, flows, sched = [], [], [], [], []
+        for gi in range(len(prog.groups)):
             for w in range(NW):
-                sched.append((len(flows), len(per_warp[w])))
-                for fi, j in per_warp[w]:
-                    ents = [(frozenset(g["xobjs"][xs]["legs"]), frozenset(prog.objs[yo].legs), xs, yo, sign)
-                            for xs, yo, sign in g["entries"][j]]
-                    classes, covered = self._classes_for([(e[0], e[1]) for e in ents])
-                    # every entry goes to the compatible class with the fewest entries so far
-                    members = [[] for _ in classes]
-                    for i in sorted(range(len(ents)), key=lambda i: sum(i in c for c in covered)):
-                        k = min((k for k in range(len(classes)) if i in covered[k]), key=lambda k: len(members[k]))
-                        members[k].append(i)
-                    assert all(members)
-                    rec0, cls0 = len(recs), len(cls_tab)
-                    for (R, C), mem in zip(classes, members):
-                        T = tuple(l for l in range(npar) if l not in R and l not in C)
-                        # helicity of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
+                mine = [f for f in flows_raw if f[0] == gi and f[1] == w]
+                sched.append((len(flows), len(mine)))
+                for _, _, acc, j, cls_out in mine:
+                    rec0, cls0, nent = len(recs), len(cls_tab), 0
+                    for R, C, T, recs_c in cls_out:
+                        # accumulator slot of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
                         ct = np.zeros((32, 4), dtype=np.uint32)
                         for lane in range(32):
                             row, c2 = lane >> 2, lane & 3
@@ -276,58 +330,23 @@ class Streams:
                                 h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
                                 ct[lane, t] = 16 * acc_swizzle(h)
                         cls_tab.append(ct)
-                        for n_, i in enumerate(mem):
-                            X, Y, xs, yo, sign = ents[i]
-                            xl, yl = tuple(sorted(X)), tuple(sorted(Y))
-                            swapped = not (frozenset(R) <= X)
-                            al, bl = (yl, xl) if swapped else (xl, yl)          # legs of the A-side / B-side operand
-                            a_off = (lambda v: self._obj_off(yo, v)) if swapped else (lambda v: 16 * (self.xslot[gi][xs] + perm(v)))
-                            b_off = (lambda v: 16 * (self.xslot[gi][xs] + perm(v))) if swapped else (lambda v: self._obj_off(yo, v))
-                            assert set(R) <= set(al) and set(C) <= set(bl)
-                            mask = sum(1 << b for b in range(len(T)) if T[b] in al)     # tile bits that select the A fragment
-                            ta = [b for b in range(len(T)) if T[b] in al]
-                            tb = [b for b in range(len(T)) if T[b] not in al]
-                            na, nb = 1 << len(ta), 1 << len(tb)
-                            shape = (1 if swapped else 0) | (mask << 1)
-                            shapes.add((shape, na, nb))
-                            rec = np.zeros((8, 4), dtype=np.uint32)
-                            for row in range(8):
-                                offs = []
-                                for a in range(na):
-                                    v = sum(((row >> b) & 1) << al.index(R[b]) for b in range(3))
-                                    v |= sum(((a >> q) & 1) << al.index(T[ta[q]]) for q in range(len(ta)))
-                                    offs.append(a_off(v))
-                                aw = [0, 0]
-                                for q, o in enumerate(offs):
-                                    aw[q >> 1] |= o << (16 * (q & 1))
-                                offs = []
-                                c2, ri = row >> 1, row & 1
-                                for b_ in range(nb):
-                                    v = sum(((c2 >> b) & 1) << bl.index(C[b]) for b in range(2))
-                                    v |= sum(((b_ >> q) & 1) << bl.index(T[tb[q]]) for q in range(len(tb)))
-                                    offs.append(b_off(v) + 8 * ri)
-                                bw = [0, 0]
-                                for q, o in enumerate(offs):
-                                    bw[q >> 1] |= o << (16 * (q & 1))
-                                # word layout: A offsets fill x (, y); B offsets follow in the next free word(s)
-                                words = aw[: (na + 1) // 2] + bw[: (nb + 1) // 2]
-                                assert len(words) <= 3
-                                words += [0] * (3 - len(words))
-                                flags = shape | ((1 if n_ == len(mem) - 1 else 0) << 4) | ((1 if n_ == 0 else 0) << 5) | \
-                                        ((1 if sign < 0 else 0) << 31)
-                                rec[row] = words + [flags]
-                            recs.append(rec)
-                    flows.append((rec0, len(ents) | (len(classes) << 8) | ((fi % NW) << 16), cls0, j))
+                        recs_c = sorted(recs_c, key=lambda sr: codes.index(sr[0]))        # stable: by shape
+                        counts = [sum(1 for sh, _ in recs_c if sh == c) for c in codes]
+                        assert all(c < 16 for c in counts)
+                        cls_hdr.append(sum(c << (4 * k) for k, c in enumerate(counts)))
+                        recs += [r for _, r in recs_c]
+                        nent += len(recs_c)
+                    flows.append((rec0, len(cls_out) | (nent << 8) | (acc << 16), cls0, j))
         self.p3rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 8, 4)
         self.p3cls = np.asarray(cls_tab, dtype=np.uint32).reshape(-1, 32, 4)
+        self.p3clsh = np.asarray(cls_hdr, dtype=np.int32)
         self.p3flow = np.asarray(flows, dtype=np.int32).reshape(-1, 4)
         self.p3sched = np.asarray(sched, dtype=np.int32).reshape(-1, 2)
-        self.p3shapes = sorted(shapes)
 
     # ---------------------------------------------------------------------------------------------
     def tables(self):
         i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w)
-        ncls = self.p3flow[:, 1] >> 8 & 0xFF
+        ncls = self.p3flow[:, 1] & 0xFF
         return {
             "npar": self.npar, "ncolor": self.ncolor, "ngroups": len(self.prog.groups), "nw": NW, "ntile": self.ntile,
             "ns_obj": self.ns_obj, "obj_plane": self.obj_plane, "ns_stage": self.ns_stage, "stage_plane": self.stage_plane,
@@ -336,8 +355,8 @@ class Streams:
             "obj": i32(self.obj_tab, 4), "term": i32(self.p1_terms, 4), "p1_items": np.asarray(self.p1_items, np.int32),
             "p1_level": np.asarray(self.p1_level, np.int32),
             "p2rec": self.p2rec, "p2sched": self.p2sched, "chunk_types": self.chunk_types,
-            "p3rec": self.p3rec, "p3cls": self.p3cls, "p3flow": self.p3flow, "p3sched": self.p3sched,
-            "p3shapes": self.p3shapes,
+            "p3rec": self.p3rec, "p3cls": self.p3cls, "p3clsh": self.p3clsh, "p3flow": self.p3flow, "p3sched": self.p3sched,
+            "p3shapes": self.p3shapes, "p3shape_codes": self.p3shape_codes,
         }
 
 

@@ -143,55 +143,50 @@ def evaluate(T, mom, mt, wt):
             f0, nf = (int(x) for x in T["p3sched"][g * nw + w])
             for f in range(f0, f0 + nf):
                 rec0, info, cls0, jamp = (int(x) for x in T["p3flow"][f])
-                nent, ncls = info & 0xFF, (info >> 8) & 0xFF
+                ncls, nent = info & 0xFF, (info >> 8) & 0xFF
                 accum = np.zeros(nh, dtype=complex)            # the flow's accumulator in shared memory, [slot]
                 written = np.zeros(nh, dtype=bool)
-                cls, frag = cls0, None
-                for e in range(rec0, rec0 + nent):
-                    rec = T["p3rec"][e]
-                    flags = int(rec[0, 3])
-                    shape, lastc, firstc, neg = flags & 0xF, (flags >> 4) & 1, (flags >> 5) & 1, (flags >> 31) & 1
-                    assert all(int(rec[r, 3]) == flags for r in range(8))
-                    swapped, mask = shape & 1, shape >> 1
-                    na = 1 << bin(mask).count("1")
-                    nb = ntile // na
-                    if firstc:
-                        frag = np.zeros((32, ntile), dtype=complex)
-                    aplanes, bplanes = (obj, stage) if swapped else (stage, obj)
-                    for lane in range(32):
-                        row, kk = lane >> 2, lane & 3
-                        words = [int(x) for x in rec[row, :3]]
-                        halves = [w_ >> (16 * q) & 0xFFFF for w_ in words for q in range(2)]
-                        a_offs = halves[:na]
-                        b_offs = halves[2 * ((na + 1) // 2):][:nb]
-                        # A fragment of this lane: component kk of the variant of row `row`; B fragment: component kk of
-                        # the variant of complex column row >> 1, real or imaginary half by row & 1
-                        for t in range(ntile):
-                            ai = sum(((t >> b) & 1) << i for i, b in enumerate([b for b in range(8) if (mask >> b) & 1]))
-                            bi = sum(((t >> b) & 1) << i for i, b in enumerate([b for b in range(ntile.bit_length() - 1) if not (mask >> b) & 1]))
-                            # the MMA sums over kk; emulate by letting lane (row, c2) gather all four components itself
-                            if True:
+                codes = T["p3shape_codes"]
+                e = rec0
+                for cls in range(cls0, cls0 + ncls):
+                    hdr = int(T["p3clsh"][cls])
+                    frag = np.zeros((32, ntile), dtype=complex)    # register fragments of the class
+                    for k, code in enumerate(codes):               # one run of entries per shape, in the kernel's order
+                        for _ in range((hdr >> (4 * k)) & 15):
+                            rec = T["p3rec"][e]
+                            e += 1
+                            flags = int(rec[0, 3])
+                            assert all(int(rec[r, 3]) == flags for r in range(8)) and (flags & 0xF) == code
+                            neg = (flags >> 31) & 1
+                            swapped, mask = code & 1, code >> 1
+                            na = 1 << bin(mask).count("1")
+                            nb = ntile // na
+                            aplanes, bplanes = (obj, stage) if swapped else (stage, obj)
+                            for lane in range(32):
+                                # the MMA sums over the component index lane % 4 of the fragments; emulate it by letting lane
+                                # (row r_, complex column c2) gather all four components of both operands itself
                                 r_, c2 = lane >> 2, lane & 3
-                                arow = [int(x) for x in rec[r_, :3]]
-                                ah = [w_ >> (16 * q) & 0xFFFF for w_ in arow for q in range(2)][:na]
-                                # column c2 is served by record rows 2 c2 (re half) and 2 c2 + 1 (im half): same slot, +8 bytes
-                                brow = [int(x) for x in rec[2 * c2, :3]]
-                                bh = [w_ >> (16 * q) & 0xFFFF for w_ in brow for q in range(2)][2 * ((na + 1) // 2):][:nb]
-                                brow1 = [int(x) for x in rec[2 * c2 + 1, :3]]
-                                bh1 = [w_ >> (16 * q) & 0xFFFF for w_ in brow1 for q in range(2)][2 * ((na + 1) // 2):][:nb]
-                                assert bh[bi] % 16 == 0 and bh1[bi] == bh[bi] + 8
-                                Xv, Yv = aplanes.load(ah[ai]), bplanes.load(bh[bi])
-                                val = np.sum(Xv * Yv)
-                                frag[lane, t] += -val if neg else val
-                    if lastc:
-                        for lane in range(32):
-                            for t in range(ntile):
-                                off = int(T["p3cls"][cls][lane, t])
-                                assert off % 16 == 0
-                                accum[off // 16] += frag[lane, t]
-                                written[off // 16] = True
-                        cls += 1
-                assert cls == cls0 + ncls and written.all()
+                                for t in range(ntile):
+                                    ai = sum(((t >> b_) & 1) << i for i, b_ in enumerate([b_ for b_ in range(8) if (mask >> b_) & 1]))
+                                    bi = sum(((t >> b_) & 1) << i for i, b_ in
+                                             enumerate([b_ for b_ in range(ntile.bit_length() - 1) if not (mask >> b_) & 1]))
+                                    arow = [int(x) for x in rec[r_, :3]]
+                                    ah = [w_ >> (16 * q) & 0xFFFF for w_ in arow for q in range(2)][:na]
+                                    # column c2 is served by record rows 2 c2 (re half) and 2 c2 + 1 (im half): same slot, +8 bytes
+                                    brow = [int(x) for x in rec[2 * c2, :3]]
+                                    bh = [w_ >> (16 * q) & 0xFFFF for w_ in brow for q in range(2)][2 * ((na + 1) // 2):][:nb]
+                                    brow1 = [int(x) for x in rec[2 * c2 + 1, :3]]
+                                    bh1 = [w_ >> (16 * q) & 0xFFFF for w_ in brow1 for q in range(2)][2 * ((na + 1) // 2):][:nb]
+                                    assert bh[bi] % 16 == 0 and bh1[bi] == bh[bi] + 8
+                                    val = np.sum(aplanes.load(ah[ai]) * bplanes.load(bh[bi]))
+                                    frag[lane, t] += -val if neg else val
+                    for lane in range(32):
+                        for t in range(ntile):
+                            off = int(T["p3cls"][cls][lane, t])
+                            assert off % 16 == 0
+                            accum[off // 16] += frag[lane, t]
+                            written[off // 16] = True
+                assert e == rec0 + nent and written.all()
                 for h in range(nh):
                     J[jamp][h] = accum[_acc_swizzle(h)]
     assert not np.isnan(J).any()

@@ -77,14 +77,14 @@ def test_program_matches_oracle_per_helicity(name, n, hels, params):
         assert abs(mh / mh_o[1][h] - 1) < 1e-10, (h, mh, mh_o[1][h])
 
 
-@pytest.mark.parametrize("name,n,gp,nev", [("gg_ttxgg", 4, 0, 2), ("gg_ttxggg", 5, 2, 1)])
-def test_helicity_shared_streams_match_oracle(name, n, gp, nev, params):
+@pytest.mark.parametrize("name,n,nev", [("gg_ttxgg", 4, 2), ("gg_ttxggg", 5, 1)])
+def test_helicity_shared_streams_match_oracle(name, n, nev, params):
     """the device streams of the helicity-shared kernel (gen/hs_streams.py: merged four-gluon vertices, X.Y split, chunks,
     classes, packed offsets), interpreted lane by lane by tests/hs_eval.py, give the oracle's per-helicity colour-summed
     |M|^2 for EVERY helicity -- the program that is the default for these processes, checked without a GPU"""
     import hs_eval
-    from paper_2510_05392_b200.gen import hs_streams
-    T = hs_streams.build(n, gp).tables()
+    from paper_2510_05392_b200.gen import emit_hs, hs_streams
+    T = hs_streams.build(n, emit_hs.GROUP_PREFIX[n]).tables()          # the grouping the library is built with
     C = np.array([[float(x) for x in r] for r in colour.colour_matrix(n)])
     gs = math.sqrt(4 * math.pi * params["aS"])
     p = inputs.momenta(name, nev, seed=7)

@@ -190,7 +190,7 @@ def _full_size_sample(proc, process, nevt, nrandom, seed):
     library processes separately (jamps buffer chunks)"""
     rng = np.random.default_rng(seed)
     edge = min(1024, nevt // 4)
-    parts = [np.arange(edge), np.arange(nevt - edge, nevt), rng.integers(0, nevt, nrandom)]
+    parts = [np.arange(edge), np.arange(nevt - edge, nevt), edge + rng.choice(nevt - 2 * edge, min(nrandom, nevt - 2 * edge), replace=False)]
     elem = 8 if proc.precision == 0 else 4
     per_evt = proc.ngood * proc.ncolor * 2 * elem
     ce = max(128, ((proc.get_option("jamp_chunk_mib") << 20) // per_evt) // 128 * 128)
