@@ -5,14 +5,20 @@
 // recompute every wavefunction, with up to 121 wavefunctions + 120 jamps of per-thread state (PAPER.md:101-119, 141,
 // 187) -- 12 KB per thread, i.e. local-memory traffic.  Here the state that depends on few helicities lives once per
 // event in shared memory (<= 8 variants per object; phase 1), the vertices are contracted with all branches but the
-// largest once per variant (phase 2: straight-line code per chunk type, chunks dealt to the warps at build time), and the
-// per-helicity work is a stream of 4-component complex dot products evaluated for all helicities at once on the FP64
-// tensor path (phase 3), accumulated in register fragments per class of entries.  Every jamp is finished on chip and
-// written once, coalesced, to the jamps buffer, rows ordered (event, helicity).
+// largest once per variant (phase 2: straight-line code per chunk type) and the per-helicity work is a stream of
+// 4-component complex dot products evaluated for all helicities at once on the FP64 tensor path (phase 3), accumulated in
+// register fragments per class of entries.  Every jamp is finished on chip and written once, coalesced, to the jamps
+// buffer, rows ordered (event, helicity).
+//
+// Scheduling inside the CTA: the work items of a step -- the colour flows of group g (phase 3) and, when the staging area
+// is double-buffered (HsCfg::NBUF = 2), the phase-2 units of group g + 1 -- are dealt to the warps at build time by their
+// instruction counts (gen/hs_streams.py _schedule), with ONE barrier per step; a warp pulls the records of its next item
+// into L1 while it works on the current one.  The paper's counterpart is the sequence of diagram-group kernels on
+// helicity streams; here a "group" never leaves the SM.
 //
 // Every shared-memory address of phases 2 and 3 comes precomputed from the streams: an argument costs one 16-bit
 // extraction, its four components are immediate offsets (component planes), and there is no interpretation of opcodes
-// inside a chunk or an entry (the opcode sequence is a template parameter).
+// inside a chunk or an entry (the opcode sequence / the shape is a template parameter).
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -25,11 +31,18 @@ namespace mg {
 
 struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
-    const uint2* p2rec; const int2* p2sched;
-    const uint4* p3rec; const uint2* p3cls; const int* p3clsh; const int4* p3flow; const int2* p3sched;
-    int ncolor;
+    const uint2* p2rec; const unsigned* wsched; const unsigned* witem;
+    const uint4* p3rec; const uint2* p3cls; const int* p3clsh; const int4* p3flow;
+    int ncolor, nflow, ncls, nsched, nitem;
     int p1_level[4];
 };
+
+// the small tables every work item starts from, copied to shared memory once per (persistent) CTA
+struct HsSmemTabs {
+    const int4* p3flow; const int* p3clsh; const unsigned* wsched; const unsigned* witem;
+};
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // variant of an argument object: bit j = bit ((code >> 3j) & 7) of the parent's variant (7 = none; variants are < 128)
 __device__ __forceinline__ int sub_variant(int var, int code)
@@ -215,10 +228,10 @@ __host__ __device__ constexpr int pext_c(int t, int m)
 }
 
 // SWAP = 0: rows from the pair object X (staging area), columns from Y (object area); 1: the other way round.
-// MASK: tile bits that select the A fragment.  kA2 / kB2 = (lane % 4) * plane of the A / B operand, in both 16-bit halves.
+// MASK: tile bits that select the A fragment.  abase / bbase = plane (lane % 4) of the A / B operand's area.
 template <int SWAP, int MASK, int NTILE>
-__device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const char* __restrict__ bbase, unsigned kA2, unsigned kB2,
-                                         const uint4 e, double (&f)[4 * NTILE])
+__device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const char* __restrict__ bbase, const uint4 e,
+                                         double (&f)[4 * NTILE])
 {
     constexpr int NA = 1 << popc_c(MASK), NB = NTILE / NA, AW = (NA + 1) / 2;
     const unsigned w[3] = { e.x, e.y, e.z };
@@ -227,13 +240,13 @@ __device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const c
     double b0[NB], b1[NB];
 #pragma unroll
     for (int a = 0; a < NA; a++) {
-        const unsigned word = w[a >> 1] + kA2;
+        const unsigned word = w[a >> 1];
         const unsigned off = (a & 1) ? (word >> 16) : (word & 0xFFFFu);
         xa[a] = *reinterpret_cast<const double2*>(abase + off);
     }
 #pragma unroll
     for (int b = 0; b < NB; b++) {
-        const unsigned word = w[AW + (b >> 1)] + kB2;
+        const unsigned word = w[AW + (b >> 1)];
         const unsigned off = (b & 1) ? (word >> 16) : (word & 0xFFFFu);
         b0[b] = *reinterpret_cast<const double*>(bbase + off);           // odd column (im out): Im, even: Re
         b1[b] = *reinterpret_cast<const double*>(bbase + (off ^ 8u));    // odd column: Re, even: Im
@@ -254,18 +267,19 @@ __device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const c
     }
 }
 
-// the n entries of shape CODE (= swapped | mask << 1; < 0: shape not used by this process) of the current class
+// the n entries of shape CODE (= swapped | mask << 1; < 0: shape not used by this process) of the current class;
+// objl / stgl = plane (lane % 4) of the object area / of the group's staging area
 template <int CODE, int NTILE>
-__device__ __forceinline__ void p3_run(int n, const uint4* __restrict__& rp, uint4& nxt, const char* __restrict__ obj,
-                                       const char* __restrict__ stage, unsigned kO2, unsigned kS2, double (&f)[4 * NTILE])
+__device__ __forceinline__ void p3_run(int n, const uint4* __restrict__& rp, uint4& nxt, const char* __restrict__ objl,
+                                       const char* __restrict__ stgl, double (&f)[4 * NTILE])
 {
     if constexpr (CODE >= 0) {
         for (int i = 0; i < n; i++) {
             const uint4 en = nxt;
             rp += 8;
             nxt = __ldg(rp);
-            if constexpr (CODE & 1) p3_entry<1, (CODE >> 1), NTILE>(obj, stage, kO2, kS2, en, f);
-            else p3_entry<0, (CODE >> 1), NTILE>(stage, obj, kS2, kO2, en, f);
+            if constexpr (CODE & 1) p3_entry<1, (CODE >> 1), NTILE>(objl, stgl, en, f);
+            else p3_entry<0, (CODE >> 1), NTILE>(stgl, objl, en, f);
         }
     }
 }
@@ -298,26 +312,117 @@ __device__ __forceinline__ int acc_swizzle(int h)
     return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7));
 }
 
-// T2 = type of the jamps buffer (double: MG_FP64, float: MG_MIXED -- PAPER.md:122 "FPTYPE=m")
+// one colour flow (phase 3): class by class, one run of entries per shape, then the finished jamp of all helicity
+// combinations is written out
 template <int NG, typename T2>
-__global__ void __launch_bounds__(32 * HS_NW, 2) hs_diagrams_kernel(const HsDev d, const HsLaunch a)
+__device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, const HsLaunch& a, int fl, int e, const char* __restrict__ objl,
+                                        const char* __restrict__ stgl, char* __restrict__ accs, int warp, int lane,
+                                        const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32])
 {
     using Cfg = HsCfg<NG>;
-    constexpr int NPAR = Cfg::NPAR, NH = 1 << NPAR, NTILE = Cfg::NTILE;
+    constexpr int NH = 1 << Cfg::NPAR, NTILE = Cfg::NTILE;
+    const int4 fd = tb.p3flow[fl];
+    const int ncls = fd.y & 0xFF, jamp = fd.w;
+    // one accumulator per flow of the group, or per warp when a group has more flows than the CTA has warps
+    char* __restrict__ acc = accs + (size_t)(Cfg::MAX_FLOWS > Cfg::NW ? warp : (fd.y >> 16)) * (NH * 16);
+    const uint4* __restrict__ rp = d.p3rec + (size_t)fd.x * 8 + (lane >> 2);
+    const uint2* __restrict__ cp = d.p3cls + (size_t)fd.z * 32 + lane;
+    const int* __restrict__ hp = tb.p3clsh + fd.z;
+    uint4 nxt = __ldg(rp);                  // the record of the next entry is always in flight
+    uint2 cl = __ldg(cp);
+    for (int c = 0; c < ncls; c++) {
+        const int h_ = hp[c];
+        const uint2 cl_ = cl;
+        cl = __ldg(cp + 32 * (c + 1));      // (one past the end: inside the blob)
+        double f[4 * NTILE];
+#pragma unroll
+        for (int q = 0; q < 4 * NTILE; q++) f[q] = 0.0;
+        p3_run<Cfg::SHAPE0, NTILE>(h_ & 15, rp, nxt, objl, stgl, f);
+        p3_run<Cfg::SHAPE1, NTILE>((h_ >> 4) & 15, rp, nxt, objl, stgl, f);
+        p3_run<Cfg::SHAPE2, NTILE>((h_ >> 8) & 15, rp, nxt, objl, stgl, f);
+        p3_run<Cfg::SHAPE3, NTILE>((h_ >> 12) & 15, rp, nxt, objl, stgl, f);
+        p3_flush<NTILE>(acc, cl_, f, c == 0);
+    }
+    __syncwarp();
+    T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
+#pragma unroll
+    for (int j = 0; j < NH / 32; j++) {
+        const int h = lane + 32 * j, pos = posr[j];
+        if (pos >= 0) {
+            const double2 v = *reinterpret_cast<const double2*>(acc + 16 * acc_swizzle(h));
+            const size_t row = (size_t)e * a.nrow_evt + pos;
+            if (a.tile_major) {
+                T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)jamp * 128 + (row & 127);
+                o[0] = T2(v.x); o[(size_t)d.ncolor * 128] = T2(v.y);
+            } else {
+                out[(size_t)jamp * a.rows + row] = T2(v.x);
+                out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// one unit of phase 2: the chunks of the same 32 (pair object, variant) items; the next chunk's records are in flight
+template <int NG>
+__device__ __forceinline__ void p2_unit(const HsDev& d, int chunk0, int nchunk, const char* __restrict__ obj,
+                                        const char* __restrict__ Ks, char* __restrict__ stage, int lane)
+{
+    using Cfg = HsCfg<NG>;
     constexpr int OBJ_PLANE = Cfg::OBJ_PLANE, STG_PLANE = Cfg::STG_PLANE;
+    const uint2* __restrict__ rp = d.p2rec + (size_t)chunk0 * 128 + lane;
+    uint2 n0 = __ldg(rp), n1 = __ldg(rp + 32), n2 = __ldg(rp + 64), n3 = __ldg(rp + 96);
+    wf<double> acc;
+#pragma unroll
+    for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
+    for (int c = 0; c < nchunk; c++) {
+        const uint2 r0 = n0, r1 = n1, r2 = n2, r3 = n3;
+        rp += 128;
+        if (c + 1 < nchunk) { n0 = __ldg(rp); n1 = __ldg(rp + 32); n2 = __ldg(rp + 64); n3 = __ldg(rp + 96); }
+        switch (r0.y & 0xFFFu) {
+#define HS_CASE(CT) case CT: p2_chunk<CT, OBJ_PLANE, STG_PLANE>(obj, Ks, stage, r0, r1, r2, r3, acc); break;
+            HS_CHUNK_TYPES(HS_CASE)
+#undef HS_CASE
+            default: break;
+        }
+    }
+}
+
+// T2 = type of the jamps buffer (double: MG_FP64, float: MG_MIXED -- PAPER.md:122 "FPTYPE=m")
+template <int NG, typename T2>
+__global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagrams_kernel(const HsDev d, const HsLaunch a)
+{
+    using Cfg = HsCfg<NG>;
+    constexpr int NPAR = Cfg::NPAR, NH = 1 << NPAR, NW = Cfg::NW, NBUF = Cfg::NBUF, NGROUPS = Cfg::NGROUPS;
+    constexpr int OBJ_PLANE = Cfg::OBJ_PLANE, STG_PLANE = Cfg::STG_PLANE;
+    constexpr int NACC = Cfg::MAX_FLOWS > NW ? NW : Cfg::MAX_FLOWS;
     extern __shared__ __align__(128) char sm[];
     char* __restrict__ obj = sm;
-    char* __restrict__ stage = sm + 4 * OBJ_PLANE;
-    char* __restrict__ accs = stage + 4 * STG_PLANE;
-    char* __restrict__ Ks = accs + Cfg::MAX_FLOWS * NH * 16;
+    char* __restrict__ stage0 = sm + 4 * OBJ_PLANE;
+    char* __restrict__ accs = stage0 + NBUF * 4 * STG_PLANE;
+    char* __restrict__ Ks = accs + NACC * NH * 16;
     double* __restrict__ pm = reinterpret_cast<double*>(Ks + 32 * Cfg::NLEGSETS);
+    HsSmemTabs tb;
+    {
+        int4* t0 = reinterpret_cast<int4*>(pm + 4 * NPAR);
+        int* t1 = reinterpret_cast<int*>(t0 + d.nflow);
+        unsigned* t2 = reinterpret_cast<unsigned*>(t1 + d.ncls);
+        unsigned* t3 = t2 + d.nsched;
+        for (int i = threadIdx.x; i < d.nflow; i += blockDim.x) t0[i] = __ldg(d.p3flow + i);
+        for (int i = threadIdx.x; i < d.ncls; i += blockDim.x) t1[i] = __ldg(d.p3clsh + i);
+        for (int i = threadIdx.x; i < d.nsched; i += blockDim.x) t2[i] = __ldg(d.wsched + i);
+        for (int i = threadIdx.x; i < d.nitem; i += blockDim.x) t3[i] = __ldg(d.witem + i);
+        tb.p3flow = t0; tb.p3clsh = t1; tb.wsched = t2; tb.witem = t3;
+    }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NTH = 32 * HS_NW;
-    // lane constants of phase 3: (lane % 4) * plane in both 16-bit halves
-    const unsigned kS2 = (unsigned)((lane & 3) * STG_PLANE) * 0x10001u, kO2 = (unsigned)((lane & 3) * OBJ_PLANE) * 0x10001u;
+    constexpr int NTH = 32 * NW;
+    const char* __restrict__ objl = obj + (lane & 3) * OBJ_PLANE;             // plane of this lane's fragment component
     int posr[NH / 32];                                  // rows of this lane's helicity combinations (write-out of phase 3)
 #pragma unroll
     for (int j = 0; j < NH / 32; j++) posr[j] = a.d_pos[lane + 32 * j];
+    // steps of one event: NBUF = 2: step s = phase 3 of group s - 1 together with phase 2 of group s (s = 0 .. NGROUPS);
+    //                     NBUF = 1: step 2 g = phase 2 of group g, step 2 g + 1 = phase 3 of group g
+    constexpr int NSTEPS = NBUF == 2 ? NGROUPS + 1 : 2 * NGROUPS;
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
         // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
         for (int i = tid; i < 4 * NPAR; i += NTH) pm[i] = a.mom[(size_t)e * (4 * NPAR) + i];
@@ -347,80 +452,34 @@ __global__ void __launch_bounds__(32 * HS_NW, 2) hs_diagrams_kernel(const HsDev 
             }
             __syncthreads();
         }
-        for (int g = 0; g < Cfg::NGROUPS; g++) {
-            // phase 2: pair objects of this group; this warp's chunks (static schedule), next chunk's records in flight
-            {
-                const int2 sc = __ldg(d.p2sched + g * HS_NW + warp);
-                const uint2* __restrict__ rp = d.p2rec + (size_t)sc.x * 128 + lane;
-                uint2 n0 = make_uint2(0u, 0u), n1 = n0, n2 = n0, n3 = n0;
-                if (sc.y > 0) { n0 = __ldg(rp); n1 = __ldg(rp + 32); n2 = __ldg(rp + 64); n3 = __ldg(rp + 96); }
-                wf<double> acc;
-#pragma unroll
-                for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
-                for (int c = 0; c < sc.y; c++) {
-                    const uint2 r0 = n0, r1 = n1, r2 = n2, r3 = n3;
-                    rp += 128;
-                    if (c + 1 < sc.y) { n0 = __ldg(rp); n1 = __ldg(rp + 32); n2 = __ldg(rp + 64); n3 = __ldg(rp + 96); }
-                    if (r0.y & 0x1000u) {
-#pragma unroll
-                        for (int q = 0; q < 4; q++) acc.c[q] = mk<double>(0.0, 0.0);
-                    }
-                    switch (r0.y & 0xFFFu) {
-#define HS_CASE(CT) case CT: p2_chunk<CT, OBJ_PLANE, STG_PLANE>(obj, Ks, stage, r0, r1, r2, r3, acc); break;
-                        HS_CHUNK_TYPES(HS_CASE)
-#undef HS_CASE
-                        default: break;
-                    }
+        for (int s = 0; s < NSTEPS; s++) {
+            // staging buffer the units of this step fill, and the one its colour flows read
+            const int b2 = NBUF == 2 ? (s & 1) : 0, b3 = NBUF == 2 ? ((s - 1) & 1) : 0;
+            char* __restrict__ stage2 = stage0 + b2 * 4 * STG_PLANE;
+            const char* __restrict__ stgl3 = stage0 + b3 * 4 * STG_PLANE + (lane & 3) * STG_PLANE;
+            const unsigned sc = tb.wsched[s * NW + warp];
+            const unsigned* __restrict__ ip = tb.witem + (sc & 0xFFFFu);
+            const int n = sc >> 16;
+            // pull the records of an item into L1: entry records (128 B each) by lanes 0 .., class tables (256 B each) by
+            // lanes 16 .. for a colour flow; the chunks (1 KB each) of a unit
+            auto pull = [&](unsigned it) {
+                if (it >> 31) {
+                    if (lane < 8 * (int)((it >> 16) & 0xFF))
+                        prefetch_l1(reinterpret_cast<const char*>(d.p2rec) + (1024u * (it & 0xFFFFu) + 128u * lane));
+                } else {
+                    const int4 fd = tb.p3flow[it];
+                    const bool cls = lane >= 16;
+                    const unsigned cnt = cls ? 2u * (fd.y & 0xFF) : ((fd.y >> 8) & 0xFF);
+                    const char* base = cls ? reinterpret_cast<const char*>(d.p3cls) : reinterpret_cast<const char*>(d.p3rec);
+                    const unsigned first = cls ? 256u * fd.z : 128u * fd.x;
+                    if ((unsigned)(lane & 15) < cnt) prefetch_l1(base + (first + 128u * (lane & 15)));
                 }
-            }
-            __syncthreads();
-            // phase 3: the jamps of this group; this warp's colour flows, class by class, one run of entries per shape
-            {
-                const int2 sc = __ldg(d.p3sched + g * HS_NW + warp);
-                for (int fl = sc.x; fl < sc.x + sc.y; fl++) {
-                    const int4 fd = __ldg(d.p3flow + fl);
-                    const int ncls = fd.y & 0xFF, jamp = fd.w;
-                    char* __restrict__ acc = accs + (size_t)(fd.y >> 16) * (NH * 16);
-                    const uint4* __restrict__ rp = d.p3rec + (size_t)fd.x * 8 + (lane >> 2);
-                    const uint2* __restrict__ cp = d.p3cls + (size_t)fd.z * 32 + lane;
-                    const int* __restrict__ hp = d.p3clsh + fd.z;
-                    uint4 nxt = __ldg(rp);                  // the record of the next entry is always in flight
-                    int hdr = __ldg(hp);
-                    uint2 cl = __ldg(cp);
-                    for (int c = 0; c < ncls; c++) {
-                        const int h_ = hdr;
-                        const uint2 cl_ = cl;
-                        hdr = __ldg(hp + c + 1);            // (one past the end: inside the blob)
-                        cl = __ldg(cp + 32 * (c + 1));
-                        double f[4 * NTILE];
-#pragma unroll
-                        for (int q = 0; q < 4 * NTILE; q++) f[q] = 0.0;
-                        p3_run<Cfg::SHAPE0, NTILE>(h_ & 15, rp, nxt, obj, stage, kO2, kS2, f);
-                        p3_run<Cfg::SHAPE1, NTILE>((h_ >> 4) & 15, rp, nxt, obj, stage, kO2, kS2, f);
-                        p3_run<Cfg::SHAPE2, NTILE>((h_ >> 8) & 15, rp, nxt, obj, stage, kO2, kS2, f);
-                        p3_run<Cfg::SHAPE3, NTILE>((h_ >> 12) & 15, rp, nxt, obj, stage, kO2, kS2, f);
-                        p3_flush<NTILE>(acc, cl_, f, c == 0);
-                    }
-                    __syncwarp();
-                    // the finished jamp of this colour flow, all helicity combinations
-                    T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
-#pragma unroll
-                    for (int j = 0; j < NH / 32; j++) {
-                        const int h = lane + 32 * j, pos = posr[j];
-                        if (pos >= 0) {
-                            const double2 v = *reinterpret_cast<const double2*>(acc + 16 * acc_swizzle(h));
-                            const size_t row = (size_t)e * a.nrow_evt + pos;
-                            if (a.tile_major) {
-                                T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)jamp * 128 + (row & 127);
-                                o[0] = T2(v.x); o[(size_t)d.ncolor * 128] = T2(v.y);
-                            } else {
-                                out[(size_t)jamp * a.rows + row] = T2(v.x);
-                                out[(size_t)(d.ncolor + jamp) * a.rows + row] = T2(v.y);
-                            }
-                        }
-                    }
-                    __syncwarp();
-                }
+            };
+            for (int k = 0; k < n; k++) {
+                const unsigned it = ip[k];
+                if (k + 1 < n) pull(ip[k + 1]);
+                if (it >> 31) p2_unit<NG>(d, it & 0xFFFFu, (it >> 16) & 0xFF, obj, Ks, stage2, lane);
+                else p3_flow<NG, T2>(d, tb, a, it, e, objl, stgl3, accs, warp, lane, posr);
             }
             __syncthreads();
         }
@@ -434,10 +493,20 @@ struct HsContext {
     HsDev d;
     void* blob = nullptr;
     size_t smem = 0;
+    int threads = 0, ctas = 1, sms = 0;
 };
 
 const HsTables* hs_host_tables(const HsContext* c) { return c->t; }
 size_t hs_smem_bytes(const HsContext* c) { return c->smem; }
+
+template <int NG> static size_t smem_bytes(const HsTables* t)
+{
+    using Cfg = HsCfg<NG>;
+    constexpr int NACC = Cfg::MAX_FLOWS > Cfg::NW ? Cfg::NW : Cfg::MAX_FLOWS;
+    return 4 * (size_t)Cfg::OBJ_PLANE + Cfg::NBUF * 4 * (size_t)Cfg::STG_PLANE + (size_t)NACC * (16u << Cfg::NPAR) +
+           32 * (size_t)Cfg::NLEGSETS + 32 * (size_t)Cfg::NPAR +
+           16 * (size_t)t->nflow + 4 * (size_t)t->ncls + 4 * (size_t)t->nsteps * Cfg::NW + 4 * (size_t)t->nitem;
+}
 
 template <int NG> static cudaError_t set_smem(size_t smem)
 {
@@ -455,13 +524,20 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     if (!t) return cudaErrorInvalidValue;
     HsContext* c = new HsContext;
     c->t = t; c->ngluon = ngluon;
+    int c_nw = 0;
+    switch (ngluon) {
+#define HS_NWOF(N) case N: c_nw = HsCfg<N>::NW; break;
+        HS_PROCESSES(HS_NWOF)
+#undef HS_NWOF
+        default: delete c; return cudaErrorInvalidValue;
+    }
     // one device blob, every table 256-byte aligned
     struct Part { const void* src; size_t bytes; size_t off; };
     Part parts[11] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
                        { t->p1_items, sizeof(int) * t->np1, 0 }, { t->legset_mask, sizeof(int) * t->nlegsets, 0 },
-                       { t->p2rec, sizeof(unsigned) * 256 * (size_t)t->nchunk, 0 }, { t->p2sched, sizeof(int) * 2 * HS_NW * t->ngroups, 0 },
+                       { t->p2rec, sizeof(unsigned) * 256 * (size_t)t->nchunk, 0 }, { t->wsched, sizeof(unsigned) * (size_t)t->nsteps * (c_nw), 0 },
                        { t->p3rec, sizeof(unsigned) * 32 * (size_t)t->nentry, 0 }, { t->p3cls, sizeof(unsigned) * 64 * (size_t)t->ncls, 0 },
-                       { t->p3flow, sizeof(int) * 4 * t->nflow, 0 }, { t->p3sched, sizeof(int) * 2 * HS_NW * t->ngroups, 0 },
+                       { t->p3flow, sizeof(int) * 4 * t->nflow, 0 }, { t->witem, sizeof(unsigned) * (size_t)t->nitem, 0 },
                        { t->p3clsh, sizeof(int) * (size_t)t->ncls, 0 } };
     size_t total = 0;
     for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
@@ -476,16 +552,19 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     HsDev& d = c->d;
     d.obj = (const int4*)(b + parts[0].off); d.term = (const int4*)(b + parts[1].off);
     d.p1_items = (const int*)(b + parts[2].off); d.legset_mask = (const int*)(b + parts[3].off);
-    d.p2rec = (const uint2*)(b + parts[4].off); d.p2sched = (const int2*)(b + parts[5].off);
+    d.p2rec = (const uint2*)(b + parts[4].off); d.wsched = (const unsigned*)(b + parts[5].off);
     d.p3rec = (const uint4*)(b + parts[6].off); d.p3cls = (const uint2*)(b + parts[7].off);
-    d.p3flow = (const int4*)(b + parts[8].off); d.p3sched = (const int2*)(b + parts[9].off);
+    d.p3flow = (const int4*)(b + parts[8].off); d.witem = (const unsigned*)(b + parts[9].off);
     d.p3clsh = (const int*)(b + parts[10].off);
-    d.ncolor = t->ncolor;
+    d.ncolor = t->ncolor; d.nflow = t->nflow; d.ncls = t->ncls; d.nsched = t->nsteps * c_nw; d.nitem = t->nitem;
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
-    c->smem = 4 * (size_t)t->obj_plane + 4 * (size_t)t->stage_plane + (size_t)t->max_flows * (16u << t->npar) +
-              32 * (size_t)t->nlegsets + 32 * (size_t)t->npar;
     switch (ngluon) {
-#define HS_SET(N) case N: e = set_smem<N>(c->smem); break;
+#define HS_SET(N) case N: c->smem = smem_bytes<N>(t); c->threads = 32 * HsCfg<N>::NW; c->ctas = HsCfg<N>::CTAS; e = set_smem<N>(c->smem); break;
         HS_PROCESSES(HS_SET)
 #undef HS_SET
         default: e = cudaErrorInvalidValue;
@@ -505,12 +584,13 @@ void hs_destroy(HsContext* c)
 cudaError_t hs_launch(const HsContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st)
 {
     if (a.nevt <= 0) return cudaSuccess;
-    const int grid = a.nevt;                         // one CTA per event; the hardware scheduler keeps every SM full
+    const int full = c->sms * c->ctas;                // persistent CTAs: the small tables are staged once per CTA
+    const int grid = a.nevt < full ? a.nevt : full;
     switch (c->ngluon) {
 #define HS_GO(N)                                                                                           \
     case N:                                                                                                \
-        if (jamps_fp64) hs_diagrams_kernel<N, double><<<grid, 32 * HS_NW, c->smem, st>>>(c->d, a);          \
-        else hs_diagrams_kernel<N, float><<<grid, 32 * HS_NW, c->smem, st>>>(c->d, a);                      \
+        if (jamps_fp64) hs_diagrams_kernel<N, double><<<grid, c->threads, c->smem, st>>>(c->d, a);          \
+        else hs_diagrams_kernel<N, float><<<grid, c->threads, c->smem, st>>>(c->d, a);                      \
         break;
         HS_PROCESSES(HS_GO)
 #undef HS_GO

@@ -1,11 +1,11 @@
 // hs_tables.h -- device streams of the helicity-shared diagram program (written by gen/hs_streams.py through
 // gen/emit_hs.py, read by hs_kernel.cu).
 //
-// One CTA (NW = 8 warps) evaluates one event for all 2^npar helicity combinations:
+// One CTA (HsCfg<NG>::NW warps) evaluates one event for all 2^npar helicity combinations:
 //   phase 1  colour-ordered objects with <= 3 legs (signed sums of Feynman off-shell currents of one leg set), every
 //            helicity variant of their own legs, level by level, into the object area
 //   phase 2  per group of colour flows: pair objects X = raw vertex contracted with all branches but the largest (Y),
-//            into the staging area; "chunks" of 32 lanes x <= 3 terms of the same opcodes, dealt to the warps at build time
+//            into the staging area; "chunks" of 32 lanes x <= 3 terms of the same opcodes
 //   phase 3  jamp[sigma][h] = sum_entries sign * sum_c X_c[variant_x(h)] * Y_c[variant_y(h)] on the FP64 tensor path,
 //            one warp per colour flow, entries sorted into classes that share their register fragments
 //
@@ -27,7 +27,11 @@
 //                      type = one hex digit (op - 7) per term, first term in the low digit
 //               rec1..3 (term k) = { offA | offB << 16, offC }; x_v3: { offA | offB << 16, 32 legset(A) | 32 legset(B) << 16 }
 //               off* = byte offset of the argument's slot in object plane 0
-//   p2sched[group * NW + warp] = { first chunk, number of chunks }
+//   p2unit[unit] = { first chunk, number of chunks }: the chunks of the same 32 items; work item of phase 2
+//   grp[group]   = { first unit, units, first flow, flows }
+//   wsched[step * NW + warp] = first | count << 16 into witem[]: the work items of this warp in this step (static schedule,
+//               longest processing time first); witem = flow index, or 1 << 31 | chunks << 16 | first chunk for a unit.
+//               Steps: NBUF = 2: step s = flows of group s - 1 and units of group s; NBUF = 1: units(g), flows(g) alternate
 //   p3rec[entry][row = lane / 4] (uint4): x, y, z = 16-bit byte offsets of the A fragments (nA of them, whole words),
 //               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | negative << 31,
 //               shape = swapped | mask << 1 (mask: tile bits that select the A fragment); the entries of a class are
@@ -35,28 +39,27 @@
 //   p3cls[class][lane] (uint2): 16-bit byte offsets into the flow's accumulator of this lane's complex number in tiles 0..3
 //   p3clsh[class] = number of entries of shape k in bits 4k .. 4k+3
 //   p3flow[f] = { first entry, classes | entries << 8 | accumulator << 16, first class, jamp index }
-//   p3sched[group * NW + warp] = { first flow, number of flows }
 #pragma once
 
 namespace mg {
 
-constexpr int HS_NW = 8;       // warps per CTA (gen/hs_streams.py NW)
-
 struct HsTables {
     int npar, ncolor, ngroups, ntile, ns_obj, obj_plane, ns_stage, stage_plane, nlegsets, max_flows;
-    int nobj, nterm, np1, nchunk, nentry, ncls, nflow;
+    int nobj, nterm, np1, nchunk, nunit, nentry, ncls, nflow, nsteps, nitem;
     int p1_level[4];
     const int* obj;
     const int* term;
     const int* p1_items;
     const int* legset_mask;
     const unsigned* p2rec;
-    const int* p2sched;
+    const int* p2unit;
     const unsigned* p3rec;
     const unsigned* p3cls;
     const int* p3clsh;
     const int* p3flow;
-    const int* p3sched;
+    const int* grp;
+    const unsigned* wsched;
+    const unsigned* witem;
     double flops_p1, flops_p2, flops_p3;      // per event (phases 1, 2) and per (event, helicity) (phase 3)
 };
 

@@ -21,9 +21,17 @@ dot-product entries jamp[sigma][h] += sign * sum_c X_c[hx] * Y_c[hy] (phase 3). 
                  (type = one hex digit (opcode - 7) per term)
           rec1..3 (term k) = { offA | offB << 16,  offC | 0 }  or for x_v3  { offA | offB << 16,  32 lsA | (32 lsB) << 16 }
       off* = byte offsets of the argument's slot in plane 0 of the object area; ls* = leg sets (momenta K_ls).
-      Chunks are dealt to the NW warps of the CTA at build time (longest processing time first), p2sched[group][warp].
+      The chunks of the same 32 items form a UNIT (the accumulators stay in registers from one chunk to the next);
+      units are the work items of phase 2 (p2unit[unit] = {first chunk, chunks}; grp[group] = {first unit, units,
+      first flow, flows}).
 
-  phase 3  one warp = one colour flow.  The entries of a flow are sorted into CLASSES: a class fixes which three legs
+  schedule  The kernel runs an event as a sequence of STEPS with one barrier each.  With a double-buffered staging area
+      (nbuf = 2) step s = the colour flows of group s - 1 (phase 3) together with the units of group s (phase 2); with
+      nbuf = 1 phases 2 and 3 of a group are two steps.  The items of a step are dealt to the nw warps of the CTA at
+      build time, longest processing time first, by their instruction counts (ITEM_COST):
+          wsched[step * nw + warp] = first | count << 16   into   witem[] = flow index  or  1 << 31 | chunks << 16 | first chunk
+
+  phase 3  one work item = one colour flow.  The entries of a flow are sorted into CLASSES: a class fixes which three legs
       index the 8 rows of the m8n8k4 FP64 MMA tile (R), which two legs its 4 complex columns (C) and which legs the tiles
       (T), so that all entries of a class accumulate into the SAME register fragments; only when a class is finished are
       the fragments added to the flow's accumulator in shared memory (slot = acc_swizzle(helicity)).  An entry fits a
@@ -46,14 +54,18 @@ import numpy as np
 
 from . import co_program
 
-NW = 8                      # warps per CTA
 MAXCHUNK = 3                # terms per phase-2 chunk
 
 OPS = co_program.OPS
+OPNAME = {v: k for k, v in OPS.items()}
 # order of the phase-2 opcodes inside an item (chunks are cut from the sorted list)
 X_ORDER = ["x_v3", "x_v4s", "x_v4", "x_row", "x_col", "x_bil"]
-# relative cost of a term (flops of emit_hs.FLOPS + accumulation), for the static schedule
+# relative cost of a term (flops of emit_hs.FLOPS + accumulation): order of the units inside a group
 X_COST = {"x_row": 72, "x_col": 72, "x_bil": 80, "x_v3": 134, "x_v4": 112, "x_v4s": 170}
+# instructions per work item (counted in the SASS of csrc/hs_kernel.cu), for the static schedule: per phase-2 term by
+# opcode, per chunk, per phase-3 entry, per class, per flow
+ITEM_COST = {"x_row": 75, "x_col": 75, "x_bil": 85, "x_v3": 125, "x_v4": 100, "x_v4s": 140, "chunk": 35, "unit": 25,
+             "entry": 62, "class": 75, "flow": 110}
 
 
 def chunk_code(ops):
@@ -89,8 +101,9 @@ def _subvar(v, parent, child):
 
 
 class Streams:
-    def __init__(self, prog: co_program.Program):
+    def __init__(self, prog: co_program.Program, nw=8, nbuf=1):
         self.prog = prog
+        self.nw, self.nbuf = nw, nbuf
         self.npar = prog.npar
         self.ncolor = prog.ncolor
         self.ntile = 1 << (self.npar - 5)
@@ -98,6 +111,7 @@ class Streams:
         self._objects()
         self._phase2()
         self._phase3()
+        self._schedule()
 
     # ---------------------------------------------------------------------------------------------
     def _lsid(self, legs):
@@ -153,7 +167,8 @@ class Streams:
     def _phase2(self):
         prog = self.prog
         chunk_types = {}          # tuple of opcodes -> id
-        recs, sched = [], []      # recs: [chunk][4][32][2] uint32
+        recs, unit_tab, grp_units = [], [], []      # recs: [chunk][4][32][2] uint32
+        self.unit_cost = []
         self.xslot = []           # per group: list of first staging slots of its pair objects
         ns_stage = 0
         for g in prog.groups:
@@ -166,7 +181,7 @@ class Streams:
         self.trash_slot = ns_stage                      # padding lanes store here
         self.ns_stage = ns_stage + 2
         self.stage_plane = plane_bytes(self.ns_stage)
-        assert 4 * self.stage_plane < 65536 and 4 * self.obj_plane < 65536, "16-bit byte offsets"
+        assert self.stage_plane < 65536 and self.obj_plane < 65536, "16-bit byte offsets inside a plane"
         for gi, g in enumerate(prog.groups):
             by_shape = defaultdict(list)
             for k, x in enumerate(g["xobjs"]):
@@ -208,19 +223,21 @@ class Streams:
                         blocks.append(blk)
                         t0 += len(ops)
                     units.append((sum(X_COST[o] for o in shape), blocks))
-            # longest processing time first onto the NW warps
-            load = [0] * NW
-            per_warp = [[] for _ in range(NW)]
+            # work items of the group, most expensive first
+            u0 = len(unit_tab)
             for cost, blocks in sorted(units, key=lambda u: -u[0]):
-                w = min(range(NW), key=lambda i: (load[i], i))
-                load[w] += cost
-                per_warp[w] += blocks
-            for w in range(NW):
-                sched.append((len(recs), len(per_warp[w])))
-                recs += per_warp[w]
+                unit_tab.append((len(recs), len(blocks)))
+                icost = ITEM_COST["unit"]
+                for blk in blocks:
+                    ct = int(blk[0, 0, 1]) & 0xFFF
+                    icost += ITEM_COST["chunk"] + sum(ITEM_COST[OPNAME[op]] for op in chunk_types[ct])
+                self.unit_cost.append(icost)
+                recs += blocks
+            grp_units.append((u0, len(unit_tab) - u0))
         self.chunk_types = dict(sorted(chunk_types.items()))      # code -> opcodes
         self.p2rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 4, 32, 2)
-        self.p2sched = np.asarray(sched, dtype=np.int32).reshape(-1, 2)
+        self.p2unit = np.asarray(unit_tab, dtype=np.int32).reshape(-1, 2)
+        self._grp_units = grp_units
 
     # ---------------------------------------------------------------------------------------------
     def _classes_for(self, ents):
@@ -248,11 +265,10 @@ class Streams:
         prog, npar = self.prog, self.npar
         ntile = self.ntile
         hbit = lambda p: npar - 1 - p
-        self.max_flows = 0
-        flows_raw = []            # per flow: (group, warp, acc, jamp, [(R, C, T, [(shape, rec)])])
+        self.max_flows = max(len(g["sigmas"]) for g in prog.groups)
+        flows_raw = []            # per flow: (group, position in the group, jamp, [(R, C, T, [(shape, rec)])])
         shapes = set()
         for gi, g in enumerate(prog.groups):
-            self.max_flows = max(self.max_flows, min(NW, len(g["sigmas"])))
             for fi, j in enumerate(g["sigmas"]):
                 ents = [(frozenset(g["xobjs"][xs]["legs"]), frozenset(prog.objs[yo].legs), xs, yo, sign)
                         for xs, yo, sign in g["entries"][j]]
@@ -307,55 +323,121 @@ class Streams:
                             rec[row] = words + [shape | ((1 if sign < 0 else 0) << 31)]
                         recs_c.append((shape, rec))
                     cls_out.append((R, C, T, recs_c))
-                flows_raw.append((gi, fi % NW, fi % NW, j, cls_out))
+                flows_raw.append((gi, fi, j, cls_out))
         self.p3shapes = sorted(shapes)
         codes = [sh for sh, _, _ in self.p3shapes]
         assert len(codes) <= 4, "the class header holds four shape counts"
         self.p3shape_codes = codes
-        recs, cls_tab, cls_hdr, flows, sched = [], [], [], [], []
+        recs, cls_tab, cls_hdr, flows, grp = [], [], [], [], []
         for gi in range(len(prog.groups)):
-            for w in range(NW):
-                mine = [f for f in flows_raw if f[0] == gi and f[1] == w]
-                sched.append((len(flows), len(mine)))
-                for _, _, acc, j, cls_out in mine:
-                    rec0, cls0, nent = len(recs), len(cls_tab), 0
-                    for R, C, T, recs_c in cls_out:
-                        # accumulator slot of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
-                        ct = np.zeros((32, 4), dtype=np.uint32)
-                        for lane in range(32):
-                            row, c2 = lane >> 2, lane & 3
-                            for t in range(ntile):
-                                h = sum(((row >> b) & 1) << hbit(R[b]) for b in range(3))
-                                h |= sum(((c2 >> b) & 1) << hbit(C[b]) for b in range(2))
-                                h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
-                                ct[lane, t] = 16 * acc_swizzle(h)
-                        cls_tab.append(ct)
-                        recs_c = sorted(recs_c, key=lambda sr: codes.index(sr[0]))        # stable: by shape
-                        counts = [sum(1 for sh, _ in recs_c if sh == c) for c in codes]
-                        assert all(c < 16 for c in counts)
-                        cls_hdr.append(sum(c << (4 * k) for k, c in enumerate(counts)))
-                        recs += [r for _, r in recs_c]
-                        nent += len(recs_c)
-                    flows.append((rec0, len(cls_out) | (nent << 8) | (acc << 16), cls0, j))
+            mine = [f for f in flows_raw if f[0] == gi]
+            grp.append(self._grp_units[gi] + (len(flows), len(mine)))
+            for _, fi, j, cls_out in mine:
+                rec0, cls0, nent = len(recs), len(cls_tab), 0
+                for R, C, T, recs_c in cls_out:
+                    # accumulator slot of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
+                    ct = np.zeros((32, 4), dtype=np.uint32)
+                    for lane in range(32):
+                        row, c2 = lane >> 2, lane & 3
+                        for t in range(ntile):
+                            h = sum(((row >> b) & 1) << hbit(R[b]) for b in range(3))
+                            h |= sum(((c2 >> b) & 1) << hbit(C[b]) for b in range(2))
+                            h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
+                            ct[lane, t] = 16 * acc_swizzle(h)
+                    cls_tab.append(ct)
+                    recs_c = sorted(recs_c, key=lambda sr: codes.index(sr[0]))        # stable: by shape
+                    counts = [sum(1 for sh, _ in recs_c if sh == c) for c in codes]
+                    assert all(c < 16 for c in counts)
+                    cls_hdr.append(sum(c << (4 * k) for k, c in enumerate(counts)))
+                    recs += [r for _, r in recs_c]
+                    nent += len(recs_c)
+                flows.append((rec0, len(cls_out) | (nent << 8) | (fi << 16), cls0, j))
         self.p3rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 8, 4)
         self.p3cls = np.asarray(cls_tab, dtype=np.uint32).reshape(-1, 32, 4)
         self.p3clsh = np.asarray(cls_hdr, dtype=np.int32)
         self.p3flow = np.asarray(flows, dtype=np.int32).reshape(-1, 4)
-        self.p3sched = np.asarray(sched, dtype=np.int32).reshape(-1, 2)
+        self.grp = np.asarray(grp, dtype=np.int32).reshape(-1, 4)
+
+    # ---------------------------------------------------------------------------------------------
+    def steps(self):
+        """[(group whose flows run (or None), group whose units run (or None))] in execution order"""
+        ng = len(self.prog.groups)
+        if self.nbuf == 2:
+            return [(s - 1 if s >= 1 else None, s if s < ng else None) for s in range(ng + 1)]
+        return [x for g in range(ng) for x in ((None, g), (g, None))]
+
+    def _schedule(self):
+        nw = self.nw
+        wsched, witem = [], []
+        self.step_load = []
+        for g3, g2 in self.steps():
+            items = []                                   # (cost, code)
+            if g3 is not None:
+                _, _, f0, nf = (int(x) for x in self.grp[g3])
+                for f in range(f0, f0 + nf):
+                    info = int(self.p3flow[f][1])
+                    cost = ITEM_COST["flow"] + ITEM_COST["class"] * (info & 0xFF) + ITEM_COST["entry"] * ((info >> 8) & 0xFF)
+                    items.append((cost, f))
+            if g2 is not None:
+                u0, nu, _, _ = (int(x) for x in self.grp[g2])
+                for u in range(u0, u0 + nu):
+                    c0, nc = (int(x) for x in self.p2unit[u])
+                    assert c0 < 65536 and nc < 256
+                    items.append((self.unit_cost[u], (1 << 31) | (nc << 16) | c0))
+            load = [0] * nw
+            per_warp = [[] for _ in range(nw)]
+            for cost, code in sorted(items, key=lambda it: (-it[0], it[1])):
+                w = min(range(nw), key=lambda i: (load[i], i))
+                load[w] += cost
+                per_warp[w].append((cost, code))
+            # hill climbing on the makespan: move or swap items between the most loaded warp and any other
+            improved = True
+            while improved:
+                improved = False
+                hi = max(range(nw), key=lambda i: (load[i], -i))
+                for lo in sorted(range(nw), key=lambda i: (load[i], i)):
+                    if lo == hi:
+                        continue
+                    best = None
+                    for a_, (ca, _) in enumerate(per_warp[hi]):
+                        for b_, (cb, _) in [(-1, (0, 0))] + list(enumerate(per_warp[lo])):
+                            new = max(load[hi] - ca + cb, load[lo] + ca - cb)
+                            if new < load[hi] and (best is None or new < best[0]):
+                                best = (new, a_, b_)
+                    if best is not None:
+                        _, a_, b_ = best
+                        ia = per_warp[hi].pop(a_)
+                        load[hi] -= ia[0]; load[lo] += ia[0]
+                        if b_ >= 0:
+                            ib = per_warp[lo].pop(b_)
+                            load[lo] -= ib[0]; load[hi] += ib[0]
+                            per_warp[hi].append(ib)
+                        per_warp[lo].append(ia)
+                        improved = True
+                        break
+            per_warp = [[code for _, code in sorted(pw, key=lambda it: (-it[0], it[1]))] for pw in per_warp]
+            self.step_load.append(load)
+            for w in range(nw):
+                assert len(witem) < 65536 and len(per_warp[w]) < 65536
+                wsched.append(len(witem) | (len(per_warp[w]) << 16))
+                witem += per_warp[w]
+        self.wsched = np.asarray(wsched, dtype=np.uint32)
+        self.witem = np.asarray(witem, dtype=np.uint32)
 
     # ---------------------------------------------------------------------------------------------
     def tables(self):
         i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w)
         ncls = self.p3flow[:, 1] & 0xFF
         return {
-            "npar": self.npar, "ncolor": self.ncolor, "ngroups": len(self.prog.groups), "nw": NW, "ntile": self.ntile,
+            "npar": self.npar, "ncolor": self.ncolor, "ngroups": len(self.prog.groups), "ntile": self.ntile,
             "ns_obj": self.ns_obj, "obj_plane": self.obj_plane, "ns_stage": self.ns_stage, "stage_plane": self.stage_plane,
             "nlegsets": len(self.legsets), "max_flows": self.max_flows, "max_classes": int(ncls.max()),
             "legset_mask": np.asarray([sum(1 << p for p in legs) for legs in self.legsets], np.int32),
             "obj": i32(self.obj_tab, 4), "term": i32(self.p1_terms, 4), "p1_items": np.asarray(self.p1_items, np.int32),
             "p1_level": np.asarray(self.p1_level, np.int32),
-            "p2rec": self.p2rec, "p2sched": self.p2sched, "chunk_types": self.chunk_types,
-            "p3rec": self.p3rec, "p3cls": self.p3cls, "p3clsh": self.p3clsh, "p3flow": self.p3flow, "p3sched": self.p3sched,
+            "p2rec": self.p2rec, "p2unit": self.p2unit, "grp": self.grp, "chunk_types": self.chunk_types,
+            "nw": self.nw, "nbuf": self.nbuf, "nsteps": len(self.steps()), "wsched": self.wsched, "witem": self.witem,
+            "p3rec": self.p3rec, "p3cls": self.p3cls, "p3clsh": self.p3clsh, "p3flow": self.p3flow,
             "p3shapes": self.p3shapes, "p3shape_codes": self.p3shape_codes,
         }
 
@@ -363,8 +445,8 @@ class Streams:
 _CACHE = {}
 
 
-def build(n, group_prefix):
-    key = (n, group_prefix)
+def build(n, group_prefix, nw=8, nbuf=1):
+    key = (n, group_prefix, nw, nbuf)
     if key not in _CACHE:
-        _CACHE[key] = Streams(co_program.build(n, group_prefix))
+        _CACHE[key] = Streams(co_program.build(n, group_prefix), nw, nbuf)
     return _CACHE[key]

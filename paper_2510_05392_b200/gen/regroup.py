@@ -4,12 +4,14 @@ A group of colour flows shares one staging area of pair objects X (phase 2 of cs
 flows of different groups need is recomputed in each of them.  Grouping the flows by a common prefix of sigma (the
 round-1 choice) recomputes 2.8 x the distinct X terms of g g -> t tbar g g g; the sharing actually follows the dihedral
 orbits of sigma (rotations and reversal of the gluon word: a purely gluonic four-leg current is common to
-(abcd e), (e abcd), (dcba e), (e dcba)), and a whole orbit (10 flows, 1200 staging slots) does not fit two CTAs per SM.
-This module searches, deterministically (seeded simulated annealing), the partition into groups of `gsize` flows with
-the smallest phase-2 cost under the staging capacity, and writes it to gen/flow_groups_n<n>.txt, which co_program reads.
-PAPER.md:424-452 is the paper's version of the same trade-off (diagram groups: fewer kernels vs hand-off traffic).
+(abcd e), (e abcd), (dcba e), (e dcba)).  One orbit = 10 flows and 1200 staging slots (77 KB); the kernel therefore runs
+one 16-warp CTA per SM with a double-buffered staging area.  `main` writes the orbit partition to
+gen/flow_groups_n<n>.txt, which co_program reads; `search` (seeded simulated annealing under a staging capacity) is the
+generic tool for other group sizes (6 flows within 832 slots: cost 4.65e6 against 4.20e6 for the orbits and 6.67e6 for
+prefix groups).  PAPER.md:424-452 is the paper's version of the same trade-off (diagram groups: fewer kernels against
+hand-off traffic).
 
-  python -m paper_2510_05392_b200.gen.regroup 5        # rewrites gen/flow_groups_n5.txt (a few minutes)
+  python -m paper_2510_05392_b200.gen.regroup 5        # rewrites gen/flow_groups_n5.txt
 """
 from __future__ import annotations
 
@@ -89,25 +91,38 @@ def load(n, sigmas):
     return groups
 
 
-def main(n, gsize=6, cap_slots=832, seeds=(12,), iters=1500000):
+def dihedral_orbits(sigmas):
+    """orbits of the colour flows under rotations and reversal of the gluon word"""
+    index = {tuple(s): j for j, s in enumerate(sigmas)}
+    seen, out = set(), []
+    for j, s_ in enumerate(sigmas):
+        if j in seen:
+            continue
+        s_ = tuple(s_)
+        orb = set()
+        for r in range(len(s_)):
+            t = s_[r:] + s_[:r]
+            orb |= {index[t], index[t[::-1]]}
+        seen |= orb
+        out.append(sorted(orb))
+    return out
+
+
+def main(n):
     from . import co_program
     prog = co_program.build(n, 0)
     xs = flow_xsets(prog)
-    best = None
-    for seed in seeds:
-        r = search(xs, gsize, cap_slots, seed, iters)
-        print(f"seed {seed}: cost {r[1]} max slots {r[2]}", file=sys.stderr)
-        if best is None or r[1] < best[1]:
-            best = r
-    groups, cost, slots = best
+    groups = dihedral_orbits(prog.sigmas)
+    costs = [group_cost(xs, g) for g in groups]
+    cost, slots = sum(c for c, _ in costs), max(s_ for _, s_ in costs)
     once = group_cost(xs, sorted(xs))[0]
     with open(path(n), "w") as f:
         f.write(f"# groups of colour flows of g g -> t tbar + {n - 2} g for the helicity-shared kernel; written by gen/regroup.py\n"
-                f"# gsize {gsize}, staging capacity {cap_slots} slots: phase-2 cost {cost} (every pair object once: {once}), "
-                f"largest group {slots} slots\n")
+                f"# dihedral orbits of the gluon word: phase-2 cost {cost} (every pair object once: {once}), "
+                f"largest group {slots} staging slots\n")
         for g in groups:
             f.write(" ".join("".join(map(str, prog.sigmas[j])) for j in g) + "\n")
-    return best
+    return groups, cost, slots
 
 
 if __name__ == "__main__":

@@ -60,7 +60,7 @@ def _x_term(op, A, B, Z, kA, kB):
 
 def evaluate(T, mom, mt, wt):
     """jamps[ncolor][2^npar] (without the g^n factor) of one event from the streams T = Streams.tables()"""
-    npar, nw, ntile = T["npar"], T["nw"], T["ntile"]
+    npar, ntile = T["npar"], T["ntile"]
     k = [mom[i] * (1 if i < 2 else -1) for i in range(npar)]
     K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
     obj = _Planes(T["obj_plane"])
@@ -110,9 +110,10 @@ def evaluate(T, mom, mt, wt):
     J = np.full((T["ncolor"], nh), np.nan + 0j, dtype=complex)
     for g in range(T["ngroups"]):
         stage = _Planes(T["stage_plane"])
-        # phase 2: chunks of every warp
-        for w in range(nw):
-            c0, nc = (int(x) for x in T["p2sched"][g * nw + w])
+        u0, nu, f0, nf = (int(x) for x in T["grp"][g])
+        # phase 2: the units of the group (work items; each keeps its accumulators from one chunk to the next)
+        for u in range(u0, u0 + nu):
+            c0, nc = (int(x) for x in T["p2unit"][u])
             acc = np.zeros((32, 4), dtype=complex)
             for c in range(c0, c0 + nc):
                 blk = T["p2rec"][c]
@@ -138,9 +139,8 @@ def evaluate(T, mom, mt, wt):
                         acc[lane] += -r if (r0x >> (16 + j)) & 1 else r
                     if last:
                         stage.store(r0x & 0xFFFF, acc[lane])
-        # phase 3: colour flows of every warp
-        for w in range(nw):
-            f0, nf = (int(x) for x in T["p3sched"][g * nw + w])
+        # phase 3: the colour flows of the group (work items)
+        if True:
             for f in range(f0, f0 + nf):
                 rec0, info, cls0, jamp = (int(x) for x in T["p3flow"][f])
                 ncls, nent = info & 0xFF, (info >> 8) & 0xFF

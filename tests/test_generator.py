@@ -84,7 +84,22 @@ def test_helicity_shared_streams_match_oracle(name, n, nev, params):
     |M|^2 for EVERY helicity -- the program that is the default for these processes, checked without a GPU"""
     import hs_eval
     from paper_2510_05392_b200.gen import emit_hs, hs_streams
-    T = hs_streams.build(n, emit_hs.GROUP_PREFIX[n]).tables()          # the grouping the library is built with
+    k = emit_hs.KERNEL_CFG[n]
+    st = hs_streams.build(n, emit_hs.GROUP_PREFIX[n], k["nw"], k["nbuf"])          # what the library is built with
+    T = st.tables()
+    # the static schedule deals every work item of every step to exactly one warp
+    for s_, (g3, g2) in enumerate(st.steps()):
+        want = []
+        if g3 is not None:
+            want += list(range(int(T["grp"][g3][2]), int(T["grp"][g3][2] + T["grp"][g3][3])))
+        if g2 is not None:
+            u0, nu = int(T["grp"][g2][0]), int(T["grp"][g2][1])
+            want += [(1 << 31) | (int(T["p2unit"][u][1]) << 16) | int(T["p2unit"][u][0]) for u in range(u0, u0 + nu)]
+        got = []
+        for w in range(k["nw"]):
+            sc = int(T["wsched"][s_ * k["nw"] + w])
+            got += [int(x) for x in T["witem"][sc & 0xFFFF:(sc & 0xFFFF) + (sc >> 16)]]
+        assert sorted(got) == sorted(want), s_
     C = np.array([[float(x) for x in r] for r in colour.colour_matrix(n)])
     gs = math.sqrt(4 * math.pi * params["aS"])
     p = inputs.momenta(name, nev, seed=7)
