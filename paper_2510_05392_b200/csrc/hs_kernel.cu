@@ -12,8 +12,7 @@
 //
 // Scheduling inside the CTA: the work items of a step -- the colour flows of group g (phase 3) and, when the staging area
 // is double-buffered (HsCfg::NBUF = 2), the phase-2 units of group g + 1 -- are dealt to the warps at build time by their
-// instruction counts (gen/hs_streams.py _schedule), with ONE barrier per step; a warp pulls the records of its next item
-// into L1 while it works on the current one.  The paper's counterpart is the sequence of diagram-group kernels on
+// instruction counts (gen/hs_streams.py _schedule), with ONE barrier per step.  The paper's counterpart is the sequence of diagram-group kernels on
 // helicity streams; here a "group" never leaves the SM.
 //
 // Every shared-memory address of phases 2 and 3 comes precomputed from the streams: an argument costs one 16-bit
@@ -31,7 +30,7 @@ namespace mg {
 
 struct HsDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
-    const uint2* p2rec; const unsigned* wsched; const unsigned* witem;
+    const uint2* p2rec; const uint2* wsched; const unsigned* witem;
     const uint4* p3rec; const uint2* p3cls; const int* p3clsh; const int4* p3flow;
     int ncolor, nflow, ncls, nsched, nitem;
     int p1_level[4];
@@ -39,10 +38,10 @@ struct HsDev {
 
 // the small tables every work item starts from, copied to shared memory once per (persistent) CTA
 struct HsSmemTabs {
-    const int4* p3flow; const int* p3clsh; const unsigned* wsched; const unsigned* witem;
+    const int4* p3flow; const int* p3clsh; const uint2* wsched; const unsigned* witem;
 };
 
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 
 // variant of an argument object: bit j = bit ((code >> 3j) & 7) of the parent's variant (7 = none; variants are < 128)
 __device__ __forceinline__ int sub_variant(int var, int code)
@@ -363,10 +362,12 @@ __device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, co
     __syncwarp();
 }
 
-// one unit of phase 2: the chunks of the same 32 (pair object, variant) items; the next chunk's records are in flight
+// the phase-2 work of a warp in a step: a contiguous run of chunks; a unit (the chunks of the same 32 (pair object,
+// variant) items) starts where rec0 says "first" (accumulators zeroed) and ends at "last" (result stored, p2_chunk).
+// The records of the next chunk are in flight while the current one is evaluated.
 template <int NG>
-__device__ __forceinline__ void p2_unit(const HsDev& d, int chunk0, int nchunk, const char* __restrict__ obj,
-                                        const char* __restrict__ Ks, char* __restrict__ stage, int lane)
+__device__ __forceinline__ void p2_run(const HsDev& d, int chunk0, int nchunk, const char* __restrict__ obj,
+                                       const char* __restrict__ Ks, char* __restrict__ stage, int lane)
 {
     using Cfg = HsCfg<NG>;
     constexpr int OBJ_PLANE = Cfg::OBJ_PLANE, STG_PLANE = Cfg::STG_PLANE;
@@ -377,8 +378,12 @@ __device__ __forceinline__ void p2_unit(const HsDev& d, int chunk0, int nchunk, 
     for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
     for (int c = 0; c < nchunk; c++) {
         const uint2 r0 = n0, r1 = n1, r2 = n2, r3 = n3;
-        rp += 128;
-        if (c + 1 < nchunk) { n0 = __ldg(rp); n1 = __ldg(rp + 32); n2 = __ldg(rp + 64); n3 = __ldg(rp + 96); }
+        rp += 128;                                       // (one chunk past the end of the table: inside the blob)
+        n0 = __ldg(rp); n1 = __ldg(rp + 32); n2 = __ldg(rp + 64); n3 = __ldg(rp + 96);
+        if (r0.y & 0x1000u) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) acc.c[q] = mk<double>(0.0, 0.0);
+        }
         switch (r0.y & 0xFFFu) {
 #define HS_CASE(CT) case CT: p2_chunk<CT, OBJ_PLANE, STG_PLANE>(obj, Ks, stage, r0, r1, r2, r3, acc); break;
             HS_CHUNK_TYPES(HS_CASE)
@@ -406,8 +411,8 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
     {
         int4* t0 = reinterpret_cast<int4*>(pm + 4 * NPAR);
         int* t1 = reinterpret_cast<int*>(t0 + d.nflow);
-        unsigned* t2 = reinterpret_cast<unsigned*>(t1 + d.ncls);
-        unsigned* t3 = t2 + d.nsched;
+        uint2* t2 = reinterpret_cast<uint2*>(t1 + ((d.ncls + 1) & ~1));
+        unsigned* t3 = reinterpret_cast<unsigned*>(t2 + d.nsched);
         for (int i = threadIdx.x; i < d.nflow; i += blockDim.x) t0[i] = __ldg(d.p3flow + i);
         for (int i = threadIdx.x; i < d.ncls; i += blockDim.x) t1[i] = __ldg(d.p3clsh + i);
         for (int i = threadIdx.x; i < d.nsched; i += blockDim.x) t2[i] = __ldg(d.wsched + i);
@@ -457,30 +462,11 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
             const int b2 = NBUF == 2 ? (s & 1) : 0, b3 = NBUF == 2 ? ((s - 1) & 1) : 0;
             char* __restrict__ stage2 = stage0 + b2 * 4 * STG_PLANE;
             const char* __restrict__ stgl3 = stage0 + b3 * 4 * STG_PLANE + (lane & 3) * STG_PLANE;
-            const unsigned sc = tb.wsched[s * NW + warp];
-            const unsigned* __restrict__ ip = tb.witem + (sc & 0xFFFFu);
-            const int n = sc >> 16;
-            // pull the records of an item into L1: entry records (128 B each) by lanes 0 .., class tables (256 B each) by
-            // lanes 16 .. for a colour flow; the chunks (1 KB each) of a unit
-            auto pull = [&](unsigned it) {
-                if (it >> 31) {
-                    if (lane < 8 * (int)((it >> 16) & 0xFF))
-                        prefetch_l1(reinterpret_cast<const char*>(d.p2rec) + (1024u * (it & 0xFFFFu) + 128u * lane));
-                } else {
-                    const int4 fd = tb.p3flow[it];
-                    const bool cls = lane >= 16;
-                    const unsigned cnt = cls ? 2u * (fd.y & 0xFF) : ((fd.y >> 8) & 0xFF);
-                    const char* base = cls ? reinterpret_cast<const char*>(d.p3cls) : reinterpret_cast<const char*>(d.p3rec);
-                    const unsigned first = cls ? 256u * fd.z : 128u * fd.x;
-                    if ((unsigned)(lane & 15) < cnt) prefetch_l1(base + (first + 128u * (lane & 15)));
-                }
-            };
-            for (int k = 0; k < n; k++) {
-                const unsigned it = ip[k];
-                if (k + 1 < n) pull(ip[k + 1]);
-                if (it >> 31) p2_unit<NG>(d, it & 0xFFFFu, (it >> 16) & 0xFF, obj, Ks, stage2, lane);
-                else p3_flow<NG, T2>(d, tb, a, it, e, objl, stgl3, accs, warp, lane, posr);
-            }
+            const uint2 sc = tb.wsched[s * NW + warp];
+            const unsigned* __restrict__ ip = tb.witem + (sc.x & 0xFFFFu);
+            const int nfl = sc.x >> 16;
+            for (int k = 0; k < nfl; k++) p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr);
+            if (sc.y >> 16) p2_run<NG>(d, sc.y & 0xFFFFu, sc.y >> 16, obj, Ks, stage2, lane);
             __syncthreads();
         }
     }
@@ -505,7 +491,7 @@ template <int NG> static size_t smem_bytes(const HsTables* t)
     constexpr int NACC = Cfg::MAX_FLOWS > Cfg::NW ? Cfg::NW : Cfg::MAX_FLOWS;
     return 4 * (size_t)Cfg::OBJ_PLANE + Cfg::NBUF * 4 * (size_t)Cfg::STG_PLANE + (size_t)NACC * (16u << Cfg::NPAR) +
            32 * (size_t)Cfg::NLEGSETS + 32 * (size_t)Cfg::NPAR +
-           16 * (size_t)t->nflow + 4 * (size_t)t->ncls + 4 * (size_t)t->nsteps * Cfg::NW + 4 * (size_t)t->nitem;
+           16 * (size_t)t->nflow + 4 * (size_t)((t->ncls + 1) & ~1) + 8 * (size_t)t->nsteps * Cfg::NW + 4 * (size_t)t->nitem;
 }
 
 template <int NG> static cudaError_t set_smem(size_t smem)
@@ -535,7 +521,7 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     struct Part { const void* src; size_t bytes; size_t off; };
     Part parts[11] = { { t->obj, sizeof(int) * 4 * t->nobj, 0 }, { t->term, sizeof(int) * 4 * t->nterm, 0 },
                        { t->p1_items, sizeof(int) * t->np1, 0 }, { t->legset_mask, sizeof(int) * t->nlegsets, 0 },
-                       { t->p2rec, sizeof(unsigned) * 256 * (size_t)t->nchunk, 0 }, { t->wsched, sizeof(unsigned) * (size_t)t->nsteps * (c_nw), 0 },
+                       { t->p2rec, sizeof(unsigned) * 256 * (size_t)t->nchunk, 0 }, { t->wsched, sizeof(unsigned) * 2 * (size_t)t->nsteps * (c_nw), 0 },
                        { t->p3rec, sizeof(unsigned) * 32 * (size_t)t->nentry, 0 }, { t->p3cls, sizeof(unsigned) * 64 * (size_t)t->ncls, 0 },
                        { t->p3flow, sizeof(int) * 4 * t->nflow, 0 }, { t->witem, sizeof(unsigned) * (size_t)t->nitem, 0 },
                        { t->p3clsh, sizeof(int) * (size_t)t->ncls, 0 } };
@@ -552,7 +538,7 @@ cudaError_t hs_create(int ngluon, HsContext** out)
     HsDev& d = c->d;
     d.obj = (const int4*)(b + parts[0].off); d.term = (const int4*)(b + parts[1].off);
     d.p1_items = (const int*)(b + parts[2].off); d.legset_mask = (const int*)(b + parts[3].off);
-    d.p2rec = (const uint2*)(b + parts[4].off); d.wsched = (const unsigned*)(b + parts[5].off);
+    d.p2rec = (const uint2*)(b + parts[4].off); d.wsched = (const uint2*)(b + parts[5].off);
     d.p3rec = (const uint4*)(b + parts[6].off); d.p3cls = (const uint2*)(b + parts[7].off);
     d.p3flow = (const int4*)(b + parts[8].off); d.witem = (const unsigned*)(b + parts[9].off);
     d.p3clsh = (const int*)(b + parts[10].off);

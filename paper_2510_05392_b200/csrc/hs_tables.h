@@ -27,10 +27,11 @@
 //                      type = one hex digit (op - 7) per term, first term in the low digit
 //               rec1..3 (term k) = { offA | offB << 16, offC }; x_v3: { offA | offB << 16, 32 legset(A) | 32 legset(B) << 16 }
 //               off* = byte offset of the argument's slot in object plane 0
-//   p2unit[unit] = { first chunk, number of chunks }: the chunks of the same 32 items; work item of phase 2
+//   p2unit[unit] = { first chunk, number of chunks }: the chunks of the same 32 items (host side only: schedule, tests)
 //   grp[group]   = { first unit, units, first flow, flows }
-//   wsched[step * NW + warp] = first | count << 16 into witem[]: the work items of this warp in this step (static schedule,
-//               longest processing time first); witem = flow index, or 1 << 31 | chunks << 16 | first chunk for a unit.
+//   wsched[step * NW + warp] = { first flow item | flows << 16, first chunk | chunks << 16 }: the work of this warp in this
+//               step (static schedule, longest processing time first): its colour flows (witem[] = flow indices), then ONE
+//               contiguous run of chunks -- p2rec is stored in execution order.
 //               Steps: NBUF = 2: step s = flows of group s - 1 and units of group s; NBUF = 1: units(g), flows(g) alternate
 //   p3rec[entry][row = lane / 4] (uint4): x, y, z = 16-bit byte offsets of the A fragments (nA of them, whole words),
 //               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | negative << 31,

@@ -28,8 +28,10 @@ dot-product entries jamp[sigma][h] += sign * sum_c X_c[hx] * Y_c[hy] (phase 3). 
   schedule  The kernel runs an event as a sequence of STEPS with one barrier each.  With a double-buffered staging area
       (nbuf = 2) step s = the colour flows of group s - 1 (phase 3) together with the units of group s (phase 2); with
       nbuf = 1 phases 2 and 3 of a group are two steps.  The items of a step are dealt to the nw warps of the CTA at
-      build time, longest processing time first, by their instruction counts (ITEM_COST):
-          wsched[step * nw + warp] = first | count << 16   into   witem[] = flow index  or  1 << 31 | chunks << 16 | first chunk
+      build time, longest processing time first, by their instruction counts (ITEM_COST).  The chunk records are stored
+      in execution order, so that the phase-2 work of a warp in a step is ONE contiguous run of chunks (rec0 says where
+      a unit starts -- accumulators zeroed -- and where it ends -- result stored):
+          wsched[step * nw + warp] = { first flow item | flows << 16, first chunk | chunks << 16 },  witem[] = flow index
 
   phase 3  one work item = one colour flow.  The entries of a flow are sorted into CLASSES: a class fixes which three legs
       index the 8 rows of the m8n8k4 FP64 MMA tile (R), which two legs its 4 complex columns (C) and which legs the tiles
@@ -369,6 +371,7 @@ class Streams:
     def _schedule(self):
         nw = self.nw
         wsched, witem = [], []
+        new_recs, new_unit = [], [None] * len(self.p2unit)
         self.step_load = []
         for g3, g2 in self.steps():
             items = []                                   # (cost, code)
@@ -381,9 +384,7 @@ class Streams:
             if g2 is not None:
                 u0, nu, _, _ = (int(x) for x in self.grp[g2])
                 for u in range(u0, u0 + nu):
-                    c0, nc = (int(x) for x in self.p2unit[u])
-                    assert c0 < 65536 and nc < 256
-                    items.append((self.unit_cost[u], (1 << 31) | (nc << 16) | c0))
+                    items.append((self.unit_cost[u], (1 << 31) | u))
             load = [0] * nw
             per_warp = [[] for _ in range(nw)]
             for cost, code in sorted(items, key=lambda it: (-it[0], it[1])):
@@ -415,13 +416,23 @@ class Streams:
                         per_warp[lo].append(ia)
                         improved = True
                         break
-            per_warp = [[code for _, code in sorted(pw, key=lambda it: (-it[0], it[1]))] for pw in per_warp]
             self.step_load.append(load)
             for w in range(nw):
-                assert len(witem) < 65536 and len(per_warp[w]) < 65536
-                wsched.append(len(witem) | (len(per_warp[w]) << 16))
-                witem += per_warp[w]
-        self.wsched = np.asarray(wsched, dtype=np.uint32)
+                mine = sorted(per_warp[w], key=lambda it: (-it[0], it[1]))
+                fl = [code for _, code in mine if not code >> 31]
+                un = [code & 0x7FFFFFFF for _, code in mine if code >> 31]          # unit indices (old numbering)
+                c0 = len(new_recs)
+                for u in un:
+                    oc, nc = (int(x) for x in self.p2unit[u])
+                    new_unit[u] = (len(new_recs), nc)
+                    new_recs += [self.p2rec[oc + k] for k in range(nc)]
+                assert len(witem) < 65536 and len(fl) < 65536 and len(new_recs) < 65536
+                wsched.append((len(witem) | (len(fl) << 16), c0 | ((len(new_recs) - c0) << 16)))
+                witem += fl
+        assert len(new_recs) == len(self.p2rec) and all(u is not None for u in new_unit)
+        self.p2rec = np.asarray(new_recs, dtype=np.uint32).reshape(-1, 4, 32, 2)
+        self.p2unit = np.asarray(new_unit, dtype=np.int32).reshape(-1, 2)
+        self.wsched = np.asarray(wsched, dtype=np.uint32).reshape(-1, 2)
         self.witem = np.asarray(witem, dtype=np.uint32)
 
     # ---------------------------------------------------------------------------------------------

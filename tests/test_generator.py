@@ -87,19 +87,23 @@ def test_helicity_shared_streams_match_oracle(name, n, nev, params):
     k = emit_hs.KERNEL_CFG[n]
     st = hs_streams.build(n, emit_hs.GROUP_PREFIX[n], k["nw"], k["nbuf"])          # what the library is built with
     T = st.tables()
-    # the static schedule deals every work item of every step to exactly one warp
+    # the static schedule deals every colour flow and every chunk of every step to exactly one warp, units unbroken
     for s_, (g3, g2) in enumerate(st.steps()):
-        want = []
-        if g3 is not None:
-            want += list(range(int(T["grp"][g3][2]), int(T["grp"][g3][2] + T["grp"][g3][3])))
+        want_f = list(range(int(T["grp"][g3][2]), int(T["grp"][g3][2] + T["grp"][g3][3]))) if g3 is not None else []
+        want_c = []
         if g2 is not None:
             u0, nu = int(T["grp"][g2][0]), int(T["grp"][g2][1])
-            want += [(1 << 31) | (int(T["p2unit"][u][1]) << 16) | int(T["p2unit"][u][0]) for u in range(u0, u0 + nu)]
-        got = []
+            for u in range(u0, u0 + nu):
+                want_c += list(range(int(T["p2unit"][u][0]), int(T["p2unit"][u][0] + T["p2unit"][u][1])))
+        got_f, got_c = [], []
         for w in range(k["nw"]):
-            sc = int(T["wsched"][s_ * k["nw"] + w])
-            got += [int(x) for x in T["witem"][sc & 0xFFFF:(sc & 0xFFFF) + (sc >> 16)]]
-        assert sorted(got) == sorted(want), s_
+            sf, sc = (int(x) for x in T["wsched"][s_ * k["nw"] + w])
+            got_f += [int(x) for x in T["witem"][sf & 0xFFFF:(sf & 0xFFFF) + (sf >> 16)]]
+            run = list(range(sc & 0xFFFF, (sc & 0xFFFF) + (sc >> 16)))
+            got_c += run
+            if run:          # a run starts with the first chunk of a unit and ends with the last chunk of one
+                assert (int(T["p2rec"][run[0]][0, 0, 1]) >> 12) & 1 and (int(T["p2rec"][run[-1]][0, 0, 1]) >> 13) & 1
+        assert sorted(got_f) == want_f and sorted(got_c) == sorted(want_c), s_
     C = np.array([[float(x) for x in r] for r in colour.colour_matrix(n)])
     gs = math.sqrt(4 * math.pi * params["aS"])
     p = inputs.momenta(name, nev, seed=7)
