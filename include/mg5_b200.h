@@ -106,6 +106,25 @@ int mg_set_good_helicities(mg_process* p, const unsigned char* h_mask);
 int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
                    size_t ws_bytes, void* cuda_stream);
 
+/* The rest of the paper's ME-engine interface (the engine "also receives other inputs": an event-by-event
+ * running alpha_s(Q^2), and "two random numbers for each event", from which it selects "a color and a helicity for event
+ * ievt" -- Table 1; the alpha_s-dependent couplings are computed in a kernel of their own).
+ * All extra pointers are DEVICE arrays of nevt elements and may be NULL (then this is mg_sigma_batch):
+ *   d_alphas : alpha_s of each event.  The couplings kernel computes G = sqrt(4 pi alpha_s(e)); every diagram of the g g ->
+ *              t tbar + gluons processes carries G^n, so d_me[e] is the card's matrix element times (alpha_s(e)/aS)^n
+ *              (e+ e- -> mu+ mu- does not depend on it).
+ *   d_rndhel, d_selhel : uniform numbers in [0, 1) -> helicity index h (numbering above) of the first good helicity k, in
+ *              increasing h, with  rnd * sum_j me_hj < sum_{j <= k} me_hj  (reading A15).
+ *   d_rndcol, d_selcol : -> colour flow c (index of the permutation sigma in lexicographic order, the order of
+ *              mg_color_matrix) chosen the same way from the weights  w_c = sum_{good h} |J_c,h|^2.
+ * A selection output needs its random-number input and vice versa (MG_EINVAL otherwise).
+ * ws_bytes must be >= mg_workspace_bytes_ex(p, nevt, d_selcol != NULL): the colour selection reads the jamps buffer, which
+ * the MG_DIAG_THREAD kernel with MG_CS_FUSED does not otherwise write. */
+int mg_sigma_batch_ex(mg_process* p, const double* d_momenta, int nevt, const double* d_alphas, const double* d_rndhel,
+                      const double* d_rndcol, double* d_me, int* d_selhel, int* d_selcol, void* d_workspace, size_t ws_bytes,
+                      void* cuda_stream);
+size_t mg_workspace_bytes_ex(const mg_process* p, int nevt, int want_selcol);
+
 /* Same from HOST buffers (pinned memory recommended): copies h_momenta to an internal device buffer, runs the
  * batch, copies me back, synchronises.  The library allocates and owns the device buffers it needs here. */
 int mg_sigma_batch_host(mg_process* p, const double* h_momenta, int nevt, double* h_me);

@@ -5,3 +5,4 @@ Nothing here imports the CUDA package's kernels, generator or binding.
 """
 from .me_oracle import (build, color_matrix, me_ggttx, me_eemumu, partial_amplitudes, matrix_elements,
                         su3_generators, DENOM, NGLUONS)  # noqa: F401
+from . import selection  # noqa: F401,E402

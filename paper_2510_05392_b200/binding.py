@@ -22,7 +22,8 @@ PRECISIONS = {"fp64": MG_FP64, "d": MG_FP64, "mixed": MG_MIXED, "m": MG_MIXED, "
 _ERR = {-1: "MG_EINVAL", -2: "MG_ENODEV", -3: "MG_ENOMEM", -4: "MG_ECUDA", -5: "MG_ESTATE"}
 
 EXPORTS = ["mg_init_process", "mg_process_info", "mg_process_flops", "mg_set_parameters", "mg_set_option", "mg_get_option",
-           "mg_workspace_bytes", "mg_helicity_filter", "mg_set_good_helicities", "mg_sigma_batch",
+           "mg_workspace_bytes", "mg_workspace_bytes_ex", "mg_helicity_filter", "mg_set_good_helicities", "mg_sigma_batch",
+           "mg_sigma_batch_ex",
            "mg_sigma_batch_host", "mg_last_helicity_terms", "mg_last_stage_ms", "mg_last_launch_count", "mg_color_sum", "mg_color_matrix",
            "mg_measure_peak", "mg_last_error", "mg_destroy"]
 
@@ -54,6 +55,9 @@ def load_library() -> ctypes.CDLL:
     lib.mg_helicity_filter.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_size_t, vp, ctypes.POINTER(ctypes.c_ubyte), ip]
     lib.mg_set_good_helicities.argtypes = [vp, ctypes.POINTER(ctypes.c_ubyte)]
     lib.mg_sigma_batch.argtypes = [vp, vp, ctypes.c_int, vp, vp, ctypes.c_size_t, vp]
+    lib.mg_sigma_batch_ex.argtypes = [vp, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
+    lib.mg_workspace_bytes_ex.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    lib.mg_workspace_bytes_ex.restype = ctypes.c_size_t
     lib.mg_sigma_batch_host.argtypes = [vp, vp, ctypes.c_int, vp]
     lib.mg_last_helicity_terms.argtypes = [vp, ctypes.c_int, vp, vp, vp]
     lib.mg_last_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
@@ -125,8 +129,8 @@ class Process:
     def _stream(self):
         return ctypes.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
 
-    def _workspace(self, nevt):
-        need = self.lib.mg_workspace_bytes(self.h, nevt)
+    def _workspace(self, nevt, want_selcol=False):
+        need = self.lib.mg_workspace_bytes_ex(self.h, nevt, 1 if want_selcol else 0)
         if self._ws is None or self._ws.numel() < need:
             self._ws = self._torch.empty(max(need, 256), dtype=self._torch.uint8, device=f"cuda:{self.device}")
         return self._ws
@@ -180,6 +184,25 @@ class Process:
         self._check(self.lib.mg_sigma_batch(self.h, d_momenta.data_ptr(), nevt, d_me.data_ptr(), ws.data_ptr(), ws.numel(),
                                             self._stream()))
         return d_me
+
+    def sigma_batch_ex(self, d_momenta, alphas=None, rndhel=None, rndcol=None):
+        """mg_sigma_batch_ex: optional per-event alpha_s and the two random numbers per event (cuda fp64 [nevt] each);
+        returns (d_me, d_selhel or None, d_selcol or None), the selections as cuda int32 [nevt]. Asynchronous."""
+        t = self._torch
+        assert d_momenta.is_cuda and d_momenta.dtype == t.float64 and d_momenta.is_contiguous()
+        nevt = d_momenta.shape[0]
+        for x in (alphas, rndhel, rndcol):
+            assert x is None or (x.is_cuda and x.dtype == t.float64 and x.is_contiguous() and x.shape == (nevt,))
+        d_me = t.empty(nevt, dtype=t.float64, device=d_momenta.device)
+        selhel = t.empty(nevt, dtype=t.int32, device=d_momenta.device) if rndhel is not None else None
+        selcol = t.empty(nevt, dtype=t.int32, device=d_momenta.device) if rndcol is not None else None
+        if self.ngood is None and nevt > 0:
+            self.helicity_filter(d_momenta)
+        ws = self._workspace(nevt, rndcol is not None)
+        ptr = lambda x: x.data_ptr() if x is not None else None
+        self._check(self.lib.mg_sigma_batch_ex(self.h, d_momenta.data_ptr(), nevt, ptr(alphas), ptr(rndhel), ptr(rndcol),
+                                               d_me.data_ptr(), ptr(selhel), ptr(selcol), ws.data_ptr(), ws.numel(), self._stream()))
+        return d_me, selhel, selcol
 
     def sigma_batch_host(self, h_momenta: np.ndarray, h_me: np.ndarray | None = None):
         """host buffers in, host buffer out (copies inside the library, synchronous)"""

@@ -293,23 +293,35 @@ static int chunk_events(const mg_process* p, int nevt, int nhel)
     return (int)ce;
 }
 
-static size_t ws_bytes_for(const mg_process* p, int nevt, int nhel)
+// optional inputs / outputs of mg_sigma_batch_ex (all DEVICE, any may be NULL)
+struct Extras {
+    const double* alphas = nullptr; const double* rndhel = nullptr; const double* rndcol = nullptr;
+    int* selhel = nullptr; int* selcol = nullptr;
+};
+
+static size_t ws_bytes_for(const mg_process* p, int nevt, int nhel, bool need_jamps = false)
 {
-    size_t b = align256((size_t)nhel * nevt * sizeof(double));
-    if ((p->color_sum == MG_CS_TENSOR || p->diagrams == MG_DIAG_SHARED) && nevt > 0) {
+    size_t b = align256((size_t)nhel * nevt * sizeof(double)) + align256((size_t)nevt * sizeof(double));   // me_h, coupling factors
+    if ((p->color_sum == MG_CS_TENSOR || p->diagrams == MG_DIAG_SHARED || need_jamps) && nevt > 0) {
         const int ce = chunk_events(p, nevt, nhel);
         b += align256(color_sum_padded_rows((long)nhel * ce) * p->d->ncolor * 2 * cs_elem(p));
     }
     return b;
 }
 
-extern "C" size_t mg_workspace_bytes(const mg_process* p, int nevt)
+static size_t workspace_bytes(const mg_process* p, int nevt, bool need_jamps)
 {
     if (!p || nevt < 0) return 0;
     const int nprobe = nevt < 1024 ? nevt : 1024;
-    size_t a = ws_bytes_for(p, nevt, p->good.empty() ? p->d->ncomb : (int)p->good.size());
+    size_t a = ws_bytes_for(p, nevt, p->good.empty() ? p->d->ncomb : (int)p->good.size(), need_jamps);
     size_t b = p->good.empty() ? align256((size_t)p->d->ncomb * nprobe * sizeof(double)) : 0;   // filter uses FUSED
     return a > b ? a : b;
+}
+
+extern "C" size_t mg_workspace_bytes(const mg_process* p, int nevt) { return workspace_bytes(p, nevt, false); }
+extern "C" size_t mg_workspace_bytes_ex(const mg_process* p, int nevt, int want_selcol)
+{
+    return workspace_bytes(p, nevt, want_selcol != 0 && p && p->d->ncolor > 1);
 }
 
 __global__ void helicity_sum_kernel(const double* __restrict__ meh, int nhel, int nevt, double* __restrict__ me)
@@ -319,6 +331,99 @@ __global__ void helicity_sum_kernel(const double* __restrict__ meh, int nhel, in
     double s = 0.0;
     for (int h = 0; h < nhel; h++) s += meh[(size_t)h * nevt + e];
     me[e] = s;
+}
+
+// alpha_s-dependent couplings, one thread per event ("an event-by-event running QCD coupling constant
+// alpha_s(Q^2)"; the dependent couplings are computed in a kernel of their own): G = sqrt(4 pi alpha_s(e));
+// every diagram of these processes carries G^order, so the squared amplitude scales by (G(e)^2 / G_card^2)^order
+__global__ void couplings_kernel(const double* __restrict__ alphas, int nevt, int order, double g2_card, double* __restrict__ gfac)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nevt) return;
+    const double g2 = 4.0 * 3.14159265358979323846 * alphas[e];
+    double f = 1.0;
+    for (int k = 0; k < order; k++) f *= g2 / g2_card;
+    gfac[e] = f;
+}
+
+// helicity sum with the per-event coupling factor and the helicity selection ("Randomly select a color and
+// a helicity for event ievt"; reading A15): the first good helicity k (increasing h) with rnd * sum < cum_k
+__global__ void helicity_sum_select_kernel(const double* __restrict__ meh, int nhel, int nevt, const double* __restrict__ gfac,
+                                           const double* __restrict__ rndhel, const int* __restrict__ good,
+                                           double* __restrict__ me, int* __restrict__ selhel)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nevt) return;
+    double s = 0.0;
+    for (int h = 0; h < nhel; h++) s += meh[(size_t)h * nevt + e];
+    me[e] = gfac ? gfac[e] * s : s;
+    if (selhel) {
+        const double target = rndhel[e] * s;
+        double c = 0.0;
+        int k = 0;
+        for (; k < nhel - 1; k++) {
+            c += meh[(size_t)k * nevt + e];
+            if (target < c) break;
+        }
+        selhel[e] = good[k];
+    }
+}
+
+// colour selection: weight of colour flow c = sum over good helicities of |J_c|^2; the first c with rnd * sum < cum_c.
+// One warp per event; lanes stride over the event's rows.  LAYOUT 0: [2][nc][rows], row = el * nhel + ih (event-major);
+// 1: [2][nc][rows], row = ih * ne + el (helicity-major); 2: tile-major [row / 128][2][nc][128], row = el * nhel + ih
+template <typename T, int LAYOUT>
+__global__ void __launch_bounds__(128) select_color_kernel(const T* __restrict__ J, int nc, int nhel, int ne, long rows,
+                                                            const double* __restrict__ rndcol, int e0, int* __restrict__ selcol)
+{
+    extern __shared__ double wsm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int el = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (el >= ne) return;
+    double* w = wsm + (size_t)warp * nc;
+    for (int c = 0; c < nc; c++) {
+        double s = 0.0;
+        for (int ih = lane; ih < nhel; ih += 32) {
+            double re, im;
+            if (LAYOUT == 2) {
+                const long row = (long)el * nhel + ih;
+                const T* t = J + (row >> 7) * (256L * nc) + (long)c * 128 + (row & 127);
+                re = (double)t[0]; im = (double)t[128L * nc];
+            } else {
+                const long row = LAYOUT == 0 ? (long)el * nhel + ih : (long)ih * ne + el;
+                re = (double)J[(long)c * rows + row]; im = (double)J[(long)(nc + c) * rows + row];
+            }
+            s += re * re + im * im;
+        }
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) w[c] = s;
+    }
+    __syncwarp();
+    if (lane == 0) {
+        double tot = 0.0;
+        for (int c = 0; c < nc; c++) tot += w[c];
+        const double target = rndcol[e0 + el] * tot;
+        double cum = 0.0;
+        int c = 0;
+        for (; c < nc - 1; c++) {
+            cum += w[c];
+            if (target < cum) break;
+        }
+        selcol[e0 + el] = c;
+    }
+}
+
+template <typename T>
+static cudaError_t launch_select_color(int layout, const void* J, int nc, int nhel, int ne, long rows, const double* rnd, int e0,
+                                       int* sel, cudaStream_t st)
+{
+    const int warps = 4;
+    const unsigned grid = (unsigned)((ne + warps - 1) / warps);
+    const size_t sm = sizeof(double) * warps * nc;
+    if (layout == 0) select_color_kernel<T, 0><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
+    else if (layout == 1) select_color_kernel<T, 1><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
+    else select_color_kernel<T, 2><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
+    return cudaGetLastError();
 }
 
 static int set_good(mg_process* p, const std::vector<int>& good)
@@ -436,8 +541,8 @@ static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
     return MG_OK;
 }
 
-extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
-                              size_t ws_bytes, void* cuda_stream)
+static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                            size_t ws_bytes, void* cuda_stream, const Extras& ex)
 {
     if (!p || nevt < 0) return fail(p, MG_EINVAL, "bad arguments");
     if (nevt == 0) return MG_OK;
@@ -445,16 +550,28 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
     if (((size_t)d_workspace & 255) != 0) return fail(p, MG_EINVAL, "workspace must be 256-byte aligned");
     CUDA_TRY(p, cudaSetDevice(p->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (ws_bytes < mg_workspace_bytes(p, nevt)) return fail(p, MG_EINVAL, "workspace too small");
+    if ((ex.selhel != nullptr) != (ex.rndhel != nullptr) || (ex.selcol != nullptr) != (ex.rndcol != nullptr))
+        return fail(p, MG_EINVAL, "a selection output needs its random-number input and vice versa");
+    const bool want_col = ex.selcol != nullptr && p->d->ncolor > 1;
+    if (ws_bytes < workspace_bytes(p, nevt, want_col)) return fail(p, MG_EINVAL, "workspace too small");
     if (p->good.empty()) {
         const int nprobe = nevt < 1024 ? nevt : 1024;
         int rc = mg_helicity_filter(p, d_momenta, nprobe, d_workspace, ws_bytes, cuda_stream, nullptr, nullptr);
         if (rc != MG_OK) return rc;
-        if (ws_bytes < mg_workspace_bytes(p, nevt)) return fail(p, MG_EINVAL, "workspace too small");
+        if (ws_bytes < workspace_bytes(p, nevt, want_col)) return fail(p, MG_EINVAL, "workspace too small");
     }
     const int nhel = (int)p->good.size();
     double* d_meh = (double*)d_workspace;
-    char* d_j = (char*)d_workspace + align256((size_t)nhel * nevt * sizeof(double));
+    double* d_gfac = (double*)((char*)d_workspace + align256((size_t)nhel * nevt * sizeof(double)));
+    char* d_j = (char*)d_gfac + align256((size_t)nevt * sizeof(double));
+    // colour selection reads the jamps: the thread kernel then takes its jamps-buffer path whatever "color_sum" says
+    const int color_sum = want_col ? MG_CS_TENSOR : p->color_sum;
+    auto select_color = [&](int layout, const void* J, int ne, long rows, int e0) -> cudaError_t {
+        if (!want_col) return cudaSuccess;
+        p->launches++;
+        return p->precision == MG_FP64 ? launch_select_color<double>(layout, J, p->d->ncolor, nhel, ne, rows, ex.rndcol, e0, ex.selcol, st)
+                                       : launch_select_color<float>(layout, J, p->d->ncolor, nhel, ne, rows, ex.rndcol, e0, ex.selcol, st);
+    };
     p->timed = false; p->ev_n = 0; p->launches = 0;
     MARK(-1);
     if (p->diagrams == MG_DIAG_SHARED) {
@@ -481,9 +598,10 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             else
                 ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st, tile_major);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("colour sum: ") + cudaGetErrorString(ce_));
+            CUDA_TRY(p, select_color(tile_major ? 2 : 0, d_j, ne, a.rows, e0));
             MARK(1);
         }
-    } else if (p->color_sum == MG_CS_FUSED) {
+    } else if (color_sum == MG_CS_FUSED) {
         DiagLaunch a = base_launch(p, d_momenta, nevt);
         a.d_hel = p->d_good; a.d_meh = d_meh; a.mode = MG_CS_FUSED;
         int rc = run_diagrams(p, a, st);
@@ -505,15 +623,41 @@ extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, 
             cudaError_t ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("color_sum_tensor: ") + cudaGetErrorString(ce_));
             p->launches++;
+            CUDA_TRY(p, select_color(1, d_j, ne, a.rows, e0));
             MARK(1);
         }
     }
-    helicity_sum_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, d_me);
+    if (ex.selcol && !want_col) CUDA_TRY(p, cudaMemsetAsync(ex.selcol, 0, (size_t)nevt * sizeof(int), st));      // one colour flow
+    if (ex.alphas || ex.selhel) {
+        if (ex.alphas) {
+            couplings_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(ex.alphas, nevt, p->d->coupling_order, 4.0 * M_PI * p->aS, d_gfac);
+            CUDA_TRY(p, cudaGetLastError());
+            p->launches++;
+        }
+        helicity_sum_select_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, ex.alphas ? d_gfac : nullptr, ex.rndhel,
+                                                                       p->d_good, d_me, ex.selhel);
+    } else
+        helicity_sum_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, d_me);
     CUDA_TRY(p, cudaGetLastError());
     p->launches++;
     MARK(2);
     p->timed = p->timing != 0;
     return MG_OK;
+}
+
+extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                              size_t ws_bytes, void* cuda_stream)
+{
+    return sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, Extras());
+}
+
+extern "C" int mg_sigma_batch_ex(mg_process* p, const double* d_momenta, int nevt, const double* d_alphas, const double* d_rndhel,
+                                 const double* d_rndcol, double* d_me, int* d_selhel, int* d_selcol, void* d_workspace,
+                                 size_t ws_bytes, void* cuda_stream)
+{
+    Extras ex;
+    ex.alphas = d_alphas; ex.rndhel = d_rndhel; ex.rndcol = d_rndcol; ex.selhel = d_selhel; ex.selcol = d_selcol;
+    return sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, ex);
 }
 
 extern "C" int mg_last_launch_count(const mg_process* p, int* launches)

@@ -262,3 +262,47 @@ def test_mixed_color_sum_variants_agree(B):
         else:
             assert _relerr(me, ref).max() < 2e-5, opts
         proc.close()
+
+
+def _near_boundary(weights, rnd, tol):
+    """True where rnd * total lies within tol * total of a cumulative boundary (the choice may then differ by rounding)"""
+    cum = np.cumsum(weights, axis=1)
+    tot = cum[:, -1:]
+    return (np.abs(cum - rnd[:, None] * tot) < tol * tot).any(axis=1)
+
+
+@pytest.mark.parametrize("process,prec,nevt", [("epem_mupmum", "fp64", 600), ("gg_ttx", "fp64", 300), ("gg_ttxg", "fp64", 150),
+                                               ("gg_ttxgg", "fp64", 70), ("gg_ttxggg", "fp64", 24), ("gg_ttxggg", "mixed", 24)])
+def test_running_alphas_and_selection(B, process, prec, nevt):
+    """mg_sigma_batch_ex (PAPER.md:77, 99-100): per-event alpha_s, selected helicity and colour, against oracle/selection.py;
+    index-exact except where the random number sits on a cumulative boundary (validity rule, A15)"""
+    from oracle import selection
+    mom = inputs.momenta(process, nevt, seed=21)
+    rng = np.random.default_rng(9)
+    al = inputs.PARAMS["aS"] * (0.7 + 0.6 * rng.random(nevt))
+    rh, rc = rng.random(nevt), rng.random(nevt)
+    proc = B.init_process(process, prec)
+    cu = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    mask = proc.helicity_filter(cu(mom))
+    good = np.nonzero(mask)[0]
+    me, sh, sc = proc.sigma_batch_ex(cu(mom), cu(al), cu(rh), cu(rc))
+    me, sh, sc = me.cpu().numpy(), sh.cpu().numpy(), sc.cpu().numpy()
+    ref, rsh, rsc = selection.select(process, mom, inputs.PARAMS, rh, rc, alphas=al, good=good)
+    tol_me, tol_sel = (1e-10, 1e-9) if prec == "fp64" else (1e-3, 1e-4)
+    assert _relerr(me, ref).max() < tol_me
+    _, mh = _oracle(process, mom, per_helicity=True)
+    ok_h = ~_near_boundary(mh[:, good], rh, tol_sel)
+    assert ok_h.sum() > 0.9 * nevt and (sh[ok_h] == rsh[ok_h]).all()
+    assert np.isin(sh, good).all()
+    if process == "epem_mupmum":
+        assert (sc == 0).all()
+    else:
+        w = selection.color_weights(process, mom, inputs.PARAMS, good)
+        ok_c = ~_near_boundary(w, rc, tol_sel)
+        assert ok_c.sum() > 0.9 * nevt and (sc[ok_c] == rsc[ok_c]).all()
+        assert sc.min() >= 0 and sc.max() < proc.ncolor
+    # without the extras the call is mg_sigma_batch
+    me0, none_h, none_c = proc.sigma_batch_ex(cu(mom))
+    assert none_h is None and none_c is None
+    assert _relerr(me0.cpu().numpy(), proc.sigma_batch(cu(mom)).cpu().numpy()).max() == 0
+    proc.close()

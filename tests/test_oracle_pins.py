@@ -476,3 +476,74 @@ def test_p10_double_vs_long_double(proc, nev, tol, params):
 
 def test_denominators():
     assert oracle.DENOM == {"epem_mupmum": 4.0, "gg_ttx": 256.0, "gg_ttxg": 256.0, "gg_ttxgg": 512.0, "gg_ttxggg": 1536.0}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# helicity / colour selection and running alpha_s (reading A15)
+def test_selection_inverse_cdf_basics():
+    from oracle import selection
+    w = [0.0, 2.0, 0.0, 1.0, 1.0]
+    assert selection.inverse_cdf(w, 0.0) == 1                   # zero-weight entries are never chosen
+    assert selection.inverse_cdf(w, 0.4999) == 1 and selection.inverse_cdf(w, 0.5) == 3
+    assert selection.inverse_cdf(w, 0.75) == 4 and selection.inverse_cdf(w, 1.0 - 1e-16) == 4
+    # frequencies follow the weights (brute force over a fine grid of random numbers)
+    counts = np.bincount([selection.inverse_cdf(w, (i + 0.5) / 4000) for i in range(4000)], minlength=5)
+    assert list(counts) == [0, 2000, 0, 1000, 1000]
+
+
+def test_selection_helicity_against_closed_form_eemumu(params):
+    """e+ e- -> mu+ mu-: the chosen helicity is the inverse CDF of the CLOSED-FORM per-helicity weights
+    (1 +- cos theta)^2 |e^2 + g g' s / (s - mZ^2 + i mZ wZ)|^2 over the good helicities 5, 6, 9, 10 (pin P1's formula)"""
+    from oracle import selection
+    nevt = 64
+    p = inputs.momenta("epem_mupmum", nevt, seed=11)
+    rng = np.random.default_rng(5)
+    rh, rc = rng.random(nevt), rng.random(nevt)
+    me, sh, sc = selection.select("epem_mupmum", p, params, rh, rc)
+    e2, gl, gr = _ee_couplings(params)
+    s = 1500.0 ** 2
+    prop = s / (s - params["mZ"] ** 2 + 1j * params["mZ"] * params["wZ"])
+    for e in range(nevt):
+        ct = np.dot(p[e, 1, 1:], p[e, 3, 1:]) / (np.linalg.norm(p[e, 1, 1:]) * np.linalg.norm(p[e, 3, 1:]))
+        w = {}
+        for h in (5, 6, 9, 10):
+            le = 1 if (h >> 2) & 1 else -1                      # helicity of the e- (particle 1)
+            lm = 1 if h & 1 else -1                             # helicity of the mu- (particle 3)
+            ge, gm = (gr if le > 0 else gl), (gr if lm > 0 else gl)
+            w[h] = (1 + (1 if le == lm else -1) * ct) ** 2 * abs(e2 + ge * gm * prop) ** 2
+        tot = sum(w.values())
+        cum, want = 0.0, 10
+        for h in (5, 6, 9, 10):
+            cum += w[h]
+            if rh[e] * tot < cum:
+                want = h
+                break
+        assert sh[e] == want, (e, sh[e], want)
+    assert (sc == 0).all()
+
+
+def test_selection_colour_bose_and_alphas(params):
+    """g g -> t tbar: exchanging the two beam gluons maps the colour flow (0,1) onto (1,0), so the colour weights swap and
+    the chosen colour follows; me with a running alpha_s is the card's me times (alpha_s / aS)^2; the choices do not depend
+    on alpha_s"""
+    from oracle import selection
+    nevt = 24
+    p = inputs.momenta("gg_ttx", nevt, seed=13)
+    q = p.copy()
+    q[:, [0, 1]] = q[:, [1, 0]]
+    q[:, :, 3] *= -1                                            # rotate by pi about x: beams back to (+z, -z) ...
+    q[:, :, 2] *= -1                                            # ... a proper rotation, so helicities are unchanged
+    good = np.arange(16)
+    w = selection.color_weights("gg_ttx", p, params, good)
+    wq = selection.color_weights("gg_ttx", q, params, good)
+    assert np.abs(wq[:, ::-1] / w - 1).max() < 1e-10
+    assert np.abs(w[:, 0] / w[:, 1] - 1).max() > 0.05           # the two flows really differ
+    rng = np.random.default_rng(6)
+    rh, rc = rng.random(nevt), rng.random(nevt)
+    me, sh, sc = selection.select("gg_ttx", p, params, rh, rc)
+    _, _, scq = selection.select("gg_ttx", q, params, rh, 1.0 - rc)         # mirrored CDF <-> mirrored random number
+    assert (scq == 1 - sc).all()
+    al = params["aS"] * (0.8 + 0.4 * rng.random(nevt))
+    me2, sh2, sc2 = selection.select("gg_ttx", p, params, rh, rc, alphas=al)
+    assert np.abs(me2 / (me * (al / params["aS"]) ** 2) - 1).max() < 1e-12
+    assert (sh2 == sh).all() and (sc2 == sc).all()
