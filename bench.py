@@ -26,9 +26,21 @@ sys.path.insert(0, ROOT)
 
 from paper_2510_05392_b200 import inputs  # noqa: E402
 
-# DRAM bytes per event of the diagram kernel from the committed ncu --set full capture (profiles/r1_summary.md:
-# dram__bytes_read.sum + dram__bytes_write.sum = 3.3 MB + 948.3 MB for 4096 events); algorithmic = the jamps, 245 760 B
-NCU_DRAM_BYTES_PER_EVENT = {("gg_ttxggg", "fp64"): (3.291648e6 + 948.265216e6) / 4096}
+# DRAM bytes of the dominant kernel from the committed ncu --set full captures: profiles/dram_traffic.csv holds one row per
+# capture (process, precision, events of the launch, dram__bytes_read.sum, dram__bytes_write.sum, capture file); the figure is
+# scaled to the timed launch by the event count.  No row for the timed (process, precision) -> "traffic": null.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+
+
+def ncu_dram_bytes_per_event(process, precision):
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, None
+    last = None
+    for line in open(TRAFFIC_CSV):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 6 and f[0] == process and f[1] == precision:
+            last = ((float(f[3]) + float(f[4])) / float(f[2]), f[5])
+    return last if last else (None, None)
 
 HEADLINE = "gg_ttxggg"      # BASELINE.json configs[4]: the process the north star's roofline targets are set on
 METRIC = "matrix elements/sec"
@@ -167,13 +179,13 @@ def spawn_ranks(argv, gpus):
     return subprocess.call(cmd)
 
 
-def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world, flush, opts=None, dist=None):
-    """returns dict with device-timed throughput of `steps` batches"""
+def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world, flush, opts=None, dist=None, stages=True):
+    """returns dict with device-timed throughput of `steps` batches (stages: also the per-stage CUDA-event times)"""
     dev = torch.cuda.current_device()
     proc = B.Process(process, precision, dev)
     for k, v in (opts or {}).items():
         proc.set_option(k, v)
-    proc.set_option("timing", 1)
+    proc.set_option("timing", 1 if stages else 0)
     mom_h = inputs.momenta(process, nevt, seed=1, first_event=shard_first_event(rank, nevt))
     d_mom = torch.from_numpy(mom_h).to(f"cuda:{dev}")
     mask = proc.helicity_filter(d_mom)
@@ -195,7 +207,8 @@ def time_process(torch, B, process, precision, nevt, steps, warmup, rank, world,
         proc.sigma_batch(d_mom, d_me)
         ev[i][1].record()
         ev[i][1].synchronize()
-        stage += np.array(proc.last_stage_ms())
+        if stages:
+            stage += np.array(proc.last_stage_ms())
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in ev)
     ms = reduce_max_ms(ms, dist, f"cuda:{dev}")
@@ -282,11 +295,12 @@ def main():
     if not shared and proc.get_option("color_sum") == 0:
         alg_flop += (2.0 * proc.ncolor * (proc.ncolor + 1) + 4.0 * proc.ncolor) * nevt * r["ngood"]   # fused triangular colour sum
     achieved = alg_flop / (diag_ms * 1e-3) * 1e-12
+    dram_per_event, dram_src = ncu_dram_bytes_per_event(process, args.precision) if shared else (None, None)
     roofline = {"bound": "alu", "kernel": "hs_diagrams_kernel" if shared else "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak if fp64_peak else None,
-                "traffic": (NCU_DRAM_BYTES_PER_EVENT[(process, args.precision)] * nevt
-                            if shared and (process, args.precision) in NCU_DRAM_BYTES_PER_EVENT else None),
-                "traffic_source": "ncu capture at 4096 events (profiles/r1_summary.md), scaled to this launch by the event count",
+                "traffic": dram_per_event * nevt if dram_per_event else None,
+                "traffic_source": (f"ncu --set full capture {dram_src} (profiles/dram_traffic.csv), scaled to this launch by the "
+                                   "event count") if dram_per_event else None,
                 "peak_source": "fp64 FMA probe kernel measured in this run (mg_measure_peak, burst); "
                                "MEASURED_PEAKS.json holds no fp64 figure",
                 "flop_per_event_helicity": proc.diagram_flops, "kernel_ms": diag_ms,
@@ -309,13 +323,23 @@ def main():
                                                          "helicity_sum": r["stage_ms"][2]},
            "roofline": roofline, "clocks": clocks}
 
-    if rank == 0 and args.ramp:
-        ramp, n = {}, 32
-        while n <= nevt:
-            q = time_process(torch, B, process, args.precision, n, 5, 3, 0, 1, flush, opts)
-            ramp[str(n)] = q["value"]
-            q["proc"].close()
+    if rank == 0 and (args.ramp or not args.no_extras):
+        # the paper's small-grid curves (MEs/s against events per batch): plain launches, and the
+        # same launch sequence replayed as a CUDA graph (option "graph")
+        sizes, n = [], 32
+        while n < nevt:
+            sizes.append(n)
             n *= 4
+        ramp = {"plain": {}, "graph": {}}
+        for n in sizes:
+            for mode in ("plain", "graph"):
+                q = time_process(torch, B, process, args.precision, n, 10, 3, 0, 1, None, dict(opts, graph=1 if mode == "graph" else 0),
+                                 stages=False)
+                ramp[mode][str(n)] = q["value"]
+                q["proc"].close()
+        ramp["plain"][str(nevt)] = r["value"]
+        peak = max(ramp["plain"].values())
+        ramp["events_for_90pct_of_peak"] = min(int(k) for k, v in ramp["plain"].items() if v >= 0.9 * peak)
         out["ramp_MEs_per_s"] = ramp
     if rank == 0 and not args.no_extras:
         # end to end through the host-buffer entry point: pinned host momenta -> device -> me -> host, every step

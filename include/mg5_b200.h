@@ -76,7 +76,11 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
 /* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
  * MG_DIAG_THREAD kernel, multiple of 32, <= 256),
  * "hs_color_alu" (MG_DIAG_SHARED in MG_MIXED: 1 = scalar-ALU fp32 colour-sum kernel instead of the tcgen05 one),
- * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1).
+ * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1),
+ * "max_streams" (MG_SCHED_STREAMS: helicities share this many streams round robin, 0 = one each),
+ * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the
+ * arguments and the handle's state are unchanged; ignored while "timing" = 1; mg_get_option
+ * "graph_replays" counts the replays of the current graph).
  * Unknown key, bad value, or a combination that cannot run (helicity streams with the MG_DIAG_SHARED kernel, which has
  * no per-helicity launches) -> MG_EINVAL, nothing changed. */
 int mg_set_option(mg_process* p, const char* key, int value);

@@ -31,6 +31,24 @@ struct mg_process {
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
     int diagrams = MG_DIAG_THREAD, hs_color_alu = 0;
+    int max_streams = 0;       // MG_SCHED_STREAMS: helicity h runs on stream h % max_streams (0 = one stream per helicity)
+    int graph = 0;             // replay the launch sequence of a batch as a CUDA graph
+    // the captured batch: valid for exactly these arguments and this state of the handle (epoch)
+    struct GraphKey {
+        const double* mom = nullptr; double* me = nullptr; void* ws = nullptr; int nevt = 0; cudaStream_t st = nullptr;
+        const void* ex[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
+        long epoch = -1;
+        bool operator==(const GraphKey& o) const
+        {
+            return mom == o.mom && me == o.me && ws == o.ws && nevt == o.nevt && st == o.st && epoch == o.epoch &&
+                   !memcmp(ex, o.ex, sizeof ex);
+        }
+    } gkey;
+    cudaGraphExec_t gexec = nullptr;
+    cudaStream_t gstream = nullptr;          // capture / replay stream when the caller passes the legacy default stream
+    cudaEvent_t gev_in = nullptr, gev_out = nullptr;
+    long epoch = 0;            // bumped by every call that changes what a batch launches
+    int graph_replays = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 1L << 30;
@@ -185,6 +203,10 @@ extern "C" void mg_destroy(mg_process* p)
     for (auto e : p->ev_join) cudaEventDestroy(e);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     for (auto e : p->ev_pool) cudaEventDestroy(e);
+    if (p->gexec) cudaGraphExecDestroy(p->gexec);
+    if (p->gstream) cudaStreamDestroy(p->gstream);
+    if (p->gev_in) cudaEventDestroy(p->gev_in);
+    if (p->gev_out) cudaEventDestroy(p->gev_out);
     delete p;
 }
 
@@ -233,6 +255,7 @@ extern "C" int mg_set_parameters(mg_process* p, const char* const* keys, const d
     if (!(tmp.aEWM1 > 0) || !(tmp.mZ > 0) || !(tmp.mW > 0) || !(tmp.mW < tmp.mZ) || !(tmp.mT >= 0) || !(tmp.aS > 0) ||
         !(tmp.wZ >= 0) || !(tmp.wT >= 0))
         return fail(p, MG_EINVAL, "parameter out of range");
+    p->epoch++;
     p->aEWM1 = tmp.aEWM1; p->mZ = tmp.mZ; p->wZ = tmp.wZ; p->mW = tmp.mW; p->mT = tmp.mT; p->wT = tmp.wT; p->aS = tmp.aS;
     return MG_OK;
 }
@@ -264,7 +287,13 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
     } else if (!strcmp(key, "jamp_chunk_mib")) {
         if (value < 1) return fail(p, MG_EINVAL, "bad jamp_chunk_mib");
         p->jamp_chunk_bytes = (long)value << 20;
+    } else if (!strcmp(key, "max_streams")) {
+        if (value < 0 || value > 1024) return fail(p, MG_EINVAL, "bad max_streams");
+        p->max_streams = value;
+    } else if (!strcmp(key, "graph")) {
+        p->graph = value != 0;
     } else return fail(p, MG_EINVAL, std::string("unknown option ") + key);
+    p->epoch++;
     return MG_OK;
 }
 
@@ -278,6 +307,9 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "hs_color_alu")) *value = p->hs_color_alu;
     else if (!strcmp(key, "timing")) *value = p->timing;
     else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
+    else if (!strcmp(key, "max_streams")) *value = p->max_streams;
+    else if (!strcmp(key, "graph")) *value = p->graph;
+    else if (!strcmp(key, "graph_replays")) *value = p->graph_replays;
     else return MG_EINVAL;
     return MG_OK;
 }
@@ -429,6 +461,7 @@ static cudaError_t launch_select_color(int layout, const void* J, int nc, int nh
 static int set_good(mg_process* p, const std::vector<int>& good)
 {
     p->good = good;
+    p->epoch++;
     if (!good.empty()) {
         CUDA_TRY(p, cudaMemcpy(p->d_good, good.data(), good.size() * sizeof(int), cudaMemcpyHostToDevice));
         std::vector<int> pos(p->d->ncomb, -1);
@@ -526,16 +559,21 @@ static int run_diagrams(mg_process* p, DiagLaunch a, cudaStream_t st)
         CUDA_TRY(p, p->d->launch(p->precision, a, st));
         p->launches++;
     } else {
-        int rc = ensure_streams(p, nhel);
+        // one stream per good helicity, or a fixed number of them shared round robin ("study how
+        // many streams are actually useful, and limit them to a fixed number")
+        const int ns = p->max_streams > 0 && p->max_streams < nhel ? p->max_streams : nhel;
+        int rc = ensure_streams(p, ns);
         if (rc != MG_OK) return rc;
         CUDA_TRY(p, cudaEventRecord(p->ev_fork, st));
+        for (int s_ = 0; s_ < ns; s_++) CUDA_TRY(p, cudaStreamWaitEvent(p->streams[s_], p->ev_fork, 0));
         for (int h = 0; h < nhel; h++) {
-            CUDA_TRY(p, cudaStreamWaitEvent(p->streams[h], p->ev_fork, 0));
             a.hel_base = h; a.nhel = 1;
-            CUDA_TRY(p, p->d->launch(p->precision, a, p->streams[h]));
+            CUDA_TRY(p, p->d->launch(p->precision, a, p->streams[h % ns]));
             p->launches++;
-            CUDA_TRY(p, cudaEventRecord(p->ev_join[h], p->streams[h]));
-            CUDA_TRY(p, cudaStreamWaitEvent(st, p->ev_join[h], 0));
+        }
+        for (int s_ = 0; s_ < ns; s_++) {
+            CUDA_TRY(p, cudaEventRecord(p->ev_join[s_], p->streams[s_]));
+            CUDA_TRY(p, cudaStreamWaitEvent(st, p->ev_join[s_], 0));
         }
     }
     return MG_OK;
@@ -645,10 +683,65 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
     return MG_OK;
 }
 
+// option "graph": the launch sequence of a batch (diagram kernels on their helicity streams, colour sums, selections, helicity
+// sum) is captured into a CUDA graph on its first execution and replayed while the arguments and the handle's state stay
+// the same -- the paper's gpuDiagrams wrapper ("configures graphs on its first execution ... on
+// subsequent executions it runs kernels via graphs rather than launching them individually")
+static int sigma_batch_graph(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace, size_t ws_bytes,
+                             void* cuda_stream, const Extras& ex)
+{
+    if (!p) return MG_EINVAL;
+    if (!p->graph || p->timing || nevt <= 0)
+        return sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, ex);
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    cudaStream_t user = (cudaStream_t)cuda_stream;
+    if (p->good.empty()) {          // the filter synchronises: not capturable, and it changes what a batch launches
+        if (!d_momenta || !d_workspace) return fail(p, MG_EINVAL, "NULL buffer");
+        int rc = mg_helicity_filter(p, d_momenta, nevt < 1024 ? nevt : 1024, d_workspace, ws_bytes, cuda_stream, nullptr, nullptr);
+        if (rc != MG_OK) return rc;
+    }
+    // the legacy default stream cannot be captured: run on a library stream ordered after / before it with events
+    cudaStream_t st = user;
+    if (user == nullptr || user == cudaStreamLegacy) {
+        if (!p->gstream) {
+            CUDA_TRY(p, cudaStreamCreateWithFlags(&p->gstream, cudaStreamNonBlocking));
+            CUDA_TRY(p, cudaEventCreateWithFlags(&p->gev_in, cudaEventDisableTiming));
+            CUDA_TRY(p, cudaEventCreateWithFlags(&p->gev_out, cudaEventDisableTiming));
+        }
+        st = p->gstream;
+        CUDA_TRY(p, cudaEventRecord(p->gev_in, user));
+        CUDA_TRY(p, cudaStreamWaitEvent(st, p->gev_in, 0));
+    }
+    mg_process::GraphKey key;
+    key.mom = d_momenta; key.me = d_me; key.ws = d_workspace; key.nevt = nevt; key.st = st; key.epoch = p->epoch;
+    key.ex[0] = ex.alphas; key.ex[1] = ex.rndhel; key.ex[2] = ex.rndcol; key.ex[3] = ex.selhel; key.ex[4] = ex.selcol;
+    if (!(p->gexec && key == p->gkey)) {
+        if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
+        CUDA_TRY(p, cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed));
+        const int rc = sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, st, ex);
+        cudaGraph_t g = nullptr;
+        const cudaError_t ce = cudaStreamEndCapture(st, &g);          // always leave capture mode
+        if (rc != MG_OK) { if (g) cudaGraphDestroy(g); return rc; }
+        if (ce != cudaSuccess) return fail(p, MG_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
+        const cudaError_t ci = cudaGraphInstantiate(&p->gexec, g, 0);
+        cudaGraphDestroy(g);
+        if (ci != cudaSuccess) { p->gexec = nullptr; return fail(p, MG_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ci)); }
+        p->gkey = key;
+        p->graph_replays = 0;
+    } else
+        p->graph_replays++;
+    CUDA_TRY(p, cudaGraphLaunch(p->gexec, st));
+    if (st != user) {
+        CUDA_TRY(p, cudaEventRecord(p->gev_out, st));
+        CUDA_TRY(p, cudaStreamWaitEvent(user, p->gev_out, 0));
+    }
+    return MG_OK;
+}
+
 extern "C" int mg_sigma_batch(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
                               size_t ws_bytes, void* cuda_stream)
 {
-    return sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, Extras());
+    return sigma_batch_graph(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, Extras());
 }
 
 extern "C" int mg_sigma_batch_ex(mg_process* p, const double* d_momenta, int nevt, const double* d_alphas, const double* d_rndhel,
@@ -657,7 +750,7 @@ extern "C" int mg_sigma_batch_ex(mg_process* p, const double* d_momenta, int nev
 {
     Extras ex;
     ex.alphas = d_alphas; ex.rndhel = d_rndhel; ex.rndcol = d_rndcol; ex.selhel = d_selhel; ex.selcol = d_selcol;
-    return sigma_batch_impl(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, ex);
+    return sigma_batch_graph(p, d_momenta, nevt, d_me, d_workspace, ws_bytes, cuda_stream, ex);
 }
 
 extern "C" int mg_last_launch_count(const mg_process* p, int* launches)

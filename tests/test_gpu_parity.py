@@ -306,3 +306,32 @@ def test_running_alphas_and_selection(B, process, prec, nevt):
     assert none_h is None and none_c is None
     assert _relerr(me0.cpu().numpy(), proc.sigma_batch(cu(mom)).cpu().numpy()).max() == 0
     proc.close()
+
+
+def test_graph_replay_and_capped_streams(B):
+    """options "graph" and "max_streams": the same numbers as the plain launch sequence,
+    the graph is captured once and replayed, and re-captured when the arguments or the handle's state change"""
+    for process, nevt in (("gg_ttxg", 777), ("gg_ttxggg", 130)):
+        mom = torch.from_numpy(inputs.momenta(process, nevt, seed=4)).cuda()
+        ref_p = B.init_process(process, "fp64")
+        ref = ref_p.sigma_batch(mom).cpu().numpy()
+        ref_p.close()
+        proc = B.init_process(process, "fp64")
+        if process == "gg_ttxg":
+            proc.set_option("schedule", 1)
+            proc.set_option("max_streams", 5)
+        proc.set_option("graph", 1)
+        me = torch.empty(nevt, dtype=torch.float64, device="cuda")
+        for it in range(4):
+            proc.sigma_batch(mom, me)
+            assert _relerr(me.cpu().numpy(), ref).max() < 1e-12, (process, it)
+        assert proc.get_option("graph_replays") == 3
+        with torch.cuda.stream(torch.cuda.Stream()):                 # a non-default stream: captured in place
+            proc.sigma_batch(mom, me)
+            torch.cuda.current_stream().synchronize()
+        assert proc.get_option("graph_replays") == 0 and _relerr(me.cpu().numpy(), ref).max() < 1e-12
+        proc.set_parameters(aS=0.2)                                   # state change: new capture, new numbers
+        proc.sigma_batch(mom, me)
+        n = {"gg_ttxg": 3, "gg_ttxggg": 5}[process]
+        assert _relerr(me.cpu().numpy(), ref * (0.2 / inputs.PARAMS["aS"]) ** n).max() < 1e-11
+        proc.close()
