@@ -133,6 +133,9 @@ static int upload_tables(mg_process* p)
     if (p->precision == MG_FP64) {
         std::vector<double> lp; int ncp = 0;
         if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
+        std::vector<double> frag;
+        color_cholesky_fragments(ncp, lp, frag);               // row-major factor, then its fragment-order copy
+        lp.insert(lp.end(), frag.begin(), frag.end());
         CUDA_TRY(p, cudaMalloc(&p->d_chol, lp.size() * sizeof(double)));
         CUDA_TRY(p, cudaMemcpy(p->d_chol, lp.data(), lp.size() * sizeof(double), cudaMemcpyHostToDevice));
     } else {

@@ -123,6 +123,159 @@ __global__ void __launch_bounds__(128) color_sum_dmma_kernel(const double* __res
     if (ak == 0) map.store(meh, row, s);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// DMMA kernel for ncolor a multiple of 24 (24, 120 colours): persistent CTAs of 16 warps, one per SM.
+//   - the Cholesky factor sits in shared memory in FRAGMENT order: one 32-double block per (k-step, n-tile) pair on or
+//     below the diagonal, element [lane] = L[4 ks + lane % 4][8 j + lane / 4], so that a B fragment is one conflict-free
+//     LDS.64 per lane (color_cholesky_fragments);
+//   - the jamps stream through a 4-stage cp.async ring of [2 parts][24 colours][64 rows] chunks (row stride 68 doubles:
+//     the A-fragment reads of a half-warp, 4 rows x 4 colours, fall into 16 different bank pairs);
+//   - a tile = 64 rows; warps 2 p and 2 p + 1 share the rows 8 p .. 8 p + 7 (re and im parts: two m8 tiles per B fragment)
+//     and split the n-tiles between them with equal numbers of MMAs (lists TA / TB below); the k loop is fully unrolled,
+//     so the triangular skipping costs no predicated issue slots;
+//   - epilogue: sum of squares of the accumulators, quad reduction, the two warps of a pair meet at a named barrier.
+// Issued MMAs per 8 complex rows: 2 * 240 of 2 * 450 (ncolor = 120) -- the factor 2 of the paper's triangular trick
+// (PAPER.md:303, 328).
+template <int NT> struct CsCfg {
+    static constexpr int NC = 8 * NT, KC = 24, NCHUNK = NC / KC, ROWS = 64, RS = 68, STAGES = 4, WARPS = 16;
+    static constexpr int NKS = NC / 4;                                       // k-steps
+    static constexpr int STAGE_DOUBLES = 2 * KC * RS;
+    __host__ __device__ static constexpr int ntile_of(int ks) { return ks / 2 + 1; }      // n-tiles with 8 j <= 4 ks + 3
+    __host__ __device__ static constexpr int block_of(int ks, int j)
+    {
+        int o = 0;
+        for (int i = 0; i < ks; i++) o += ntile_of(i);
+        return o + j;
+    }
+    static constexpr int NBLK = block_of(NKS, 0);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)NBLK * 32 + (size_t)STAGES * STAGE_DOUBLES + 2 * WARPS * 8);
+    // n-tiles of the two warps of a pair: tile j costs (NT - j) k-step pairs; dealt heaviest first to the lighter warp
+    __host__ __device__ static constexpr bool in_half(int j, int half)
+    {
+        int la = 0, lb = 0;
+        bool mine = false;
+        for (int t = 0; t < NT; t++) {
+            const bool to_a = la <= lb;
+            if (to_a) la += NT - t; else lb += NT - t;
+            if (t == j) mine = (half == 0) == to_a;
+        }
+        return mine;
+    }
+    // accumulator slot of n-tile j inside its half, and the largest number of n-tiles of a half
+    __host__ __device__ static constexpr int slot_of(int j, int half)
+    {
+        int s = 0;
+        for (int t = 0; t < j; t++) s += in_half(t, half) ? 1 : 0;
+        return s;
+    }
+    static constexpr int MAXS = slot_of(NT, 0) > slot_of(NT, 1) ? slot_of(NT, 0) : slot_of(NT, 1);
+};
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+
+template <int NT, int HALF>
+__device__ __forceinline__ void cs2_chunk(const double* __restrict__ Ls, const double* __restrict__ xs, int chunk, int lane,
+                                          double (&acc)[CsCfg<NT>::MAXS][4])
+{
+    using C = CsCfg<NT>;
+    const int ar = lane >> 2, ak = lane & 3;
+    // this lane's A elements of the chunk: colour kk + ak, row ar (re part, then im part)
+    const double* __restrict__ xa = xs + ak * C::RS + ar;
+#pragma unroll
+    for (int c = 0; c < C::NCHUNK; c++) {
+        if (c != chunk) continue;               // (chunk is uniform; the body below is specialised per chunk)
+#pragma unroll
+        for (int kk = 0; kk < C::KC; kk += 4) {
+            const int ks = (c * C::KC + kk) / 4;
+            const double a_re = xa[kk * C::RS], a_im = xa[(C::KC + kk) * C::RS];
+#pragma unroll
+            for (int j = 0; j < NT; j++) {
+                if (j < C::ntile_of(ks) && C::in_half(j, HALF)) {
+                    const double b = Ls[C::block_of(ks, j) * 32 + lane];
+                    const int sl = C::slot_of(j, HALF);          // (constant after unrolling)
+                    dmma(acc[sl][0], acc[sl][1], a_re, b);
+                    dmma(acc[sl][2], acc[sl][3], a_im, b);
+                }
+            }
+        }
+    }
+}
+
+template <int NT>
+__global__ void __launch_bounds__(512, 1) color_sum_dmma2_kernel(const double* __restrict__ Lfrag, const double* __restrict__ X,
+                                                                 long rows_padded, RowMap map, double* __restrict__ meh)
+{
+    using C = CsCfg<NT>;
+    extern __shared__ __align__(16) double csm[];
+    double* __restrict__ Ls = csm;
+    double* __restrict__ Xs = Ls + (size_t)C::NBLK * 32;
+    double* __restrict__ part = Xs + (size_t)C::STAGES * C::STAGE_DOUBLES;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, pair = warp >> 1, half = warp & 1;
+    for (int i = tid; i < C::NBLK * 32; i += blockDim.x) Ls[i] = Lfrag[i];
+    const long ntile_rows = rows_padded / C::ROWS;
+    const long my_tiles = blockIdx.x < ntile_rows ? (ntile_rows - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const long nq = my_tiles * C::NCHUNK;                      // chunks this CTA streams
+    auto issue = [&](long q) {                                 // chunk q -> stage q % STAGES (16-byte pieces, 1536 per chunk)
+        if (q < nq) {
+            const long tile = blockIdx.x + (q / C::NCHUNK) * gridDim.x;
+            const int c0 = (int)(q % C::NCHUNK) * C::KC;
+            double* dst = Xs + (size_t)(q % C::STAGES) * C::STAGE_DOUBLES;
+            for (int pc = tid; pc < 2 * C::KC * (C::ROWS / 2); pc += 512) {
+                const int seg = pc % (C::ROWS / 2), pk = pc / (C::ROWS / 2);          // pk = part * KC + colour
+                const int prt = pk / C::KC, kc = pk % C::KC;
+                cp_async16(dst + pk * C::RS + 2 * seg, X + ((long)prt * C::NC + c0 + kc) * rows_padded + tile * C::ROWS + 2 * seg);
+            }
+        }
+        cp_async_commit();
+    };
+    for (int q = 0; q < C::STAGES - 1; q++) issue(q);
+    double acc[C::MAXS][4];
+#pragma unroll
+    for (int j = 0; j < C::MAXS; j++) { acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.0; }
+    for (long q = 0; q < nq; q++) {
+        cp_async_wait<C::STAGES - 2>();
+        __syncthreads();                                       // chunk q has landed; everybody is done with chunk q - 1
+        issue(q + C::STAGES - 1);
+        const double* xs = Xs + (size_t)(q % C::STAGES) * C::STAGE_DOUBLES + 8 * pair;
+        const int chunk = (int)(q % C::NCHUNK);
+        if (half == 0) cs2_chunk<NT, 0>(Ls, xs, chunk, lane, acc);
+        else cs2_chunk<NT, 1>(Ls, xs, chunk, lane, acc);
+        if (chunk == C::NCHUNK - 1) {
+            double s = 0.0;
+#pragma unroll
+            for (int j = 0; j < C::MAXS; j++) {          // (a slot this half does not use stays zero)
+                s += acc[j][0] * acc[j][0] + acc[j][1] * acc[j][1] + acc[j][2] * acc[j][2] + acc[j][3] * acc[j][3];
+                acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.0;
+            }
+            s += __shfl_xor_sync(0xffffffffu, s, 1);
+            s += __shfl_xor_sync(0xffffffffu, s, 2);
+            if (half == 1 && (lane & 3) == 0) part[warp * 8 + (lane >> 2)] = s;
+            pair_barrier(1 + pair);
+            if (half == 0 && (lane & 3) == 0) {
+                const long tile = blockIdx.x + (q / C::NCHUNK) * gridDim.x;
+                map.store(meh, tile * C::ROWS + 8 * pair + (lane >> 2), s + part[(warp + 1) * 8 + (lane >> 2)]);
+            }
+        }
+    }
+    cp_async_wait<0>();
+}
+
+// the Cholesky factor in the fragment order of color_sum_dmma2_kernel: block (ks, j), j <= ks / 2, element [lane] =
+// L[4 ks + lane % 4][8 j + lane / 4]; lp = the padded row-major factor of color_cholesky_padded
+void color_cholesky_fragments(int ncp, const std::vector<double>& lp, std::vector<double>& frag)
+{
+    frag.clear();
+    for (int ks = 0; ks < ncp / 4; ks++)
+        for (int j = 0; j <= ks / 2; j++)
+            for (int lane = 0; lane < 32; lane++) frag.push_back(lp[(size_t)(4 * ks + lane % 4) * ncp + 8 * j + lane / 4]);
+}
+
 // Cholesky factor of the integer colour matrix, computed on the host in long double and zero-padded to a
 // multiple of 8 columns; the caller (api.cu) uploads it once per handle.  Returns false if C is not
 // positive definite.
@@ -158,14 +311,30 @@ cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const
     const int warps = 4;
     const unsigned grid = (unsigned)((rows_padded / 8 + warps - 1) / warps);
     const double* X = (const double*)d_jamps;
-#define LAUNCH(NT) color_sum_dmma_kernel<NT><<<grid, warps * 32, 0, st>>>(d_chol, X, ncolor, rows_padded, map, d_meh)
+    if (ncp / 8 == 1) {
+        color_sum_dmma_kernel<1><<<grid, warps * 32, 0, st>>>(d_chol, X, ncolor, rows_padded, map, d_meh);
+        return cudaGetLastError();
+    }
+    // 24 / 120 colours: the persistent kernel; d_chol holds the row-major factor followed by its fragment-order copy
+    const double* d_frag = d_chol + (size_t)ncp * ncp;
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long tiles = rows_padded / 64;
+    const unsigned g2 = (unsigned)(tiles < sms ? tiles : sms);
+#define LAUNCH2(NT)                                                                                                       \
+    {                                                                                                                     \
+        cudaError_t e_ = cudaFuncSetAttribute(color_sum_dmma2_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+                                              (int)CsCfg<NT>::SMEM);                                                      \
+        if (e_ != cudaSuccess) return e_;                                                                                 \
+        color_sum_dmma2_kernel<NT><<<g2, 512, CsCfg<NT>::SMEM, st>>>(d_frag, X, rows_padded, map, d_meh);                 \
+    }
     switch (ncp / 8) {
-        case 1: LAUNCH(1); break;
-        case 3: LAUNCH(3); break;
-        case 15: LAUNCH(15); break;
+        case 3: LAUNCH2(3); break;
+        case 15: LAUNCH2(15); break;
         default: return cudaErrorInvalidValue;
     }
-#undef LAUNCH
+#undef LAUNCH2
     return cudaGetLastError();
 }
 

@@ -44,6 +44,9 @@ cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const
 
 // host: L with C = L L^T (lower-triangular, row-major, zero-padded to ncp = 8*ceil(ncolor/8) columns)
 bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out);
+// host: the same factor in the fragment order of the persistent DMMA kernel (color_sum.cu); the device image handed to
+// color_sum_tensor as d_factor in MG_FP64 is lp followed by frag
+void color_cholesky_fragments(int ncp, const std::vector<double>& lp, std::vector<double>& frag);
 
 // host: two-term TF32 image [hi | lo] of the Cholesky factor in the tcgen05 shared-memory layout (color_sum_tf32.cu)
 bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img);
