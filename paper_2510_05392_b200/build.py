@@ -24,9 +24,9 @@ LIB = os.path.join(HERE, "libmg5_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
-# per-file extra flags: the 1240-diagram process is compiled without the all-fp32 instantiation unless
-# MG_FP32_ALL=1 (compile time), see DESIGN.md
-EXTRA = {"proc_gg_ttxggg.cu": ["-DMG_NO_FP32"] if os.environ.get("MG_FP32_ALL", "0") != "1" else []}
+# per-file extra flags (none at present: the all-fp32 instantiation of the 1240-diagram process is a translation unit of
+# its own, generated/proc_gg_ttxggg_f32.cu, so that it compiles in parallel with the fp64 one)
+EXTRA = {}
 
 
 import re

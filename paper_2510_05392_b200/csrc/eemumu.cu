@@ -48,6 +48,7 @@ struct P_epem_mupmum {
     {
         epem_mupmum::jamps<T>(pe, ihel, ph, j);
     }
+    static cudaError_t launch_f32(const DiagLaunch& a, cudaStream_t st) { return launch_t<P_epem_mupmum, float, float>(a, st); }
 };
 
 const ProcessDesc* desc_epem_mupmum()

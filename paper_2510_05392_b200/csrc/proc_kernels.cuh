@@ -69,25 +69,32 @@ static cudaError_t launch_any(int precision, const DiagLaunch& a, cudaStream_t s
     switch (precision) {
         case 0: return launch_t<P, double, double>(a, st);
         case 1: return launch_t<P, double, float>(a, st);
-#ifndef MG_NO_FP32
-        case 2: return launch_t<P, float, float>(a, st);
-#endif
+        case 2: return P::launch_f32(a, st);
         default: return cudaErrorInvalidValue;
     }
 }
 
 }  // namespace mg
 
-#ifdef MG_NO_FP32
+// the all-fp32 instantiation: in this translation unit (default), in one of its own (MG_EXT_FP32: MG_DEFINE_GG_PROCESS_F32
+// there), or left out (MG_NO_FP32; mg_init_process then refuses MG_FP32 for the process)
+#if defined(MG_NO_FP32)
 #define MG_HAS_FP32 false
+#define MG_F32_BODY(NS) return cudaErrorInvalidValue;
+#define MG_F32_DECL(NS)
+#elif defined(MG_EXT_FP32)
+#define MG_HAS_FP32 true
+#define MG_F32_BODY(NS) return launch_f32_##NS(a, st);
+#define MG_F32_DECL(NS) cudaError_t launch_f32_##NS(const DiagLaunch& a, cudaStream_t st);
 #else
 #define MG_HAS_FP32 true
+#define MG_F32_BODY(NS) return launch_t<P_##NS, float, float>(a, st);
+#define MG_F32_DECL(NS)
 #endif
 
-// Defines the traits struct and the descriptor of a generated process namespace NS.
-#define MG_DEFINE_GG_PROCESS(NS, NGROUPS)                                                                  \
+#define MG_DEFINE_GG_PROCESS_F32(NS)                                                                       \
     namespace mg {                                                                                         \
-    struct P_##NS {                                                                                        \
+    struct P32_##NS {                                                                                      \
         static constexpr int NPAR = NS::NPAR, NCOLOR = NS::NCOLOR;                                         \
         template <typename T>                                                                              \
         static __device__ __forceinline__ void jamps(const double* pe, int ihel, const phys<T>& ph, cx<T>* j) \
@@ -95,6 +102,23 @@ static cudaError_t launch_any(int precision, const DiagLaunch& a, cudaStream_t s
             NS::jamps<T>(pe, ihel, ph.mt, ph.wt, j);                                                       \
         }                                                                                                  \
     };                                                                                                     \
+    cudaError_t launch_f32_##NS(const DiagLaunch& a, cudaStream_t st) { return launch_t<P32_##NS, float, float>(a, st); } \
+    }
+
+// Defines the traits struct and the descriptor of a generated process namespace NS.
+#define MG_DEFINE_GG_PROCESS(NS, NGROUPS)                                                                  \
+    namespace mg {                                                                                         \
+    MG_F32_DECL(NS)                                                                                        \
+    struct P_##NS {                                                                                        \
+        static constexpr int NPAR = NS::NPAR, NCOLOR = NS::NCOLOR;                                         \
+        template <typename T>                                                                              \
+        static __device__ __forceinline__ void jamps(const double* pe, int ihel, const phys<T>& ph, cx<T>* j) \
+        {                                                                                                  \
+            NS::jamps<T>(pe, ihel, ph.mt, ph.wt, j);                                                       \
+        }                                                                                                  \
+        static cudaError_t launch_f32(const DiagLaunch& a, cudaStream_t st);                               \
+    };                                                                                                     \
+    cudaError_t P_##NS::launch_f32(const DiagLaunch& a, cudaStream_t st) { MG_F32_BODY(NS) }               \
     const ProcessDesc* desc_##NS()                                                                         \
     {                                                                                                      \
         static const ProcessDesc d = { #NS, NS::NGLUON, NS::NPAR, NS::NCOMB, NS::NCOLOR, NS::NDIAGRAMS,    \

@@ -126,7 +126,9 @@ class Streams:
     def _objects(self):
         prog = self.prog
         self._ls, self.legsets = {}, []
-        order = sorted(range(len(prog.objs)), key=lambda i: (len(prog.objs[i].legs), i))
+        # level by level; inside a level objects with the same sequence of opcodes are neighbours, so that the lanes of a
+        # warp of phase 1 (lane = (object, variant)) mostly run the same code
+        order = sorted(range(len(prog.objs)), key=lambda i: (len(prog.objs[i].legs), tuple(t.op for t in prog.objs[i].terms), i))
         self.obj_order = order
         self.obj_slot = {}
         slot = 0

@@ -62,8 +62,6 @@ def test_fp64_parity_and_mask(B, process):
 @pytest.mark.parametrize("process", list(SMALL))
 @pytest.mark.parametrize("precision", ["mixed", "fp32"])
 def test_reduced_precision_parity(B, process, precision):
-    if process == "gg_ttxggg" and precision == "fp32":
-        pytest.skip("all-fp32 instantiation of the 1240-diagram kernel is not built by default (compile time)")
     nevt = SMALL[process]
     mom = inputs.momenta(process, nevt)
     proc = B.init_process(process, precision)
@@ -335,3 +333,27 @@ def test_graph_replay_and_capped_streams(B):
         n = {"gg_ttxg": 3, "gg_ttxggg": 5}[process]
         assert _relerr(me.cpu().numpy(), ref * (0.2 / inputs.PARAMS["aS"]) ** n).max() < 1e-11
         proc.close()
+
+
+@pytest.mark.parametrize("process,nevt", [("epem_mupmum", 4096), ("gg_ttx", 4096), ("gg_ttxg", 4096), ("gg_ttxgg", 2048),
+                                          ("gg_ttxggg", 2048)])
+def test_precision_error_study(B, process, nevt):
+    """the paper's three floating-point modes d / m / f against the fp64 oracle on the same events:
+    relative-error histograms ('full fp32 mode with its own error study'; the numbers are kept in
+    profiles/r2_precision_study.md).  Flat RAMBO without cuts reaches deep into the soft / collinear regions, where the
+    amplitudes of single diagrams cancel by many orders of magnitude: that is where fp32 amplitudes lose their digits."""
+    mom = inputs.momenta(process, nevt, seed=31)
+    ref = _oracle(process, mom)
+    d_mom = torch.from_numpy(mom).cuda()
+    stats = {}
+    for prec in ("fp64", "mixed", "fp32"):
+        proc = B.init_process(process, prec)
+        me = proc.sigma_batch(d_mom).cpu().numpy()
+        proc.close()
+        err = _relerr(me, ref)
+        _histogram(err, f"{process} {prec}")
+        stats[prec] = (float(np.median(err)), float(np.quantile(err, 0.99)), float(err.max()))
+    assert stats["fp64"][2] < 1e-10
+    assert stats["mixed"][0] < 2e-4 and stats["mixed"][2] < 1e-3
+    # all-fp32: the median stays at single-precision level; the tail is what the study is about (no bound on the maximum)
+    assert stats["fp32"][0] < 2e-4, stats["fp32"]
