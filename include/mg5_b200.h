@@ -81,6 +81,8 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
  * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the
  * arguments and the handle's state are unchanged; ignored while "timing" = 1; mg_get_option
  * "graph_replays" counts the replays of the current graph).
+ * With "diagrams" = MG_DIAG_SHARED the jamps always go through the workspace and the tensor-core colour sum ("color_sum" and
+ * "block" then only affect the helicity filter and MG_DIAG_THREAD).
  * Unknown key, bad value, or a combination that cannot run (helicity streams with the MG_DIAG_SHARED kernel, which has
  * no per-helicity launches) -> MG_EINVAL, nothing changed. */
 int mg_set_option(mg_process* p, const char* key, int value);

@@ -268,18 +268,14 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     Tf32Cfg c;
     if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128 || c.nchunks > 8 || c.a_stages > 4 || c.raw_stages > TF32_MAX_RAW)
         return cudaErrorInvalidValue;
-    static int sms = 0;
-    static size_t smem_set = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
+    // per call, for the CURRENT device: the attribute is per device and a process may hold handles on several
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const size_t smem = tf32_smem_bytes(c);
-    if (smem > smem_set) {
+    {
         cudaError_t e = cudaFuncSetAttribute(color_sum_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        smem_set = smem;
     }
     Tf32Args a;
     a.X = (const float*)d_jamps; a.Bimg = (const float*)d_factor_img; a.out = d_meh; a.rows_padded = rows_padded;
