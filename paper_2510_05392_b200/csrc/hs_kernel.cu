@@ -316,7 +316,7 @@ __device__ __forceinline__ int acc_swizzle(int h)
 template <int NG, typename T2>
 __device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, const HsLaunch& a, int fl, int e, const char* __restrict__ objl,
                                         const char* __restrict__ stgl, char* __restrict__ accs, int warp, int lane,
-                                        const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32])
+                                        const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32], uint4 nxt, uint2 cl)
 {
     using Cfg = HsCfg<NG>;
     constexpr int NH = 1 << Cfg::NPAR, NTILE = Cfg::NTILE;
@@ -327,8 +327,8 @@ __device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, co
     const uint4* __restrict__ rp = d.p3rec + (size_t)fd.x * 8 + (lane >> 2);
     const uint2* __restrict__ cp = d.p3cls + (size_t)fd.z * 32 + lane;
     const int* __restrict__ hp = tb.p3clsh + fd.z;
-    uint4 nxt = __ldg(rp);                  // the record of the next entry is always in flight
-    uint2 cl = __ldg(cp);
+    // nxt = the first entry's record, cl = the first class table (loaded by the caller, ahead of time where it can):
+    // the record of the next entry is always in flight
     for (int c = 0; c < ncls; c++) {
         const int h_ = hp[c];
         const uint2 cl_ = cl;
@@ -367,12 +367,12 @@ __device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, co
 // The records of the next chunk are in flight while the current one is evaluated.
 template <int NG>
 __device__ __forceinline__ void p2_run(const HsDev& d, int chunk0, int nchunk, const char* __restrict__ obj,
-                                       const char* __restrict__ Ks, char* __restrict__ stage, int lane)
+                                       const char* __restrict__ Ks, char* __restrict__ stage, int lane, uint2 n0, uint2 n1, uint2 n2,
+                                       uint2 n3)
 {
     using Cfg = HsCfg<NG>;
     constexpr int OBJ_PLANE = Cfg::OBJ_PLANE, STG_PLANE = Cfg::STG_PLANE;
-    const uint2* __restrict__ rp = d.p2rec + (size_t)chunk0 * 128 + lane;
-    uint2 n0 = __ldg(rp), n1 = __ldg(rp + 32), n2 = __ldg(rp + 64), n3 = __ldg(rp + 96);
+    const uint2* __restrict__ rp = d.p2rec + (size_t)chunk0 * 128 + lane;          // n0 .. n3 = the records of chunk0
     wf<double> acc;
 #pragma unroll
     for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
@@ -445,6 +445,25 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
             K[0] = k0; K[1] = k1; K[2] = k2; K[3] = k3;
         }
         __syncthreads();
+        // HsCfg::PRE (measured per process: -6 % for g g -> t tbar g g, +3 % for g g -> t tbar g g g, where it is off): the
+        // first records a warp needs in a step are loaded BEFORE the barrier that ends the previous step (the tables do
+        // not depend on the event): pa = the first entry record of its first colour flow, pb.x/.y = that flow's first class
+        // table; a warp without flows gets the four records of its first chunk instead (pa, pb).
+        uint4 pa = make_uint4(0u, 0u, 0u, 0u), pb = pa;
+        auto preload = [&](int s) {
+            if (!Cfg::PRE || s >= NSTEPS) return;
+            const uint2 sc = tb.wsched[s * NW + warp];
+            if (sc.x >> 16) {
+                const int4 fd = tb.p3flow[tb.witem[sc.x & 0xFFFFu]];
+                pa = __ldg(d.p3rec + (size_t)fd.x * 8 + (lane >> 2));
+                const uint2 c = __ldg(d.p3cls + (size_t)fd.z * 32 + lane);
+                pb.x = c.x; pb.y = c.y;
+            } else if (sc.y >> 16) {
+                const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
+                const uint2 r0 = __ldg(rp), r1 = __ldg(rp + 32), r2 = __ldg(rp + 64), r3 = __ldg(rp + 96);
+                pa = make_uint4(r0.x, r0.y, r1.x, r1.y); pb = make_uint4(r2.x, r2.y, r3.x, r3.y);
+            }
+        };
         // phase 1: objects, level by level
         for (int lvl = 0; lvl < 3; lvl++) {
             for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += NTH) {
@@ -455,6 +474,7 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
                 p1_terms<OBJ_PLANE>(d, obj, Ks, pm, o.z, o.w, var, o.y >> 8, a.mt, a.wt, acc);
                 st_wf<OBJ_PLANE>(obj, 16u * (unsigned)(o.x + perm(var)), acc);
             }
+            if (lvl == 2) preload(0);
             __syncthreads();
         }
         for (int s = 0; s < NSTEPS; s++) {
@@ -464,9 +484,33 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
             const char* __restrict__ stgl3 = stage0 + b3 * 4 * STG_PLANE + (lane & 3) * STG_PLANE;
             const uint2 sc = tb.wsched[s * NW + warp];
             const unsigned* __restrict__ ip = tb.witem + (sc.x & 0xFFFFu);
-            const int nfl = sc.x >> 16;
-            for (int k = 0; k < nfl; k++) p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr);
-            if (sc.y >> 16) p2_run<NG>(d, sc.y & 0xFFFFu, sc.y >> 16, obj, Ks, stage2, lane);
+            const int nfl = sc.x >> 16, nch = sc.y >> 16;
+            uint2 c0 = make_uint2(pa.x, pa.y), c1 = make_uint2(pa.z, pa.w), c2 = make_uint2(pb.x, pb.y), c3 = make_uint2(pb.z, pb.w);
+            if (Cfg::PRE && nfl > 0 && nch > 0) {
+                // the chunk run's first records travel through the colour flow(s) in registers
+                const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
+                c0 = __ldg(rp); c1 = __ldg(rp + 32); c2 = __ldg(rp + 64); c3 = __ldg(rp + 96);
+            }
+#ifndef HS_SKIP_P3
+            for (int k = 0; k < nfl; k++) {
+                uint4 nxt = pa;
+                uint2 cl = make_uint2(pb.x, pb.y);
+                if (!Cfg::PRE || k > 0) {
+                    const int4 fd = tb.p3flow[ip[k]];
+                    nxt = __ldg(d.p3rec + (size_t)fd.x * 8 + (lane >> 2));
+                    cl = __ldg(d.p3cls + (size_t)fd.z * 32 + lane);
+                }
+                p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr, nxt, cl);
+            }
+#endif
+            if (!Cfg::PRE && nch > 0) {
+                const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
+                c0 = __ldg(rp); c1 = __ldg(rp + 32); c2 = __ldg(rp + 64); c3 = __ldg(rp + 96);
+            }
+#ifndef HS_SKIP_P2
+            if (nch) p2_run<NG>(d, sc.y & 0xFFFFu, nch, obj, Ks, stage2, lane, c0, c1, c2, c3);
+#endif
+            preload(s + 1);
             __syncthreads();
         }
     }
