@@ -266,23 +266,6 @@ __device__ __forceinline__ void p3_entry(const char* __restrict__ abase, const c
     }
 }
 
-// the n entries of shape CODE (= swapped | mask << 1; < 0: shape not used by this process) of the current class;
-// objl / stgl = plane (lane % 4) of the object area / of the group's staging area
-template <int CODE, int NTILE>
-__device__ __forceinline__ void p3_run(int n, const uint4* __restrict__& rp, uint4& nxt, const char* __restrict__ objl,
-                                       const char* __restrict__ stgl, double (&f)[4 * NTILE])
-{
-    if constexpr (CODE >= 0) {
-        for (int i = 0; i < n; i++) {
-            const uint4 en = nxt;
-            rp += 8;
-            nxt = __ldg(rp);
-            if constexpr (CODE & 1) p3_entry<1, (CODE >> 1), NTILE>(objl, stgl, en, f);
-            else p3_entry<0, (CODE >> 1), NTILE>(stgl, objl, en, f);
-        }
-    }
-}
-
 // add the fragments of a finished class to the flow's accumulator (first class: plain store)
 template <int NTILE>
 __device__ __forceinline__ void p3_flush(char* __restrict__ acc, const uint2 cl, const double (&f)[4 * NTILE], bool first)
@@ -311,38 +294,92 @@ __device__ __forceinline__ int acc_swizzle(int h)
     return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7));
 }
 
-// one colour flow (phase 3): class by class, one run of entries per shape, then the finished jamp of all helicity
-// combinations is written out
-template <int NG, typename T2>
-__device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, const HsLaunch& a, int fl, int e, const char* __restrict__ objl,
-                                        const char* __restrict__ stgl, char* __restrict__ accs, int warp, int lane,
-                                        const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32], uint4 nxt, uint2 cl)
+// ------------------------------------------------------------------------------------------------------------
+// one colour flow (phase 3) as STRAIGHT-LINE code.  The classes of a flow come in a canonical order and the sequence of
+// their headers H0 .. H4 (count of entries per shape; the flow's SIGNATURE, gen/hs_streams.py) is a template parameter,
+// so every entry's shape, every record's address and every class boundary is a compile-time constant: no loop, no
+// dispatch inside a flow; the records of a class are loaded while the previous class is evaluated.  HsCfg::P3_PAD: all
+// flows of the process are padded to ONE signature -- a slot a flow does not use carries the skip bit (record word w,
+// bit 8), a class it does not use has header 0 in p3clsh -- because the SM's instruction cache is smaller than this
+// kernel (2 -> 5: three instantiations measured 13 % slower than one although they execute 17 % fewer instructions).
+template <int NG> __host__ __device__ constexpr int shape_code(int k)
+{
+    return k == 0 ? HsCfg<NG>::SHAPE0 : k == 1 ? HsCfg<NG>::SHAPE1 : k == 2 ? HsCfg<NG>::SHAPE2 : HsCfg<NG>::SHAPE3;
+}
+__host__ __device__ constexpr int hdr_entries(int h) { return (h & 15) + ((h >> 4) & 15) + ((h >> 8) & 15) + ((h >> 12) & 15); }
+__host__ __device__ constexpr int max_c(int a, int b) { return a > b ? a : b; }
+
+template <int N> struct P3Recs { uint4 r[N]; };
+
+template <int NE, int NMAX> __device__ __forceinline__ void p3_load_class(P3Recs<NMAX>& q, const uint4* __restrict__ rp, int e0)
+{
+#pragma unroll
+    for (int i = 0; i < NE; i++) q.r[i] = __ldg(rp + 8 * (e0 + i));
+}
+
+template <int NG, int H, int K, int I0, int NMAX>
+__device__ __forceinline__ void p3_static_run(const P3Recs<NMAX>& q, const char* __restrict__ objl, const char* __restrict__ stgl,
+                                              double (&f)[4 * HsCfg<NG>::NTILE])
+{
+    constexpr int CODE = shape_code<NG>(K), N = (H >> (4 * K)) & 15, NTILE = HsCfg<NG>::NTILE;
+    if constexpr (CODE >= 0 && N > 0) {
+#pragma unroll
+        for (int i = 0; i < N; i++) {
+            if (((HsCfg<NG>::P3_ALWAYS >> K) & 1) || !(q.r[I0 + i].w & 0x100u)) {        // (uniform over the warp)
+                if constexpr (CODE & 1) p3_entry<1, (CODE >> 1), NTILE>(objl, stgl, q.r[I0 + i], f);
+                else p3_entry<0, (CODE >> 1), NTILE>(stgl, objl, q.r[I0 + i], f);
+            }
+        }
+    }
+}
+
+// class C of the flow (header H, first entry E0); HN = header of the next class (its records are put in flight first)
+template <int NG, int H, int HN, int E0, int C, int NMAX>
+__device__ __forceinline__ void p3_static_class(const P3Recs<NMAX>& q, P3Recs<NMAX>& qn, const uint4* __restrict__ rp,
+                                                const uint2* __restrict__ cp, const int* __restrict__ hp,
+                                                const char* __restrict__ objl, const char* __restrict__ stgl, char* __restrict__ acc)
+{
+    constexpr int NTILE = HsCfg<NG>::NTILE;
+    if constexpr (H != 0) {
+        if constexpr (HN != 0) p3_load_class<hdr_entries(HN), NMAX>(qn, rp, E0 + hdr_entries(H));
+        if (HsCfg<NG>::P3_PAD && C > 0 && hp[C] == 0) return;      // a padded flow does not have this class
+        const uint2 cl = __ldg(cp + 32 * C);
+        double f[4 * NTILE];
+#pragma unroll
+        for (int i = 0; i < 4 * NTILE; i++) f[i] = 0.0;
+        constexpr int n0 = H & 15, n1 = (H >> 4) & 15, n2 = (H >> 8) & 15;
+        p3_static_run<NG, H, 0, 0, NMAX>(q, objl, stgl, f);
+        p3_static_run<NG, H, 1, n0, NMAX>(q, objl, stgl, f);
+        p3_static_run<NG, H, 2, n0 + n1, NMAX>(q, objl, stgl, f);
+        p3_static_run<NG, H, 3, n0 + n1 + n2, NMAX>(q, objl, stgl, f);
+        p3_flush<NTILE>(acc, cl, f, C == 0);
+    }
+}
+
+template <int NG, typename T2, int H0, int H1, int H2, int H3, int H4>
+__device__ __forceinline__ void p3_flow_sig(const HsDev& d, const HsSmemTabs& tb, const HsLaunch& a, const int4 fd, int e,
+                                            const char* __restrict__ objl, const char* __restrict__ stgl, char* __restrict__ accs,
+                                            int warp, int lane, const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32])
 {
     using Cfg = HsCfg<NG>;
-    constexpr int NH = 1 << Cfg::NPAR, NTILE = Cfg::NTILE;
-    const int4 fd = tb.p3flow[fl];
-    const int ncls = fd.y & 0xFF, jamp = fd.w;
+    constexpr int NH = 1 << Cfg::NPAR;
+    constexpr int NMAX = max_c(max_c(max_c(hdr_entries(H0), hdr_entries(H1)), max_c(hdr_entries(H2), hdr_entries(H3))), hdr_entries(H4));
+    constexpr int E1 = hdr_entries(H0), E2 = E1 + hdr_entries(H1), E3 = E2 + hdr_entries(H2), E4 = E3 + hdr_entries(H3);
+    const int jamp = fd.w;
     // one accumulator per flow of the group, or per warp when a group has more flows than the CTA has warps
-    char* __restrict__ acc = accs + (size_t)(Cfg::MAX_FLOWS > Cfg::NW ? warp : (fd.y >> 16)) * (NH * 16);
+    char* __restrict__ acc = accs + (size_t)(Cfg::MAX_FLOWS > Cfg::NW ? warp : ((fd.y >> 16) & 0xFF)) * (NH * 16);
     const uint4* __restrict__ rp = d.p3rec + (size_t)fd.x * 8 + (lane >> 2);
     const uint2* __restrict__ cp = d.p3cls + (size_t)fd.z * 32 + lane;
     const int* __restrict__ hp = tb.p3clsh + fd.z;
-    // nxt = the first entry's record, cl = the first class table (loaded by the caller, ahead of time where it can):
-    // the record of the next entry is always in flight
-    for (int c = 0; c < ncls; c++) {
-        const int h_ = hp[c];
-        const uint2 cl_ = cl;
-        cl = __ldg(cp + 32 * (c + 1));      // (one past the end: inside the blob)
-        double f[4 * NTILE];
-#pragma unroll
-        for (int q = 0; q < 4 * NTILE; q++) f[q] = 0.0;
-        p3_run<Cfg::SHAPE0, NTILE>(h_ & 15, rp, nxt, objl, stgl, f);
-        p3_run<Cfg::SHAPE1, NTILE>((h_ >> 4) & 15, rp, nxt, objl, stgl, f);
-        p3_run<Cfg::SHAPE2, NTILE>((h_ >> 8) & 15, rp, nxt, objl, stgl, f);
-        p3_run<Cfg::SHAPE3, NTILE>((h_ >> 12) & 15, rp, nxt, objl, stgl, f);
-        p3_flush<NTILE>(acc, cl_, f, c == 0);
-    }
+    P3Recs<NMAX> qa, qb;                      // record sets of the current / the next class, alternating
+    p3_load_class<hdr_entries(H0), NMAX>(qa, rp, 0);
+    p3_static_class<NG, H0, H1, 0, 0, NMAX>(qa, qb, rp, cp, hp, objl, stgl, acc);
+    p3_static_class<NG, H1, H2, E1, 1, NMAX>(qb, qa, rp, cp, hp, objl, stgl, acc);
+    p3_static_class<NG, H2, H3, E2, 2, NMAX>(qa, qb, rp, cp, hp, objl, stgl, acc);
+    p3_static_class<NG, H3, H4, E3, 3, NMAX>(qb, qa, rp, cp, hp, objl, stgl, acc);
+    p3_static_class<NG, H4, 0, E4, 4, NMAX>(qa, qb, rp, cp, hp, objl, stgl, acc);
     __syncwarp();
+    // the finished jamp of this colour flow, all helicity combinations
     T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
 #pragma unroll
     for (int j = 0; j < NH / 32; j++) {
@@ -360,6 +397,23 @@ __device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, co
         }
     }
     __syncwarp();
+}
+
+template <int NG, typename T2>
+__device__ __forceinline__ void p3_flow(const HsDev& d, const HsSmemTabs& tb, const HsLaunch& a, int fl, int e,
+                                        const char* __restrict__ objl, const char* __restrict__ stgl, char* __restrict__ accs,
+                                        int warp, int lane, const int (&posr)[(1 << HsCfg<NG>::NPAR) / 32])
+{
+    const int4 fd = tb.p3flow[fl];
+#define HS_SIG_CASE(ID, H0, H1, H2, H3, H4) \
+    case ID: p3_flow_sig<NG, T2, H0, H1, H2, H3, H4>(d, tb, a, fd, e, objl, stgl, accs, warp, lane, posr); break;
+    if constexpr (NG == 4) {
+        switch ((fd.y >> 24) & 0x7F) { HS_FLOW_SIGS_4(HS_SIG_CASE) default: break; }
+    } else {
+        static_assert(NG == 5, "add the process's HS_FLOW_SIGS list here");
+        switch ((fd.y >> 24) & 0x7F) { HS_FLOW_SIGS_5(HS_SIG_CASE) default: break; }
+    }
+#undef HS_SIG_CASE
 }
 
 // the phase-2 work of a warp in a step: a contiguous run of chunks; a unit (the chunks of the same 32 (pair object,
@@ -447,18 +501,12 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
         __syncthreads();
         // HsCfg::PRE (measured per process: -6 % for g g -> t tbar g g, +3 % for g g -> t tbar g g g, where it is off): the
         // first records a warp needs in a step are loaded BEFORE the barrier that ends the previous step (the tables do
-        // not depend on the event): pa = the first entry record of its first colour flow, pb.x/.y = that flow's first class
-        // table; a warp without flows gets the four records of its first chunk instead (pa, pb).
+        // not depend on the event): pa, pb = the four records of the first chunk of a warp that has no colour flow in that step.
         uint4 pa = make_uint4(0u, 0u, 0u, 0u), pb = pa;
         auto preload = [&](int s) {
             if (!Cfg::PRE || s >= NSTEPS) return;
             const uint2 sc = tb.wsched[s * NW + warp];
-            if (sc.x >> 16) {
-                const int4 fd = tb.p3flow[tb.witem[sc.x & 0xFFFFu]];
-                pa = __ldg(d.p3rec + (size_t)fd.x * 8 + (lane >> 2));
-                const uint2 c = __ldg(d.p3cls + (size_t)fd.z * 32 + lane);
-                pb.x = c.x; pb.y = c.y;
-            } else if (sc.y >> 16) {
+            if (!(sc.x >> 16) && (sc.y >> 16)) {
                 const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
                 const uint2 r0 = __ldg(rp), r1 = __ldg(rp + 32), r2 = __ldg(rp + 64), r3 = __ldg(rp + 96);
                 pa = make_uint4(r0.x, r0.y, r1.x, r1.y); pb = make_uint4(r2.x, r2.y, r3.x, r3.y);
@@ -492,16 +540,7 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
                 c0 = __ldg(rp); c1 = __ldg(rp + 32); c2 = __ldg(rp + 64); c3 = __ldg(rp + 96);
             }
 #ifndef HS_SKIP_P3
-            for (int k = 0; k < nfl; k++) {
-                uint4 nxt = pa;
-                uint2 cl = make_uint2(pb.x, pb.y);
-                if (!Cfg::PRE || k > 0) {
-                    const int4 fd = tb.p3flow[ip[k]];
-                    nxt = __ldg(d.p3rec + (size_t)fd.x * 8 + (lane >> 2));
-                    cl = __ldg(d.p3cls + (size_t)fd.z * 32 + lane);
-                }
-                p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr, nxt, cl);
-            }
+            for (int k = 0; k < nfl; k++) p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr);
 #endif
             if (!Cfg::PRE && nch > 0) {
                 const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;

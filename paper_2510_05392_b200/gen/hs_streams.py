@@ -42,7 +42,9 @@ dot-product entries jamp[sigma][h] += sign * sum_c X_c[hx] * Y_c[hy] (phase 3). 
       adds (lane % 4) * PLANE) and a flag word; per (class, lane) the accumulator offsets of the lane's tiles.  Inside a
       class the entries are sorted by SHAPE (which operand gives the rows, which tile bits select the A fragment) and
       the class header holds the number of entries of each shape, so that the kernel runs one tight loop per shape
-      with no per-entry dispatch.
+      with no per-entry dispatch.  The classes of a flow come in a canonical order; the sequence of their headers is the
+      flow's SIGNATURE (p3flow[f].y bits 24..30) and the kernel instantiates straight-line code per signature
+      (HS_FLOW_SIGS_<n> in generated/hs_gen.h); with pad = 1 all flows are padded to ONE signature (skip bits).
 
 Everything here is integer bookkeeping of an exact rewriting; tests/hs_eval.py interprets these very streams in numpy and
 tests/test_generator.py compares the resulting jamps with the oracle (CPU, no kernel involved).
@@ -103,9 +105,9 @@ def _subvar(v, parent, child):
 
 
 class Streams:
-    def __init__(self, prog: co_program.Program, nw=8, nbuf=1):
+    def __init__(self, prog: co_program.Program, nw=8, nbuf=1, pad=0):
         self.prog = prog
-        self.nw, self.nbuf = nw, nbuf
+        self.nw, self.nbuf, self.pad = nw, nbuf, pad
         self.npar = prog.npar
         self.ncolor = prog.ncolor
         self.ntile = 1 << (self.npar - 5)
@@ -333,29 +335,60 @@ class Streams:
         assert len(codes) <= 4, "the class header holds four shape counts"
         self.p3shape_codes = codes
         recs, cls_tab, cls_hdr, flows, grp = [], [], [], [], []
+        counts_of = lambda recs_c: tuple(sum(1 for sh, _ in recs_c if sh == c) for c in codes)
+        # A flow's classes come in a canonical order (by their shape counts); the sequence of their headers is the flow's
+        # SIGNATURE, and the kernel runs every signature as its own straight-line code.  pad = 1: ONE signature for the
+        # whole process -- max_cls classes, each with hmax[k] slots for the entries of shape k; missing entries / classes
+        # are slots with the SKIP bit (record word w bit 8) / header 0 -- because the instruction cache of the SM is smaller
+        # than the kernel (2 -> 5: three signatures measured 13 % slower than one although they execute fewer instructions).
+        max_cls = max(len(f[3]) for f in flows_raw)
+        hmax = [max(counts_of(co[3])[k] for f in flows_raw for co in f[3]) for k in range(len(codes))]
+        assert all(c < 16 for c in hmax) and max_cls <= 5
+        pack = lambda counts: sum(c << (4 * k) for k, c in enumerate(counts))
+        self.flow_sigs = {}       # sequence of class headers -> signature id
+        # shapes present in EVERY slot need no skip test
+        self.p3_always = sum(1 << k for k in range(len(codes))
+                             if not self.pad or (all(counts_of(co[3])[k] == hmax[k] for f in flows_raw for co in f[3]) and
+                                                 all(len(f[3]) == max_cls for f in flows_raw)))
+        skip_rec = np.zeros((8, 4), dtype=np.uint32)
+        skip_rec[:, 3] = 0x100
+        self.flow_real_entries = []
         for gi in range(len(prog.groups)):
             mine = [f for f in flows_raw if f[0] == gi]
             grp.append(self._grp_units[gi] + (len(flows), len(mine)))
             for _, fi, j, cls_out in mine:
-                rec0, cls0, nent = len(recs), len(cls_tab), 0
-                for R, C, T, recs_c in cls_out:
-                    # accumulator slot of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
+                rec0, cls0 = len(recs), len(cls_tab)
+                cls_out = sorted(cls_out, key=lambda co: tuple(-x for x in counts_of(co[3])))
+                nreal, sig = 0, []
+                for ci in range(max_cls if self.pad else len(cls_out)):
                     ct = np.zeros((32, 4), dtype=np.uint32)
-                    for lane in range(32):
-                        row, c2 = lane >> 2, lane & 3
-                        for t in range(ntile):
-                            h = sum(((row >> b) & 1) << hbit(R[b]) for b in range(3))
-                            h |= sum(((c2 >> b) & 1) << hbit(C[b]) for b in range(2))
-                            h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
-                            ct[lane, t] = 16 * acc_swizzle(h)
+                    if ci < len(cls_out):
+                        R, C, T, recs_c = cls_out[ci]
+                        # accumulator slot of (lane, tile): rows <-> R, complex columns <-> C, tiles <-> T
+                        for lane in range(32):
+                            row, c2 = lane >> 2, lane & 3
+                            for t in range(ntile):
+                                h = sum(((row >> b) & 1) << hbit(R[b]) for b in range(3))
+                                h |= sum(((c2 >> b) & 1) << hbit(C[b]) for b in range(2))
+                                h |= sum(((t >> b) & 1) << hbit(T[b]) for b in range(len(T)))
+                                ct[lane, t] = 16 * acc_swizzle(h)
+                        counts = counts_of(recs_c)
+                        cls_hdr.append(pack(counts))
+                        for k, code in enumerate(codes):
+                            mine_k = [r for sh, r in recs_c if sh == code]
+                            recs += mine_k + ([skip_rec] * (hmax[k] - len(mine_k)) if self.pad else [])
+                        nreal += len(recs_c)
+                        sig.append(pack(hmax) if self.pad else pack(counts))
+                    else:
+                        cls_hdr.append(0)
+                        recs += [skip_rec] * sum(hmax)
+                        sig.append(pack(hmax))
                     cls_tab.append(ct)
-                    recs_c = sorted(recs_c, key=lambda sr: codes.index(sr[0]))        # stable: by shape
-                    counts = [sum(1 for sh, _ in recs_c if sh == c) for c in codes]
-                    assert all(c < 16 for c in counts)
-                    cls_hdr.append(sum(c << (4 * k) for k, c in enumerate(counts)))
-                    recs += [r for _, r in recs_c]
-                    nent += len(recs_c)
-                flows.append((rec0, len(cls_out) | (nent << 8) | (fi << 16), cls0, j))
+                sid = self.flow_sigs.setdefault(tuple(sig), len(self.flow_sigs))
+                assert fi < 256 and sid < 128
+                flows.append((rec0, len(sig) | ((len(recs) - rec0) << 8) | (fi << 16) | (sid << 24), cls0, j))
+                self.flow_real_entries.append((len(cls_out), nreal))
+        assert not self.pad or len(self.flow_sigs) == 1
         self.p3rec = np.asarray(recs, dtype=np.uint32).reshape(-1, 8, 4)
         self.p3cls = np.asarray(cls_tab, dtype=np.uint32).reshape(-1, 32, 4)
         self.p3clsh = np.asarray(cls_hdr, dtype=np.int32)
@@ -380,8 +413,8 @@ class Streams:
             if g3 is not None:
                 _, _, f0, nf = (int(x) for x in self.grp[g3])
                 for f in range(f0, f0 + nf):
-                    info = int(self.p3flow[f][1])
-                    cost = ITEM_COST["flow"] + ITEM_COST["class"] * (info & 0xFF) + ITEM_COST["entry"] * ((info >> 8) & 0xFF)
+                    ncls_real, nent_real = self.flow_real_entries[f]
+                    cost = ITEM_COST["flow"] + ITEM_COST["class"] * ncls_real + ITEM_COST["entry"] * nent_real
                     items.append((cost, f))
             if g2 is not None:
                 u0, nu, _, _ = (int(x) for x in self.grp[g2])
@@ -451,15 +484,15 @@ class Streams:
             "p2rec": self.p2rec, "p2unit": self.p2unit, "grp": self.grp, "chunk_types": self.chunk_types,
             "nw": self.nw, "nbuf": self.nbuf, "nsteps": len(self.steps()), "wsched": self.wsched, "witem": self.witem,
             "p3rec": self.p3rec, "p3cls": self.p3cls, "p3clsh": self.p3clsh, "p3flow": self.p3flow,
-            "p3shapes": self.p3shapes, "p3shape_codes": self.p3shape_codes,
+            "p3shapes": self.p3shapes, "p3shape_codes": self.p3shape_codes, "flow_sigs": dict(self.flow_sigs), "p3_pad": self.pad, "p3_always": self.p3_always,
         }
 
 
 _CACHE = {}
 
 
-def build(n, group_prefix, nw=8, nbuf=1):
-    key = (n, group_prefix, nw, nbuf)
+def build(n, group_prefix, nw=8, nbuf=1, pad=0):
+    key = (n, group_prefix, nw, nbuf, pad)
     if key not in _CACHE:
-        _CACHE[key] = Streams(co_program.build(n, group_prefix), nw, nbuf)
+        _CACHE[key] = Streams(co_program.build(n, group_prefix), nw, nbuf, pad)
     return _CACHE[key]

@@ -147,16 +147,24 @@ def evaluate(T, mom, mt, wt):
                 accum = np.zeros(nh, dtype=complex)            # the flow's accumulator in shared memory, [slot]
                 written = np.zeros(nh, dtype=bool)
                 codes = T["p3shape_codes"]
+                sig = [hs for hs, i in T["flow_sigs"].items() if i == (info >> 24) & 0x7F][0]      # slots per class
+                assert ncls == len(sig)
                 e = rec0
                 for cls in range(cls0, cls0 + ncls):
                     hdr = int(T["p3clsh"][cls])
+                    hslots = sig[cls - cls0]
                     frag = np.zeros((32, ntile), dtype=complex)    # register fragments of the class
-                    for k, code in enumerate(codes):               # one run of entries per shape, in the kernel's order
-                        for _ in range((hdr >> (4 * k)) & 15):
+                    nreal = 0
+                    for k, code in enumerate(codes):               # the slots of shape k, in the kernel's order
+                        for _ in range((hslots >> (4 * k)) & 15):
                             rec = T["p3rec"][e]
                             e += 1
                             flags = int(rec[0, 3])
-                            assert all(int(rec[r, 3]) == flags for r in range(8)) and (flags & 0xF) == code
+                            assert all(int(rec[r, 3]) == flags for r in range(8))
+                            if flags & 0x100:                      # slot not used by this flow
+                                continue
+                            assert (flags & 0xF) == code and hdr != 0
+                            nreal += 1
                             neg = (flags >> 31) & 1
                             swapped, mask = code & 1, code >> 1
                             na = 1 << bin(mask).count("1")
@@ -180,6 +188,9 @@ def evaluate(T, mom, mt, wt):
                                     assert bh[bi] % 16 == 0 and bh1[bi] == bh[bi] + 8
                                     val = np.sum(aplanes.load(ah[ai]) * bplanes.load(bh[bi]))
                                     frag[lane, t] += -val if neg else val
+                    assert nreal == sum((hdr >> (4 * k)) & 15 for k in range(4))
+                    if hdr == 0:                                   # class not used by this flow: the kernel skips its flush
+                        continue
                     for lane in range(32):
                         for t in range(ntile):
                             off = int(T["p3cls"][cls][lane, t])

@@ -85,7 +85,7 @@ def test_helicity_shared_streams_match_oracle(name, n, nev, params):
     import hs_eval
     from paper_2510_05392_b200.gen import emit_hs, hs_streams
     k = emit_hs.KERNEL_CFG[n]
-    st = hs_streams.build(n, emit_hs.GROUP_PREFIX[n], k["nw"], k["nbuf"])          # what the library is built with
+    st = emit_hs.streams(n)                                                        # what the library is built with
     T = st.tables()
     # the static schedule deals every colour flow and every chunk of every step to exactly one warp, units unbroken
     for s_, (g3, g2) in enumerate(st.steps()):
