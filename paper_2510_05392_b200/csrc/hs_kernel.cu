@@ -539,16 +539,12 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
                 const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
                 c0 = __ldg(rp); c1 = __ldg(rp + 32); c2 = __ldg(rp + 64); c3 = __ldg(rp + 96);
             }
-#ifndef HS_SKIP_P3
             for (int k = 0; k < nfl; k++) p3_flow<NG, T2>(d, tb, a, ip[k], e, objl, stgl3, accs, warp, lane, posr);
-#endif
             if (!Cfg::PRE && nch > 0) {
                 const uint2* __restrict__ rp = d.p2rec + (size_t)(sc.y & 0xFFFFu) * 128 + lane;
                 c0 = __ldg(rp); c1 = __ldg(rp + 32); c2 = __ldg(rp + 64); c3 = __ldg(rp + 96);
             }
-#ifndef HS_SKIP_P2
             if (nch) p2_run<NG>(d, sc.y & 0xFFFFu, nch, obj, Ks, stage2, lane, c0, c1, c2, c3);
-#endif
             preload(s + 1);
             __syncthreads();
         }
