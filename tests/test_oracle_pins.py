@@ -547,3 +547,53 @@ def test_selection_colour_bose_and_alphas(params):
     me2, sh2, sc2 = selection.select("gg_ttx", p, params, rh, rc, alphas=al)
     assert np.abs(me2 / (me * (al / params["aS"]) ** 2) - 1).max() < 1e-12
     assert (sh2 == sh).all() and (sc2 == sc).all()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P8: collinear limit.  When two final-state gluons i, j become collinear (p_i = z p, p_j = (1 - z) p),
+#   sum_{hel, col} |M_{n+1}|^2  ->  (2 g^2 / s_ij) Phat_gg(z) sum |M_n|^2   after the average over the azimuth of the pair,
+#   Phat_gg(z) = 2 C_A [ z/(1-z) + (1-z)/z + z(1-z) ],  C_A = 3   (textbook, e.g. Ellis-Stirling-Webber ch. 5).
+# This ties the (n+1)-gluon amplitudes, colour matrix and coupling power to the n-gluon ones: a wrong normalisation of
+# A(sigma) or of C_{sigma sigma'} at ONE multiplicity (which the per-multiplicity pins P3-P6 cannot see, being ratios or
+# invariances) breaks it.  me = sum / denom, so the test uses me * denom; the identical-gluon factor (n-2)! inside denom is
+# a convention (reading A3: it belongs to the phase-space symmetry factor and MG5aMC puts it into the ME) -- the limit does
+# not fix it, the last assertion only records the convention's ratio.
+def _split_collinear(p, z, kt, phi):
+    """massless p -> two massless momenta z p + kT - ..., (1 - z) p - kT - ... (Sudakov decomposition, exact on-shell;
+    their sum differs from p by O(kT^2 / E))"""
+    E = p[0]
+    d = p[1:] / np.linalg.norm(p[1:])
+    a = np.cross(d, [0.0, 0.0, 1.0] if abs(d[2]) < 0.9 else [1.0, 0.0, 0.0])
+    a /= np.linalg.norm(a)
+    b = np.cross(d, a)
+    kT = kt * (math.cos(phi) * a + math.sin(phi) * b)
+    nbar = np.array([1.0, *(-d)])                       # light-like, opposite direction
+    K = np.array([0.0, *kT])
+    pi = z * p + K + (kt * kt / (2 * z * mdot(p, nbar).real)) * nbar
+    pj = (1 - z) * p - K + (kt * kt / (2 * (1 - z) * mdot(p, nbar).real)) * nbar
+    return pi, pj
+
+
+@pytest.mark.parametrize("proc_n,proc_n1,ng", [("gg_ttxg", "gg_ttxgg", 3), ("gg_ttxgg", "gg_ttxggg", 4)])
+def test_p8_collinear_limit_links_multiplicities(proc_n, proc_n1, ng, params):
+    P = dict(params, wT=0.0)
+    g2 = 4 * math.pi * P["aS"]
+    p = inputs.momenta(proc_n, 3, seed=17)
+    nphi = 8
+    for e in range(3):
+        me_n = oracle.matrix_elements(proc_n, p[e:e + 1], P)[0]
+        last = p.shape[1] - 1                               # split the last final-state gluon
+        for z in (0.3, 0.6):
+            kt = 1e-4 * p[e, last, 0]
+            vals = []
+            for k in range(nphi):
+                pi, pj = _split_collinear(p[e, last], z, kt, 2 * math.pi * (k + 0.5) / nphi)
+                q = np.concatenate([p[e, :last], pi[None], pj[None]])[None]
+                vals.append(oracle.matrix_elements(proc_n1, q, P)[0])
+            sij = 2 * mdot(pi, pj).real
+            phat = 2 * 3.0 * (z / (1 - z) + (1 - z) / z + z * (1 - z))
+            ratio = np.mean(vals) * oracle.DENOM[proc_n1] / (me_n * oracle.DENOM[proc_n])
+            want = 2 * g2 / sij * phat
+            assert abs(ratio / want - 1) < 2e-3, (proc_n1, e, z, ratio / want)
+    # convention of reading A3: denom_{n+1} / denom_n = (n - 1)! / (n - 2)!
+    assert oracle.DENOM[proc_n1] / oracle.DENOM[proc_n] == ng - 1
