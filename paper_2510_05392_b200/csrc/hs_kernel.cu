@@ -33,7 +33,7 @@ struct HsDev {
     const uint2* p2rec; const uint2* wsched; const unsigned* witem;
     const uint4* p3rec; const uint2* p3cls; const int* p3clsh; const int4* p3flow;
     int ncolor, nflow, ncls, nsched, nitem;
-    int p1_level[4];
+    int2 p1sched[3][16];       // [level - 1][warp] = { first item, blocks of 32 items }
 };
 
 // the small tables every work item starts from, copied to shared memory once per (persistent) CTA
@@ -514,8 +514,10 @@ __global__ void __launch_bounds__(32 * HsCfg<NG>::NW, HsCfg<NG>::CTAS) hs_diagra
         };
         // phase 1: objects, level by level
         for (int lvl = 0; lvl < 3; lvl++) {
-            for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += NTH) {
-                const int it = __ldg(d.p1_items + i);
+            const int2 ps = d.p1sched[lvl][warp];
+            for (int b = 0; b < ps.y; b++) {
+                const int it = __ldg(d.p1_items + ps.x + 32 * b + lane);
+                if (it < 0) continue;
                 const int4 o = __ldg(d.obj + (it >> 8));
                 const int var = it & 0xFF;
                 wf<double> acc;
@@ -627,7 +629,9 @@ cudaError_t hs_create(int ngluon, HsContext** out)
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
     }
-    for (int i = 0; i < 4; i++) d.p1_level[i] = t->p1_level[i];
+    for (int l = 0; l < 3; l++)
+        for (int w = 0; w < 16; w++)
+            d.p1sched[l][w] = w < c_nw ? make_int2(t->p1sched[2 * (l * c_nw + w)], t->p1sched[2 * (l * c_nw + w) + 1]) : make_int2(0, 0);
     switch (ngluon) {
 #define HS_SET(N) case N: c->smem = smem_bytes<N>(t); c->threads = 32 * HsCfg<N>::NW; c->ctas = HsCfg<N>::CTAS; e = set_smem<N>(c->smem); break;
         HS_PROCESSES(HS_SET)

@@ -20,7 +20,9 @@
 //               ops: 0 ext_v, 1 ext_ql, 2 ext_qr, 3 v3, 4 v4, 5 ffv_l, 6 ffv_r, 7 ffv_p (currents with propagator, phase 1);
 //                    8 x_row, 9 x_col, 10 x_bil, 11 x_v3, 12 x_v4, 13 x_v4s (raw vertices, phase 2; 13 = both orderings of
 //                    the four-gluon vertex that share the middle argument: 2 (p.r) q - (q.r) p - (q.p) r)
-//   p1_items  = obj << 8 | variant, level by level; p1_level[l] .. p1_level[l+1] is level l+1
+//   p1_items  = obj << 8 | variant (-1: idle lane), level by level (p1_level[l] .. p1_level[l+1] is level l+1), in blocks of 32
+//               lanes with one sequence of opcodes; p1sched[(level - 1) * NW + warp] = { first item, blocks }: the blocks this
+//               warp evaluates (dealt at build time, longest first)
 //   legset_mask[s] = particles of leg set s (bit p); K_s = sum of all-incoming momenta
 //   p2rec[chunk][4][lane] (uint2):
 //               rec0 = { byte offset of the item's slot in staging plane 0 | sign bits << 16, type | first << 12 | last << 13 },
@@ -61,6 +63,7 @@ struct HsTables {
     const int* grp;
     const unsigned* wsched;
     const unsigned* witem;
+    const int* p1sched;
     double flops_p1, flops_p2, flops_p3;      // per event (phases 1, 2) and per (event, helicity) (phase 3)
 };
 

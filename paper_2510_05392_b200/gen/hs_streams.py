@@ -155,13 +155,35 @@ class Streams:
                     w[1 + k] = self.obj_slot[x] | (_subpos(o.legs, prog.objs[x].legs) << 16)
                 terms.append(w)
             obj_tab.append([self.obj_slot[i], len(o.legs) | (self._lsid(o.legs) << 8), t0, len(o.terms)])
-        p1_items, p1_level = [], [0]
+        # phase-1 items (object << 8 | variant) in blocks of 32 lanes with one sequence of opcodes each (-1 = idle lane); the
+        # blocks of a level are dealt to the nw warps at build time, longest processing time first (cost = flops of the
+        # terms), and stored warp by warp: p1sched[level * nw + warp] = (first item, blocks)
+        from .emit_hs import FLOPS
+        p1_items, p1_level, p1sched = [], [0], []
         for lvl in (1, 2, 3):
+            by_shape = defaultdict(list)
             for new, i in enumerate(order):
                 if len(prog.objs[i].legs) == lvl:
-                    p1_items += [(new << 8) | v for v in range(1 << lvl)]
+                    shape = tuple(t.op for t in prog.objs[i].terms)
+                    by_shape[shape] += [(new << 8) | v for v in range(1 << lvl)]
+            blocks = []
+            for shape, items in sorted(by_shape.items()):
+                cost = sum(FLOPS[o] + 8 for o in shape)
+                for k in range(0, len(items), 32):
+                    blk = items[k:k + 32]
+                    blocks.append((cost, blk + [-1] * (32 - len(blk))))
+            load = [0] * self.nw
+            per_warp = [[] for _ in range(self.nw)]
+            for cost, blk in sorted(blocks, key=lambda b: (-b[0], b[1])):
+                w = min(range(self.nw), key=lambda i: (load[i], i))
+                load[w] += cost
+                per_warp[w].append(blk)
+            for w in range(self.nw):
+                p1sched.append((len(p1_items), len(per_warp[w])))
+                for blk in per_warp[w]:
+                    p1_items += blk
             p1_level.append(len(p1_items))
-        assert max(len(o.legs) for o in prog.objs) <= 3
+        self.p1sched = p1sched
         self.obj_tab, self.p1_terms, self.p1_items, self.p1_level = obj_tab, terms, p1_items, p1_level
         self._index_of = index_of
 
@@ -480,7 +502,7 @@ class Streams:
             "nlegsets": len(self.legsets), "max_flows": self.max_flows, "max_classes": int(ncls.max()),
             "legset_mask": np.asarray([sum(1 << p for p in legs) for legs in self.legsets], np.int32),
             "obj": i32(self.obj_tab, 4), "term": i32(self.p1_terms, 4), "p1_items": np.asarray(self.p1_items, np.int32),
-            "p1_level": np.asarray(self.p1_level, np.int32),
+            "p1_level": np.asarray(self.p1_level, np.int32), "p1sched": np.asarray(self.p1sched, np.int32).reshape(-1, 2),
             "p2rec": self.p2rec, "p2unit": self.p2unit, "grp": self.grp, "chunk_types": self.chunk_types,
             "nw": self.nw, "nbuf": self.nbuf, "nsteps": len(self.steps()), "wsched": self.wsched, "witem": self.witem,
             "p3rec": self.p3rec, "p3cls": self.p3cls, "p3clsh": self.p3clsh, "p3flow": self.p3flow,

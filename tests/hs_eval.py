@@ -70,6 +70,8 @@ def evaluate(T, mom, mt, wt):
         return obj.load(16 * ((w & 0xFFFF) + _perm(_sub(var, (w >> 16) & 0x1FF))))
 
     for it in T["p1_items"]:
+        if int(it) < 0:                       # idle lane of a block
+            continue
         o, var = int(it) >> 8, int(it) & 0xFF
         slot0, info, t0, nt = (int(x) for x in T["obj"][o])
         kout = K[info >> 8]
