@@ -76,6 +76,9 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
 /* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
  * MG_DIAG_THREAD kernel, multiple of 32, <= 256),
  * "hs_color_alu" (MG_DIAG_SHARED in MG_MIXED: 1 = scalar-ALU fp32 colour-sum kernel instead of the tcgen05 one),
+ * "tf32_direct" (MG_DIAG_SHARED in MG_MIXED with the tcgen05 kernel, default 1: the diagram kernel writes the jamps as TF32
+ * values straight in the tensor-core operand layout and the contraction accumulates J Lhi + J Llo; 0: fp32 jamps, two-term
+ * split of J inside the contraction, three products),
  * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1),
  * "max_streams" (MG_SCHED_STREAMS: helicities share this many streams round robin, 0 = one each),
  * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the

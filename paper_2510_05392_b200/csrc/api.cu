@@ -30,7 +30,7 @@ struct mg_process {
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
     int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
-    int diagrams = MG_DIAG_THREAD, hs_color_alu = 0;
+    int diagrams = MG_DIAG_THREAD, hs_color_alu = 0, tf32_direct = 1;
     int max_streams = 0;       // MG_SCHED_STREAMS: helicity h runs on stream h % max_streams (0 = one stream per helicity)
     int graph = 0;             // replay the launch sequence of a batch as a CUDA graph
     // the captured batch: valid for exactly these arguments and this state of the handle (epoch)
@@ -285,6 +285,8 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         p->diagrams = value;
     } else if (!strcmp(key, "hs_color_alu")) {
         p->hs_color_alu = value != 0;
+    } else if (!strcmp(key, "tf32_direct")) {
+        p->tf32_direct = value != 0;
     } else if (!strcmp(key, "timing")) {
         p->timing = value != 0;
     } else if (!strcmp(key, "jamp_chunk_mib")) {
@@ -308,6 +310,7 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "block")) *value = p->block;
     else if (!strcmp(key, "diagrams")) *value = p->diagrams;
     else if (!strcmp(key, "hs_color_alu")) *value = p->hs_color_alu;
+    else if (!strcmp(key, "tf32_direct")) *value = p->tf32_direct;
     else if (!strcmp(key, "timing")) *value = p->timing;
     else if (!strcmp(key, "jamp_chunk_mib")) *value = (int)(p->jamp_chunk_bytes >> 20);
     else if (!strcmp(key, "max_streams")) *value = p->max_streams;
@@ -406,7 +409,8 @@ __global__ void helicity_sum_select_kernel(const double* __restrict__ meh, int n
 
 // colour selection: weight of colour flow c = sum over good helicities of |J_c|^2; the first c with rnd * sum < cum_c.
 // One warp per event; lanes stride over the event's rows.  LAYOUT 0: [2][nc][rows], row = el * nhel + ih (event-major);
-// 1: [2][nc][rows], row = ih * ne + el (helicity-major); 2: tile-major [row / 128][2][nc][128], row = el * nhel + ih
+// 1: [2][nc][rows], row = ih * ne + el (helicity-major); 2: tile-major [row / 128][2][nc][128], row = el * nhel + ih;
+// 3: the tcgen05 operand layout of csrc/color_sum_tf32.cu (per tile and part: chunks of 24 colours as K-major core matrices)
 template <typename T, int LAYOUT>
 __global__ void __launch_bounds__(128) select_color_kernel(const T* __restrict__ J, int nc, int nhel, int ne, long rows,
                                                             const double* __restrict__ rndcol, int e0, int* __restrict__ selcol)
@@ -420,7 +424,12 @@ __global__ void __launch_bounds__(128) select_color_kernel(const T* __restrict__
         double s = 0.0;
         for (int ih = lane; ih < nhel; ih += 32) {
             double re, im;
-            if (LAYOUT == 2) {
+            if (LAYOUT == 3) {
+                const long row = (long)el * nhel + ih;
+                const unsigned m = (unsigned)(row & 127);
+                const T* t = J + (row >> 7) * (256L * nc) + (long)(c / 24) * (24 * 128) + (m >> 3) * 192 + ((c % 24) >> 2) * 32 + (m & 7) * 4 + (c & 3);
+                re = (double)t[0]; im = (double)t[128L * nc];
+            } else if (LAYOUT == 2) {
                 const long row = (long)el * nhel + ih;
                 const T* t = J + (row >> 7) * (256L * nc) + (long)c * 128 + (row & 127);
                 re = (double)t[0]; im = (double)t[128L * nc];
@@ -457,6 +466,7 @@ static cudaError_t launch_select_color(int layout, const void* J, int nc, int nh
     const size_t sm = sizeof(double) * warps * nc;
     if (layout == 0) select_color_kernel<T, 0><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
     else if (layout == 1) select_color_kernel<T, 1><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
+    else if (layout == 3) select_color_kernel<T, 3><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
     else select_color_kernel<T, 2><<<grid, 32 * warps, sm, st>>>((const T*)J, nc, nhel, ne, rows, rnd, e0, sel);
     return cudaGetLastError();
 }
@@ -625,8 +635,10 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
             a.mom = d_momenta + (size_t)e0 * p->d->npar * 4; a.nevt = ne; a.d_pos = p->d_pos; a.nrow_evt = nhel;
             a.d_jamps = d_j; a.rows = color_sum_padded_rows(rows); a.mt = p->mT; a.wt = p->wT;
             // tcgen05 colour sum: one contiguous block per 128-row tile, so that a chunk of colours is ONE bulk copy
-            const bool tile_major = p->precision != MG_FP64 && !p->hs_color_alu;
-            a.tile_major = tile_major ? 1 : 0;
+            // (2: straight in the operand layout, TF32-rounded -- the contraction then needs neither converter warps nor the
+            //  low term of the jamps; needs chunks of 24 colours)
+            const int tile_major = p->precision != MG_FP64 && !p->hs_color_alu ? (p->d->ncolor % 24 == 0 && p->tf32_direct ? 2 : 1) : 0;
+            a.tile_major = tile_major;
             CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
@@ -639,7 +651,7 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
             else
                 ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st, tile_major);
             if (ce_ != cudaSuccess) return fail(p, MG_ECUDA, std::string("colour sum: ") + cudaGetErrorString(ce_));
-            CUDA_TRY(p, select_color(tile_major ? 2 : 0, d_j, ne, a.rows, e0));
+            CUDA_TRY(p, select_color(tile_major == 2 ? 3 : (tile_major ? 2 : 0), d_j, ne, a.rows, e0));
             MARK(1);
         }
     } else if (color_sum == MG_CS_FUSED) {

@@ -298,10 +298,10 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
-                           double* d_meh, cudaStream_t st, bool tile_major);
+                           double* d_meh, cudaStream_t st, int tile_major);
 
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
-                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, bool tile_major)
+                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, int tile_major)
 {
     if (!is_fp64) return color_sum_tf32(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st, tile_major);
     if (tile_major) return cudaErrorInvalidValue;

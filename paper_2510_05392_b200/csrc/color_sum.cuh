@@ -39,8 +39,9 @@ cudaError_t color_sum_alu(bool is_fp64, int ncolor, const void* d_cmat, const vo
 //   d_factor: DEVICE Cholesky factor of C: fp64 [ncp][ncp] padded (color_cholesky_padded), or the two-term TF32
 //             image of it (tf32_build_factor_image) for fp32
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
-                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, bool tile_major = false);
-// tile_major (fp32 only): d_jamps is [rows_padded / 128][2][ncolor][128] instead of [2][ncolor][rows_padded]
+                             long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, int tile_major = 0);
+// tile_major (fp32 only): 1: d_jamps is [rows_padded / 128][2][ncolor][128] instead of [2][ncolor][rows_padded];
+// 2: the tcgen05 operand layout, TF32-rounded by the producer (color_sum_tf32.cu "direct": no converter warps, two products)
 
 // host: L with C = L L^T (lower-triangular, row-major, zero-padded to ncp = 8*ceil(ncolor/8) columns)
 bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp, int* ncp_out);

@@ -98,12 +98,13 @@ struct Tf32Args {
 
 constexpr int TF32_THREADS = 512;
 constexpr int TF32_MAX_RAW = 8;
+constexpr int TF32_MAX_A = 12;
 
 __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const Tf32Args a)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ uint64_t raw_full[TF32_MAX_RAW], raw_empty[TF32_MAX_RAW];
-    __shared__ uint64_t a_full[4], a_empty[4], acc_full[2], acc_empty[2];
+    __shared__ uint64_t a_full[TF32_MAX_A], a_empty[TF32_MAX_A], acc_full[2], acc_empty[2];
     __shared__ uint32_t tmem_slot;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -111,13 +112,17 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
     const size_t a_bytes = (size_t)a.KC * 128 * 4;             // one A term of one stage = one raw stage
     float* Bs = reinterpret_cast<float*>(smem);
     unsigned char* As = smem + 2 * b_bytes;                    // [a_stages][hi | lo]
-    const int R = a.raw_stages, NA = a.a_stages;
-    unsigned char* Rs = As + (size_t)2 * NA * a_bytes;         // [raw_stages][KC][128] fp32
+    // direct mode (tile_major = 2): the A ring holds one TF32 term per stage and takes the raw ring's space as well --
+    // the ring depth is what hides the HBM latency (3 stages: 2.3 TB/s, 11 stages: measured in profiles/)
+    const bool direct = a.tile_major == 2;
+    const int R = a.raw_stages, NA = direct ? (2 * a.a_stages + a.raw_stages < TF32_MAX_A ? 2 * a.a_stages + a.raw_stages : TF32_MAX_A) : a.a_stages;
+    const size_t a_stride = direct ? a_bytes : 2 * a_bytes;   // bytes per A stage
+    unsigned char* Rs = As + (size_t)2 * a.a_stages * a_bytes; // [raw_stages][KC][128] fp32 (not in direct mode)
     const uint32_t tcols = 4 * a.NP <= 32 ? 32 : (4 * a.NP <= 64 ? 64 : (4 * a.NP <= 128 ? 128 : (4 * a.NP <= 256 ? 256 : 512)));
 
     if (tid == 0) {
         for (int s = 0; s < R; s++) { tc5::mbar_init(&raw_full[s], 1); tc5::mbar_init(&raw_empty[s], 8); }
-        for (int s = 0; s < NA; s++) { tc5::mbar_init(&a_full[s], 8); tc5::mbar_init(&a_empty[s], 1); }
+        for (int s = 0; s < NA; s++) { tc5::mbar_init(&a_full[s], a.tile_major == 2 ? 1 : 8); tc5::mbar_init(&a_empty[s], 1); }
         for (int s = 0; s < 2; s++) { tc5::mbar_init(&acc_full[s], 1); tc5::mbar_init(&acc_empty[s], 4); }
         tc5::mbar_fence_init();
     }
@@ -136,7 +141,24 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
     const long ntiles = a.rows_padded / 128;
     const int cpt = 2 * a.nchunks;                             // chunks per tile (re part, then im part)
 
-    if (warp == 0) {
+    if (warp == 0 && a.tile_major == 2) {
+        // ---- TMA producer, direct: the jamps are already TF32 values in the operand layout: one 12 KB bulk copy per chunk
+        //      straight into the A ring (no raw ring, no converters, no low term of X) ----
+        if (lane == 0) {
+            uint32_t sa = 0, ph = 1;                 // stage and the parity to wait for (no division in this loop)
+            for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                const float* xt = a.X + (size_t)tile * (256 * a.nc);
+                for (int part = 0; part < 2; part++)
+                    for (int c = a.nchunks - 1; c >= 0; c--) {
+                        tc5::mbar_wait(&a_empty[sa], ph);
+                        tc5::mbar_arrive_expect_tx(&a_full[sa], (uint32_t)a_bytes);
+                        tc5::tma_load_1d(As + (size_t)sa * a_stride, xt + ((size_t)part * a.nc + c * a.KC) * 128, (uint32_t)a_bytes, &a_full[sa]);
+                        if (++sa == (uint32_t)NA) { sa = 0; ph ^= 1; }
+                    }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 0) {
         // ---- TMA producer: lane 0 waits for the stage and posts the byte count, then lane kk copies colour kk ----
         uint32_t q = 0;
         for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -164,32 +186,54 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
     } else if (warp == 1) {
         // ---- MMA issuer ----
         if (lane == 0) {
+            // this loop is ONE thread: nothing but waits, descriptor additions and the MMAs may be in it (the first version
+            // divided by nchunks and by the ring depth per chunk and rebuilt every descriptor: 10 us per tile)
             const uint32_t b_base = tc5::smem_u32(Bs), a_base = tc5::smem_u32(As);
             const uint32_t sbo = (uint32_t)(a.KC / 4) * 128;
-            uint32_t q = 0, tl = 0;
+            const int nks = a.KC / 8;
+            const uint64_t ks_step = 256 >> 4;                       // one k-step (two core-matrix columns) in descriptor units
+            uint64_t dbh[8], dbl[8];
+            uint32_t ides[8];
+#pragma unroll
+            for (int c = 0; c < 8; c++) {
+                const int cc = c < a.nchunks ? c : 0;
+                dbh[c] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[cc] * 4, 128, sbo);
+                dbl[c] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[cc] * 4 + (uint32_t)b_bytes, 128, sbo);
+                ides[c] = tc5::idesc_tf32(a.chunk_n[cc], 0, 0);
+            }
+            const uint64_t da0 = tc5::smem_desc(a_base, 128, sbo);
+            const uint64_t a_step = (uint64_t)(a_stride >> 4), al_off = (uint64_t)(a_bytes >> 4);
+            uint32_t sa = 0, ph = 0, tl = 0;
             for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, tl++) {
                 const uint32_t buf = tl & 1;
                 tc5::mbar_wait(&acc_empty[buf], ((tl >> 1) & 1) ^ 1);
                 tc5::tc_fence_after();
-                for (int j = 0; j < cpt; j++, q++) {
-                    const int part = j / a.nchunks, ci = j % a.nchunks, c = a.nchunks - 1 - ci;
-                    const uint32_t sa = q % NA;
-                    tc5::mbar_wait(&a_full[sa], (q / NA) & 1);
-                    tc5::tc_fence_after();
+                for (int part = 0; part < 2; part++) {
                     const uint32_t tm_d = tmem + buf * 2 * a.NP + part * a.NP;
-                    const uint32_t idesc = tc5::idesc_tf32(a.chunk_n[c], 0, 0);
-                    const uint32_t ah = a_base + (uint32_t)(sa * 2 * a_bytes), al = ah + (uint32_t)a_bytes;
-                    const uint32_t bh = b_base + (uint32_t)a.chunk_off[c] * 4, bl = bh + (uint32_t)b_bytes;
-                    for (int ks = 0; ks < a.KC / 8; ks++) {
-                        const uint64_t dah = tc5::smem_desc(ah + ks * 256, 128, sbo), dal = tc5::smem_desc(al + ks * 256, 128, sbo);
-                        const uint64_t dbh = tc5::smem_desc(bh + ks * 256, 128, sbo), dbl = tc5::smem_desc(bl + ks * 256, 128, sbo);
-                        tc5::mma_tf32(tm_d, dah, dbh, idesc, (ci | ks) != 0);
-                        tc5::mma_tf32(tm_d, dal, dbh, idesc, 1);
-                        tc5::mma_tf32(tm_d, dah, dbl, idesc, 1);
+#pragma unroll
+                    for (int ci = 0; ci < 8; ci++) {
+                        if (ci < a.nchunks) {
+                            const int c = a.nchunks - 1 - ci;
+                            tc5::mbar_wait(&a_full[sa], ph);
+                            tc5::tc_fence_after();
+                            // (c is a run-time index into register arrays: resolved by the unrolled selects below)
+                            uint64_t bh = dbh[0], bl = dbl[0];
+                            uint32_t id = ides[0];
+#pragma unroll
+                            for (int t = 1; t < 8; t++)
+                                if (c == t) { bh = dbh[t]; bl = dbl[t]; id = ides[t]; }
+                            const uint64_t dah = da0 + a_step * sa;
+                            for (int ks = 0; ks < nks; ks++) {
+                                tc5::mma_tf32(tm_d, dah + ks_step * ks, bh + ks_step * ks, id, (ci | ks) != 0);
+                                if (!direct) tc5::mma_tf32(tm_d, dah + al_off + ks_step * ks, bh + ks_step * ks, id, 1);
+                                tc5::mma_tf32(tm_d, dah + ks_step * ks, bl + ks_step * ks, id, 1);
+                            }
+                            tc5::mma_commit(&a_empty[sa]);
+                            if (++sa == (uint32_t)NA) { sa = 0; ph ^= 1; }
+                        }
                     }
-                    tc5::mma_commit(&a_empty[sa]);
-                    if (j == cpt - 1) tc5::mma_commit(&acc_full[buf]);
                 }
+                tc5::mma_commit(&acc_full[buf]);
             }
         }
         __syncwarp();
@@ -217,7 +261,7 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
             if (lane == 0) tc5::mbar_arrive(&acc_empty[buf]);
             a.map.store(a.out, tile * 128 + r, (double)s0 + (double)s1 + ((double)s2 + (double)s3));
         }
-    } else if (warp >= 8) {
+    } else if (warp >= 8 && a.tile_major != 2) {
         // ---- converters: 8 warps; thread = (row m of the tile, half of the chunk's colour quads) ----
         const int m = (tid - 256) & 127, half = (tid - 256) >> 7;
         const int nq = a.KC / 4, q0 = half * nq / 2, q1 = (half + 1) * nq / 2;
@@ -263,9 +307,10 @@ static size_t tf32_smem_bytes(const Tf32Cfg& c)
 }
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
-                           double* d_meh, cudaStream_t st, bool tile_major)
+                           double* d_meh, cudaStream_t st, int tile_major)
 {
     Tf32Cfg c;
+    if (tile_major == 2 && ncolor % 24 != 0) return cudaErrorInvalidValue;
     if (!tf32_cfg(ncolor, &c) || !d_factor_img || rows_padded % 128 || c.nchunks > 8 || c.a_stages > 4 || c.raw_stages > TF32_MAX_RAW)
         return cudaErrorInvalidValue;
     // per call, for the CURRENT device: the attribute is per device and a process may hold handles on several
@@ -279,7 +324,7 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     }
     Tf32Args a;
     a.X = (const float*)d_jamps; a.Bimg = (const float*)d_factor_img; a.out = d_meh; a.rows_padded = rows_padded;
-    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.raw_stages = c.raw_stages; a.a_stages = c.a_stages; a.map = map; a.tile_major = tile_major ? 1 : 0;
+    a.nc = c.nc; a.KP = c.KP; a.NP = c.NP; a.KC = c.KC; a.nchunks = c.nchunks; a.raw_stages = c.raw_stages; a.a_stages = c.a_stages; a.map = map; a.tile_major = tile_major;
     a.b_floats = (int)chunk_off(c, c.nchunks);
     for (int i = 0; i < 8; i++) { a.chunk_off[i] = i < c.nchunks ? (int)chunk_off(c, i) : 0; a.chunk_n[i] = i < c.nchunks ? chunk_n(c, i) : 0; }
     const long ntiles = rows_padded / 128;

@@ -68,6 +68,14 @@ template <int PLANE> __device__ __forceinline__ void st_wf(char* __restrict__ ar
     for (int c = 0; c < 4; c++) *reinterpret_cast<double2*>(area + off + c * PLANE) = make_double2(w.c[c].re, w.c[c].im);
 }
 
+// fp32 -> TF32 (10 explicit significand bits), round to nearest: the tensor core would truncate
+__device__ __forceinline__ float to_tf32(float x)
+{
+    unsigned u;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
+    return __uint_as_float(u);
+}
+
 __device__ __forceinline__ p4<double> ld_k(const char* __restrict__ Ks, unsigned off)
 {
     const double2 a = *reinterpret_cast<const double2*>(Ks + off), b = *reinterpret_cast<const double2*>(Ks + off + 16);
@@ -387,7 +395,16 @@ __device__ __forceinline__ void p3_flow_sig(const HsDev& d, const HsSmemTabs& tb
         if (pos >= 0) {
             const double2 v = *reinterpret_cast<const double2*>(acc + 16 * acc_swizzle(h));
             const size_t row = (size_t)e * a.nrow_evt + pos;
-            if (a.tile_major) {
+            if (a.tile_major == 2) {
+                // tcgen05 operand layout (csrc/color_sum_tf32.cu, "direct"): per 128-row tile and part, chunks of 24 colours
+                // as K-major core matrices [row / 8][colour quad][row % 8][colour % 4], values rounded to TF32
+                if constexpr (sizeof(T2) == 4) {
+                    const unsigned m = (unsigned)(row & 127);
+                    float* __restrict__ o = reinterpret_cast<float*>(out) + (row >> 7) * (size_t)(256 * d.ncolor) +
+                                            (size_t)(jamp / 24) * (24 * 128) + (m >> 3) * 192 + ((jamp % 24) >> 2) * 32 + (m & 7) * 4 + (jamp & 3);
+                    o[0] = to_tf32((float)v.x); o[(size_t)d.ncolor * 128] = to_tf32((float)v.y);
+                }
+            } else if (a.tile_major) {
                 T2* __restrict__ o = out + (row >> 7) * (size_t)(256 * d.ncolor) + (size_t)jamp * 128 + (row & 127);
                 o[0] = T2(v.x); o[(size_t)d.ncolor * 128] = T2(v.y);
             } else {

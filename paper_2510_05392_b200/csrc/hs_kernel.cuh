@@ -13,7 +13,8 @@ struct HsLaunch {
     int nrow_evt;          // rows per event (= number of good helicities)
     void* d_jamps;         // DEVICE [2][ncolor][rows] fp64 or fp32; row = event * nrow_evt + pos[h]
     long rows;             // row stride of the jamps buffer
-    int tile_major;        // 1: [row / 128][2][ncolor][128] (one contiguous block per 128-row tile: TMA-friendly) instead
+    int tile_major;        // 2: the tcgen05 operand layout, TF32-rounded (fp32 jamps, ncolor % 24 == 0; color_sum_tf32.cu);
+                           // 1: [row / 128][2][ncolor][128] (one contiguous block per 128-row tile: TMA-friendly) instead
     double mt, wt;
 };
 

@@ -250,7 +250,9 @@ def test_mixed_color_sum_variants_agree(B):
     mom = inputs.momenta("gg_ttxggg", 203, seed=5)
     d_mom = torch.from_numpy(mom).cuda()
     ref = None
-    for opts in ({}, {"hs_color_alu": 1}, {"diagrams": 0, "color_sum": 1}):
+    # reference = the fp32 ALU kernel; the split-TF32 contraction (three products) agrees to fp32 level, the direct one (jamps
+    # rounded to TF32 by the diagram kernel, two products) to the TF32 rounding of J averaged over 120 colours
+    for opts, tol in (({"hs_color_alu": 1}, 0.0), ({"tf32_direct": 0}, 2e-5), ({}, 1e-4), ({"diagrams": 0, "color_sum": 1}, 2e-5)):
         proc = B.init_process("gg_ttxggg", "mixed")
         for k, v in opts.items():
             proc.set_option(k, v)
@@ -258,7 +260,9 @@ def test_mixed_color_sum_variants_agree(B):
         if ref is None:
             ref = me
         else:
-            assert _relerr(me, ref).max() < 2e-5, opts
+            err = _relerr(me, ref)
+            print(opts, "median", np.median(err), "max", err.max())
+            assert err.max() < tol, opts
         proc.close()
 
 
