@@ -12,8 +12,9 @@
 //
 // Scheduling inside the CTA: the work items of a step -- the colour flows of group g (phase 3) and, when the staging area
 // is double-buffered (HsCfg::NBUF = 2), the phase-2 units of group g + 1 -- are dealt to the warps at build time by their
-// instruction counts (gen/hs_streams.py _schedule), with ONE barrier per step.  The paper's counterpart is the sequence of diagram-group kernels on
-// helicity streams; here a "group" never leaves the SM.
+// instruction counts (gen/hs_streams.py _schedule), with ONE barrier per step; phase 1 is dealt the same way, in blocks of
+// 32 items with one sequence of opcodes.  The paper's counterpart is the sequence of diagram-group kernels on helicity
+// streams; here a "group" never leaves the SM.
 //
 // Every shared-memory address of phases 2 and 3 comes precomputed from the streams: an argument costs one 16-bit
 // extraction, its four components are immediate offsets (component planes), and there is no interpretation of opcodes
@@ -40,8 +41,6 @@ struct HsDev {
 struct HsSmemTabs {
     const int4* p3flow; const int* p3clsh; const uint2* wsched; const unsigned* witem;
 };
-
-
 
 // variant of an argument object: bit j = bit ((code >> 3j) & 7) of the parent's variant (7 = none; variants are < 128)
 __device__ __forceinline__ int sub_variant(int var, int code)

@@ -36,12 +36,15 @@
 //               contiguous run of chunks -- p2rec is stored in execution order.
 //               Steps: NBUF = 2: step s = flows of group s - 1 and units of group s; NBUF = 1: units(g), flows(g) alternate
 //   p3rec[entry][row = lane / 4] (uint4): x, y, z = 16-bit byte offsets of the A fragments (nA of them, whole words),
-//               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | negative << 31,
+//               then of the B fragments (nB; + 8 for odd rows: the imaginary half), w = shape | skip << 8 | negative << 31,
 //               shape = swapped | mask << 1 (mask: tile bits that select the A fragment); the entries of a class are
-//               sorted by shape, in the order HsCfg<NG>::SHAPE0..3
+//               sorted by shape, in the order HsCfg<NG>::SHAPE0..3; skip: a slot of a padded flow that holds no entry
 //   p3cls[class][lane] (uint2): 16-bit byte offsets into the flow's accumulator of this lane's complex number in tiles 0..3
-//   p3clsh[class] = number of entries of shape k in bits 4k .. 4k+3
-//   p3flow[f] = { first entry, classes | entries << 8 | accumulator << 16, first class, jamp index }
+//   p3clsh[class] = number of (real) entries of shape k in bits 4k .. 4k+3; 0 = a class a padded flow does not have
+//   p3flow[f] = { first entry, classes | entry slots << 8 | accumulator << 16 | signature << 24, first class, jamp index };
+//               signature = id of the flow's sequence of class headers (slots per shape), HS_FLOW_SIGS_<n> in
+//               generated/hs_gen.h: the kernel runs each signature as straight-line code; HsCfg::P3_PAD = 1: all flows padded
+//               to one signature
 #pragma once
 
 namespace mg {
