@@ -361,3 +361,22 @@ def test_precision_error_study(B, process, nevt):
     assert stats["mixed"][0] < 2e-4 and stats["mixed"][2] < 1e-3
     # all-fp32: the median stays at single-precision level; the tail is what the study is about (no bound on the maximum)
     assert stats["fp32"][0] < 2e-4, stats["fp32"]
+
+
+@pytest.mark.parametrize("process,prec,nevt", [("gg_ttxgg", "fp64", 131), ("gg_ttxggg", "fp64", 67), ("gg_ttxggg", "mixed", 67)])
+def test_partial_helicity_mask_on_the_shared_kernel(B, process, prec, nevt):
+    """a good-helicity list that is a strict subset (rows per event not a multiple of anything, skipped helicities inside the
+    CTA-per-event kernel, ragged 128-row tiles of the tensor-core colour sums): me = the oracle's sum over exactly those"""
+    mom = inputs.momenta(process, nevt, seed=23)
+    _, mh = _oracle(process, mom, per_helicity=True)
+    ncomb = mh.shape[1]
+    mask = np.zeros(ncomb, dtype=np.uint8)
+    mask[::3] = 1
+    mask[5] = 1
+    proc = B.init_process(process, prec)
+    proc.set_good_helicities(mask)
+    me = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+    ref = mh[:, mask.astype(bool)].sum(axis=1)
+    err = _relerr(me, ref)
+    assert err.max() < (1e-10 if prec == "fp64" else 1e-3), err.max()
+    proc.close()
