@@ -100,12 +100,15 @@ constexpr int TF32_THREADS = 512;
 constexpr int TF32_MAX_RAW = 8;
 constexpr int TF32_MAX_A = 12;
 
+template <bool DIRECT>
 __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const Tf32Args a)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ uint64_t raw_full[TF32_MAX_RAW], raw_empty[TF32_MAX_RAW];
     __shared__ uint64_t a_full[TF32_MAX_A], a_empty[TF32_MAX_A], acc_full[2], acc_empty[2];
     __shared__ uint32_t tmem_slot;
+    __shared__ uint64_t tab_b[8][2];          // per chunk: descriptors of its slice of L_hi / L_lo (MMA issuer)
+    __shared__ uint32_t tab_id[8];            // per chunk: instruction descriptor (accumulator width)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const size_t b_bytes = (size_t)a.b_floats * 4;             // one factor image
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
     unsigned char* As = smem + 2 * b_bytes;                    // [a_stages][hi | lo]
     // direct mode (tile_major = 2): the A ring holds one TF32 term per stage and takes the raw ring's space as well --
     // the ring depth is what hides the HBM latency (3 stages: 2.3 TB/s, 11 stages: measured in profiles/)
-    const bool direct = a.tile_major == 2;
+    constexpr bool direct = DIRECT;            // (a.tile_major == 2)
     const int R = a.raw_stages, NA = direct ? (2 * a.a_stages + a.raw_stages < TF32_MAX_A ? 2 * a.a_stages + a.raw_stages : TF32_MAX_A) : a.a_stages;
     const size_t a_stride = direct ? a_bytes : 2 * a_bytes;   // bytes per A stage
     unsigned char* Rs = As + (size_t)2 * a.a_stages * a_bytes; // [raw_stages][KC][128] fp32 (not in direct mode)
@@ -122,9 +125,16 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
 
     if (tid == 0) {
         for (int s = 0; s < R; s++) { tc5::mbar_init(&raw_full[s], 1); tc5::mbar_init(&raw_empty[s], 8); }
-        for (int s = 0; s < NA; s++) { tc5::mbar_init(&a_full[s], a.tile_major == 2 ? 1 : 8); tc5::mbar_init(&a_empty[s], 1); }
-        for (int s = 0; s < 2; s++) { tc5::mbar_init(&acc_full[s], 1); tc5::mbar_init(&acc_empty[s], 4); }
+        for (int s = 0; s < NA; s++) { tc5::mbar_init(&a_full[s], direct ? 1 : 8); tc5::mbar_init(&a_empty[s], 1); }
+        for (int s = 0; s < 2; s++) { tc5::mbar_init(&acc_full[s], direct ? 2 : 1); tc5::mbar_init(&acc_empty[s], 4); }
         tc5::mbar_fence_init();
+        // per chunk: descriptors of its slice of L_hi / L_lo and the instruction descriptor (read by the MMA issuers)
+        const uint32_t b_base = tc5::smem_u32(Bs), sbo0 = (uint32_t)(a.KC / 4) * 128;
+        for (int c = 0; c < a.nchunks; c++) {
+            tab_b[c][0] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[c] * 4, 128, sbo0);
+            tab_b[c][1] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[c] * 4 + (uint32_t)b_bytes, 128, sbo0);
+            tab_id[c] = tc5::idesc_tf32(a.chunk_n[c], 0, 0);
+        }
     }
     if (warp == 2) tc5::tmem_alloc(&tmem_slot, tcols);
     {   // resident factor image
@@ -141,15 +151,15 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
     const long ntiles = a.rows_padded / 128;
     const int cpt = 2 * a.nchunks;                             // chunks per tile (re part, then im part)
 
-    if (warp == 0 && a.tile_major == 2) {
+    if (warp == 0 && direct) {
         // ---- TMA producer, direct: the jamps are already TF32 values in the operand layout: one 12 KB bulk copy per chunk
         //      straight into the A ring (no raw ring, no converters, no low term of X) ----
         if (lane == 0) {
             uint32_t sa = 0, ph = 1;                 // stage and the parity to wait for (no division in this loop)
             for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
                 const float* xt = a.X + (size_t)tile * (256 * a.nc);
-                for (int part = 0; part < 2; part++)
-                    for (int c = a.nchunks - 1; c >= 0; c--) {
+                for (int c = a.nchunks - 1; c >= 0; c--)
+                    for (int part = 0; part < 2; part++) {             // re, im alternate: one MMA-issuing thread each
                         tc5::mbar_wait(&a_empty[sa], ph);
                         tc5::mbar_arrive_expect_tx(&a_full[sa], (uint32_t)a_bytes);
                         tc5::tma_load_1d(As + (size_t)sa * a_stride, xt + ((size_t)part * a.nc + c * a.KC) * 128, (uint32_t)a_bytes, &a_full[sa]);
@@ -183,54 +193,42 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
             }
         }
         __syncwarp();
-    } else if (warp == 1) {
-        // ---- MMA issuer ----
+    } else if (warp == 1 || (direct && warp == 3)) {
+        // ---- MMA issuer(s).  Each is ONE thread: nothing but waits, descriptor additions and the MMAs may be in its loop (the
+        //      first version divided by nchunks and by the ring depth per chunk and rebuilt every descriptor: 10 us per tile).
+        //      Direct mode has two of them, warp 1 for the re part and warp 3 for the im part (independent accumulator
+        //      columns, alternate stages of the ring): the issue rate of one thread was the limit of the kernel ----
         if (lane == 0) {
-            // this loop is ONE thread: nothing but waits, descriptor additions and the MMAs may be in it (the first version
-            // divided by nchunks and by the ring depth per chunk and rebuilt every descriptor: 10 us per tile)
-            const uint32_t b_base = tc5::smem_u32(Bs), a_base = tc5::smem_u32(As);
+            const int me = warp == 3 ? 1 : 0;
+            const uint32_t a_base = tc5::smem_u32(As);
             const uint32_t sbo = (uint32_t)(a.KC / 4) * 128;
             const int nks = a.KC / 8;
-            const uint64_t ks_step = 256 >> 4;                       // one k-step (two core-matrix columns) in descriptor units
-            uint64_t dbh[8], dbl[8];
-            uint32_t ides[8];
-#pragma unroll
-            for (int c = 0; c < 8; c++) {
-                const int cc = c < a.nchunks ? c : 0;
-                dbh[c] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[cc] * 4, 128, sbo);
-                dbl[c] = tc5::smem_desc(b_base + (uint32_t)a.chunk_off[cc] * 4 + (uint32_t)b_bytes, 128, sbo);
-                ides[c] = tc5::idesc_tf32(a.chunk_n[cc], 0, 0);
-            }
+            const uint32_t ks_step = 256 >> 4;                       // one k-step (two core-matrix columns) in descriptor units
             const uint64_t da0 = tc5::smem_desc(a_base, 128, sbo);
-            const uint64_t a_step = (uint64_t)(a_stride >> 4), al_off = (uint64_t)(a_bytes >> 4);
-            uint32_t sa = 0, ph = 0, tl = 0;
+            const uint32_t a_step = (uint32_t)(a_stride >> 4), al_off = (uint32_t)(a_bytes >> 4);
+            const uint32_t adv = direct ? 2 : 1;                     // stages per chunk of this thread
+            uint32_t sa = direct ? me : 0, ph = 0, tl = 0;
             for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, tl++) {
                 const uint32_t buf = tl & 1;
                 tc5::mbar_wait(&acc_empty[buf], ((tl >> 1) & 1) ^ 1);
                 tc5::tc_fence_after();
-                for (int part = 0; part < 2; part++) {
+                for (int part = direct ? me : 0; part < (direct ? me + 1 : 2); part++) {
                     const uint32_t tm_d = tmem + buf * 2 * a.NP + part * a.NP;
-#pragma unroll
-                    for (int ci = 0; ci < 8; ci++) {
-                        if (ci < a.nchunks) {
-                            const int c = a.nchunks - 1 - ci;
-                            tc5::mbar_wait(&a_full[sa], ph);
-                            tc5::tc_fence_after();
-                            // (c is a run-time index into register arrays: resolved by the unrolled selects below)
-                            uint64_t bh = dbh[0], bl = dbl[0];
-                            uint32_t id = ides[0];
-#pragma unroll
-                            for (int t = 1; t < 8; t++)
-                                if (c == t) { bh = dbh[t]; bl = dbl[t]; id = ides[t]; }
-                            const uint64_t dah = da0 + a_step * sa;
-                            for (int ks = 0; ks < nks; ks++) {
-                                tc5::mma_tf32(tm_d, dah + ks_step * ks, bh + ks_step * ks, id, (ci | ks) != 0);
-                                if (!direct) tc5::mma_tf32(tm_d, dah + al_off + ks_step * ks, bh + ks_step * ks, id, 1);
-                                tc5::mma_tf32(tm_d, dah + ks_step * ks, bl + ks_step * ks, id, 1);
-                            }
-                            tc5::mma_commit(&a_empty[sa]);
-                            if (++sa == (uint32_t)NA) { sa = 0; ph ^= 1; }
+                    for (int ci = 0; ci < a.nchunks; ci++) {
+                        const int c = a.nchunks - 1 - ci;
+                        const uint64_t bh = tab_b[c][0], bl = tab_b[c][1];
+                        const uint32_t id = tab_id[c];
+                        const uint64_t dah = da0 + a_step * sa;
+                        tc5::mbar_wait(&a_full[sa], ph);
+                        tc5::tc_fence_after();
+                        for (int ks = 0; ks < nks; ks++) {
+                            tc5::mma_tf32(tm_d, dah + ks_step * ks, bh + ks_step * ks, id, (ci | ks) != 0);
+                            if (!direct) tc5::mma_tf32(tm_d, dah + al_off + ks_step * ks, bh + ks_step * ks, id, 1);
+                            tc5::mma_tf32(tm_d, dah + ks_step * ks, bl + ks_step * ks, id, 1);
                         }
+                        tc5::mma_commit(&a_empty[sa]);
+                        sa += adv;
+                        if (sa >= (uint32_t)NA) { sa -= NA; ph ^= 1; }
                     }
                 }
                 tc5::mma_commit(&acc_full[buf]);
@@ -261,7 +259,7 @@ __global__ void __launch_bounds__(TF32_THREADS, 1) color_sum_tf32_kernel(const T
             if (lane == 0) tc5::mbar_arrive(&acc_empty[buf]);
             a.map.store(a.out, tile * 128 + r, (double)s0 + (double)s1 + ((double)s2 + (double)s3));
         }
-    } else if (warp >= 8 && a.tile_major != 2) {
+    } else if (warp >= 8 && !direct) {
         // ---- converters: 8 warps; thread = (row m of the tile, half of the chunk's colour quads) ----
         const int m = (tid - 256) & 127, half = (tid - 256) >> 7;
         const int nq = a.KC / 4, q0 = half * nq / 2, q1 = (half + 1) * nq / 2;
@@ -319,7 +317,8 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const size_t smem = tf32_smem_bytes(c);
     {
-        cudaError_t e = cudaFuncSetAttribute(color_sum_tf32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(color_sum_tf32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(color_sum_tf32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     Tf32Args a;
@@ -329,7 +328,8 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
     for (int i = 0; i < 8; i++) { a.chunk_off[i] = i < c.nchunks ? (int)chunk_off(c, i) : 0; a.chunk_n[i] = i < c.nchunks ? chunk_n(c, i) : 0; }
     const long ntiles = rows_padded / 128;
     const int grid = (int)(ntiles < sms ? ntiles : sms);      // one CTA per SM: each owns its TMEM columns
-    color_sum_tf32_kernel<<<grid, TF32_THREADS, smem, st>>>(a);
+    if (tile_major == 2) color_sum_tf32_kernel<true><<<grid, TF32_THREADS, smem, st>>>(a);
+    else color_sum_tf32_kernel<false><<<grid, TF32_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
