@@ -323,7 +323,7 @@ def main():
                                                          "helicity_sum": r["stage_ms"][2]},
            "roofline": roofline, "clocks": clocks}
 
-    if rank == 0 and (args.ramp or not args.no_extras):
+    if rank == 0 and (args.ramp or (world == 1 and not args.no_extras)):          # (one-GPU study: not in multi-rank runs)
         # the paper's small-grid curves (MEs/s against events per batch): plain launches, and the
         # same launch sequence replayed as a CUDA graph (option "graph")
         sizes, n = [], 32
