@@ -306,6 +306,29 @@ def main():
                 "flop_per_event_helicity": proc.diagram_flops, "kernel_ms": diag_ms,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
 
+    # second kernel of the step, the colour sum: FP64 tensor bound (DMMA, issued flop of the triangular contraction) in fp64,
+    # HBM bound (it reads the jamps once) in mixed precision
+    cs_roofline = None
+    cs_ms = r["stage_ms"][1]
+    if shared and cs_ms > 0:
+        rows = nevt * r["ngood"]
+        nc = proc.ncolor
+        if args.precision in ("fp64", "d"):
+            nt = (nc + 7) // 8
+            pairs = sum(ks // 2 + 1 for ks in range(2 * nt))                   # (k-step, n-tile) pairs on or below the diagonal
+            flop = rows / 8 * pairs * 2 * 512.0                                # x 2 parts, 512 flop per m8n8k4
+            dmma_peak = B.measure_peak(2, local)
+            ach = flop / (cs_ms * 1e-3) * 1e-12
+            cs_roofline = {"bound": "tensor", "kernel": "color_sum_dmma2_kernel", "achieved": ach, "peak": dmma_peak, "unit": "TFLOP/s",
+                           "frac": ach / dmma_peak, "kernel_ms": cs_ms, "flop_counted": "issued DMMA (triangular k-step x n-tile pairs)",
+                           "peak_source": "mma.sync.m8n8k4.f64 probe measured in this run (mg_measure_peak kind 2)"}
+        elif not proc.get_option("hs_color_alu"):
+            nbytes = rows * nc * 2 * 4.0
+            ach = nbytes / (cs_ms * 1e-3) * 1e-9
+            cs_roofline = {"bound": "hbm", "kernel": "color_sum_tf32_kernel", "achieved": ach, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                           "frac": ach / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None, "kernel_ms": cs_ms,
+                           "bytes_counted": "the fp32 jamps, read once", "peak_source": peak_src}
+
     out = {"metric": METRIC, "value": r["value"], "unit": "MEs/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64" if args.precision in ("fp64", "d") else ("f64+f32" if args.precision in ("mixed", "m") else "f32"),
@@ -321,7 +344,7 @@ def main():
                       "l2": "256 MiB device memset between timed steps (outside the per-step event pairs)"},
            "gpu_launches": r["launches"], "stage_ms": {"diagrams": r["stage_ms"][0], "color_sum": r["stage_ms"][1],
                                                          "helicity_sum": r["stage_ms"][2]},
-           "roofline": roofline, "clocks": clocks}
+           "roofline": roofline, "roofline_color_sum": cs_roofline, "clocks": clocks}
 
     if rank == 0 and (args.ramp or (world == 1 and not args.no_extras)):          # (one-GPU study: not in multi-rank runs)
         # the paper's small-grid curves (MEs/s against events per batch): plain launches, and the
