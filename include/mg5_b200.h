@@ -79,7 +79,8 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
  * "tf32_direct" (MG_DIAG_SHARED in MG_MIXED with the tcgen05 kernel, default 1: the diagram kernel writes the jamps as TF32
  * values straight in the tensor-core operand layout and the contraction accumulates J Lhi + J Llo; 0: fp32 jamps, two-term
  * split of J inside the contraction, three products),
- * "jamp_chunk_mib" (size of the jamps buffer inside the workspace), "timing" (0/1),
+ * "jamp_chunk_mib" (size of the jamps buffer inside the workspace; default 16384 = every BASELINE.json batch in one chunk;
+ * smaller values trade workspace for more launches), "timing" (0/1),
  * "max_streams" (MG_SCHED_STREAMS: helicities share this many streams round robin, 0 = one each),
  * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the
  * arguments and the handle's state are unchanged; ignored while "timing" = 1; mg_get_option

@@ -51,7 +51,7 @@ struct mg_process {
     int graph_replays = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
-    long jamp_chunk_bytes = 1L << 30;
+    long jamp_chunk_bytes = 16L << 30;     // one chunk for every BASELINE.json batch (180 GB of HBM3e); smaller via "jamp_chunk_mib"
     // good helicities
     std::vector<int> good;
     int* d_good = nullptr;     // DEVICE [ncomb]

@@ -221,6 +221,12 @@ def test_full_size_sampled(B, process):
     err = _relerr(me[idx], _oracle(process, mom[idx]))
     _histogram(err, f"{process} fp64 full size")
     assert err.max() < 1e-10
+    if process in ("gg_ttxgg", "gg_ttxggg"):
+        # the default jamps buffer holds the whole batch; with a 1 GiB buffer the batch goes through several diagram /
+        # colour-sum launches (for gg_ttxggg 16 chunks of 4352 events): same numbers, event by event, over the FULL batch
+        proc.set_option("jamp_chunk_mib", 1024)
+        me2 = proc.sigma_batch(torch.from_numpy(mom).cuda()).cpu().numpy()
+        assert _relerr(me2, me).max() < 1e-13
     proc.close()
 
 
