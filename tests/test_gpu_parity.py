@@ -3,6 +3,8 @@
 Tolerances (BASELINE.json north_star): fp64 relative 1e-10 per event; mixed/fp32 median 2e-4, max 1e-3;
 helicity mask exact.  Sizes span several thread blocks and a ragged tail.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -186,6 +188,8 @@ def _full_size_sample(proc, process, nevt, nrandom, seed):
     """indices compared with the oracle at the full batch size (SURVEY.md §8(c) oracle cost note): the first and the last
     1024 events, `nrandom` seeded random ones, and the events on both sides of every boundary between the event chunks the
     library processes separately (jamps buffer chunks)"""
+    if os.environ.get("MG_FULL_PARITY") == "1":          # every event of the batch (minutes of oracle time for gg_ttxggg)
+        return np.arange(nevt)
     rng = np.random.default_rng(seed)
     edge = min(1024, nevt // 4)
     parts = [np.arange(edge), np.arange(nevt - edge, nevt), edge + rng.choice(nevt - 2 * edge, min(nrandom, nevt - 2 * edge), replace=False)]
@@ -195,6 +199,25 @@ def _full_size_sample(proc, process, nevt, nrandom, seed):
     b = np.arange(ce, nevt, ce)
     parts += [b - 1, b]
     return np.unique(np.concatenate(parts))
+
+
+def _assert_fp64_parity(process, mom, me, err, tol=1e-10):
+    """fp64 bar: relative 1e-10 per event against the fp64 oracle.  An event beyond it goes to the arbiter of reading A12
+    (DESIGN.md): the long-double build of the oracle.  In the collinear / soft corners of uncut RAMBO the diagrams (and the
+    Berends-Giele currents) cancel by many orders of magnitude and BOTH fp64 evaluations lose digits -- over the full 65 536
+    events of g g -> t tbar g g g this happens once (a gluon at pT/E = 1e-3 to a beam: the fp64 oracle is 1.3e-9 off its own
+    long-double value, profiles/r2_full_parity.md).  Such an event passes iff the fp64 oracle itself misses the arbiter
+    by more than the tolerance and the CUDA result is no farther from the arbiter than three times that."""
+    bad = np.nonzero(err >= tol)[0]
+    if bad.size == 0:
+        return
+    assert bad.size <= max(1, me.size // 10000), f"{bad.size} events beyond {tol}: not a rounding corner"
+    ld = oracle.matrix_elements(process, mom[bad], inputs.PARAMS, long_double=True)
+    ref = _oracle(process, mom[bad])
+    for k, i in enumerate(bad):
+        e_ref, e_gpu = abs(ref[k] / ld[k] - 1), abs(me[i] / ld[k] - 1)
+        print(f"\n[arbiter] event {i}: gpu/oracle64-1 = {err[i]:.2e}, oracle64/ld-1 = {e_ref:.2e}, gpu/ld-1 = {e_gpu:.2e}")
+        assert e_ref > tol and e_gpu < 3 * e_ref, (i, err[i], e_ref, e_gpu)
 
 
 def _histogram(err, label):
@@ -220,7 +243,7 @@ def test_full_size_sampled(B, process):
     assert idx.size >= min(4096, nevt // 5) and idx[0] == 0 and idx[-1] == nevt - 1
     err = _relerr(me[idx], _oracle(process, mom[idx]))
     _histogram(err, f"{process} fp64 full size")
-    assert err.max() < 1e-10
+    _assert_fp64_parity(process, mom[idx], me[idx], err)
     if process in ("gg_ttxgg", "gg_ttxggg"):
         # the default jamps buffer holds the whole batch; with a 1 GiB buffer the batch goes through several diagram /
         # colour-sum launches (for gg_ttxggg 16 chunks of 4352 events): same numbers, event by event, over the FULL batch
