@@ -74,7 +74,7 @@ int mg_process_flops(const mg_process* p, double* diagram_flops, double* color_f
 int mg_set_parameters(mg_process* p, const char* const* keys, const double* values, int n);
 
 /* Options: "color_sum" (MG_CS_*), "schedule" (MG_SCHED_*), "diagrams" (MG_DIAG_*), "block" (threads per block of the
- * MG_DIAG_THREAD kernel, multiple of 32, <= 256),
+ * MG_DIAG_THREAD kernel, multiple of 32, <= 256; default 64, the fastest of 32..256 on B200 for g g -> t tbar (g)),
  * "hs_color_alu" (MG_DIAG_SHARED in MG_MIXED: 1 = scalar-ALU fp32 colour-sum kernel instead of the tcgen05 one),
  * "tf32_direct" (MG_DIAG_SHARED in MG_MIXED with the tcgen05 kernel, default 1: the diagram kernel writes the jamps as TF32
  * values straight in the tensor-core operand layout and the contraction accumulates J Lhi + J Llo; 0: fp32 jamps, two-term

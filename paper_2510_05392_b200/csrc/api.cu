@@ -29,7 +29,7 @@ struct mg_process {
     // parameters (BASELINE.json card)
     double aEWM1 = 132.507, mZ = 91.188, wZ = 2.4414, mW = 80.419, mT = 173.0, wT = 1.4915, aS = 0.118;
     // options
-    int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 128, timing = 0;
+    int color_sum = MG_CS_FUSED, schedule = MG_SCHED_GRID, block = 64, timing = 0;       // (block: 64 measured best for g g -> t tbar (g))
     int diagrams = MG_DIAG_THREAD, hs_color_alu = 0, tf32_direct = 1;
     int max_streams = 0;       // MG_SCHED_STREAMS: helicity h runs on stream h % max_streams (0 = one stream per helicity)
     int graph = 0;             // replay the launch sequence of a batch as a CUDA graph

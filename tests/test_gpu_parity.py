@@ -82,7 +82,7 @@ def test_scheduling_variants_agree(B, process):
     d_mom = torch.from_numpy(mom).cuda()
     base = None
     for opts in ({"diagrams": 0}, {"diagrams": 0, "schedule": 1}, {"diagrams": 0, "color_sum": 1},
-                 {"diagrams": 0, "color_sum": 1, "schedule": 1}, {"diagrams": 0, "block": 64},
+                 {"diagrams": 0, "color_sum": 1, "schedule": 1}, {"diagrams": 0, "block": 128},
                  {"diagrams": 1}, {"diagrams": 1, "jamp_chunk_mib": 1}):
         if opts.get("diagrams") == 1 and process in ("gg_ttx", "gg_ttxg"):
             continue                                   # the helicity-shared program exists for >= 2 final-state gluons
