@@ -58,9 +58,9 @@
 typedef ORC_REAL real;
 typedef ORC_REAL _Complex cplx;
 
-#define MAXG 5            /* max number of gluons */
-#define MAXPERM 120
-#define NCODE 32768       /* 8^5 tuple codes, digits 1..5 */
+#define MAXG 6            /* max number of gluons (g g -> t tbar g g g g: Table 2) */
+#define MAXPERM 720
+#define NCODE 262144      /* 8^6 tuple codes, digits 1..6 */
 
 /* ------------------------------------------------------------------------------------------ */
 /* permutations of n in lexicographic order                                                    */
@@ -165,6 +165,64 @@ int orc_color_matrix(int n, double* C /* [n!][n!] */, double* max_imag)
     double mi = 0;
     for (size_t i = 0; i < (size_t)np * np; i++) {
         C[i] = creal(acc[i]);
+        if (fabs(cimag(acc[i])) > mi) mi = fabs(cimag(acc[i]));
+    }
+    if (max_imag) *max_imag = mi;
+    free(acc);
+    return np;
+}
+
+/* First row only, C_{id,s'} for all s', by the same brute force.  With 6 gluons the full double loop over (s, s')
+ * inside the 8^6 colour assignments is out of reach (1.2e12 3x3 products); renaming the summed adjoint indices
+ * a_i -> a_{s(i)} in the definition gives C_{s s'} = C_{id, s^-1 o s'}, which the Python front end uses to fill the
+ * matrix from this row.  The identity itself is pinned against the full brute force for n <= 5
+ * (tests/test_oracle_pins.py).  Returns n!.                                                    */
+int orc_color_matrix_row0(int n, double* row /* [n!] */, double* max_imag)
+{
+    if (n < 1 || n > MAXG) return -1;
+    double _Complex T[8][3][3];
+    su3_generators(T);
+    static int perm[MAXPERM][MAXG];
+    int np = perms_lex(n, perm);
+    long nassign = 1;
+    for (int i = 0; i < n; i++) nassign *= 8;
+    double _Complex* acc = calloc((size_t)np, sizeof(double _Complex));
+#pragma omp parallel
+    {
+        double _Complex* loc = calloc((size_t)np, sizeof(double _Complex));
+#pragma omp for schedule(static)
+        for (long code = 0; code < nassign; code++) {
+            int a[MAXG];
+            long c = code;
+            for (int i = 0; i < n; i++) { a[i] = (int)(c % 8); c /= 8; }
+            double _Complex M0[3][3];
+            for (int s = 0; s < np; s++) {
+                double _Complex M[3][3], N[3][3];
+                memcpy(M, T[a[perm[s][0]]], sizeof(M));
+                for (int k = 1; k < n; k++) {
+                    const double _Complex (*X)[3] = T[a[perm[s][k]]];
+                    for (int i = 0; i < 3; i++)
+                        for (int j = 0; j < 3; j++) {
+                            double _Complex v = 0;
+                            for (int l = 0; l < 3; l++) v += M[i][l] * X[l][j];
+                            N[i][j] = v;
+                        }
+                    memcpy(M, N, sizeof(M));
+                }
+                if (s == 0) memcpy(M0, M, sizeof(M));      /* lexicographic order: permutation 0 is the identity */
+                double _Complex v = 0;
+                for (int i = 0; i < 3; i++)
+                    for (int j = 0; j < 3; j++) v += M0[i][j] * conj(M[i][j]);
+                loc[s] += v;
+            }
+        }
+#pragma omp critical
+        for (int i = 0; i < np; i++) acc[i] += loc[i];
+        free(loc);
+    }
+    double mi = 0;
+    for (int i = 0; i < np; i++) {
+        row[i] = creal(acc[i]);
         if (fabs(cimag(acc[i])) > mi) mi = fabs(cimag(acc[i]));
     }
     if (max_imag) *max_imag = mi;
@@ -288,7 +346,7 @@ typedef struct {
 } bg_t;
 
 static int tcode(const int* t, int len)
-{   /* ordered tuple -> code (base 8, digits 1..5) */
+{   /* ordered tuple -> code (base 8, digits 1..6) */
     int c = 0;
     for (int i = len - 1; i >= 0; i--) c = c * 8 + (t[i] + 1);
     return c;

@@ -19,8 +19,9 @@ _SRC = os.path.join(_HERE, "me_oracle.c")
 
 # number of gluons per process and the averaging/symmetry factor denom (reading A3):
 # gg initial state 2*2 spins * 8*8 colours = 256, times (n-2)! for identical final gluons; e+e-: 2*2.
-NGLUONS = {"gg_ttx": 2, "gg_ttxg": 3, "gg_ttxgg": 4, "gg_ttxggg": 5}
-DENOM = {"epem_mupmum": 4.0, "gg_ttx": 256.0, "gg_ttxg": 256.0, "gg_ttxgg": 512.0, "gg_ttxggg": 1536.0}
+NGLUONS = {"gg_ttx": 2, "gg_ttxg": 3, "gg_ttxgg": 4, "gg_ttxggg": 5, "gg_ttxgggg": 6}
+DENOM = {"epem_mupmum": 4.0, "gg_ttx": 256.0, "gg_ttxg": 256.0, "gg_ttxgg": 512.0, "gg_ttxggg": 1536.0,
+         "gg_ttxgggg": 6144.0}
 
 
 def _lib_path(long_double: bool) -> str:
@@ -47,6 +48,8 @@ def _lib(long_double: bool = False) -> ctypes.CDLL:
     ip = ctypes.POINTER(ctypes.c_int)
     lib.orc_color_matrix.argtypes = [ctypes.c_int, dp, dp]
     lib.orc_color_matrix.restype = ctypes.c_int
+    lib.orc_color_matrix_row0.argtypes = [ctypes.c_int, dp, dp]
+    lib.orc_color_matrix_row0.restype = ctypes.c_int
     lib.orc_ggttx_partial.argtypes = [ctypes.c_int, dp, ip, ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, dp]
     lib.orc_ggttx_partial.restype = ctypes.c_int
     lib.orc_me_ggttx.argtypes = [ctypes.c_int, dp, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double,
@@ -71,8 +74,29 @@ def su3_generators() -> np.ndarray:
     return out[..., 0] + 1j * out[..., 1]
 
 
+def color_matrix_from_row0(n: int):
+    """(C, max |imag|) with C_{s s'} = C_{id, s^-1 o s'} filled from the brute-force first row (orc_color_matrix_row0)."""
+    import itertools
+    nperm = math.factorial(n)
+    row = np.zeros(nperm)
+    mi = ctypes.c_double(0.0)
+    if _lib().orc_color_matrix_row0(n, _dp(row), ctypes.byref(mi)) != nperm:
+        raise RuntimeError("orc_color_matrix_row0 failed")
+    perms = list(itertools.permutations(range(n)))            # lexicographic, like perms_lex in the C file
+    rank = {p: i for i, p in enumerate(perms)}
+    C = np.zeros((nperm, nperm))
+    for i, s in enumerate(perms):
+        inv = [0] * n
+        for pos, g in enumerate(s):
+            inv[g] = pos
+        C[i] = row[[rank[tuple(inv[g] for g in t)] for t in perms]]
+    return C, mi.value
+
+
 @lru_cache(maxsize=None)
 def _color_matrix_cached(n: int):
+    if n >= 6:
+        return color_matrix_from_row0(n)
     nperm = math.factorial(n)
     C = np.zeros((nperm, nperm))
     mi = ctypes.c_double(0.0)

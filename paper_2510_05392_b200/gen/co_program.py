@@ -174,18 +174,76 @@ class Program:
         sign = combo[0][1]
         canon = tuple((i, s * sign) for i, s in combo)
         if canon not in self._combo:
-            o = self._new_obj(kind, legs)
-            for i, s in canon:
-                o.terms.append(self._term_of_current(self.proc.currents[i], s))
+            if len(legs) <= 3:
+                o = self._new_obj(kind, legs)
+                for i, s in canon:
+                    o.terms.append(self._term_of_current(self.proc.currents[i], s))
+            else:
+                terms = self._factorised_terms(canon, word, sign, legs)      # creates the argument objects first
+                o = self._new_obj(kind, legs)
+                o.terms = terms
             self._combo[canon] = o.id
         return self._combo[canon], sign
+
+    def _factorised_terms(self, canon, word, sign, legs):
+        """terms of a colour-ordered object with more than 3 legs, sum_c s_c c with s_c = sign * col_c[word]: its Feynman
+        currents c = V(a_1, .., a_k) have arguments with up to 3 legs, which are not objects themselves, so the sum is
+        factorised the way the amplitudes are (module docstring, (2)): col_c[word] = t * prod_i col_{a_i}[w_i] with w_i
+        the sub-word of `word` seen by a_i and t = +-1 fixed by (vertex, leg sets, word); V is multilinear, hence
+            sum_c s_c c = sum over (vertex, leg sets) of  sign t V(O_1, .., O_k),  O_i = sum_a col_a[w_i] a.
+        The currents sort their arguments by id (v3, and the first two of v4: vertex function and colour are both odd
+        under that exchange); here they are put in the order of their leg sets, so that one (vertex, leg sets) class is one
+        term.  `_check_expansion` expands the result back into Feynman currents."""
+        cur = self.proc.currents
+        found = {}
+        for cid, s_c in canon:
+            c = cur[cid]
+            args = [cur[i] for i in c.args]
+            flip = 1
+            if c.op in ("v3", "v4") and min(args[0].legs) > min(args[1].legs):
+                args[0], args[1] = args[1], args[0]
+                flip = -1                                  # Lorentz part alone changes sign (the colour is read off c.col)
+            words = [_key_word(a, word) for a in args]
+            prod = 1
+            for a, w in zip(args, words):
+                prod *= a.col.get(w, 0)
+            assert prod in (1, -1), "coefficient of a current does not factorise"
+            objs = tuple(self.object_for(a.kind, a.legs, w) for a, w in zip(args, words))
+            t = s_c * prod * flip
+            for _, os_ in objs:
+                t *= os_
+            key = (c.op, tuple(o for o, _ in objs))
+            assert found.setdefault(key, t) == t
+        # expansion check: the terms, multiplied out over the Feynman currents of their argument objects, are exactly canon
+        import itertools
+        inv_combo = getattr(self, "_members", None)
+        if inv_combo is None:
+            inv_combo = self._members = {}
+        for cn, oid in self._combo.items():
+            inv_combo.setdefault(oid, list(cn))
+        for fid, oid in self._fobj.items():
+            inv_combo.setdefault(oid, [(fid, 1)])
+        got = {}
+        for (op, ids), t in found.items():
+            for pick in itertools.product(*[inv_combo[o] for o in ids]):
+                fids, co = [f for f, _ in pick], t
+                for _, s_ in pick:
+                    co *= s_
+                if op in ("v3", "v4") and fids[0] > fids[1]:
+                    fids[0], fids[1] = fids[1], fids[0]
+                    co = -co
+                c = self.proc._memo.get((op, tuple(fids)))
+                assert c is not None, "factorised object holds a current that no diagram has"
+                got[c.id] = got.get(c.id, 0) + co
+        assert {k: v for k, v in got.items() if v} == dict(canon), "factorised object differs from its Feynman currents"
+        return [Term(t, op, ids, tuple(sorted(legs))) for (op, ids), t in sorted(found.items())]
 
     # ---------------------------------------------------------------------------------------------
     def _build_evals(self):
         """per colour flow sigma: the distinct vertex evaluations (op, ((object, sign), ...)) -> sign"""
         proc = self.proc
         cur = proc.currents
-        assert max(len(c.legs) for c in cur) <= 3, "centroid branches with more than 3 legs are not supported"
+        assert max(len(c.legs) for c in cur) <= 4, "centroid branches with more than 4 legs are not supported"
         inv = {v: k for k, v in proc.rank.items()}
         self.sigmas = [inv[j] for j in range(self.ncolor)]
         self.evals = [dict() for _ in range(self.ncolor)]

@@ -283,11 +283,29 @@ def _lower_diagram(proc, diagram, dindex, prefer):
     g = _diagram_graph(proc, diagram)
     size = _branch_sizes(g)
     best = None
+
+    def legs_of(u, frm):
+        if g.kind[u][0] == "ext":
+            return {g.kind[u][1]}
+        out = set()
+        for w in g.adj[u]:
+            if w != frm:
+                out |= legs_of(w, u)
+        return out
+
     for u in range(len(g.kind)):
         if g.kind[u][0] == "ext":
             continue
         worst = max(size(w, u) for w in g.adj[u])
-        score = (worst, prefer.get(g.kind[u][0], 0), u)
+        # 8 external legs: a propagator can split them 4 | 4 and both of its end vertices are centroids.  Take the end on
+        # the top quark's side, whatever the vertices are: the set of diagrams cut at (vertex, leg sets) is then the full
+        # product of the sub-diagrams of its branches, which the colour factorisation of gen/co_program.py needs.  (With
+        # 6 legs the 3 | 3 tie is left to `prefer`, as the committed tables of g g -> t tbar g g were built.)
+        tie = 0
+        if proc.npar >= 8 and 2 * worst == proc.npar:
+            big = next(w for w in g.adj[u] if size(w, u) == worst)
+            tie = 1 if 2 in legs_of(big, u) else 0
+        score = (worst, tie, prefer.get(g.kind[u][0], 0), u)
         if best is None or score < best[0]:
             best = (score, u)
     centre = best[1]

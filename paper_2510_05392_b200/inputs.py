@@ -45,6 +45,8 @@ PROCESSES = {
     "gg_ttxg": {"final": ["mT", "mT", 0.0], "nevt": 524288},
     "gg_ttxgg": {"final": ["mT", "mT", 0.0, 0.0], "nevt": 262144},
     "gg_ttxggg": {"final": ["mT", "mT", 0.0, 0.0, 0.0], "nevt": 65536},
+    # SURVEY.md §8(f) row 3 (Table 2 and Tables 5-8 of the paper; not a BASELINE.json config): batch size chosen here
+    "gg_ttxgggg": {"final": ["mT", "mT", 0.0, 0.0, 0.0, 0.0], "nevt": 4096},
 }
 
 
