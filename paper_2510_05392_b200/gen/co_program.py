@@ -23,8 +23,9 @@ Two exact rewritings of that sum (neither changes what is
   the per-helicity work of one jamp is a short sum of 4-component complex dot products and each jamp is
   complete when its loop ends -- no per-thread jamp array.
 
-Tables (all int32, see `Tables`): objects + terms (phase 1), per group of colour flows the pair objects
-+ terms (phase 2) and the dot-product entries (phase 3), the variant lookup, the leg sets.
+With 6 gluons a branch can hold 4 legs; such a colour-ordered object is itself factorised over the objects of its own
+branches (`_factorised_terms`).  The program is lowered to device tables by gen/hs_streams.py (tuned kernel, <= 5 gluons)
+and gen/hsg_tables.py (generic kernel).
 """
 from __future__ import annotations
 
@@ -361,128 +362,6 @@ class Program:
         return {"name": self.name, "objects": len(self.objs), "object_variants": ov, "groups": len(self.groups),
                 "xobjs_per_group_max": max(nx), "x_variants_per_group_max": max(xv), "dot_entries": ne,
                 "x_term_variants": nt, "obj_term_variants": sum(len(o.terms) << len(o.legs) for o in self.objs)}
-
-    # ---------------------------------------------------------------------------------------------
-    def tables(self):
-        """flatten to the int32 arrays read by csrc/hs_kernel.cu (layout documented in csrc/hs_tables.h)"""
-        npar = self.npar
-        # objects sorted by number of legs (phase 1 runs level by level); ids are remapped
-        order = sorted(range(len(self.objs)), key=lambda i: (len(self.objs[i].legs), i))
-        remap = {old: new for new, old in enumerate(order)}
-        objs = [self.objs[i] for i in order]
-        legsets, ls_id = [], {}
-
-        def lsid(legs):
-            if legs not in ls_id:
-                ls_id[legs] = len(legsets)
-                legsets.append(legs)
-            return ls_id[legs]
-
-        def subpos(parent, child):
-            """9-bit code p0 | p1<<3 | p2<<6: position in the parent's variant index of the j-th leg of the child
-            (7 = none: the parent variant has no such bit, so it reads as 0)"""
-            pos = [parent.index(p) for p in child]
-            assert len(pos) <= 3 and all(q < 7 for q in pos)
-            pos += [7] * (3 - len(pos))
-            return pos[0] | (pos[1] << 3) | (pos[2] << 6)
-
-        terms = []
-        pending = []          # (term index, argument slot, object id before remapping): offsets are filled in below
-
-        def add_terms(tl, parent_legs):
-            first = len(terms)
-            for t in tl:
-                if t.op.startswith("ext"):
-                    terms.append([OPS[t.op] | ((1 if t.sign < 0 else 0) << 8), t.args[0], 0, 0])
-                    continue
-                ls = [lsid(self.objs[x].legs) for x in t.args]
-                assert all(l < 256 for l in ls)
-                w = [OPS[t.op] | ((1 if t.sign < 0 else 0) << 8) | (ls[0] << 16) | (ls[1] << 24), 0, 0, 0]
-                for k, x in enumerate(t.args):
-                    w[1 + k] = subpos(parent_legs, self.objs[x].legs) << 16
-                    pending.append((len(terms), 1 + k, x))
-                terms.append(w)
-            return first, len(tl)
-
-        obj_tab, off = [], 0
-        for o in objs:
-            t0, nt = add_terms(o.terms, o.legs)
-            o_off = off
-            off += 4 << len(o.legs)
-            obj_tab.append([o_off, len(o.legs) | (lsid(o.legs) << 8), t0, nt])
-        obj_area = off                                        # complex numbers
-        obj_off = {o.id: obj_tab[i][0] for i, o in enumerate(objs)}
-        # phase-1 items per level
-        p1_items, p1_level = [], [0]
-        for lvl in (1, 2, 3):
-            for i, o in enumerate(objs):
-                if len(o.legs) == lvl:
-                    p1_items += [(i << 8) | v for v in range(1 << lvl)]
-            p1_level.append(len(p1_items))
-        # groups
-        vrows, vrow_id, hdep = [], {}, []
-
-        def vrow(xlegs):
-            if xlegs not in vrow_id:
-                ylegs = tuple(p for p in range(npar) if p not in xlegs)
-                # phase 3 on the FP64 tensor path: swizzled accumulator index of (x variant, y variant) = hdep_x ^ hdep_y
-                dep = lambda v, legs: sum(((v >> j) & 1) << (npar - 1 - p) for j, p in enumerate(legs))
-                hdep.append([acc_swizzle(dep(v, xlegs)) if v < (1 << len(xlegs)) else 0 for v in range(32)] +
-                            [acc_swizzle(dep(v, ylegs)) if v < (1 << len(ylegs)) else 0 for v in range(8)])
-                row = []
-                for h in range(1 << npar):
-                    hb = [(h >> (npar - 1 - p)) & 1 for p in range(npar)]
-                    vx = sum(hb[p] << j for j, p in enumerate(xlegs))
-                    vy = sum(hb[p] << j for j, p in enumerate(ylegs))
-                    row.append(vx | (vy << 8))
-                vrow_id[xlegs] = len(vrows)
-                vrows.append(row)
-            return vrow_id[xlegs]
-
-        grp_tab, x_tab, x_items, sig_tab, ent_tab = [], [], [], [], []
-        stage_max = 0
-        for g in self.groups:
-            x0, xi0, s0 = len(x_tab), len(x_items), len(sig_tab)
-            soff, slots = 0, []
-            for k, x in enumerate(g["xobjs"]):
-                t0, nt = add_terms(x["terms"], x["legs"])
-                slots.append(soff)
-                x_tab.append([soff, len(x["legs"]), t0, nt])
-                soff += 4 << len(x["legs"])
-            stage_max = max(stage_max, soff)
-            # phase-2 work units: 32 lanes = 32 (pair object, variant) items whose term lists have the same shape, so
-            # that a warp runs them in lockstep; units are handed out dynamically, most expensive first
-            sig = lambda x: (-(1 << len(x["legs"])), -len(x["terms"]), tuple(t.op for t in x["terms"]))
-            flat = []
-            for k in sorted(range(len(g["xobjs"])), key=lambda k: sig(g["xobjs"][k])):
-                flat += [((k << 8) | v, len(g["xobjs"][k]["terms"])) for v in range(1 << len(g["xobjs"][k]["legs"]))]
-            units = [flat[i:i + 32] for i in range(0, len(flat), 32)]
-            units.sort(key=lambda u: -max(c for _, c in u))
-            for u in units:
-                x_items += [it for it, _ in u] + [-1] * (32 - len(u))
-            for j in g["sigmas"]:
-                e0 = len(ent_tab)
-                for xs, yo, sign in g["entries"][j]:
-                    x = g["xobjs"][xs]
-                    y = objs[remap[yo]]
-                    ent_tab.append([slots[xs] | ((1 << len(x["legs"])) << 16),
-                                    obj_tab[remap[yo]][0] | ((1 << len(y.legs)) << 16), vrow(x["legs"]), sign])
-                sig_tab.append([j, e0, len(ent_tab) - e0, 0])
-            grp_tab.append([x0, xi0, len(x_items) - xi0, s0, len(sig_tab) - s0, 0, 0, 0])
-        for ti, slot_, x in pending:                          # argument offsets inside the object area
-            terms[ti][slot_] |= obj_off[x]
-        ls_mask = [sum(1 << p for p in legs) for legs in legsets]
-        i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w) if len(a) else np.zeros((0, w), np.int32)
-        return {
-            "npar": npar, "ncolor": self.ncolor, "obj_area": obj_area, "stage_area": stage_max,
-            "nobj": len(objs), "nlegsets": len(legsets), "ngroups": len(grp_tab),
-            "obj": i32(obj_tab, 4), "term": i32(terms, 4), "p1_items": np.asarray(p1_items, np.int32),
-            "p1_level": np.asarray(p1_level, np.int32), "legset_mask": np.asarray(ls_mask, np.int32),
-            "group": i32(grp_tab, 8), "xobj": i32(x_tab, 4), "x_items": np.asarray(x_items, np.int32),
-            "sigma": i32(sig_tab, 4), "entry": i32(ent_tab, 4),
-            "vtab": np.asarray(vrows, np.int32).astype(np.uint16).reshape(-1, 1 << npar),
-            "hdep": np.asarray(hdep, np.int32).astype(np.uint8).reshape(-1, 40),
-        }
 
 
 _CACHE = {}

@@ -1,0 +1,108 @@
+"""numpy interpreter of the tables of the generic helicity-shared kernel (gen/hsg_tables.py) -- CPU TEST HELPER.
+
+Executes what one CTA of csrc/hsg_kernel.cu executes for one event from the same packed tables (objects, pair objects,
+entries, variant lookup); every opcode is restated with the plain gamma-matrix helpers of tests/ir_eval.py.  So the
+generator's factorisation at 6 gluons (4-leg colour-ordered objects, the X.Y split and its signs, the packing) is checked
+against the oracle on CPU before any kernel runs.  Not product, not oracle; nothing here is imported by the package.
+"""
+import numpy as np
+
+import ir_eval as ir
+
+G = ir.G
+
+
+def _sub(v, code):
+    return sum(((v >> ((code >> (3 * j)) & 7)) & 1) << j for j in range(4))
+
+
+def _x_term(op, A, B, Z, kA, kB):
+    if op == 8:
+        return A @ ir.slash(B)
+    if op == 9:
+        return ir.slash(A) @ B
+    if op == 10:
+        return np.array([A @ ir.GAM[mu] @ B for mu in range(4)])
+    if op == 11:
+        return ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A
+    if op == 12:
+        return ir.mdot(A, Z) * B - ir.mdot(B, Z) * A
+    if op == 13:
+        return 2 * ir.mdot(A, Z) * B - ir.mdot(B, Z) * A - ir.mdot(A, B) * Z
+    raise ValueError(op)
+
+
+def evaluate(T, mom, mt, wt):
+    """jamps[ncolor][2^npar] (without the g^n factor) of one event"""
+    npar = T["npar"]
+    k = [mom[i] * (1 if i < 2 else -1) for i in range(npar)]
+    K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
+    area = np.full((T["nslot"], 4), np.nan + 0j, dtype=complex)
+
+    def arg(w, var):
+        return area[(w & 0xFFFF) + _sub(var, (w >> 16) & 0xFFF)]
+
+    for it in T["p1_items"]:
+        o, var = int(it) >> 8, int(it) & 0xFF
+        slot0, info, t0, nt = (int(x) for x in T["obj"][o])
+        kout = K[info >> 8]
+        acc = np.zeros(4, dtype=complex)
+        for t in T["term"][t0:t0 + nt]:
+            w0, w1, w2, w3 = (int(x) & 0xFFFFFFFF for x in t)
+            op, neg = w0 & 0xFF, (w0 >> 8) & 1
+            hel = 1 if var & 1 else -1
+            if op == 0:
+                e = ir.polvec(mom[w1], hel)
+                r = e if w1 < 2 else e.conj()
+            elif op == 1:
+                r = ir.u_spinor(mom[2], mt, hel).conj() @ ir.GAM[0]
+            elif op == 2:
+                r = ir.v_spinor(mom[3], mt, hel)
+            else:
+                A, B = arg(w1, var), arg(w2, var)
+                kA, kB = K[(w0 >> 16) & 0xFF], K[(w0 >> 24) & 0xFF]
+                if op == 3:
+                    r = (ir.mdot(A, B) * (kA - kB) + ir.mdot(2 * kB + kA, A) * B - ir.mdot(2 * kA + kB, B) * A) / ir.mdot(kout, kout)
+                elif op == 4:
+                    Z = arg(w3, var)
+                    r = (ir.mdot(A, Z) * B - ir.mdot(B, Z) * A) / ir.mdot(kout, kout)
+                elif op == 5:
+                    q = -kout
+                    r = A @ ir.slash(B) @ (ir.slash(q) + mt * np.eye(4)) / (ir.mdot(q, q) - mt * mt + 1j * mt * wt)
+                elif op == 6:
+                    q = kout
+                    r = (ir.slash(q) + mt * np.eye(4)) @ ir.slash(A) @ B / (ir.mdot(q, q) - mt * mt + 1j * mt * wt)
+                elif op == 7:
+                    r = np.array([A @ ir.GAM[mu] @ B for mu in range(4)]) / ir.mdot(kout, kout)
+                else:
+                    raise ValueError(op)
+            acc = acc + (-r if neg else r)
+        assert np.isnan(area[slot0 + var]).all()
+        area[slot0 + var] = acc
+
+    for a, b in T["xitem"]:
+        a, b = int(a) & 0xFFFFFFFF, int(b) & 0xFFFFFFFF
+        t0, nt = a & 0xFFFFFF, a >> 24
+        slot, var, vec = b & 0xFFFFF, (b >> 20) & 0xFF, (b >> 28) & 1
+        acc = np.zeros(4, dtype=complex)
+        for t in T["term"][t0:t0 + nt]:
+            w0, w1, w2, w3 = (int(x) & 0xFFFFFFFF for x in t)
+            op, neg = w0 & 0xFF, (w0 >> 8) & 1
+            A, B = arg(w1, var), arg(w2, var)
+            Z = arg(w3, var) if op in (12, 13) else None
+            r = _x_term(op, A, B, Z, K[(w0 >> 16) & 0xFF], K[(w0 >> 24) & 0xFF])
+            assert (op >= 10) == bool(vec)
+            acc = acc + (-r if neg else r)
+        assert np.isnan(area[slot]).all()
+        area[slot] = G * acc if vec else acc
+    assert not np.isnan(area).any()
+
+    nh = 1 << npar
+    J = np.zeros((T["ncolor"], nh), dtype=complex)
+    for j, e0, ne, _ in T["flow"]:
+        for xs, ys, row, sign in T["entry"][e0:e0 + ne]:
+            vt = T["vtab"][row].astype(np.int64)
+            X = area[int(xs) + (vt & 0xFF)]
+            Y = area[int(ys) + (vt >> 8)]
+            J[j] += int(sign) * np.sum(X * Y, axis=1)
+    return J

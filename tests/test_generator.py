@@ -112,3 +112,21 @@ def test_helicity_shared_streams_match_oracle(name, n, nev, params):
         J = hs_eval.evaluate(T, p[e], params["mT"], params["wT"])
         mh = np.einsum("ih,ij,jh->h", J.conj(), C, J).real * gs ** (2 * n) / oracle.DENOM[name]
         assert np.abs(mh / mh_o[e] - 1).max() < 1e-10
+
+
+@pytest.mark.parametrize("name,n", [("gg_ttxgg", 4), ("gg_ttxggg", 5), ("gg_ttxgggg", 6)])
+def test_generic_tables_match_oracle(name, n, params):
+    """the tables of the generic helicity-shared kernel (gen/hsg_tables.py; the program of g g -> t tbar g g g g with its
+    4-leg colour-ordered objects, Table 2 at PAPER.md:180-187), interpreted by tests/hsg_eval.py, give the oracle's
+    per-helicity colour-summed |M|^2 for EVERY helicity (colour matrix: the oracle's, brute force)"""
+    import hsg_eval
+    from paper_2510_05392_b200.gen import hsg_tables
+    T = hsg_tables.tables(n)
+    assert T["ncolor"] == math.factorial(n) and len(T["flow"]) == T["ncolor"]
+    C = oracle.color_matrix(n)
+    gs = math.sqrt(4 * math.pi * params["aS"])
+    p = inputs.momenta(name, 1, seed=7)
+    _, mh_o = oracle.matrix_elements(name, p, params, per_helicity=True)
+    J = hsg_eval.evaluate(T, p[0], params["mT"], params["wT"])
+    mh = np.einsum("ih,ij,jh->h", J.conj(), C, J).real * gs ** (2 * n) / oracle.DENOM[name]
+    assert np.abs(mh / mh_o[0] - 1).max() < 1e-9
