@@ -153,7 +153,7 @@ class Process:
 
     def helicity_filter(self, d_momenta, nprobe=None):
         nevt = d_momenta.shape[0]
-        nprobe = min(nevt, 1024) if nprobe is None else nprobe
+        nprobe = min(nevt, self.get_option("probe_events")) if nprobe is None else nprobe
         ws = self._workspace(max(nevt, nprobe))
         mask = (ctypes.c_ubyte * self.ncomb)()
         ng = ctypes.c_int()

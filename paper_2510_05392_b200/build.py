@@ -61,9 +61,10 @@ def _compile(src, verbose):
 
 
 def build(verbose: bool = False, jobs: int | None = None) -> str:
-    from .gen import emit_cuda, emit_hs
+    from .gen import emit_cuda, emit_hs, emit_hsg
     emit_cuda.generate_all(GEN)
     emit_hs.emit(GEN)
+    emit_hsg.emit(GEN)
     os.makedirs(OBJ, exist_ok=True)
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(GEN, "*.cu")))
     # biggest first

@@ -10,12 +10,14 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
 #include "../../include/mg5_b200.h"
 #include "color_sum.cuh"
 #include "hs_kernel.cuh"
+#include "hsg_kernel.cuh"
 #include "mg_internal.cuh"
 
 using namespace mg;
@@ -50,6 +52,7 @@ struct mg_process {
     long epoch = 0;            // bumped by every call that changes what a batch launches
     int graph_replays = 0;
     HsContext* hs = nullptr;   // helicity-shared program (gg processes)
+    HsgContext* hsg = nullptr; // generic helicity-shared kernel (g g -> t tbar g g g g: the only diagram kernel it has)
     int* d_pos = nullptr;      // DEVICE [ncomb]: position of helicity h in the good list, -1 = not good
     long jamp_chunk_bytes = 16L << 30;     // one chunk for every BASELINE.json batch (180 GB of HBM3e); smaller via "jamp_chunk_mib"
     // good helicities
@@ -108,6 +111,53 @@ static double make_norm(const mg_process* p)
     return pow(g2, p->d->coupling_order) / (p->d->denom * p->d->cden);
 }
 
+// g g -> t tbar g g g g (Table 2): no thread-per-(event, helicity) kernel (launch =
+// NULL), the generic helicity-shared kernel only.  The colour matrix is expanded from its first row:
+// C[s][s'] = row0[rank(s^-1 o s')], permutations in lexicographic order (gen/colour.py colour_matrix).
+static const ProcessDesc* desc_gg_ttxgggg()
+{
+    static ProcessDesc d;
+    static std::vector<int> cmat;
+    static bool done = false;
+    if (done) return &d;
+    const HsgTables* t = hsg_tables(6);
+    if (!t) return nullptr;
+    const int n = 6, np = t->ncolor;
+    std::vector<std::vector<int>> perms;
+    std::vector<int> a(n);
+    for (int i = 0; i < n; i++) a[i] = i;
+    do perms.push_back(a); while (std::next_permutation(a.begin(), a.end()));
+    auto rank = [&](const std::vector<int>& q) {            // lexicographic rank
+        int r = 0;
+        for (int i = 0; i < n; i++) {
+            int smaller = 0;
+            for (int j = i + 1; j < n; j++) smaller += q[j] < q[i];
+            int f = 1;
+            for (int k = 2; k <= n - 1 - i; k++) f *= k;
+            r += smaller * f;
+        }
+        return r;
+    };
+    cmat.assign((size_t)np * np, 0);
+    for (int i = 0; i < np; i++) {
+        int inv[6];
+        for (int pos = 0; pos < n; pos++) inv[perms[i][pos]] = pos;
+        for (int j = 0; j < np; j++) {
+            std::vector<int> rel(n);
+            for (int pos = 0; pos < n; pos++) rel[pos] = inv[perms[j][pos]];
+            cmat[(size_t)i * np + j] = t->cmat_row0[rank(rel)];
+        }
+    }
+    d.name = "gg_ttxgggg"; d.ngluon = 6; d.npar = 8; d.ncomb = 256; d.ncolor = np; d.ndiagrams = t->ndiagrams;
+    d.namps = 0; d.ncurrents = t->nobj; d.ngroups = 1;
+    d.denom = 256.0 * 24.0;            // 2*2 spins, 8*8 colours of the beams, 4! identical final gluons (reading A3)
+    d.cden = t->cden; d.cmat = cmat.data();
+    d.flops = (t->flops_p1 + t->flops_p2) / 256.0 + t->flops_p3;
+    d.coupling_order = 6; d.has_fp32 = false; d.launch = nullptr;
+    done = true;
+    return &d;
+}
+
 extern "C" const char* mg_last_error(const mg_process* p) { return p ? p->err.c_str() : g_init_error.c_str(); }
 
 static int upload_tables(mg_process* p)
@@ -130,7 +180,12 @@ static int upload_tables(mg_process* p)
         CUDA_TRY(p, cudaMemcpy(p->d_cmat64, h64.data(), n2 * sizeof(double), cudaMemcpyHostToDevice));
     }
     if (p->precision == MG_FP64) p->d_cmat64 = p->d_cmat;
-    if (p->precision == MG_FP64) {
+    if (p->precision == MG_FP64 && d->ncolor > 128) {
+        std::vector<double> frag; int rank = 0;
+        if (!color_cholesky_big(d->ncolor, d->cmat, frag, &rank)) return fail(p, MG_ESTATE, "colour matrix is not positive semi-definite");
+        CUDA_TRY(p, cudaMalloc(&p->d_chol, frag.size() * sizeof(double)));
+        CUDA_TRY(p, cudaMemcpy(p->d_chol, frag.data(), frag.size() * sizeof(double), cudaMemcpyHostToDevice));
+    } else if (p->precision == MG_FP64) {
         std::vector<double> lp; int ncp = 0;
         if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
         std::vector<double> frag;
@@ -165,7 +220,11 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     else if (!strcmp(name, "gg_ttxg")) d = desc_gg_ttxg();
     else if (!strcmp(name, "gg_ttxgg")) d = desc_gg_ttxgg();
     else if (!strcmp(name, "gg_ttxggg")) d = desc_gg_ttxggg();
+    else if (!strcmp(name, "gg_ttxgggg")) d = desc_gg_ttxgggg();
     else return fail(nullptr, MG_EINVAL, std::string("unknown process ") + name);
+    if (!d) return fail(nullptr, MG_EINVAL, std::string("library built without ") + name);
+    if (!d->launch && precision != MG_FP64)
+        return fail(nullptr, MG_EINVAL, std::string(name) + " runs in MG_FP64 only (generic helicity-shared kernel + DMMA colour sum)");
     if (precision == MG_FP32 && !d->has_fp32)
         return fail(nullptr, MG_EINVAL, std::string("library built without the MG_FP32 instantiation of ") + name);
     int ndev = 0;
@@ -183,7 +242,11 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     p->d = d; p->precision = precision; p->device = device;
     int rc = upload_tables(p);
     if (rc != MG_OK) { g_init_error = p->err; mg_destroy(p); return rc; }
-    if (hs_tables(d->ngluon) && precision != MG_FP32) {       // helicity-shared program: g g -> t tbar + >= 2 g
+    if (!d->launch) {                                         // the generic helicity-shared kernel is the only diagram kernel
+        cudaError_t e = hsg_create(d->ngluon, &p->hsg);
+        if (e != cudaSuccess) { g_init_error = std::string("hsg_create: ") + cudaGetErrorString(e); mg_destroy(p); return e == cudaErrorMemoryAllocation ? MG_ENOMEM : MG_ECUDA; }
+        p->diagrams = MG_DIAG_SHARED;
+    } else if (hs_tables(d->ngluon) && precision != MG_FP32) {       // helicity-shared program: g g -> t tbar + >= 2 g
         cudaError_t e = hs_create(d->ngluon, &p->hs);
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
         p->diagrams = MG_DIAG_SHARED;                         // measured default, see DESIGN.md
@@ -198,6 +261,7 @@ extern "C" void mg_destroy(mg_process* p)
     if (!p) return;
     cudaSetDevice(p->device);
     hs_destroy(p->hs);
+    hsg_destroy(p->hsg);
     cudaFree(p->d_pos);
     if (p->d_cmat64 != p->d_cmat) cudaFree(p->d_cmat64);
     cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat); cudaFree(p->d_chol);
@@ -229,7 +293,10 @@ extern "C" int mg_process_flops(const mg_process* p, double* diagram_flops, doub
     if (!p) return MG_EINVAL;
     if (diagram_flops) {
         *diagram_flops = p->d->flops;
-        if (p->diagrams == MG_DIAG_SHARED && p->hs) {
+        if (p->hsg) {
+            const HsgTables* t = hsg_host_tables(p->hsg);
+            *diagram_flops = (t->flops_p1 + t->flops_p2) / p->d->ncomb + t->flops_p3;
+        } else if (p->diagrams == MG_DIAG_SHARED && p->hs) {
             const HsTables* t = hs_host_tables(p->hs);
             *diagram_flops = (t->flops_p1 + t->flops_p2) / p->d->ncomb + t->flops_p3;
         }
@@ -279,7 +346,8 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         p->block = value;
     } else if (!strcmp(key, "diagrams")) {
         if (value != MG_DIAG_THREAD && value != MG_DIAG_SHARED) return fail(p, MG_EINVAL, "bad diagrams");
-        if (value == MG_DIAG_SHARED && !p->hs) return fail(p, MG_EINVAL, "this process/precision has no helicity-shared program");
+        if (value == MG_DIAG_THREAD && !p->d->launch) return fail(p, MG_EINVAL, "this process has the helicity-shared kernel only");
+        if (value == MG_DIAG_SHARED && !p->hs && !p->hsg) return fail(p, MG_EINVAL, "this process/precision has no helicity-shared program");
         if (value == MG_DIAG_SHARED && p->schedule == MG_SCHED_STREAMS)
             return fail(p, MG_EINVAL, "the helicity-shared kernel has no helicity streams (set schedule = 0 first)");
         p->diagrams = value;
@@ -316,6 +384,7 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "max_streams")) *value = p->max_streams;
     else if (!strcmp(key, "graph")) *value = p->graph;
     else if (!strcmp(key, "graph_replays")) *value = p->graph_replays;
+    else if (!strcmp(key, "probe_events")) *value = p->d->launch ? 1024 : 16;      // events the automatic helicity filter uses at most
     else return MG_EINVAL;
     return MG_OK;
 }
@@ -347,12 +416,26 @@ static size_t ws_bytes_for(const mg_process* p, int nevt, int nhel, bool need_ja
     return b;
 }
 
+// events of the first batch the helicity filter looks at (the generic kernel's probe goes through the jamps buffer:
+// 2.9 MB per event at 6 gluons)
+static int probe_events(const mg_process* p, int nevt)
+{
+    const int cap = p->d->launch ? 1024 : 16;
+    return nevt < cap ? nevt : cap;
+}
+
+static size_t filter_bytes(const mg_process* p, int nprobe)
+{
+    size_t b = align256((size_t)p->d->ncomb * nprobe * sizeof(double));                           // filter uses FUSED
+    if (!p->d->launch) b += align256(color_sum_padded_rows((long)p->d->ncomb * nprobe) * p->d->ncolor * 2 * sizeof(double));
+    return b;
+}
+
 static size_t workspace_bytes(const mg_process* p, int nevt, bool need_jamps)
 {
     if (!p || nevt < 0) return 0;
-    const int nprobe = nevt < 1024 ? nevt : 1024;
     size_t a = ws_bytes_for(p, nevt, p->good.empty() ? p->d->ncomb : (int)p->good.size(), need_jamps);
-    size_t b = p->good.empty() ? align256((size_t)p->d->ncomb * nprobe * sizeof(double)) : 0;   // filter uses FUSED
+    size_t b = p->good.empty() ? filter_bytes(p, probe_events(p, nevt)) : 0;
     return a > b ? a : b;
 }
 
@@ -509,13 +592,26 @@ extern "C" int mg_helicity_filter(mg_process* p, const double* d_momenta, int np
     if (!p || !d_momenta || nprobe <= 0 || !d_workspace) return fail(p, MG_EINVAL, "bad arguments");
     const int ncomb = p->d->ncomb;
     const size_t need = (size_t)ncomb * nprobe * sizeof(double);
-    if (ws_bytes < need) return fail(p, MG_EINVAL, "workspace too small for the helicity filter");
+    if (ws_bytes < filter_bytes(p, nprobe)) return fail(p, MG_EINVAL, "workspace too small for the helicity filter");
     CUDA_TRY(p, cudaSetDevice(p->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    DiagLaunch a = base_launch(p, d_momenta, nprobe);
-    a.d_hel = p->d_all; a.hel_base = 0; a.nhel = ncomb; a.d_meh = (double*)d_workspace; a.mode = MG_CS_FUSED;
-    a.d_cmat = p->d_cmat64;
-    CUDA_TRY(p, p->d->launch(MG_FP64, a, st));          // both sides decide in fp64 whatever the handle's precision (reading A5)
+    if (!p->d->launch) {
+        // generic helicity-shared kernel: every helicity combination is a row of its event (d_all = identity), then the
+        // colour sum over the probe's rows
+        const long rows = (long)ncomb * nprobe;
+        HsLaunch a;
+        a.mom = d_momenta; a.nevt = nprobe; a.d_pos = p->d_all; a.nrow_evt = ncomb;
+        a.d_jamps = (char*)d_workspace + align256(need); a.rows = color_sum_padded_rows(rows); a.mt = p->mT; a.wt = p->wT; a.tile_major = 0;
+        CUDA_TRY(p, hsg_launch(p->hsg, true, a, st));
+        RowMap map;
+        map.rows_valid = rows; map.hel_minor = ncomb; map.evt_stride = nprobe; map.e0 = 0; map.norm = make_norm(p);
+        CUDA_TRY(p, color_sum_tensor(true, p->d->ncolor, p->d_cmat, p->d_chol, a.d_jamps, a.rows, map, (double*)d_workspace, st));
+    } else {
+        DiagLaunch a = base_launch(p, d_momenta, nprobe);
+        a.d_hel = p->d_all; a.hel_base = 0; a.nhel = ncomb; a.d_meh = (double*)d_workspace; a.mode = MG_CS_FUSED;
+        a.d_cmat = p->d_cmat64;
+        CUDA_TRY(p, p->d->launch(MG_FP64, a, st));      // both sides decide in fp64 whatever the handle's precision (reading A5)
+    }
     std::vector<double> h(need / sizeof(double));
     CUDA_TRY(p, cudaMemcpyAsync(h.data(), d_workspace, need, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(p, cudaStreamSynchronize(st));
@@ -606,7 +702,7 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
     const bool want_col = ex.selcol != nullptr && p->d->ncolor > 1;
     if (ws_bytes < workspace_bytes(p, nevt, want_col)) return fail(p, MG_EINVAL, "workspace too small");
     if (p->good.empty()) {
-        const int nprobe = nevt < 1024 ? nevt : 1024;
+        const int nprobe = probe_events(p, nevt);
         int rc = mg_helicity_filter(p, d_momenta, nprobe, d_workspace, ws_bytes, cuda_stream, nullptr, nullptr);
         if (rc != MG_OK) return rc;
         if (ws_bytes < workspace_bytes(p, nevt, want_col)) return fail(p, MG_EINVAL, "workspace too small");
@@ -639,7 +735,8 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
             //  low term of the jamps; needs chunks of 24 colours)
             const int tile_major = p->precision != MG_FP64 && !p->hs_color_alu ? (p->d->ncolor % 24 == 0 && p->tf32_direct ? 2 : 1) : 0;
             a.tile_major = tile_major;
-            CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, st));
+            if (p->hsg) CUDA_TRY(p, hsg_launch(p->hsg, true, a, st));
+            else CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
             RowMap map;

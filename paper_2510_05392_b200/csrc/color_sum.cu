@@ -297,6 +297,122 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
     return true;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// DMMA kernel for a colour matrix that does not fit in shared memory (720 colours: g g -> t tbar g g g g, SURVEY.md §8(f)
+// row 3; PAPER.md:580-613 makes this contraction the point of the 2 -> 6 process).  Same triangular form Z = X L.
+//   - a CTA (16 warps) = 16 rows, their Re and Im parts: M = 32 = four m8 tiles; all 32 x NC accumulators stay in
+//     registers (NC / 8 n-tiles dealt to the warps in pairs (j, NC/8 - 1 - j): equal numbers of k-steps);
+//   - the jamps stream through a 3-stage cp.async ring of [16 colours][32] chunks (row stride 40 doubles: the A-fragment
+//     reads fall into distinct bank pairs); every A fragment serves all n-tiles of the warp;
+//   - the factor is read from global memory (L2-resident: 4 MB) in FRAGMENT order, one coalesced 256-byte read per
+//     (k-step, n-tile) and warp: element [lane] = L[4 ks + lane % 4][8 j + lane / 4]; blocks above the diagonal are skipped.
+// C is only positive SEMI-definite at 6 gluons (rank 685 of 720): the factor has zero columns there (color_cholesky_big).
+template <int NC>
+__global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __restrict__ Lf, const double* __restrict__ X,
+                                                               long rows_padded, RowMap map, double* __restrict__ meh)
+{
+    static_assert(NC % 16 == 0, "chunks of 16 colours");
+    constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 16, NCHUNK = NC / KC, STG = 3, STRIDE = 40;
+    constexpr int SLOTS = 2 * ((NPAIR + 15) / 16);
+    __shared__ __align__(16) double js[STG][KC][STRIDE];
+    __shared__ double red[16][32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long r0 = (long)blockIdx.x * 16;
+    // chunk loader: thread t < 256 copies 16 bytes: colour t / 16, part (t / 8) % 2, rows 2 (t % 8) ..
+    auto load_chunk = [&](int c) {
+        if (c < NCHUNK && tid < 256) {
+            const int k = tid >> 4, part = (tid >> 3) & 1, q = tid & 7;
+            const double* src = X + ((long)part * NC + c * KC + k) * rows_padded + r0 + 2 * q;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&js[c % STG][k][part * 16 + 2 * q]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+        }
+        asm volatile("cp.async.commit_group;");
+    };
+    double acc[SLOTS][4][2];
+#pragma unroll
+    for (int s = 0; s < SLOTS; s++)
+#pragma unroll
+        for (int m = 0; m < 4; m++) acc[s][m][0] = acc[s][m][1] = 0.0;
+    load_chunk(0);
+    load_chunk(1);
+    const int ak = lane & 3, ar = lane >> 2;
+#pragma unroll 1
+    for (int c = 0; c < NCHUNK; c++) {
+        asm volatile("cp.async.wait_group 1;");
+        __syncthreads();
+        load_chunk(c + 2);
+        const double (*jt)[STRIDE] = js[c % STG];
+#pragma unroll
+        for (int kk = 0; kk < KC / 4; kk++) {
+            const int ks = c * (KC / 4) + kk;
+            double a[4];
+#pragma unroll
+            for (int m = 0; m < 4; m++) a[m] = jt[4 * kk + ak][8 * m + ar];
+#pragma unroll
+            for (int s = 0; s < SLOTS; s++) {
+                const int pr = warp + 16 * (s >> 1);
+                const int j = (s & 1) ? NT8 - 1 - pr : pr;
+                if (pr < NPAIR && ks >= 2 * j) {
+                    const double b = __ldg(Lf + ((long)ks * NT8 + j) * 32 + lane);
+#pragma unroll
+                    for (int m = 0; m < 4; m++) dmma(acc[s][m][0], acc[s][m][1], a[m], b);
+                }
+            }
+        }
+    }
+    // sum of squares per m-row: lanes of a quad hold the 8 columns of a row
+#pragma unroll
+    for (int m = 0; m < 4; m++) {
+        double v = 0.0;
+#pragma unroll
+        for (int s = 0; s < SLOTS; s++) v += acc[s][m][0] * acc[s][m][0] + acc[s][m][1] * acc[s][m][1];
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        if (ak == 0) red[warp][8 * m + ar] = v;
+    }
+    __syncthreads();
+    if (tid < 16) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < 16; w++) v += red[w][tid] + red[w][16 + tid];       // Re part + Im part of the row
+        map.store(meh, r0 + tid, v);
+    }
+}
+
+// host: factor of a positive SEMI-definite integer matrix in the fragment order of color_sum_big_kernel (full rectangle of
+// (k-step, n-tile) blocks).  A pivot that vanishes (relative to its diagonal element) gives a zero column; the rest of that
+// column must vanish too (it does for a semi-definite matrix), else false.
+bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, int* rank_out)
+{
+    if (ncolor % 16) return false;
+    const int n = ncolor;
+    std::vector<long double> l((size_t)n * n, 0.0L);
+    std::vector<char> null(n, 0);
+    int rank = 0;
+    for (int j = 0; j < n; j++) {
+        long double s = cmat[(size_t)j * n + j];
+        for (int k = 0; k < j; k++) s -= l[(size_t)j * n + k] * l[(size_t)j * n + k];
+        const long double tol = 1e-10L * cmat[(size_t)j * n + j];
+        if (s < -tol) return false;
+        if (s <= tol) null[j] = 1; else { l[(size_t)j * n + j] = sqrtl(s); rank++; }
+        for (int i = j + 1; i < n; i++) {
+            long double t = cmat[(size_t)i * n + j];
+            for (int k = 0; k < j; k++) t -= l[(size_t)i * n + k] * l[(size_t)j * n + k];
+            if (null[j]) { if (fabsl(t) > 1e-8L * cmat[(size_t)j * n + j]) return false; }
+            else l[(size_t)i * n + j] = t / l[(size_t)j * n + j];
+        }
+    }
+    frag.assign((size_t)(n / 4) * (n / 8) * 32, 0.0);
+    for (int ks = 0; ks < n / 4; ks++)
+        for (int j = 0; j < n / 8; j++)
+            for (int lane = 0; lane < 32; lane++) {
+                const int k = 4 * ks + lane % 4, c = 8 * j + lane / 4;
+                if (k >= c) frag[((size_t)ks * (n / 8) + j) * 32 + lane] = (double)l[(size_t)k * n + c];
+            }
+    if (rank_out) *rank_out = rank;
+    return true;
+}
+
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
                            double* d_meh, cudaStream_t st, int tile_major);
 
@@ -307,6 +423,10 @@ cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const
     if (tile_major) return cudaErrorInvalidValue;
     if (!d_factor) return cudaErrorInvalidValue;
     const double* d_chol = (const double*)d_factor;
+    if (ncolor == 720) {            // d_factor: the fragment-order factor of color_cholesky_big
+        color_sum_big_kernel<720><<<(unsigned)(rows_padded / 16), 512, 0, st>>>(d_chol, (const double*)d_jamps, rows_padded, map, d_meh);
+        return cudaGetLastError();
+    }
     const int ncp = (ncolor + 7) / 8 * 8;
     const int warps = 4;
     const unsigned grid = (unsigned)((rows_padded / 8 + warps - 1) / warps);

@@ -49,6 +49,9 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 // color_sum_tensor as d_factor in MG_FP64 is lp followed by frag
 void color_cholesky_fragments(int ncp, const std::vector<double>& lp, std::vector<double>& frag);
 
+// host: factor of the (positive semi-definite) 720 x 720 matrix in the fragment order of the large-matrix DMMA kernel
+bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, int* rank_out);
+
 // host: two-term TF32 image [hi | lo] of the Cholesky factor in the tcgen05 shared-memory layout (color_sum_tf32.cu)
 bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img);
 

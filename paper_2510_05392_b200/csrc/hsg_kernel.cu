@@ -1,0 +1,268 @@
+// hsg_kernel.cu -- GENERIC helicity-shared diagram kernel (g g -> t tbar g g g g; Table 2,
+// 15 495 diagrams, 720 colour flows, 256 helicities).  Interprets the tables of gen/hsg_tables.py.
+//
+// Same three phases as the tuned kernel of the smaller processes (hs_kernel.cu): colour-ordered objects of <= 4 legs, every
+// helicity variant of their own legs once per event (phase 1); pair objects X = vertex contracted with all branches but the
+// largest, Y (phase 2); jamp[sigma][h] = sum over entries of +- sum_c X_c[variant_x(h)] Y_c[variant_y(h)] (phase 3, thread =
+// helicity combination).  What changes at this size: one event holds 5 984 object variants (383 KB) and 43 680 pair-object
+// variants (2.8 MB) -- they cannot live in shared memory.  Each (persistent) CTA owns a scratch area in GLOBAL memory, written
+// and re-read through L1/L2 by the same CTA: the paper's hand-off between diagram-group kernels through global memory
+// (PAPER.md:424-444), but inside one kernel and with barriers instead of kernel boundaries.  All pair objects of an event are
+// built once (one group of colour flows), so phase 3 runs the 720 flows without a barrier between them.
+//
+// Scratch layout: four component planes, byte(c, slot) = c * 16 * nslot + 16 * slot, so that the lanes of a warp (consecutive
+// variants) read consecutive 16-byte words of one plane.
+#include <stdint.h>
+
+#include "helas.cuh"
+#include "hsg_kernel.cuh"
+
+namespace mg {
+
+struct HsgDev {
+    const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
+    const int2* xitem; const int4* entry; const int4* flow; const unsigned short* vtab;
+    int npar, ncolor, nslot, nlegsets, nxitem, nflow, nlevel;
+    int p1_level[8];
+};
+
+static constexpr int HSG_THREADS = 256;
+
+__device__ __forceinline__ int sub_variant4(int var, int code)
+{
+    return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2) |
+           (((var >> ((code >> 9) & 7)) & 1) << 3);
+}
+
+__device__ __forceinline__ void ldw(const char* __restrict__ area, size_t plane, int slot, wf<double>& w)
+{
+#pragma unroll
+    for (int c = 0; c < 4; c++) {
+        const double2 v = *reinterpret_cast<const double2*>(area + c * plane + 16 * (size_t)slot);
+        w.c[c].re = v.x; w.c[c].im = v.y;
+    }
+}
+
+__device__ __forceinline__ void stw(char* __restrict__ area, size_t plane, int slot, const wf<double>& w)
+{
+#pragma unroll
+    for (int c = 0; c < 4; c++) *reinterpret_cast<double2*>(area + c * plane + 16 * (size_t)slot) = make_double2(w.c[c].re, w.c[c].im);
+}
+
+__device__ __forceinline__ p4<double> ldk(const double* __restrict__ Ks, int ls)
+{
+    p4<double> k = { Ks[4 * ls], Ks[4 * ls + 1], Ks[4 * ls + 2], Ks[4 * ls + 3] };
+    return k;
+}
+
+__device__ __forceinline__ void axpy(double sg, const wf<double>& r, wf<double>& acc)
+{
+#pragma unroll
+    for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
+}
+
+// T2 = type of the jamps buffer
+template <typename T2>
+__global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgDev d, const HsLaunch a, char* __restrict__ scratch)
+{
+    extern __shared__ __align__(16) double smd[];
+    double* __restrict__ Ks = smd;                               // [nlegsets][4]
+    double* __restrict__ pm = smd + 4 * d.nlegsets;              // [npar][4]
+    const int tid = threadIdx.x, NT = HSG_THREADS;
+    const int npar = d.npar, nh = 1 << npar;
+    const size_t plane = 16 * (size_t)d.nslot;
+    char* __restrict__ area = scratch + (size_t)blockIdx.x * 4 * plane;
+    T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
+    auto arg = [&](int word, int var, wf<double>& w) { ldw(area, plane, (word & 0xFFFF) + sub_variant4(var, (word >> 16) & 0xFFF), w); };
+
+    for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
+        // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
+        for (int i = tid; i < 4 * npar; i += NT) pm[i] = a.mom[(size_t)e * (4 * npar) + i];
+        __syncthreads();
+        for (int s = tid; s < d.nlegsets; s += NT) {
+            const int m = __ldg(d.legset_mask + s);
+            double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
+            for (int p = 0; p < npar; p++)
+                if ((m >> p) & 1) {
+                    const double sg = p < 2 ? 1.0 : -1.0;
+                    k0 += sg * pm[4 * p]; k1 += sg * pm[4 * p + 1]; k2 += sg * pm[4 * p + 2]; k3 += sg * pm[4 * p + 3];
+                }
+            Ks[4 * s] = k0; Ks[4 * s + 1] = k1; Ks[4 * s + 2] = k2; Ks[4 * s + 3] = k3;
+        }
+        __syncthreads();
+        // phase 1: colour-ordered objects, level by level (an object of L legs reads objects of fewer legs only)
+        for (int lvl = 0; lvl < d.nlevel; lvl++) {
+            for (int i = d.p1_level[lvl] + tid; i < d.p1_level[lvl + 1]; i += NT) {
+                const int it = __ldg(d.p1_items + i);
+                const int4 o = __ldg(d.obj + (it >> 8));
+                const int var = it & 0xFF;
+                const p4<double> K = ldk(Ks, o.y >> 8);
+                wf<double> acc;
+#pragma unroll
+                for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
+                for (int t = 0; t < o.w; t++) {
+                    const int4 w = __ldg(d.term + o.z + t);
+                    const int op = w.x & 0xFF;
+                    wf<double> r;
+                    if (op <= 2) {
+                        const int hel = (var & 1) ? 1 : -1;
+                        const double* p = pm + 4 * w.y;
+                        if (op == 0) ext_eps(p, hel, w.y >= 2, r);
+                        else if (op == 1) ext_ubar(p, a.mt, hel, r);
+                        else ext_v(p, a.mt, hel, r);
+                    } else {
+                        wf<double> A, B;
+                        arg(w.y, var, A); arg(w.z, var, B);
+                        switch (op) {
+                            case 3: v3_off(A, ldk(Ks, (w.x >> 16) & 0xFF), B, ldk(Ks, (w.x >> 24) & 0xFF), 1.0 / m2(K), r); break;
+                            case 4: { wf<double> Z; arg(w.w, var, Z); v4_off(A, B, Z, 1.0 / m2(K), r); break; }
+                            case 5: ffv_l(A, B, -K, a.mt, inv_prop(m2(K), a.mt, a.wt), r); break;
+                            case 6: ffv_r(A, B, K, a.mt, inv_prop(m2(K), a.mt, a.wt), r); break;
+                            default: ffv_p(A, B, 1.0 / m2(K), r); break;       // 7
+                        }
+                    }
+                    axpy((w.x >> 8) & 1 ? -1.0 : 1.0, r, acc);
+                }
+                stw(area, plane, o.x + var, acc);
+            }
+            __syncthreads();
+        }
+        // phase 2: pair objects (raw vertices; vector-valued ones lowered at the store for the plain dot of phase 3)
+        for (int i = tid; i < d.nxitem; i += NT) {
+            const int2 it = __ldg(d.xitem + i);
+            const int t0 = it.x & 0xFFFFFF, nt = (int)((unsigned)it.x >> 24);
+            const int slot = it.y & 0xFFFFF, var = (it.y >> 20) & 0xFF;
+            wf<double> acc;
+#pragma unroll
+            for (int c = 0; c < 4; c++) acc.c[c] = mk<double>(0.0, 0.0);
+            for (int t = 0; t < nt; t++) {
+                const int4 w = __ldg(d.term + t0 + t);
+                const int op = w.x & 0xFF;
+                wf<double> A, B, q;
+                arg(w.y, var, A); arg(w.z, var, B);
+                switch (op) {
+                    case 8: row_slash(A, make_slashed(B), q); break;
+                    case 9: slash_col(make_slashed(A), B, q); break;
+                    case 10: ffv_p_raw(A, B, q); break;
+                    case 11: v3_raw(A, ldk(Ks, (w.x >> 16) & 0xFF), B, ldk(Ks, (w.x >> 24) & 0xFF), q); break;
+                    case 12: { wf<double> Z; arg(w.w, var, Z); v4_raw(A, B, Z, q); break; }
+                    default: {                                              // 13: 2 (A.Z) B - (B.Z) A - (B.A) Z
+                        wf<double> Z; arg(w.w, var, Z);
+                        cx<double> xz = dot(A, Z);
+                        xz = xz + xz;
+                        const cx<double> yz = dot(B, Z), yx = dot(B, A);
+#pragma unroll
+                        for (int mu = 0; mu < 4; mu++) q.c[mu] = cfms(yx, Z.c[mu], cfms(yz, A.c[mu], xz * B.c[mu]));
+                        break;
+                    }
+                }
+                axpy((w.x >> 8) & 1 ? -1.0 : 1.0, q, acc);
+            }
+            if ((it.y >> 28) & 1) {
+#pragma unroll
+                for (int c = 1; c < 4; c++) acc.c[c] = -acc.c[c];
+            }
+            stw(area, plane, slot, acc);
+        }
+        __syncthreads();
+        // phase 3: the colour flows; thread = helicity combination
+        for (int h = tid; h < nh; h += NT) {
+            const int pos = a.d_pos[h];
+            const size_t row = (size_t)e * a.nrow_evt + (pos < 0 ? 0 : pos);
+            const unsigned short* __restrict__ vt = d.vtab + h;
+            for (int f = 0; f < d.nflow; f++) {
+                const int4 fl = __ldg(d.flow + f);
+                double re = 0.0, im = 0.0;
+                for (int k = 0; k < fl.z; k++) {
+                    const int4 en = __ldg(d.entry + fl.y + k);
+                    const unsigned v = __ldg(vt + (size_t)en.z * nh);
+                    wf<double> X, Y;
+                    ldw(area, plane, en.x + (int)(v & 0xFFu), X);
+                    ldw(area, plane, en.y + (int)(v >> 8), Y);
+                    double sr = 0.0, si = 0.0;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) {
+                        sr = fma(X.c[c].re, Y.c[c].re, sr); sr = fma(-X.c[c].im, Y.c[c].im, sr);
+                        si = fma(X.c[c].re, Y.c[c].im, si); si = fma(X.c[c].im, Y.c[c].re, si);
+                    }
+                    if (en.w < 0) { re -= sr; im -= si; } else { re += sr; im += si; }
+                }
+                if (pos >= 0) {
+                    out[(size_t)fl.x * a.rows + row] = T2(re);
+                    out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(im);
+                }
+            }
+        }
+        __syncthreads();                 // the next event overwrites the scratch area
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+struct HsgContext {
+    const HsgTables* t = nullptr;
+    HsgDev d;
+    void* blob = nullptr;
+    char* scratch = nullptr;
+    int grid = 0;
+    size_t smem = 0;
+};
+
+const HsgTables* hsg_host_tables(const HsgContext* c) { return c->t; }
+
+cudaError_t hsg_create(int ngluon, HsgContext** out)
+{
+    *out = nullptr;
+    const HsgTables* t = hsg_tables(ngluon);
+    if (!t) return cudaErrorInvalidValue;
+    HsgContext* c = new HsgContext;
+    c->t = t;
+    struct Part { const void* src; size_t bytes; size_t off; };
+    Part parts[8] = { { t->obj, sizeof(int) * 4 * (size_t)t->nobj, 0 }, { t->term, sizeof(int) * 4 * (size_t)t->nterm, 0 },
+                      { t->p1_items, sizeof(int) * (size_t)t->np1, 0 }, { t->legset_mask, sizeof(int) * (size_t)t->nlegsets, 0 },
+                      { t->xitem, sizeof(int) * 2 * (size_t)t->nxitem, 0 }, { t->entry, sizeof(int) * 4 * (size_t)t->nentry, 0 },
+                      { t->flow, sizeof(int) * 4 * (size_t)t->nflow, 0 },
+                      { t->vtab, sizeof(unsigned short) * ((size_t)t->nvrow << t->npar), 0 } };
+    size_t total = 0;
+    for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
+    cudaError_t e = cudaMalloc(&c->blob, total);
+    if (e != cudaSuccess) { delete c; return e; }
+    for (auto& p : parts)
+        if (p.bytes && e == cudaSuccess) e = cudaMemcpy((char*)c->blob + p.off, p.src, p.bytes, cudaMemcpyHostToDevice);
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    c->grid = 2 * sms;                                  // persistent CTAs, two per SM: one scratch area each
+    if (e == cudaSuccess) e = cudaMalloc(&c->scratch, (size_t)c->grid * 64 * (size_t)t->nslot);
+    if (e != cudaSuccess) { cudaFree(c->blob); delete c; return e; }
+    char* b = (char*)c->blob;
+    HsgDev& d = c->d;
+    d.obj = (const int4*)(b + parts[0].off); d.term = (const int4*)(b + parts[1].off);
+    d.p1_items = (const int*)(b + parts[2].off); d.legset_mask = (const int*)(b + parts[3].off);
+    d.xitem = (const int2*)(b + parts[4].off); d.entry = (const int4*)(b + parts[5].off);
+    d.flow = (const int4*)(b + parts[6].off); d.vtab = (const unsigned short*)(b + parts[7].off);
+    d.npar = t->npar; d.ncolor = t->ncolor; d.nslot = t->nslot; d.nlegsets = t->nlegsets; d.nxitem = t->nxitem;
+    d.nflow = t->nflow; d.nlevel = t->nlevel;
+    for (int l = 0; l < 8; l++) d.p1_level[l] = l <= t->nlevel ? t->p1_level[l] : 0;
+    c->smem = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar);
+    *out = c;
+    return cudaSuccess;
+}
+
+void hsg_destroy(HsgContext* c)
+{
+    if (!c) return;
+    cudaFree(c->blob);
+    cudaFree(c->scratch);
+    delete c;
+}
+
+cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st)
+{
+    if (a.nevt <= 0) return cudaSuccess;
+    const int grid = a.nevt < c->grid ? a.nevt : c->grid;
+    if (jamps_fp64) hsg_diagrams_kernel<double><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->scratch);
+    else hsg_diagrams_kernel<float><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->scratch);
+    return cudaGetLastError();
+}
+
+}  // namespace mg

@@ -1,0 +1,38 @@
+// hsg_kernel.cuh -- host interface of the generic helicity-shared diagram kernel (hsg_kernel.cu) and the layout of its
+// tables (written by gen/hsg_tables.py through gen/emit_hsg.py; packing documented in gen/hsg_tables.py).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "hs_kernel.cuh"
+
+namespace mg {
+
+struct HsgTables {
+    int npar, ncolor, ns_obj, nslot, nlegsets, nobj, nterm, np1, nxitem, nentry, nflow, nvrow, nlevel, ndiagrams;
+    int p1_level[8];
+    const int* obj;
+    const int* term;
+    const int* p1_items;
+    const int* legset_mask;
+    const int* xitem;
+    const int* entry;
+    const int* flow;
+    const unsigned short* vtab;
+    // colour matrix: numerators (over cden) of the row of the identity permutation; C[s][s'] = row0[rank(s^-1 o s')]
+    const int* cmat_row0;
+    int cden;
+    double flops_p1, flops_p2, flops_p3;      // per event (phases 1, 2) and per (event, helicity) (phase 3)
+};
+
+const HsgTables* hsg_tables(int ngluon);        // generated/hsg_tables_gen.cu; NULL if the process has none
+
+struct HsgContext;
+
+// tables and the CTAs' scratch areas go to the CURRENT device
+cudaError_t hsg_create(int ngluon, HsgContext** out);
+void hsg_destroy(HsgContext* c);
+const HsgTables* hsg_host_tables(const HsgContext* c);
+// jamps [2][ncolor][rows] (HsLaunch::tile_major is ignored: 0)
+cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
+
+}  // namespace mg

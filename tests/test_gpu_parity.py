@@ -409,3 +409,34 @@ def test_partial_helicity_mask_on_the_shared_kernel(B, process, prec, nevt):
     err = _relerr(me, ref)
     assert err.max() < (1e-10 if prec == "fp64" else 1e-3), err.max()
     proc.close()
+
+
+def test_gg_ttxgggg_parity_and_mask(B):
+    """g g -> t tbar g g g g (Table 2: 15 495 diagrams, 720 colour flows, 256
+    helicities): generic helicity-shared kernel (objects in a global scratch area) + large-matrix DMMA colour sum against the
+    oracle, per event and per helicity; 37 events = ragged against the 16-row tiles of the colour sum and the probe of 16"""
+    process, nevt = "gg_ttxgggg", 37
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, "fp64")
+    assert (proc.npar, proc.ncomb, proc.ncolor, proc.ndiagrams) == (8, 256, 720, 15495)
+    d_mom = torch.from_numpy(mom).cuda()
+    mask = proc.helicity_filter(d_mom)                        # probe = the first 16 events
+    ref, ref_h = _oracle(process, mom, per_helicity=True)
+    assert mask.all() and (ref_h[:16] / ref[:16, None] > 1e-8).any(axis=0).all()          # PAPER.md:203 row (6): 256
+    me = proc.sigma_batch(d_mom).cpu().numpy()
+    print("\n[gg_ttxgggg] max rel err", _relerr(me, ref).max())
+    _assert_fp64_parity(process, mom, me, _relerr(me, ref))
+    meh = proc.last_helicity_terms(nevt).cpu().numpy()
+    assert (np.abs(meh - ref_h.T) / ref[None, :]).max() < 1e-10
+    # only MG_FP64, only the helicity-shared kernel
+    with pytest.raises(Exception):
+        B.init_process(process, "mixed")
+    with pytest.raises(Exception):
+        proc.set_option("diagrams", 0)
+    # a partial helicity mask: the masked-out rows are not computed into the sum
+    m2 = np.zeros(256, np.uint8)
+    m2[[3, 77, 200]] = 1
+    proc.set_good_helicities(m2)
+    me2 = proc.sigma_batch(d_mom[:5].contiguous()).cpu().numpy()
+    assert _relerr(me2, ref_h[:5][:, [3, 77, 200]].sum(axis=1)).max() < 1e-10
+    proc.close()
