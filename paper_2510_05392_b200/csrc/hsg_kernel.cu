@@ -61,6 +61,37 @@ __device__ __forceinline__ void axpy(double sg, const wf<double>& r, wf<double>&
     for (int c = 0; c < 4; c++) { acc.c[c].re = fma(sg, r.c[c].re, acc.c[c].re); acc.c[c].im = fma(sg, r.c[c].im, acc.c[c].im); }
 }
 
+// one entry for the 8 helicity combinations q of particles 0, 1, 2 (bit i of q = particle i): XMASK = which of them are legs
+// of X.  They are the lowest-numbered particles, hence the lowest bits of the variant index of whichever object holds them.
+template <int XMASK>
+__device__ __forceinline__ void p3_entry8(const char* __restrict__ px, const char* __restrict__ py, size_t plane, double sg,
+                                          double (&re)[8], double (&im)[8])
+{
+    constexpr int NX = 1 << (((XMASK >> 0) & 1) + ((XMASK >> 1) & 1) + ((XMASK >> 2) & 1)), NY = 8 / NX;
+#pragma unroll
+    for (int c = 0; c < 4; c++) {
+        double2 x[NX], y[NY];
+#pragma unroll
+        for (int i = 0; i < NX; i++) x[i] = *reinterpret_cast<const double2*>(px + c * plane + 16 * i);
+#pragma unroll
+        for (int i = 0; i < NY; i++) {
+            y[i] = *reinterpret_cast<const double2*>(py + c * plane + 16 * i);
+            y[i].x *= sg; y[i].y *= sg;
+        }
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            int xo = 0, yo = 0, nx = 0, ny = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                if ((XMASK >> b) & 1) { xo |= ((q >> b) & 1) << nx; nx++; }
+                else { yo |= ((q >> b) & 1) << ny; ny++; }
+            }
+            re[q] = fma(x[xo].x, y[yo].x, re[q]); re[q] = fma(-x[xo].y, y[yo].y, re[q]);
+            im[q] = fma(x[xo].x, y[yo].y, im[q]); im[q] = fma(x[xo].y, y[yo].x, im[q]);
+        }
+    }
+}
+
 // T2 = type of the jamps buffer
 template <typename T2>
 __global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgDev d, const HsLaunch a, char* __restrict__ scratch)
@@ -165,31 +196,52 @@ __global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgD
             stw(area, plane, slot, acc);
         }
         __syncthreads();
-        // phase 3: the colour flows; thread = helicity combination
-        for (int h = tid; h < nh; h += NT) {
-            const int pos = a.d_pos[h];
-            const size_t row = (size_t)e * a.nrow_evt + (pos < 0 ? 0 : pos);
-            const unsigned short* __restrict__ vt = d.vtab + h;
-            for (int f = 0; f < d.nflow; f++) {
-                const int4 fl = __ldg(d.flow + f);
-                double re = 0.0, im = 0.0;
-                for (int k = 0; k < fl.z; k++) {
-                    const int4 en = __ldg(d.entry + fl.y + k);
-                    const unsigned v = __ldg(vt + (size_t)en.z * nh);
-                    wf<double> X, Y;
-                    ldw(area, plane, en.x + (int)(v & 0xFFu), X);
-                    ldw(area, plane, en.y + (int)(v >> 8), Y);
-                    double sr = 0.0, si = 0.0;
+        // phase 3: the colour flows, one warp per flow: lane = helicities of particles 3 .. npar-1 (the low bits of h), and
+        // every thread carries the 8 helicity combinations of particles 0, 1, 2 in registers.  Those particles are the first
+        // legs of X or of Y, so the variants a thread needs are CONSECUTIVE slots: 2^nx of X and 2^(3-nx) of Y serve 8 dot
+        // products (9 or 6 wavefunction loads instead of 16), p3_entry8.
+        {
+            const int lane = tid & 31, nlow = nh >> 3;
+            for (int f = tid >> 5; f < d.nflow * (nlow >> 5); f += NT >> 5) {
+                const int fi = f / (nlow >> 5), hl = (f % (nlow >> 5)) * 32 + lane;       // (npar = 8: one warp per flow)
+                const int4 fl = __ldg(d.flow + fi);
+                double re[8], im[8];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) {
-                        sr = fma(X.c[c].re, Y.c[c].re, sr); sr = fma(-X.c[c].im, Y.c[c].im, sr);
-                        si = fma(X.c[c].re, Y.c[c].im, si); si = fma(X.c[c].im, Y.c[c].re, si);
+                for (int q = 0; q < 8; q++) re[q] = im[q] = 0.0;
+                const unsigned short* __restrict__ vt = d.vtab + hl;
+                int4 en = __ldg(d.entry + fl.y);
+                unsigned v = __ldg(vt + (size_t)en.z * nh);
+                for (int k = 0; k < fl.z; k++) {
+                    const int4 cur = en;
+                    const unsigned cv = v;
+                    if (k + 1 < fl.z) {
+                        en = __ldg(d.entry + fl.y + k + 1);
+                        v = __ldg(vt + (size_t)en.z * nh);
                     }
-                    if (en.w < 0) { re -= sr; im -= si; } else { re += sr; im += si; }
+                    const char* __restrict__ px = area + 16 * (size_t)(cur.x + (int)(cv & 0xFFu));
+                    const char* __restrict__ py = area + 16 * (size_t)(cur.y + (int)(cv >> 8));
+                    const double sg = (cur.w & 1) ? -1.0 : 1.0;
+                    switch ((cur.w >> 1) & 7) {
+                        case 0: p3_entry8<0>(px, py, plane, sg, re, im); break;
+                        case 1: p3_entry8<1>(px, py, plane, sg, re, im); break;
+                        case 2: p3_entry8<2>(px, py, plane, sg, re, im); break;
+                        case 3: p3_entry8<3>(px, py, plane, sg, re, im); break;
+                        case 4: p3_entry8<4>(px, py, plane, sg, re, im); break;
+                        case 5: p3_entry8<5>(px, py, plane, sg, re, im); break;
+                        case 6: p3_entry8<6>(px, py, plane, sg, re, im); break;
+                        default: p3_entry8<7>(px, py, plane, sg, re, im); break;
+                    }
                 }
-                if (pos >= 0) {
-                    out[(size_t)fl.x * a.rows + row] = T2(re);
-                    out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(im);
+#pragma unroll
+                for (int q = 0; q < 8; q++) {
+                    // q bit i = helicity of particle i = bit npar-1-i of h
+                    const int h = hl | ((q & 1) << (npar - 1)) | (((q >> 1) & 1) << (npar - 2)) | (((q >> 2) & 1) << (npar - 3));
+                    const int pos = a.d_pos[h];
+                    if (pos >= 0) {
+                        const size_t row = (size_t)e * a.nrow_evt + pos;
+                        out[(size_t)fl.x * a.rows + row] = T2(re[q]);
+                        out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(im[q]);
+                    }
                 }
             }
         }

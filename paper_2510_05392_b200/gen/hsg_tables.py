@@ -22,7 +22,7 @@ Packing (int32; variant bit j <-> helicity of the j-th leg in ascending particle
   xitem[i]   = { first term | terms << 24, slot | variant << 20 | vector-valued << 28 }: one variant of a pair object; sorted
                by the sequence of opcodes.  Vector-valued (opcodes >= 10): components 1-3 are negated at the store, so that
                the contraction with Y is a plain sum over the four components
-  entry[e]   = { first slot of X, first slot of Y, row of vtab, sign }
+  entry[e]   = { first slot of X, first slot of Y, row of vtab, negative | (particles 0, 1, 2 that are legs of X) << 1 }
   flow[f]    = { colour index, first entry, entries, 0 }
   vtab[row][h] (uint16) = variant of X | variant of Y << 8 for helicity combination h (bit npar-1-p of h = particle p)
 """
@@ -137,7 +137,8 @@ def build(n):
         for xs, yo, sign in g["entries"][j]:
             x = g["xobjs"][xs]
             assert set(x["legs"]) | set(prog.objs[yo].legs) == set(range(npar))
-            entries.append([xslot[xs], slot0[yo], vrow(tuple(x["legs"])), sign])
+            flags = (1 if sign < 0 else 0) | (sum(1 << p for p in x["legs"] if p < 3) << 1)
+            entries.append([xslot[xs], slot0[yo], vrow(tuple(x["legs"])), flags])
         flows.append([j, e0, len(entries) - e0, 0])
     i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w)
     return {

@@ -100,9 +100,17 @@ def evaluate(T, mom, mt, wt):
     nh = 1 << npar
     J = np.zeros((T["ncolor"], nh), dtype=complex)
     for j, e0, ne, _ in T["flow"]:
-        for xs, ys, row, sign in T["entry"][e0:e0 + ne]:
+        for xs, ys, row, flags in T["entry"][e0:e0 + ne]:
             vt = T["vtab"][row].astype(np.int64)
             X = area[int(xs) + (vt & 0xFF)]
             Y = area[int(ys) + (vt >> 8)]
-            J[j] += int(sign) * np.sum(X * Y, axis=1)
+            J[j] += (-1 if int(flags) & 1 else 1) * np.sum(X * Y, axis=1)
+            # bits 1..3: which of particles 0, 1, 2 are legs of X -- they must then be the lowest bits of X's variant index
+            for i in range(3):
+                hbit = 1 << (npar - 1 - i)
+                dx = (vt[hbit] & 0xFF) - (vt[0] & 0xFF)
+                dy = (vt[hbit] >> 8) - (vt[0] >> 8)
+                inx = (int(flags) >> (1 + i)) & 1
+                before = sum(1 for b in range(i) if ((int(flags) >> (1 + b)) & 1) == inx)
+                assert (dx, dy) == ((1 << before, 0) if inx else (0, 1 << before))
     return J
