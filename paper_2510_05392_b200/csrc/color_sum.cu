@@ -12,6 +12,7 @@
 #include <math.h>
 #include <stdint.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "color_sum.cuh"
@@ -302,29 +303,52 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 // row 3; PAPER.md:580-613 makes this contraction the point of the 2 -> 6 process).  Same triangular form Z = X L.
 //   - a CTA (16 warps) = 16 rows, their Re and Im parts: M = 32 = four m8 tiles; all 32 x NC accumulators stay in
 //     registers (NC / 8 n-tiles dealt to the warps in pairs (j, NC/8 - 1 - j): equal numbers of k-steps);
-//   - the jamps stream through a 3-stage cp.async ring of [16 colours][32] chunks (row stride 40 doubles: the A-fragment
-//     reads fall into distinct bank pairs); every A fragment serves all n-tiles of the warp;
-//   - the factor is read from global memory (L2-resident: 4 MB) in FRAGMENT order, one coalesced 256-byte read per
-//     (k-step, n-tile) and warp: element [lane] = L[4 ks + lane % 4][8 j + lane / 4]; blocks above the diagonal are skipped.
+//   - jamps AND factor stream through a 3-stage cp.async ring, 8 colours (two k-steps) per chunk: [8][32] jamps (row stride 40
+//     doubles: the A-fragment reads fall into distinct bank pairs) and, per k-step, the factor's fragments of the n-tiles on or
+//     below the diagonal.  The factor lives in global memory (4 MB, L2-resident) in FRAGMENT order, element [lane] of block
+//     (k-step, n-tile) = L[4 ks + lane % 4][8 j + lane / 4], so that the blocks a k-step needs are ONE contiguous range and a B
+//     fragment is one conflict-free LDS.64 per lane; every A fragment serves all n-tiles of the warp.
 // C is only positive SEMI-definite at 6 gluons (rank 685 of 720): the factor has zero columns there (color_cholesky_big).
+template <int NC>
+struct CsBig {
+    static constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 8, NCHUNK = NC / KC, STG = 3, STRIDE = 40;
+    static constexpr int SLOTS = 2 * ((NPAIR + 15) / 16);
+    static constexpr size_t L_STAGE = (size_t)(KC / 4) * NT8 * 32;            // doubles: the two k-steps of a chunk, all n-tiles
+    static constexpr size_t SMEM = sizeof(double) * (STG * L_STAGE + STG * KC * STRIDE + 16 * 32);
+};
+
 template <int NC>
 __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __restrict__ Lf, const double* __restrict__ X,
                                                                long rows_padded, RowMap map, double* __restrict__ meh)
 {
-    static_assert(NC % 16 == 0, "chunks of 16 colours");
-    constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 16, NCHUNK = NC / KC, STG = 3, STRIDE = 40;
-    constexpr int SLOTS = 2 * ((NPAIR + 15) / 16);
-    __shared__ __align__(16) double js[STG][KC][STRIDE];
-    __shared__ double red[16][32];
+    using Cfg = CsBig<NC>;
+    static_assert(NC % 16 == 0, "pairs of n-tiles");
+    constexpr int NT8 = Cfg::NT8, NPAIR = Cfg::NPAIR, KC = Cfg::KC, NCHUNK = Cfg::NCHUNK, STG = Cfg::STG, STRIDE = Cfg::STRIDE;
+    constexpr int SLOTS = Cfg::SLOTS;
+    extern __shared__ __align__(16) double sm_big[];
+    double* __restrict__ ls = sm_big;                                     // [STG][KC / 4][NT8][32]: factor fragments
+    double* __restrict__ js = ls + STG * Cfg::L_STAGE;                    // [STG][KC][STRIDE]: jamps
+    double* __restrict__ red = js + STG * KC * STRIDE;                    // [16][32]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long r0 = (long)blockIdx.x * 16;
-    // chunk loader: thread t < 256 copies 16 bytes: colour t / 16, part (t / 8) % 2, rows 2 (t % 8) ..
+    // chunk c = colours 8 c .. 8 c + 7 = k-steps 2 c, 2 c + 1: the jamps (thread t < 128 copies 16 bytes: colour t / 16,
+    // part (t / 8) % 2, rows 2 (t % 8) ..) and, of either k-step, the fragments of the n-tiles 0 .. c (on or below the diagonal)
     auto load_chunk = [&](int c) {
-        if (c < NCHUNK && tid < 256) {
-            const int k = tid >> 4, part = (tid >> 3) & 1, q = tid & 7;
-            const double* src = X + ((long)part * NC + c * KC + k) * rows_padded + r0 + 2 * q;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(&js[c % STG][k][part * 16 + 2 * q]);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+        if (c < NCHUNK) {
+            const int st = c % STG;
+            if (tid < 128) {
+                const int k = tid >> 4, part = (tid >> 3) & 1, q = tid & 7;
+                const double* src = X + ((long)part * NC + c * KC + k) * rows_padded + r0 + 2 * q;
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(js + ((size_t)st * KC + k) * STRIDE + part * 16 + 2 * q);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+            }
+            const int n16 = (c + 1) * 16;                                // 16-byte pieces per k-step
+            for (int i = tid; i < 2 * n16; i += 512) {
+                const int kk = i >= n16, o = i - kk * n16;
+                const double* src = Lf + ((long)(2 * c + kk) * NT8) * 32 + 2 * o;
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(ls + (size_t)st * Cfg::L_STAGE + (size_t)kk * NT8 * 32 + 2 * o);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+            }
         }
         asm volatile("cp.async.commit_group;");
     };
@@ -333,6 +357,21 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
     for (int s = 0; s < SLOTS; s++)
 #pragma unroll
         for (int m = 0; m < 4; m++) acc[s][m][0] = acc[s][m][1] = 0.0;
+    // the n-tiles of this warp in ASCENDING order (slot s < SLOTS / 2: pair s's low tile, then the high tiles backwards), so
+    // that the tiles on or below the diagonal at chunk c are a PREFIX of the slots: its length picks a branch-free body.
+    // (A predicated-off DMMA still occupies the tensor pipe -- measured: predication made this kernel 2x slower.)
+    int jn[SLOTS];
+#pragma unroll
+    for (int s = 0; s < SLOTS; s++) {
+        const int pr = warp + 16 * (s < SLOTS / 2 ? s : SLOTS - 1 - s);
+        jn[s] = pr < NPAIR ? (s < SLOTS / 2 ? pr : NT8 - 1 - pr) : (1 << 20);         // no such pair: never active
+    }
+    static_assert(SLOTS == 6, "the switch below lists 1 .. 6 active tiles");
+#pragma unroll
+    for (int pass = 0; pass < SLOTS - 1; pass++)                                      // (a missing third pair sorts last)
+#pragma unroll
+        for (int s = 0; s + 1 < SLOTS - pass; s++)
+            if (jn[s] > jn[s + 1]) { const int t = jn[s]; jn[s] = jn[s + 1]; jn[s + 1] = t; }
     load_chunk(0);
     load_chunk(1);
     const int ak = lane & 3, ar = lane >> 2;
@@ -341,23 +380,34 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
         asm volatile("cp.async.wait_group 1;");
         __syncthreads();
         load_chunk(c + 2);
-        const double (*jt)[STRIDE] = js[c % STG];
+        const double* __restrict__ jt = js + (size_t)(c % STG) * KC * STRIDE;
+        const double* __restrict__ lt = ls + (size_t)(c % STG) * Cfg::L_STAGE + lane;
+        int nact = 0;
 #pragma unroll
-        for (int kk = 0; kk < KC / 4; kk++) {
-            const int ks = c * (KC / 4) + kk;
-            double a[4];
+        for (int s = 0; s < SLOTS; s++) nact += jn[s] <= c;
+        auto body = [&](auto NA) {
+            constexpr int NACT = decltype(NA)::value;
 #pragma unroll
-            for (int m = 0; m < 4; m++) a[m] = jt[4 * kk + ak][8 * m + ar];
+            for (int kk = 0; kk < KC / 4; kk++) {
+                double a[4];
 #pragma unroll
-            for (int s = 0; s < SLOTS; s++) {
-                const int pr = warp + 16 * (s >> 1);
-                const int j = (s & 1) ? NT8 - 1 - pr : pr;
-                if (pr < NPAIR && ks >= 2 * j) {
-                    const double b = __ldg(Lf + ((long)ks * NT8 + j) * 32 + lane);
+                for (int m = 0; m < 4; m++) a[m] = jt[(4 * kk + ak) * STRIDE + 8 * m + ar];
+#pragma unroll
+                for (int s = 0; s < NACT; s++) {
+                    const double b = lt[((size_t)kk * NT8 + jn[s]) * 32];
 #pragma unroll
                     for (int m = 0; m < 4; m++) dmma(acc[s][m][0], acc[s][m][1], a[m], b);
                 }
             }
+        };
+        switch (nact) {
+            case 1: body(std::integral_constant<int, 1>()); break;
+            case 2: body(std::integral_constant<int, 2>()); break;
+            case 3: body(std::integral_constant<int, 3>()); break;
+            case 4: body(std::integral_constant<int, 4>()); break;
+            case 5: body(std::integral_constant<int, 5>()); break;
+            case 6: body(std::integral_constant<int, 6>()); break;
+            default: break;
         }
     }
     // sum of squares per m-row: lanes of a quad hold the 8 columns of a row
@@ -368,13 +418,13 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
         for (int s = 0; s < SLOTS; s++) v += acc[s][m][0] * acc[s][m][0] + acc[s][m][1] * acc[s][m][1];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
-        if (ak == 0) red[warp][8 * m + ar] = v;
+        if (ak == 0) red[warp * 32 + 8 * m + ar] = v;
     }
     __syncthreads();
     if (tid < 16) {
         double v = 0.0;
 #pragma unroll
-        for (int w = 0; w < 16; w++) v += red[w][tid] + red[w][16 + tid];       // Re part + Im part of the row
+        for (int w = 0; w < 16; w++) v += red[w * 32 + tid] + red[w * 32 + 16 + tid];       // Re part + Im part of the row
         map.store(meh, r0 + tid, v);
     }
 }
@@ -424,7 +474,9 @@ cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const
     if (!d_factor) return cudaErrorInvalidValue;
     const double* d_chol = (const double*)d_factor;
     if (ncolor == 720) {            // d_factor: the fragment-order factor of color_cholesky_big
-        color_sum_big_kernel<720><<<(unsigned)(rows_padded / 16), 512, 0, st>>>(d_chol, (const double*)d_jamps, rows_padded, map, d_meh);
+        cudaError_t e_ = cudaFuncSetAttribute(color_sum_big_kernel<720>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CsBig<720>::SMEM);
+        if (e_ != cudaSuccess) return e_;
+        color_sum_big_kernel<720><<<(unsigned)(rows_padded / 16), 512, CsBig<720>::SMEM, st>>>(d_chol, (const double*)d_jamps, rows_padded, map, d_meh);
         return cudaGetLastError();
     }
     const int ncp = (ncolor + 7) / 8 * 8;
