@@ -108,7 +108,8 @@ def oracle_rate(process, nevt_sample, seed=1):
 
 
 # sized for about 10-30 s of oracle time on the 16 host cores of the GPU box (854 MEs/s measured for gg_ttxggg)
-ORACLE_SAMPLE = {"epem_mupmum": 16384, "gg_ttx": 65536, "gg_ttxg": 65536, "gg_ttxgg": 32768, "gg_ttxggg": 12288}
+ORACLE_SAMPLE = {"epem_mupmum": 16384, "gg_ttx": 65536, "gg_ttxg": 65536, "gg_ttxgg": 32768, "gg_ttxggg": 12288,
+                 "gg_ttxgggg": 256}
 
 
 def run_reference(args):
@@ -296,7 +297,7 @@ def main():
         alg_flop += (2.0 * proc.ncolor * (proc.ncolor + 1) + 4.0 * proc.ncolor) * nevt * r["ngood"]   # fused triangular colour sum
     achieved = alg_flop / (diag_ms * 1e-3) * 1e-12
     dram_per_event, dram_src = ncu_dram_bytes_per_event(process, args.precision) if shared else (None, None)
-    roofline = {"bound": "alu", "kernel": "hs_diagrams_kernel" if shared else "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": ("hsg_diagrams_kernel" if process == "gg_ttxgggg" else "hs_diagrams_kernel") if shared else "diagrams_kernel", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak if fp64_peak else None,
                 "traffic": dram_per_event * nevt if dram_per_event else None,
                 "traffic_source": (f"ncu --set full capture {dram_src} (profiles/dram_traffic.csv), scaled to this launch by the "
@@ -319,7 +320,7 @@ def main():
             flop = rows / 8 * pairs * 2 * 512.0                                # x 2 parts, 512 flop per m8n8k4
             dmma_peak = B.measure_peak(2, local)
             ach = flop / (cs_ms * 1e-3) * 1e-12
-            cs_roofline = {"bound": "tensor", "kernel": "color_sum_dmma2_kernel", "achieved": ach, "peak": dmma_peak, "unit": "TFLOP/s",
+            cs_roofline = {"bound": "tensor", "kernel": "color_sum_big_kernel" if nc > 128 else "color_sum_dmma2_kernel", "achieved": ach, "peak": dmma_peak, "unit": "TFLOP/s",
                            "frac": ach / dmma_peak, "kernel_ms": cs_ms, "flop_counted": "issued DMMA (triangular k-step x n-tile pairs)",
                            "peak_source": "mma.sync.m8n8k4.f64 probe measured in this run (mg_measure_peak kind 2)"}
         elif not proc.get_option("hs_color_alu"):
@@ -333,7 +334,8 @@ def main():
            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64" if args.precision in ("fp64", "d") else ("f64+f32" if args.precision in ("mixed", "m") else "f32"),
            "data": "synthetic",
-           "config": {"workload": f"{process}: {nevt} events/batch/GPU, flat RAMBO sqrt(s)=1500 GeV seed 1 (BASELINE.json config)",
+           "config": {"workload": f"{process}: {nevt} events/batch/GPU, flat RAMBO sqrt(s)=1500 GeV seed 1 ("
+                                              + ("SURVEY.md 8(f) row 3; batch size chosen here)" if process == "gg_ttxgggg" else "BASELINE.json config)"),
                       "process": process, "precision": args.precision, "nevt_per_gpu": nevt, "good_helicities": r["ngood"],
                       "diagrams": "helicity-shared (CTA = event, thread = helicity)" if shared else "thread = (event, helicity)",
                       "schedule": "helicity streams" if args.schedule else ("helicity = thread index" if shared else "helicity = grid.y"),
@@ -383,12 +385,15 @@ def main():
             per = {}
             for pname in inputs.PROCESSES:
                 for prec in ("fp64", "mixed"):
+                    if pname == "gg_ttxgggg" and prec != "fp64":          # MG_FP64 only
+                        continue
                     if pname == process and prec == args.precision:
                         per[f"{pname}/{prec}"] = {"MEs_per_s": r["value"], "ms_per_batch": r["ms_per_step"]}
                         continue
                     try:
                         q = time_process(torch, B, pname, prec, inputs.PROCESSES[pname]["nevt"], 3, 3, 0, 1, flush, opts)
                         per[f"{pname}/{prec}"] = {"MEs_per_s": q["value"], "ms_per_batch": q["ms_per_step"],
+                                                  "stage_ms": {"diagrams": q["stage_ms"][0], "color_sum": q["stage_ms"][1]},
                                                   "diagram_tflops": q["proc"].diagram_flops * inputs.PROCESSES[pname]["nevt"]
                                                   * q["ngood"] / (q["stage_ms"][0] * 1e-3) * 1e-12}
                         q["proc"].close()

@@ -303,7 +303,8 @@ def _near_boundary(weights, rnd, tol):
 
 
 @pytest.mark.parametrize("process,prec,nevt", [("epem_mupmum", "fp64", 600), ("gg_ttx", "fp64", 300), ("gg_ttxg", "fp64", 150),
-                                               ("gg_ttxgg", "fp64", 70), ("gg_ttxggg", "fp64", 24), ("gg_ttxggg", "mixed", 24)])
+                                               ("gg_ttxgg", "fp64", 70), ("gg_ttxggg", "fp64", 24), ("gg_ttxggg", "mixed", 24),
+                                               ("gg_ttxgggg", "fp64", 10)])
 def test_running_alphas_and_selection(B, process, prec, nevt):
     """mg_sigma_batch_ex (PAPER.md:77, 99-100): per-event alpha_s, selected helicity and colour, against oracle/selection.py;
     index-exact except where the random number sits on a cumulative boundary (validity rule, A15)"""
@@ -439,4 +440,33 @@ def test_gg_ttxgggg_parity_and_mask(B):
     proc.set_good_helicities(m2)
     me2 = proc.sigma_batch(d_mom[:5].contiguous()).cpu().numpy()
     assert _relerr(me2, ref_h[:5][:, [3, 77, 200]].sum(axis=1)).max() < 1e-10
+    proc.close()
+
+
+def test_gg_ttxgggg_full_batch_sampled(B):
+    """the 4096-event batch bench.py times for g g -> t tbar g g g g (12 GB of jamps, one launch per kernel), oracle on 48
+    sampled events (first, last, around the multiples of the 296 persistent CTAs' stride, random); then the same batch in
+    chunks of 128 events (jamp_chunk_mib) and as a replayed CUDA graph: identical numbers"""
+    process = "gg_ttxgggg"
+    nevt = inputs.PROCESSES[process]["nevt"]
+    mom = inputs.momenta(process, nevt)
+    proc = B.init_process(process, "fp64")
+    d_mom = torch.from_numpy(mom).cuda()
+    me = proc.sigma_batch(d_mom).cpu().numpy()
+    assert np.isfinite(me).all() and (me > 0).all()
+    rng = np.random.default_rng(4)
+    idx = np.unique(np.concatenate([[0, 1, 15, 16, 295, 296, 297, 591, 592, nevt - 2, nevt - 1],
+                                    rng.choice(nevt, 37, replace=False)]))
+    ref = _oracle(process, mom[idx])
+    _histogram(_relerr(me[idx], ref), "gg_ttxgggg full batch, sampled")
+    _assert_fp64_parity(process, mom[idx], me[idx], _relerr(me[idx], ref))
+    proc.set_option("jamp_chunk_mib", 400)                 # 128 events per chunk: 32 launches of either kernel
+    me2 = proc.sigma_batch(d_mom).cpu().numpy()
+    assert np.array_equal(me2, me)
+    proc.set_option("jamp_chunk_mib", 16384)
+    proc.set_option("graph", 1)
+    out = torch.empty(nevt, dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        proc.sigma_batch(d_mom, out)
+    assert proc.get_option("graph_replays") >= 1 and np.array_equal(out.cpu().numpy(), me)
     proc.close()
