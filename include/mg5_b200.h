@@ -54,11 +54,15 @@ enum { MG_SCHED_GRID = 0, MG_SCHED_STREAMS = 1 };
  *   MG_DIAG_THREAD : one thread per (event, helicity), the paper's layout
  *   MG_DIAG_SHARED : one CTA per event, all helicities at once; wavefunctions shared between helicities in shared
  *                    memory, jamps written to the workspace and contracted by the colour-sum kernel (g g -> t tbar +
- *                    2 or 3 gluons, MG_FP64 / MG_MIXED; the default there) */
+ *                    2 or 3 gluons, MG_FP64 / MG_MIXED; the default there; g g -> t tbar + 4 gluons: the only kernel) */
 enum { MG_DIAG_THREAD = 0, MG_DIAG_SHARED = 1 };
 
 /* Create a process.  name: "epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg" (BASELINE.json configs;
- * Table 2).  Parameters start at the BASELINE.json card.  *out is NULL on failure. */
+ * Table 2), or "gg_ttxgggg" (g g -> t tbar g g g g, Table 2's 2 -> 6 row: 15 495 diagrams, 720 colour
+ * flows, 256 helicities; Tables 5-8).  The latter runs in MG_FP64 with MG_DIAG_SHARED only (generic
+ * helicity-shared kernel, the event's wavefunctions in a per-CTA scratch area in global memory owned by the handle: about
+ * 1 GB of device memory per handle; 720-colour FP64 tensor-core colour sum): any other precision -> MG_EINVAL.
+ * Parameters start at the BASELINE.json card.  *out is NULL on failure. */
 int mg_init_process(const char* name, int precision, int device, mg_process** out);
 
 /* Static facts about the process (any pointer may be NULL). ngroups = diagram-group functions in the diagram
@@ -84,7 +88,8 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
  * "max_streams" (MG_SCHED_STREAMS: helicities share this many streams round robin, 0 = one each),
  * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the
  * arguments and the handle's state are unchanged; ignored while "timing" = 1; mg_get_option
- * "graph_replays" counts the replays of the current graph).
+ * "graph_replays" counts the replays of the current graph; mg_get_option "probe_events" = the number of events of the first
+ * batch the automatic helicity filter looks at, at most: 1024, or 16 for "gg_ttxgggg" whose probe goes through the jamps buffer).
  * With "diagrams" = MG_DIAG_SHARED the jamps always go through the workspace and the tensor-core colour sum ("color_sum" and
  * "block" then only affect the helicity filter and MG_DIAG_THREAD).
  * Unknown key, bad value, or a combination that cannot run (helicity streams with the MG_DIAG_SHARED kernel, which has
