@@ -61,6 +61,7 @@ struct mg_process {
     int* d_all = nullptr;      // DEVICE [ncomb] = 0..ncomb-1
     void* d_cmat = nullptr;    // DEVICE [ncolor^2] numerators as the colour-sum type
     void* d_cmat64 = nullptr;  // DEVICE [ncolor^2] numerators in fp64 (helicity filter; = d_cmat in MG_FP64)
+    void* d_chol64 = nullptr;  // DEVICE fp64 factor for the helicity filter of the generic kernel when d_chol is the TF32 image (else = d_chol)
     void* d_chol = nullptr;    // DEVICE Cholesky factor of the numerators for the tensor colour sum: fp64 [ncp^2] (MG_FP64) or its TF32 image
     // helicity streams
     std::vector<cudaStream_t> streams;
@@ -180,11 +181,20 @@ static int upload_tables(mg_process* p)
         CUDA_TRY(p, cudaMemcpy(p->d_cmat64, h64.data(), n2 * sizeof(double), cudaMemcpyHostToDevice));
     }
     if (p->precision == MG_FP64) p->d_cmat64 = p->d_cmat;
-    if (p->precision == MG_FP64 && d->ncolor > 128) {
+    if (d->ncolor > 128) {
+        // 720 colours: fp64 factor in fragment order (the helicity filter always decides in fp64, reading A5) and, in mixed
+        // precision, its TF32 image for the tcgen05 contraction
         std::vector<double> frag; int rank = 0;
         if (!color_cholesky_big(d->ncolor, d->cmat, frag, &rank)) return fail(p, MG_ESTATE, "colour matrix is not positive semi-definite");
-        CUDA_TRY(p, cudaMalloc(&p->d_chol, frag.size() * sizeof(double)));
-        CUDA_TRY(p, cudaMemcpy(p->d_chol, frag.data(), frag.size() * sizeof(double), cudaMemcpyHostToDevice));
+        CUDA_TRY(p, cudaMalloc(&p->d_chol64, frag.size() * sizeof(double)));
+        CUDA_TRY(p, cudaMemcpy(p->d_chol64, frag.data(), frag.size() * sizeof(double), cudaMemcpyHostToDevice));
+        if (p->precision == MG_FP64) p->d_chol = p->d_chol64;
+        else {
+            std::vector<float> img;
+            if (!tf32_big_build_factor_image(d->ncolor, d->cmat, img)) return fail(p, MG_ESTATE, "cannot build the TF32 factor image");
+            CUDA_TRY(p, cudaMalloc(&p->d_chol, img.size() * sizeof(float)));
+            CUDA_TRY(p, cudaMemcpy(p->d_chol, img.data(), img.size() * sizeof(float), cudaMemcpyHostToDevice));
+        }
     } else if (p->precision == MG_FP64) {
         std::vector<double> lp; int ncp = 0;
         if (!color_cholesky_padded(d->ncolor, d->cmat, lp, &ncp)) return fail(p, MG_ESTATE, "colour matrix is not positive definite");
@@ -223,8 +233,8 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
     else if (!strcmp(name, "gg_ttxgggg")) d = desc_gg_ttxgggg();
     else return fail(nullptr, MG_EINVAL, std::string("unknown process ") + name);
     if (!d) return fail(nullptr, MG_EINVAL, std::string("library built without ") + name);
-    if (!d->launch && precision != MG_FP64)
-        return fail(nullptr, MG_EINVAL, std::string(name) + " runs in MG_FP64 only (generic helicity-shared kernel + DMMA colour sum)");
+    if (!d->launch && precision == MG_FP32)
+        return fail(nullptr, MG_EINVAL, std::string(name) + " runs in MG_FP64 and MG_MIXED only (generic helicity-shared kernel, fp64 amplitudes)");
     if (precision == MG_FP32 && !d->has_fp32)
         return fail(nullptr, MG_EINVAL, std::string("library built without the MG_FP32 instantiation of ") + name);
     int ndev = 0;
@@ -264,6 +274,7 @@ extern "C" void mg_destroy(mg_process* p)
     hsg_destroy(p->hsg);
     cudaFree(p->d_pos);
     if (p->d_cmat64 != p->d_cmat) cudaFree(p->d_cmat64);
+    if (p->d_chol64 != p->d_chol) cudaFree(p->d_chol64);
     cudaFree(p->d_good); cudaFree(p->d_all); cudaFree(p->d_cmat); cudaFree(p->d_chol);
     cudaFree(p->d_mom_own); cudaFree(p->d_me_own); cudaFree(p->d_ws_own);
     for (auto s : p->streams) cudaStreamDestroy(s);
@@ -605,7 +616,7 @@ extern "C" int mg_helicity_filter(mg_process* p, const double* d_momenta, int np
         CUDA_TRY(p, hsg_launch(p->hsg, true, a, st));
         RowMap map;
         map.rows_valid = rows; map.hel_minor = ncomb; map.evt_stride = nprobe; map.e0 = 0; map.norm = make_norm(p);
-        CUDA_TRY(p, color_sum_tensor(true, p->d->ncolor, p->d_cmat, p->d_chol, a.d_jamps, a.rows, map, (double*)d_workspace, st));
+        CUDA_TRY(p, color_sum_tensor(true, p->d->ncolor, p->d_cmat64, p->d_chol64, a.d_jamps, a.rows, map, (double*)d_workspace, st));
     } else {
         DiagLaunch a = base_launch(p, d_momenta, nprobe);
         a.d_hel = p->d_all; a.hel_base = 0; a.nhel = ncomb; a.d_meh = (double*)d_workspace; a.mode = MG_CS_FUSED;
@@ -733,9 +744,11 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
             // tcgen05 colour sum: one contiguous block per 128-row tile, so that a chunk of colours is ONE bulk copy
             // (2: straight in the operand layout, TF32-rounded -- the contraction then needs neither converter warps nor the
             //  low term of the jamps; needs chunks of 24 colours)
-            const int tile_major = p->precision != MG_FP64 && !p->hs_color_alu ? (p->d->ncolor % 24 == 0 && p->tf32_direct ? 2 : 1) : 0;
+            // (the generic kernel has the operand layout only: options "hs_color_alu" / "tf32_direct" do not apply to it)
+            const bool alu = p->hs_color_alu && !p->hsg;
+            const int tile_major = p->precision != MG_FP64 && !alu ? (p->hsg || (p->d->ncolor % 24 == 0 && p->tf32_direct) ? 2 : 1) : 0;
             a.tile_major = tile_major;
-            if (p->hsg) CUDA_TRY(p, hsg_launch(p->hsg, true, a, st));
+            if (p->hsg) CUDA_TRY(p, hsg_launch(p->hsg, p->precision == MG_FP64, a, st));
             else CUDA_TRY(p, hs_launch(p->hs, p->precision == MG_FP64, a, st));
             p->launches += 2;                      // + the colour-sum kernel below
             MARK(0);
@@ -743,7 +756,7 @@ static int sigma_batch_impl(mg_process* p, const double* d_momenta, int nevt, do
             map.rows_valid = rows; map.hel_minor = nhel; map.evt_stride = nevt; map.e0 = e0; map.norm = make_norm(p);
             cudaError_t ce_;
             // tensor-core contraction (DMMA in MG_FP64, tcgen05 kind::tf32 otherwise) unless the ALU kernel is asked for
-            if (p->hs_color_alu && p->precision != MG_FP64)
+            if (alu && p->precision != MG_FP64)
                 ce_ = color_sum_alu(false, p->d->ncolor, p->d_cmat, d_j, a.rows, d_meh, st, &map);
             else
                 ce_ = color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, a.rows, map, d_meh, st, tile_major);

@@ -429,13 +429,12 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
     }
 }
 
-// host: factor of a positive SEMI-definite integer matrix in the fragment order of color_sum_big_kernel (full rectangle of
-// (k-step, n-tile) blocks).  A pivot that vanishes (relative to its diagonal element) gives a zero column; the rest of that
-// column must vanish too (it does for a semi-definite matrix), else false.
-bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, int* rank_out)
+// host: factor L (row-major, lower triangular, C = L L^T) of a positive SEMI-definite integer matrix, in long double.  A pivot
+// that vanishes (relative to its diagonal element) gives a zero column; the rest of that column must vanish too (it does for a
+// semi-definite matrix), else false.  color_cholesky_big: the same factor in the fragment order of color_sum_big_kernel (full
+// rectangle of (k-step, n-tile) blocks).
+bool color_cholesky_semidef(int n, const int* cmat, std::vector<double>& L, int* rank_out)
 {
-    if (ncolor % 16) return false;
-    const int n = ncolor;
     std::vector<long double> l((size_t)n * n, 0.0L);
     std::vector<char> null(n, 0);
     int rank = 0;
@@ -452,16 +451,30 @@ bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, 
             else l[(size_t)i * n + j] = t / l[(size_t)j * n + j];
         }
     }
+    L.resize((size_t)n * n);
+    for (size_t i = 0; i < L.size(); i++) L[i] = (double)l[i];
+    if (rank_out) *rank_out = rank;
+    return true;
+}
+
+bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, int* rank_out)
+{
+    if (ncolor % 16) return false;
+    const int n = ncolor;
+    std::vector<double> l;
+    if (!color_cholesky_semidef(n, cmat, l, rank_out)) return false;
     frag.assign((size_t)(n / 4) * (n / 8) * 32, 0.0);
     for (int ks = 0; ks < n / 4; ks++)
         for (int j = 0; j < n / 8; j++)
             for (int lane = 0; lane < 32; lane++) {
                 const int k = 4 * ks + lane % 4, c = 8 * j + lane / 4;
-                if (k >= c) frag[((size_t)ks * (n / 8) + j) * 32 + lane] = (double)l[(size_t)k * n + c];
+                if (k >= c) frag[((size_t)ks * (n / 8) + j) * 32 + lane] = l[(size_t)k * n + c];
             }
-    if (rank_out) *rank_out = rank;
     return true;
 }
+
+cudaError_t color_sum_tf32_big(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
+                               double* d_meh, cudaStream_t st);
 
 cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_jamps, long rows_padded, const RowMap& map,
                            double* d_meh, cudaStream_t st, int tile_major);
@@ -469,6 +482,8 @@ cudaError_t color_sum_tf32(int ncolor, const void* d_factor_img, const void* d_j
 cudaError_t color_sum_tensor(bool is_fp64, int ncolor, const void* d_cmat, const void* d_factor, const void* d_jamps,
                              long rows_padded, const RowMap& map, double* d_meh, cudaStream_t st, int tile_major)
 {
+    if (!is_fp64 && ncolor == 720)           // operand layout only (the generic diagram kernel writes it)
+        return tile_major == 2 ? color_sum_tf32_big(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st) : cudaErrorInvalidValue;
     if (!is_fp64) return color_sum_tf32(ncolor, d_factor, d_jamps, rows_padded, map, d_meh, st, tile_major);
     if (tile_major) return cudaErrorInvalidValue;
     if (!d_factor) return cudaErrorInvalidValue;

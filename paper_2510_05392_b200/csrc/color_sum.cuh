@@ -51,6 +51,10 @@ void color_cholesky_fragments(int ncp, const std::vector<double>& lp, std::vecto
 
 // host: factor of the (positive semi-definite) 720 x 720 matrix in the fragment order of the large-matrix DMMA kernel
 bool color_cholesky_big(int ncolor, const int* cmat, std::vector<double>& frag, int* rank_out);
+// host: the row-major factor itself (zero columns at null pivots)
+bool color_cholesky_semidef(int n, const int* cmat, std::vector<double>& L, int* rank_out);
+// host: TF32 image [hi | lo] of that factor, slice by slice in the order color_sum_tf32_big_kernel consumes it (720 colours)
+bool tf32_big_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img);
 
 // host: two-term TF32 image [hi | lo] of the Cholesky factor in the tcgen05 shared-memory layout (color_sum_tf32.cu)
 bool tf32_build_factor_image(int ncolor, const int* cmat, std::vector<float>& img);

@@ -28,6 +28,14 @@ struct HsgDev {
 
 static constexpr int HSG_THREADS = 256;
 
+// fp32 -> TF32 (10 explicit significand bits), round to nearest: the tensor core would truncate
+__device__ __forceinline__ float to_tf32(float x)
+{
+    unsigned u;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
+    return __uint_as_float(u);
+}
+
 __device__ __forceinline__ int sub_variant4(int var, int code)
 {
     return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2) |
@@ -239,8 +247,20 @@ __global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgD
                     const int pos = a.d_pos[h];
                     if (pos >= 0) {
                         const size_t row = (size_t)e * a.nrow_evt + pos;
-                        out[(size_t)fl.x * a.rows + row] = T2(re[q]);
-                        out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(im[q]);
+                        if (a.tile_major == 2) {
+                            // tcgen05 operand layout (color_sum_tf32_big.cu): per 128-row tile and part, chunks of 24 colours as
+                            // K-major core matrices [row / 8][colour quad][row % 8][colour % 4], values rounded to TF32
+                            if constexpr (sizeof(T2) == 4) {
+                                const unsigned m = (unsigned)(row & 127);
+                                const int jc = fl.x;
+                                float* __restrict__ o = reinterpret_cast<float*>(out) + (row >> 7) * (size_t)(256 * d.ncolor) +
+                                                        (size_t)(jc / 24) * (24 * 128) + (m >> 3) * 192 + ((jc % 24) >> 2) * 32 + (m & 7) * 4 + (jc & 3);
+                                o[0] = to_tf32((float)re[q]); o[(size_t)d.ncolor * 128] = to_tf32((float)im[q]);
+                            }
+                        } else {
+                            out[(size_t)fl.x * a.rows + row] = T2(re[q]);
+                            out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(im[q]);
+                        }
                     }
                 }
             }

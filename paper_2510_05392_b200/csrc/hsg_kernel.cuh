@@ -32,7 +32,7 @@ struct HsgContext;
 cudaError_t hsg_create(int ngluon, HsgContext** out);
 void hsg_destroy(HsgContext* c);
 const HsgTables* hsg_host_tables(const HsgContext* c);
-// jamps [2][ncolor][rows] (HsLaunch::tile_major is ignored: 0)
+// jamps [2][ncolor][rows] (tile_major = 0) or, fp32 only, the tcgen05 operand layout (tile_major = 2, ncolor % 24 == 0)
 cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
 
 }  // namespace mg

@@ -429,9 +429,9 @@ def test_gg_ttxgggg_parity_and_mask(B):
     _assert_fp64_parity(process, mom, me, _relerr(me, ref))
     meh = proc.last_helicity_terms(nevt).cpu().numpy()
     assert (np.abs(meh - ref_h.T) / ref[None, :]).max() < 1e-10
-    # only MG_FP64, only the helicity-shared kernel
+    # no all-fp32 build, only the helicity-shared kernel
     with pytest.raises(Exception):
-        B.init_process(process, "mixed")
+        B.init_process(process, "fp32")
     with pytest.raises(Exception):
         proc.set_option("diagrams", 0)
     # a partial helicity mask: the masked-out rows are not computed into the sum
@@ -469,4 +469,35 @@ def test_gg_ttxgggg_full_batch_sampled(B):
     for _ in range(3):
         proc.sigma_batch(d_mom, out)
     assert proc.get_option("graph_replays") >= 1 and np.array_equal(out.cpu().numpy(), me)
+    proc.close()
+
+
+def test_gg_ttxgggg_mixed(B):
+    """MG_MIXED for g g -> t tbar g g g g: fp64 amplitudes, jamps rounded to TF32 in the tcgen05 operand layout, the 720-colour
+    contraction tiled in N and K on the 5th-generation tensor cores (color_sum_tf32_big.cu) -- against the oracle (bar of the
+    mixed mode: median 2e-4, max 1e-3) and against the handle's own fp64 result; 200 events = 400 row tiles, ragged"""
+    process, nevt = "gg_ttxgggg", 200
+    mom = inputs.momenta(process, nevt, seed=3)
+    d_mom = torch.from_numpy(mom).cuda()
+    p64 = B.init_process(process, "fp64")
+    me64 = p64.sigma_batch(d_mom).cpu().numpy()
+    p64.close()
+    proc = B.init_process(process, "mixed")
+    me = proc.sigma_batch(d_mom).cpu().numpy()
+    err = _relerr(me, me64)
+    _histogram(err, "gg_ttxgggg mixed vs fp64")
+    assert np.median(err) < 2e-4 and err.max() < 1e-3
+    ref = _oracle(process, mom[:24])
+    assert _relerr(me64[:24], ref).max() < 1e-10
+    # colour selection reads the operand layout
+    rng = np.random.default_rng(2)
+    rc = rng.random(nevt)
+    _, _, sc = proc.sigma_batch_ex(d_mom, None, None, torch.from_numpy(rc).cuda())
+    sc = sc.cpu().numpy()
+    from oracle import selection
+    w = selection.color_weights(process, mom[:6], inputs.PARAMS, np.arange(256))
+    ok = ~_near_boundary(w, rc[:6], 1e-4)
+    cum = np.cumsum(w, axis=1)
+    want = np.array([int(np.searchsorted(cum[i], rc[i] * cum[i, -1], side="right")) for i in range(6)])
+    assert (sc[:6][ok] == want[ok]).all() and sc.min() >= 0 and sc.max() < 720
     proc.close()
