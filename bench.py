@@ -323,6 +323,17 @@ def main():
             cs_roofline = {"bound": "tensor", "kernel": "color_sum_big_kernel" if nc > 128 else "color_sum_dmma2_kernel", "achieved": ach, "peak": dmma_peak, "unit": "TFLOP/s",
                            "frac": ach / dmma_peak, "kernel_ms": cs_ms, "flop_counted": "issued DMMA (triangular k-step x n-tile pairs)",
                            "peak_source": "mma.sync.m8n8k4.f64 probe measured in this run (mg_measure_peak kind 2)"}
+        elif nc > 128:
+            # 720 colours: compute bound on the TF32 tensor path; issued MMA flop = per 128-row tile and part, per (block of
+            # 240 columns, 24-colour chunk on or below the block's diagonal) two products (L_hi, L_lo) of 128 x width x 24
+            widths = [min(240, (24 * (c - 10 * b + 1) + 15) // 16 * 16) for b in range(3) for c in range(10 * b, 30)]
+            flop = rows / 128 * 2 * sum(2 * 2.0 * 128 * w * 24 for w in widths)
+            tf32_peak = B.measure_peak(3, local)
+            ach = flop / (cs_ms * 1e-3) * 1e-12
+            cs_roofline = {"bound": "tensor", "kernel": "color_sum_tf32_big_kernel", "achieved": ach, "peak": tf32_peak, "unit": "TFLOP/s",
+                           "frac": ach / tf32_peak if tf32_peak else None, "kernel_ms": cs_ms,
+                           "flop_counted": "issued tcgen05.mma kind::tf32 (J Lhi + J Llo, triangular in 24-colour chunks)",
+                           "peak_source": "tcgen05 kind::tf32 probe measured in this run (mg_measure_peak kind 3)"}
         elif not proc.get_option("hs_color_alu"):
             nbytes = rows * nc * 2 * 4.0
             ach = nbytes / (cs_ms * 1e-3) * 1e-9
@@ -340,7 +351,7 @@ def main():
                       "diagrams": "helicity-shared (CTA = event, thread = helicity)" if shared else "thread = (event, helicity)",
                       "schedule": "helicity streams" if args.schedule else ("helicity = thread index" if shared else "helicity = grid.y"),
                       "color_sum": (("DMMA (mma.sync f64), Cholesky form" if args.precision in ("fp64", "d") else
-                                     ("ALU kernel" if proc.get_option("hs_color_alu") else "tcgen05 kind::tf32, split, Cholesky form"))
+                                     ("ALU kernel" if proc.get_option("hs_color_alu") and process != "gg_ttxgggg" else "tcgen05 kind::tf32, split, Cholesky form"))
                                     if shared else ("tensor" if proc.get_option("color_sum") == 1 else "fused ALU")),
                       "jamp_chunk_mib": proc.get_option("jamp_chunk_mib"),
                       "l2": "256 MiB device memset between timed steps (outside the per-step event pairs)"},
@@ -385,8 +396,6 @@ def main():
             per = {}
             for pname in inputs.PROCESSES:
                 for prec in ("fp64", "mixed"):
-                    if pname == "gg_ttxgggg" and prec != "fp64":          # MG_FP64 only
-                        continue
                     if pname == process and prec == args.precision:
                         per[f"{pname}/{prec}"] = {"MEs_per_s": r["value"], "ms_per_batch": r["ms_per_step"]}
                         continue

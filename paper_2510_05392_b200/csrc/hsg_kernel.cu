@@ -70,27 +70,28 @@ __device__ __forceinline__ void axpy(double sg, const wf<double>& r, wf<double>&
 }
 
 // one entry for the 8 helicity combinations q of particles 0, 1, 2 (bit i of q = particle i): XMASK = which of them are legs
-// of X.  They are the lowest-numbered particles, hence the lowest bits of the variant index of whichever object holds them.
+// of X.  They are the lowest-numbered particles, hence the HIGHEST bits of the variant index of whichever object holds them
+// (descending particle order): the variants a thread needs are sx (sy) bytes apart, index bit 0 = the largest of the three.
 template <int XMASK>
-__device__ __forceinline__ void p3_entry8(const char* __restrict__ px, const char* __restrict__ py, size_t plane, double sg,
-                                          double (&re)[8], double (&im)[8])
+__device__ __forceinline__ void p3_entry8(const char* __restrict__ px, const char* __restrict__ py, size_t plane, unsigned sx,
+                                          unsigned sy, double sg, double (&re)[8], double (&im)[8])
 {
     constexpr int NX = 1 << (((XMASK >> 0) & 1) + ((XMASK >> 1) & 1) + ((XMASK >> 2) & 1)), NY = 8 / NX;
 #pragma unroll
     for (int c = 0; c < 4; c++) {
         double2 x[NX], y[NY];
 #pragma unroll
-        for (int i = 0; i < NX; i++) x[i] = *reinterpret_cast<const double2*>(px + c * plane + 16 * i);
+        for (int i = 0; i < NX; i++) x[i] = *reinterpret_cast<const double2*>(px + c * plane + (size_t)i * sx);
 #pragma unroll
         for (int i = 0; i < NY; i++) {
-            y[i] = *reinterpret_cast<const double2*>(py + c * plane + 16 * i);
+            y[i] = *reinterpret_cast<const double2*>(py + c * plane + (size_t)i * sy);
             y[i].x *= sg; y[i].y *= sg;
         }
 #pragma unroll
         for (int q = 0; q < 8; q++) {
             int xo = 0, yo = 0, nx = 0, ny = 0;
 #pragma unroll
-            for (int b = 0; b < 3; b++) {
+            for (int b = 2; b >= 0; b--) {
                 if ((XMASK >> b) & 1) { xo |= ((q >> b) & 1) << nx; nx++; }
                 else { yo |= ((q >> b) & 1) << ny; ny++; }
             }
@@ -205,9 +206,9 @@ __global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgD
         }
         __syncthreads();
         // phase 3: the colour flows, one warp per flow: lane = helicities of particles 3 .. npar-1 (the low bits of h), and
-        // every thread carries the 8 helicity combinations of particles 0, 1, 2 in registers.  Those particles are the first
-        // legs of X or of Y, so the variants a thread needs are CONSECUTIVE slots: 2^nx of X and 2^(3-nx) of Y serve 8 dot
-        // products (9 or 6 wavefunction loads instead of 16), p3_entry8.
+        // every thread carries the 8 helicity combinations of particles 0, 1, 2 in registers: 2^nx variants of X and 2^(3-nx) of
+        // Y serve 8 dot products (9 or 6 wavefunction loads instead of 16), p3_entry8.  Variant indices run over the legs in
+        // DESCENDING particle order, so the lanes of the warp read one contiguous run of slots per load.
         {
             const int lane = tid & 31, nlow = nh >> 3;
             for (int f = tid >> 5; f < d.nflow * (nlow >> 5); f += NT >> 5) {
@@ -229,15 +230,16 @@ __global__ void __launch_bounds__(HSG_THREADS, 2) hsg_diagrams_kernel(const HsgD
                     const char* __restrict__ px = area + 16 * (size_t)(cur.x + (int)(cv & 0xFFu));
                     const char* __restrict__ py = area + 16 * (size_t)(cur.y + (int)(cv >> 8));
                     const double sg = (cur.w & 1) ? -1.0 : 1.0;
+                    const unsigned sx = 16u << ((cur.w >> 4) & 7), sy = 16u << ((cur.w >> 7) & 7);
                     switch ((cur.w >> 1) & 7) {
-                        case 0: p3_entry8<0>(px, py, plane, sg, re, im); break;
-                        case 1: p3_entry8<1>(px, py, plane, sg, re, im); break;
-                        case 2: p3_entry8<2>(px, py, plane, sg, re, im); break;
-                        case 3: p3_entry8<3>(px, py, plane, sg, re, im); break;
-                        case 4: p3_entry8<4>(px, py, plane, sg, re, im); break;
-                        case 5: p3_entry8<5>(px, py, plane, sg, re, im); break;
-                        case 6: p3_entry8<6>(px, py, plane, sg, re, im); break;
-                        default: p3_entry8<7>(px, py, plane, sg, re, im); break;
+                        case 0: p3_entry8<0>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 1: p3_entry8<1>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 2: p3_entry8<2>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 3: p3_entry8<3>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 4: p3_entry8<4>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 5: p3_entry8<5>(px, py, plane, sx, sy, sg, re, im); break;
+                        case 6: p3_entry8<6>(px, py, plane, sx, sy, sg, re, im); break;
+                        default: p3_entry8<7>(px, py, plane, sx, sy, sg, re, im); break;
                     }
                 }
 #pragma unroll

@@ -10,7 +10,9 @@ PAPER.md:424-444, here inside one kernel.  One group of colour flows (every pair
 Scratch area of one CTA: four component planes, byte(c, slot) = c * 16 * nslot + 16 * slot; variant v of an object with
 first slot s0 is slot s0 + v; the objects come first (slots [0, ns_obj)), then the pair objects.
 
-Packing (int32; variant bit j <-> helicity of the j-th leg in ascending particle order, 1 = +):
+Packing (int32; variant bit j <-> helicity of the j-th leg in DESCENDING particle order, 1 = +: phase 3 runs lane = the
+helicities of the five highest-numbered particles, so the variants the lanes of a warp read are the LOWEST bits of the index --
+one contiguous run of 16-byte words, one L1 wavefront instead of four; measured in profiles/r3_gg_ttxgggg.md):
   obj[i]     = { first slot, L | legset << 8, first term, number of terms }                      (sorted by L = number of legs)
   term[t]    = { op | negative << 8 | legset(arg0) << 16 | legset(arg1) << 24, word(arg0), word(arg1), word(arg2) }
                word(arg) = first slot of the argument object | code << 16, code = 4 x 3 bits: position in the parent's variant
@@ -22,7 +24,9 @@ Packing (int32; variant bit j <-> helicity of the j-th leg in ascending particle
   xitem[i]   = { first term | terms << 24, slot | variant << 20 | vector-valued << 28 }: one variant of a pair object; sorted
                by the sequence of opcodes.  Vector-valued (opcodes >= 10): components 1-3 are negated at the store, so that
                the contraction with Y is a plain sum over the four components
-  entry[e]   = { first slot of X, first slot of Y, row of vtab, negative | (particles 0, 1, 2 that are legs of X) << 1 }
+  entry[e]   = { first slot of X, first slot of Y, row of vtab, negative | (particles 0, 1, 2 that are legs of X) << 1 |
+                 lx << 4 | ly << 7 }: lx (ly) = number of legs of X (Y) other than particles 0, 1, 2 -- those three are the
+                 HIGHEST bits of the variant index, so the variants a thread of phase 3 needs are 2^lx (2^ly) slots apart
   flow[f]    = { colour index, first entry, entries, 0 }
   vtab[row][h] (uint16) = variant of X | variant of Y << 8 for helicity combination h (bit npar-1-p of h = particle p)
 """
@@ -38,7 +42,12 @@ FLOPS = {"ext_v": 40, "ext_ql": 60, "ext_qr": 60, "v3": 150, "v4": 90, "ffv_l": 
          "x_row": 72, "x_col": 72, "x_bil": 80, "x_v3": 134, "x_v4": 112, "x_v4s": 170}
 
 
+def _desc(legs):
+    return tuple(sorted(legs, reverse=True))
+
+
 def _code(parent, child):
+    parent, child = _desc(parent), _desc(child)
     pos = [parent.index(p) for p in child]
     assert len(pos) <= 4 and all(q < 7 for q in pos)
     pos += [7] * (4 - len(pos))
@@ -119,11 +128,12 @@ def build(n):
 
     def vrow(xlegs):
         if xlegs not in vrow_id:
-            ylegs = tuple(p for p in range(npar) if p not in xlegs)
+            ylegs = _desc(p for p in range(npar) if p not in xlegs)
+            xlegs_d = _desc(xlegs)
             row = []
             for h in range(1 << npar):
                 hb = [(h >> (npar - 1 - p)) & 1 for p in range(npar)]
-                vx = sum(hb[p] << j for j, p in enumerate(xlegs))
+                vx = sum(hb[p] << j for j, p in enumerate(xlegs_d))
                 vy = sum(hb[p] << j for j, p in enumerate(ylegs))
                 assert vx < 256 and vy < 256
                 row.append(vx | (vy << 8))
@@ -137,7 +147,9 @@ def build(n):
         for xs, yo, sign in g["entries"][j]:
             x = g["xobjs"][xs]
             assert set(x["legs"]) | set(prog.objs[yo].legs) == set(range(npar))
-            flags = (1 if sign < 0 else 0) | (sum(1 << p for p in x["legs"] if p < 3) << 1)
+            nfx = sum(1 for p in x["legs"] if p < 3)
+            lx, ly = len(x["legs"]) - nfx, (npar - len(x["legs"])) - (3 - nfx)
+            flags = (1 if sign < 0 else 0) | (sum(1 << p for p in x["legs"] if p < 3) << 1) | (lx << 4) | (ly << 7)
             entries.append([xslot[xs], slot0[yo], vrow(tuple(x["legs"])), flags])
         flows.append([j, e0, len(entries) - e0, 0])
     i32 = lambda a, w: np.asarray(a, dtype=np.int64).astype(np.int32).reshape(-1, w)

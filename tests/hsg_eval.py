@@ -105,12 +105,15 @@ def evaluate(T, mom, mt, wt):
             X = area[int(xs) + (vt & 0xFF)]
             Y = area[int(ys) + (vt >> 8)]
             J[j] += (-1 if int(flags) & 1 else 1) * np.sum(X * Y, axis=1)
-            # bits 1..3: which of particles 0, 1, 2 are legs of X -- they must then be the lowest bits of X's variant index
+            # bits 1..3: which of particles 0, 1, 2 are legs of X; they are the highest bits of the variant index of the object
+            # that holds them (descending particle order), above its lx (ly) other legs (bits 4..6, 7..9)
+            fl = int(flags)
+            lx, ly = (fl >> 4) & 7, (fl >> 7) & 7
             for i in range(3):
                 hbit = 1 << (npar - 1 - i)
                 dx = (vt[hbit] & 0xFF) - (vt[0] & 0xFF)
                 dy = (vt[hbit] >> 8) - (vt[0] >> 8)
-                inx = (int(flags) >> (1 + i)) & 1
-                before = sum(1 for b in range(i) if ((int(flags) >> (1 + b)) & 1) == inx)
-                assert (dx, dy) == ((1 << before, 0) if inx else (0, 1 << before))
+                inx = (fl >> (1 + i)) & 1
+                above = sum(1 for b in range(i + 1, 3) if ((fl >> (1 + b)) & 1) == inx)       # larger fixed particles sit below
+                assert (dx, dy) == ((1 << (lx + above), 0) if inx else (0, 1 << (ly + above)))
     return J
