@@ -59,9 +59,10 @@ enum { MG_DIAG_THREAD = 0, MG_DIAG_SHARED = 1 };
 
 /* Create a process.  name: "epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg" (BASELINE.json configs;
  * Table 2), or "gg_ttxgggg" (g g -> t tbar g g g g, Table 2's 2 -> 6 row: 15 495 diagrams, 720 colour
- * flows, 256 helicities; Tables 5-8).  The latter runs in MG_FP64 with MG_DIAG_SHARED only (generic
+ * flows, 256 helicities; Tables 5-8).  The latter runs with MG_DIAG_SHARED only (generic
  * helicity-shared kernel, the event's wavefunctions in a per-CTA scratch area in global memory owned by the handle: about
- * 1 GB of device memory per handle; 720-colour FP64 tensor-core colour sum): any other precision -> MG_EINVAL.
+ * 0.5 GB of device memory per handle) in MG_FP64 (720-colour FP64 tensor-core colour sum) and MG_MIXED (the same on tcgen05
+ * kind::tf32); MG_FP32 -> MG_EINVAL.
  * Parameters start at the BASELINE.json card.  *out is NULL on failure. */
 int mg_init_process(const char* name, int precision, int device, mg_process** out);
 
@@ -158,7 +159,9 @@ int mg_last_launch_count(const mg_process* p, int* launches);
 /* Stand-alone colour sum over rows of jamps already in DEVICE memory, layout [2][ncolor][nrows] (re block,
  * im block) of the precision's colour-sum type (fp64 for MG_FP64, fp32 otherwise):
  *   d_out[r] = sum_ij (Re J_i C_ij Re J_j + Im J_i C_ij Im J_j),  C = integer numerators (denominator NOT applied).
- * impl = MG_CS_FUSED runs the scalar-ALU triangular kernel, MG_CS_TENSOR the tensor-core kernel. */
+ * impl = MG_CS_FUSED runs the scalar-ALU triangular kernel, MG_CS_TENSOR the tensor-core kernel.
+ * "gg_ttxgggg" (720 colours): MG_CS_TENSOR in MG_FP64 only (the tcgen05 kernel of that size reads the operand layout the
+ * diagram kernel writes, not this one; there is no scalar kernel): anything else -> MG_ECUDA "invalid argument". */
 int mg_color_sum(mg_process* p, int impl, const void* d_jamps, long nrows, double* d_out, void* cuda_stream);
 
 /* Copy the integer colour matrix numerators [ncolor*ncolor] and the common denominator to HOST memory. */

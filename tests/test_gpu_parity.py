@@ -129,6 +129,18 @@ def test_standalone_color_sum_kernels(B):
                 out = proc.color_sum(dJ, impl).cpu().numpy()
                 assert np.abs(out / ref - 1).max() < tol, (process, prec, impl, np.abs(out / ref - 1).max())
             proc.close()
+    # 720 colours (g g -> t tbar g g g g): the semi-definite matrix (rank 685) through its factor with zero columns, fp64
+    # tensor kernel; random jamps have components in the null space of C, which must contribute exactly nothing
+    proc = B.init_process("gg_ttxgggg", "fp64")
+    C, den = proc.color_matrix()
+    assert den == 1944 and C.shape == (720, 720)
+    J = rng.normal(size=(2, 720, 256))
+    ref = np.einsum("pir,ij,pjr->r", J, C.astype(np.float64), J)
+    out = proc.color_sum(torch.from_numpy(J).cuda(), 1).cpu().numpy()
+    assert np.abs(out / ref - 1).max() < 1e-11
+    with pytest.raises(Exception):
+        proc.color_sum(torch.from_numpy(J).cuda(), 0)          # no scalar-ALU kernel at this size
+    proc.close()
 
 
 def test_edge_cases(B):
