@@ -156,6 +156,21 @@ int mg_last_stage_ms(mg_process* p, float ms[3]);
 /* Number of kernels the last mg_sigma_batch launched (diagram + colour-sum + helicity-sum kernels). */
 int mg_last_launch_count(const mg_process* p, int* launches);
 
+/* The same batch for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc).  Only for "gg_ttxgggg", the process whose diagram kernel needs scratch memory: here the
+ * scratch is a file-scope static __device__ array of 26 MiB inside the library (8 persistent CTAs' worth; every GPU that
+ * loads the library holds it until the process exits) instead of the handle's own areas, so the call makes no cudaMalloc /
+ * cudaFree / allocating library call and does not synchronise.  Inputs, output and workspace are the caller's, as in
+ * mg_sigma_batch (ws_bytes >= mg_workspace_bytes(p, nevt)).  Limits: nevt <= MG_NOALLOC_MAX_EVENTS, else MG_EINVAL and nothing
+ * is launched; a good-helicity list must already be installed (mg_helicity_filter / mg_set_good_helicities), else MG_ESTATE;
+ * any other process -> MG_EINVAL.  Throughput is that of 8 CTAs (about 1/18 of the GPU).  ALL calls, from every handle of the
+ * process, share the one array: calls that may overlap on the GPU (different streams) race on it -- serialise them.  The
+ * array keeps the previous call's contents; the kernel writes every word before reading it, nothing needs clearing.
+ * Results are bit-identical to mg_sigma_batch's. */
+#define MG_NOALLOC_MAX_EVENTS 256
+int mg_sigma_batch_noalloc(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                           size_t ws_bytes, void* cuda_stream);
+
 /* Stand-alone colour sum over rows of jamps already in DEVICE memory, layout [2][ncolor][nrows] (re block,
  * im block) of the precision's colour-sum type (fp64 for MG_FP64, fp32 otherwise):
  *   d_out[r] = sum_ij (Re J_i C_ij Re J_j + Im J_i C_ij Im J_j),  C = integer numerators (denominator NOT applied).

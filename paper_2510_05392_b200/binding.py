@@ -23,9 +23,11 @@ _ERR = {-1: "MG_EINVAL", -2: "MG_ENODEV", -3: "MG_ENOMEM", -4: "MG_ECUDA", -5: "
 
 EXPORTS = ["mg_init_process", "mg_process_info", "mg_process_flops", "mg_set_parameters", "mg_set_option", "mg_get_option",
            "mg_workspace_bytes", "mg_workspace_bytes_ex", "mg_helicity_filter", "mg_set_good_helicities", "mg_sigma_batch",
-           "mg_sigma_batch_ex",
+           "mg_sigma_batch_ex", "mg_sigma_batch_noalloc",
            "mg_sigma_batch_host", "mg_last_helicity_terms", "mg_last_stage_ms", "mg_last_launch_count", "mg_color_sum", "mg_color_matrix",
            "mg_measure_peak", "mg_last_error", "mg_destroy"]
+
+NOALLOC_MAX_EVENTS = 256          # MG_NOALLOC_MAX_EVENTS of include/mg5_b200.h
 
 _lib = None
 
@@ -55,6 +57,7 @@ def load_library() -> ctypes.CDLL:
     lib.mg_helicity_filter.argtypes = [vp, vp, ctypes.c_int, vp, ctypes.c_size_t, vp, ctypes.POINTER(ctypes.c_ubyte), ip]
     lib.mg_set_good_helicities.argtypes = [vp, ctypes.POINTER(ctypes.c_ubyte)]
     lib.mg_sigma_batch.argtypes = [vp, vp, ctypes.c_int, vp, vp, ctypes.c_size_t, vp]
+    lib.mg_sigma_batch_noalloc.argtypes = [vp, vp, ctypes.c_int, vp, vp, ctypes.c_size_t, vp]
     lib.mg_sigma_batch_ex.argtypes = [vp, vp, ctypes.c_int, vp, vp, vp, vp, vp, vp, vp, ctypes.c_size_t, vp]
     lib.mg_workspace_bytes_ex.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.mg_workspace_bytes_ex.restype = ctypes.c_size_t
@@ -183,6 +186,19 @@ class Process:
         ws = self._workspace(nevt)
         self._check(self.lib.mg_sigma_batch(self.h, d_momenta.data_ptr(), nevt, d_me.data_ptr(), ws.data_ptr(), ws.numel(),
                                             self._stream()))
+        return d_me
+
+    def sigma_batch_noalloc(self, d_momenta, d_me=None):
+        """mg_sigma_batch_noalloc: as sigma_batch, the library allocating nothing (gg_ttxgggg, <= NOALLOC_MAX_EVENTS events, a
+        helicity list already installed).  The output and the workspace are allocated HERE, by the caller's side."""
+        t = self._torch
+        assert d_momenta.is_cuda and d_momenta.dtype == t.float64 and d_momenta.is_contiguous()
+        nevt = d_momenta.shape[0]
+        if d_me is None:
+            d_me = t.empty(nevt, dtype=t.float64, device=d_momenta.device)
+        ws = self._workspace(nevt)
+        self._check(self.lib.mg_sigma_batch_noalloc(self.h, d_momenta.data_ptr(), nevt, d_me.data_ptr(), ws.data_ptr(), ws.numel(),
+                                                    self._stream()))
         return d_me
 
     def sigma_batch_ex(self, d_momenta, alphas=None, rndhel=None, rndcol=None):

@@ -256,6 +256,7 @@ extern "C" int mg_init_process(const char* name, int precision, int device, mg_p
         cudaError_t e = hsg_create(d->ngluon, &p->hsg);
         if (e != cudaSuccess) { g_init_error = std::string("hsg_create: ") + cudaGetErrorString(e); mg_destroy(p); return e == cudaErrorMemoryAllocation ? MG_ENOMEM : MG_ECUDA; }
         p->diagrams = MG_DIAG_SHARED;
+        hsg_static_setup(p->hsg);          // mg_sigma_batch_noalloc (a failure is reported by that call, not here)
     } else if (hs_tables(d->ngluon) && precision != MG_FP32) {       // helicity-shared program: g g -> t tbar + >= 2 g
         cudaError_t e = hs_create(d->ngluon, &p->hs);
         if (e != cudaSuccess) { g_init_error = std::string("hs_create: ") + cudaGetErrorString(e); mg_destroy(p); return MG_ECUDA; }
@@ -941,6 +942,50 @@ extern "C" int mg_color_matrix(const mg_process* p, int* h_numerators, int* deno
     if (!p) return MG_EINVAL;
     if (h_numerators) memcpy(h_numerators, p->d->cmat, sizeof(int) * p->d->ncolor * p->d->ncolor);
     if (denominator) *denominator = p->d->cden;
+    return MG_OK;
+}
+
+// The entry point that allocates nothing (include/mg5_b200.h): diagram kernel with its scratch areas in the static __device__
+// array of csrc/hsg_kernel.cu, colour sum, helicity sum -- the launch sequence of sigma_batch_impl for the generic
+// helicity-shared kernel, written out here so that no existing path changes.  No cudaMalloc / cudaFree / allocating library
+// call, no host-side containers on the success path, no synchronisation, no helicity filter.
+extern "C" int mg_sigma_batch_noalloc(mg_process* p, const double* d_momenta, int nevt, double* d_me, void* d_workspace,
+                                      size_t ws_bytes, void* cuda_stream)
+{
+    if (!p || nevt < 0) return fail(p, MG_EINVAL, "bad arguments");
+    if (!p->hsg) return fail(p, MG_EINVAL, "mg_sigma_batch_noalloc: this process has no kernel that uses scratch memory (gg_ttxgggg only)");
+    if (nevt > MG_NOALLOC_MAX_EVENTS) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "mg_sigma_batch_noalloc: nevt = %d, at most %d events per call (static scratch: 26 MiB, %d CTAs)",
+                 nevt, MG_NOALLOC_MAX_EVENTS, hsg_static_ctas(p->hsg));
+        return fail(p, MG_EINVAL, buf);
+    }
+    if (nevt == 0) return MG_OK;
+    if (!d_momenta || !d_me || !d_workspace) return fail(p, MG_EINVAL, "NULL buffer");
+    if (((size_t)d_workspace & 255) != 0) return fail(p, MG_EINVAL, "workspace must be 256-byte aligned");
+    if (p->good.empty())
+        return fail(p, MG_ESTATE, "mg_sigma_batch_noalloc: no good-helicity list (call mg_helicity_filter or mg_set_good_helicities first)");
+    if (hsg_static_ctas(p->hsg) < 1) return fail(p, MG_ESTATE, "mg_sigma_batch_noalloc: the static scratch array is too small for this process");
+    CUDA_TRY(p, cudaSetDevice(p->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nhel = (int)p->good.size();
+    const long rows = (long)nhel * nevt, rows_p = color_sum_padded_rows(rows);
+    const size_t meh_b = align256((size_t)nhel * nevt * sizeof(double)), gfac_b = align256((size_t)nevt * sizeof(double));
+    if (ws_bytes < meh_b + gfac_b + align256((size_t)rows_p * p->d->ncolor * 2 * cs_elem(p)))
+        return fail(p, MG_EINVAL, "workspace too small (mg_workspace_bytes)");
+    double* d_meh = (double*)d_workspace;
+    char* d_j = (char*)d_workspace + meh_b + gfac_b;
+    HsLaunch a;
+    a.mom = d_momenta; a.nevt = nevt; a.d_pos = p->d_pos; a.nrow_evt = nhel;
+    a.d_jamps = d_j; a.rows = rows_p; a.mt = p->mT; a.wt = p->wT;
+    a.tile_major = p->precision != MG_FP64 ? 2 : 0;
+    CUDA_TRY(p, hsg_launch_static(p->hsg, p->precision == MG_FP64, a, st));
+    RowMap map;
+    map.rows_valid = rows; map.hel_minor = nhel; map.evt_stride = nevt; map.e0 = 0; map.norm = make_norm(p);
+    CUDA_TRY(p, color_sum_tensor(p->precision == MG_FP64, p->d->ncolor, p->d_cmat, p->d_chol, d_j, rows_p, map, d_meh, st, a.tile_major));
+    helicity_sum_kernel<<<(nevt + 255) / 256, 256, 0, st>>>(d_meh, nhel, nevt, d_me);
+    CUDA_TRY(p, cudaGetLastError());
+    p->timed = false; p->launches = 3;
     return MG_OK;
 }
 

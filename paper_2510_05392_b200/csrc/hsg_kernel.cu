@@ -280,7 +280,20 @@ struct HsgContext {
     char* scratch = nullptr;
     int grid = 0;
     size_t smem = 0;
+    // hsg_launch_static: device address of hsg_static_scratch on this context's device (hsg_static_setup)
+    char* static_scratch = nullptr;
+    cudaError_t static_err = cudaErrorNotReady;
 };
+
+// Scratch areas for callers that cannot allocate (hsg_launch_static; include/mg5_b200.h mg_sigma_batch_noalloc): a file-scope
+// array of HSG_STATIC_BYTES = 26 MiB, enough for 8 persistent CTAs of g g -> t tbar g g g g (8 x 3 178 496 B).  Every GPU that
+// loads the library holds it until the process exits.  In HOST code this name is a host-side stand-in, not a device address:
+// the address a kernel may be given comes from cudaGetSymbolAddress (hsg_static_setup), per device.  All calls share the array
+// and it keeps the last call's contents; the kernel writes every slot of an event (phases 1 and 2) before it reads it (phase
+// 3), so nothing has to start at zero -- but two such launches that overlap on the GPU race on it.
+static constexpr size_t HSG_STATIC_BYTES = (size_t)26 << 20;
+static constexpr int HSG_STATIC_CTAS = 8;
+static __device__ __align__(256) unsigned char hsg_static_scratch[HSG_STATIC_BYTES];
 
 const HsgTables* hsg_host_tables(const HsgContext* c) { return c->t; }
 
@@ -321,6 +334,36 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     c->smem = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar);
     *out = c;
     return cudaSuccess;
+}
+
+// once per context, with the context's device current: the device address of the static scratch array on THAT device
+cudaError_t hsg_static_setup(HsgContext* c)
+{
+    void* ptr = nullptr;
+    c->static_err = cudaGetSymbolAddress(&ptr, hsg_static_scratch);
+    c->static_scratch = c->static_err == cudaSuccess ? (char*)ptr : nullptr;
+    return c->static_err;
+}
+
+// persistent CTAs the static array has room for (0: the process's scratch area does not fit at all)
+int hsg_static_ctas(const HsgContext* c)
+{
+    const size_t per_cta = 64 * (size_t)c->t->nslot;
+    const size_t n = HSG_STATIC_BYTES / per_cta;
+    return (int)(n < (size_t)HSG_STATIC_CTAS ? n : (size_t)HSG_STATIC_CTAS);
+}
+
+// the same kernel as hsg_launch with its scratch areas in the static array: allocates nothing, at most HSG_STATIC_CTAS CTAs
+cudaError_t hsg_launch_static(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st)
+{
+    if (a.nevt <= 0) return cudaSuccess;
+    if (!c->static_scratch) return c->static_err != cudaSuccess ? c->static_err : cudaErrorNotReady;
+    const int ctas = hsg_static_ctas(c);
+    if (ctas < 1) return cudaErrorInvalidValue;
+    const int grid = a.nevt < ctas ? a.nevt : ctas;
+    if (jamps_fp64) hsg_diagrams_kernel<double><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->static_scratch);
+    else hsg_diagrams_kernel<float><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->static_scratch);
+    return cudaGetLastError();
 }
 
 void hsg_destroy(HsgContext* c)

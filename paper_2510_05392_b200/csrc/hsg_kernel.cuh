@@ -35,4 +35,13 @@ const HsgTables* hsg_host_tables(const HsgContext* c);
 // jamps [2][ncolor][rows] (tile_major = 0) or, fp32 only, the tcgen05 operand layout (tile_major = 2, ncolor % 24 == 0)
 cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
 
+
+// The no-allocation variant (mg_sigma_batch_noalloc): the same kernel with its scratch areas in a file-scope static __device__
+// array of 26 MiB (8 CTAs' worth for g g -> t tbar g g g g).  hsg_static_setup: once per context with its device current
+// (resolves the array's device address, cudaGetSymbolAddress); hsg_launch_static calls no allocating routine.  Launches that
+// overlap on the GPU race on the shared array.
+cudaError_t hsg_static_setup(HsgContext* c);
+int hsg_static_ctas(const HsgContext* c);
+cudaError_t hsg_launch_static(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
+
 }  // namespace mg
