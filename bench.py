@@ -365,7 +365,7 @@ def main():
         sizes, n = [], 32
         while n < nevt:
             sizes.append(n)
-            n *= 4
+            n *= 2 if 512 <= n < 2048 else 4          # 32, 128, 512, 1024, 2048, 8192, ...: finer where the curves bend
         ramp = {"plain": {}, "graph": {}}
         for n in sizes:
             for mode in ("plain", "graph"):
