@@ -14,6 +14,7 @@
 // variants) read consecutive 16-byte words of one plane.
 #include <stdint.h>
 
+#include "generated/hsg_gen.h"
 #include "helas.cuh"
 #include "hsg_kernel.cuh"
 
@@ -23,11 +24,14 @@ struct HsgDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
     const int2* xitem; const int4* entry; const int4* flow; const unsigned short* vtab;
     int npar, ncolor, nslot, nlegsets, nxitem, nflow, nlevel;
+    int p3buf;                 // bytes of one phase-3 operand buffer: max over the entries of 64 (2^|X| + 2^|Y|)
     int p1_level[8];
 };
 
 // measured (4096 events, diagrams): 256 threads x 2 CTAs per SM 39.0 ms, 256 x 3 (80 registers, spills) 47.2, 512 x 1 38.0
 static constexpr int HSG_THREADS = 512, HSG_CTAS = 1;
+// phase 3: operand buffers per warp (entries in flight: the one being evaluated and HSG_P3_STAGES - 1 being copied)
+static constexpr int HSG_P3_STAGES = 2;          // (3 stages: 34.7 ms per 4096 events, 2: 33.7 -- the L1 cache left for phases 1 and 2 counts)
 
 // fp32 -> TF32 (10 explicit significand bits), round to nearest: the tensor core would truncate
 __device__ __forceinline__ float to_tf32(float x)
@@ -71,22 +75,30 @@ __device__ __forceinline__ void axpy(double sg, const wf<double>& r, wf<double>&
 }
 
 // one entry for the 8 helicity combinations q of particles 0, 1, 2 (bit i of q = particle i): XMASK = which of them are legs
-// of X.  They are the lowest-numbered particles, hence the HIGHEST bits of the variant index of whichever object holds them
-// (descending particle order): the variants a thread needs are sx (sy) bytes apart, index bit 0 = the largest of the three.
-template <int XMASK>
-__device__ __forceinline__ void p3_entry8(const char* __restrict__ px, const char* __restrict__ py, size_t plane, unsigned sx,
-                                          unsigned sy, double sg, double (&re)[8], double (&im)[8])
+// of X, LGX = number of legs of X (npar = 8: Y has 8 - LGX).  The three are the lowest-numbered particles, hence the HIGHEST
+// bits of the variant index of whichever object holds them (descending particle order), index bit 0 = the largest of the three.
+// bx = the entry's operand buffer in shared memory, [X: 4 components][2^LGX variants] then [Y: 4][2^(8 - LGX)], 16 bytes each;
+// vx, vy = this lane's variants (its five helicities): every offset below is a compile-time immediate.
+template <int XMASK, int LGX>
+__device__ __forceinline__ void p3_entry8(const char* __restrict__ bx, unsigned vx, unsigned vy, double sg, double (&re)[8], double (&im)[8])
 {
-    constexpr int NX = 1 << (((XMASK >> 0) & 1) + ((XMASK >> 1) & 1) + ((XMASK >> 2) & 1)), NY = 8 / NX;
+    constexpr int NFX = ((XMASK >> 0) & 1) + ((XMASK >> 1) & 1) + ((XMASK >> 2) & 1), NX = 1 << NFX, NY = 8 / NX;
+    constexpr int LGY = 8 - LGX, LX = LGX - NFX, LY = LGY - (3 - NFX);
+    static_assert(LX >= 0 && LY >= 0, "impossible entry kind");
+    const char* __restrict__ px = bx + 16 * vx;
+    const char* __restrict__ py = bx + (64 << LGX) + 16 * vy;
 #pragma unroll
     for (int c = 0; c < 4; c++) {
         double2 x[NX], y[NY];
 #pragma unroll
-        for (int i = 0; i < NX; i++) x[i] = *reinterpret_cast<const double2*>(px + c * plane + (size_t)i * sx);
+        for (int i = 0; i < NX; i++) {
+            x[i] = *reinterpret_cast<const double2*>(px + c * (16 << LGX) + i * (16 << LX));
+            if (NX < NY) { x[i].x *= sg; x[i].y *= sg; }
+        }
 #pragma unroll
         for (int i = 0; i < NY; i++) {
-            y[i] = *reinterpret_cast<const double2*>(py + c * plane + (size_t)i * sy);
-            y[i].x *= sg; y[i].y *= sg;
+            y[i] = *reinterpret_cast<const double2*>(py + c * (16 << LGY) + i * (16 << LY));
+            if (NX >= NY) { y[i].x *= sg; y[i].y *= sg; }
         }
 #pragma unroll
         for (int q = 0; q < 8; q++) {
@@ -102,6 +114,28 @@ __device__ __forceinline__ void p3_entry8(const char* __restrict__ px, const cha
     }
 }
 
+// copy of an entry's operands from the CTA's scratch area (planes of `plane` bytes; xs, ys = first slots of X and Y) into the
+// warp's buffer dst (shared-memory address): 4 x 2^LGX + 4 x 2^(8 - LGX) pieces of 16 bytes, lane = piece % 32
+template <int LGX>
+__device__ __forceinline__ void p3_stage(const char* __restrict__ area, unsigned plane, int xs, int ys, unsigned dst, int lane)
+{
+    constexpr int LGY = 8 - LGX, NX4 = 4 << LGX, NY4 = 4 << LGY;
+#pragma unroll
+    for (int t = 0; t < NX4 / 32; t++) {
+        const int i = lane + 32 * t;
+        const char* src = area + ((unsigned)(i >> LGX) * plane + 16u * (unsigned)(xs + (i & ((1 << LGX) - 1))));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (unsigned)i), "l"(src) : "memory");
+    }
+#pragma unroll
+    for (int t = 0; t < (NY4 + 31) / 32; t++) {
+        const int i = lane + 32 * t;
+        if (NY4 % 32 == 0 || i < NY4) {
+            const char* src = area + ((unsigned)(i >> LGY) * plane + 16u * (unsigned)(ys + (i & ((1 << LGY) - 1))));
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * (unsigned)(NX4 + i)), "l"(src) : "memory");
+        }
+    }
+}
+
 // T2 = type of the jamps buffer
 template <typename T2>
 __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(const HsgDev d, const HsLaunch a, char* __restrict__ scratch)
@@ -109,11 +143,16 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
     extern __shared__ __align__(16) double smd[];
     double* __restrict__ Ks = smd;                               // [nlegsets][4]
     double* __restrict__ pm = smd + 4 * d.nlegsets;              // [npar][4]
+    char* __restrict__ p3base = reinterpret_cast<char*>(pm + 4 * d.npar);   // [warp][HSG_P3_STAGES][p3buf]: operands of phase 3
     const int tid = threadIdx.x, NT = HSG_THREADS;
     const int npar = d.npar, nh = 1 << npar;
     const size_t plane = 16 * (size_t)d.nslot;
     char* __restrict__ area = scratch + (size_t)blockIdx.x * 4 * plane;
     T2* __restrict__ out = reinterpret_cast<T2*>(a.d_jamps);
+    int posq[8];                 // rows of this lane's 8 helicity combinations (phase 3; npar = 8: the low five bits = lane)
+#pragma unroll
+    for (int q = 0; q < 8; q++)
+        posq[q] = a.d_pos[(tid & 31) | ((q & 1) << (npar - 1)) | (((q >> 1) & 1) << (npar - 2)) | (((q >> 2) & 1) << (npar - 3))];
     auto arg = [&](int word, int var, wf<double>& w) { ldw(area, plane, (word & 0xFFFF) + sub_variant4(var, (word >> 16) & 0xFFF), w); };
 
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
@@ -210,44 +249,80 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
         // every thread carries the 8 helicity combinations of particles 0, 1, 2 in registers: 2^nx variants of X and 2^(3-nx) of
         // Y serve 8 dot products (9 or 6 wavefunction loads instead of 16), p3_entry8.  Variant indices run over the legs in
         // DESCENDING particle order, so the lanes of the warp read one contiguous run of slots per load.
+        // The operands of an entry -- ALL variants of X and of Y, 2 to 4.3 KB -- are copied from the scratch area (L2: the area
+        // is 3.2 MB, the L1 hit rate of direct loads was 51 %) into a shared-memory buffer of the warp by cp.async,
+        // HSG_P3_STAGES - 1 entries ahead of the one being evaluated: the L2 latency, which bounded the kernel (four dependent
+        // batches of loads per entry at 16 warps per SM), is off the critical path.
         {
-            const int lane = tid & 31, nlow = nh >> 3;
-            for (int f = tid >> 5; f < d.nflow * (nlow >> 5); f += NT >> 5) {
-                const int fi = f / (nlow >> 5), hl = (f % (nlow >> 5)) * 32 + lane;       // (npar = 8: one warp per flow)
-                const int4 fl = __ldg(d.flow + fi);
+            const int lane = tid & 31;
+            char* __restrict__ wbuf = p3base + (size_t)(tid >> 5) * (HSG_P3_STAGES * d.p3buf);
+            const unsigned wbuf_s = (unsigned)__cvta_generic_to_shared(wbuf);
+            auto stage = [&](const int4 en, int b) {
+                const unsigned dst = wbuf_s + (unsigned)(b * d.p3buf);
+                switch (((en.w >> 4) & 7) + __popc((en.w >> 1) & 7)) {
+                    case 4: p3_stage<4>(area, (unsigned)plane, en.x, en.y, dst, lane); break;
+                    case 5: p3_stage<5>(area, (unsigned)plane, en.x, en.y, dst, lane); break;
+                    default: p3_stage<6>(area, (unsigned)plane, en.x, en.y, dst, lane); break;
+                }
+            };
+            // Nothing a warp needs next may wait for memory: the flow header and the entry records of the warp's NEXT flow are
+            // fetched while the current one runs (lane i keeps entry i; an entry's record reaches all lanes by shuffles), and
+            // the variant lookup of entry k + 1 is fetched while entry k is evaluated.  (With 143 KB of the SM's memory in use as
+            // shared memory the L1 cache is small and mostly holds the operands of phases 1 and 2: a table read is often an L2
+            // round trip.)
+            const int NWARP = NT >> 5;
+            auto bcast = [&](const int4 m, int k) {
+                return make_int4(__shfl_sync(0xffffffffu, m.x, k), __shfl_sync(0xffffffffu, m.y, k), __shfl_sync(0xffffffffu, m.z, k),
+                                 __shfl_sync(0xffffffffu, m.w, k));
+            };
+            const unsigned short* __restrict__ vt = d.vtab + lane;
+            int f = tid >> 5;
+            int4 fl = make_int4(0, 0, 0, 0), myent = fl;
+            unsigned v = 0;
+            if (f < d.nflow) {
+                fl = __ldg(d.flow + f);
+                if (lane < fl.z) myent = __ldg(d.entry + fl.y + lane);
+                v = __ldg(vt + (size_t)__shfl_sync(0xffffffffu, myent.z, 0) * nh);
+            }
+            for (; f < d.nflow; f += NWARP) {
+                const int fn = f + NWARP;
+                int4 fl_n = make_int4(0, 0, 0, 0), myent_n = fl_n;
+                if (fn < d.nflow) fl_n = __ldg(d.flow + fn);
                 double re[8], im[8];
 #pragma unroll
                 for (int q = 0; q < 8; q++) re[q] = im[q] = 0.0;
-                const unsigned short* __restrict__ vt = d.vtab + hl;
-                int4 en = __ldg(d.entry + fl.y);
-                unsigned v = __ldg(vt + (size_t)en.z * nh);
+#pragma unroll
+                for (int k = 0; k < HSG_P3_STAGES - 1; k++) {            // one commit group per entry, empty past the end
+                    if (k < fl.z) stage(bcast(myent, k), k);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                }
+                int bcur = 0, bnew = HSG_P3_STAGES - 1;
                 for (int k = 0; k < fl.z; k++) {
-                    const int4 cur = en;
+                    if (k + HSG_P3_STAGES - 1 < fl.z) stage(bcast(myent, k + HSG_P3_STAGES - 1), bnew);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    const int4 cur = bcast(myent, k);
                     const unsigned cv = v;
-                    if (k + 1 < fl.z) {
-                        en = __ldg(d.entry + fl.y + k + 1);
-                        v = __ldg(vt + (size_t)en.z * nh);
-                    }
-                    const char* __restrict__ px = area + 16 * (size_t)(cur.x + (int)(cv & 0xFFu));
-                    const char* __restrict__ py = area + 16 * (size_t)(cur.y + (int)(cv >> 8));
+                    if (k == 0 && fn < d.nflow && lane < fl_n.z) myent_n = __ldg(d.entry + fl_n.y + lane);
+                    if (k + 1 < fl.z) v = __ldg(vt + (size_t)__shfl_sync(0xffffffffu, myent.z, k + 1) * nh);
+                    else if (fn < d.nflow) v = __ldg(vt + (size_t)__shfl_sync(0xffffffffu, myent_n.z, 0) * nh);
+                    asm volatile("cp.async.wait_group %0;" ::"n"(HSG_P3_STAGES - 1) : "memory");
+                    __syncwarp();
+                    const char* __restrict__ bx = wbuf + bcur * d.p3buf;
                     const double sg = (cur.w & 1) ? -1.0 : 1.0;
-                    const unsigned sx = 16u << ((cur.w >> 4) & 7), sy = 16u << ((cur.w >> 7) & 7);
-                    switch ((cur.w >> 1) & 7) {
-                        case 0: p3_entry8<0>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 1: p3_entry8<1>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 2: p3_entry8<2>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 3: p3_entry8<3>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 4: p3_entry8<4>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 5: p3_entry8<5>(px, py, plane, sx, sy, sg, re, im); break;
-                        case 6: p3_entry8<6>(px, py, plane, sx, sy, sg, re, im); break;
-                        default: p3_entry8<7>(px, py, plane, sx, sy, sg, re, im); break;
+                    const int lgx = ((cur.w >> 4) & 7) + __popc((cur.w >> 1) & 7);
+                    switch (((cur.w >> 1) & 7) | (lgx << 3)) {
+#define HSG_P3_CASE(M, LG) case (M) | ((LG) << 3): p3_entry8<M, LG>(bx, cv & 0xFFu, cv >> 8, sg, re, im); break;
+                        HSG_P3_COMBOS(HSG_P3_CASE)
+#undef HSG_P3_CASE
+                        default: break;                                  // (hsg_create refuses tables with another kind)
                     }
+                    __syncwarp();                                        // the buffer is free for the copy of entry k + STAGES
+                    bnew = bcur;
+                    bcur = bcur + 1 == HSG_P3_STAGES ? 0 : bcur + 1;
                 }
 #pragma unroll
                 for (int q = 0; q < 8; q++) {
-                    // q bit i = helicity of particle i = bit npar-1-i of h
-                    const int h = hl | ((q & 1) << (npar - 1)) | (((q >> 1) & 1) << (npar - 2)) | (((q >> 2) & 1) << (npar - 3));
-                    const int pos = a.d_pos[h];
+                    const int pos = posq[q];          // q bit i = helicity of particle i = bit npar-1-i of h; the low bits = lane
                     if (pos >= 0) {
                         const size_t row = (size_t)e * a.nrow_evt + pos;
                         if (a.tile_major == 2) {
@@ -266,6 +341,7 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                         }
                     }
                 }
+                fl = fl_n; myent = myent_n;
             }
         }
         __syncthreads();                 // the next event overwrites the scratch area
@@ -302,6 +378,7 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     *out = nullptr;
     const HsgTables* t = hsg_tables(ngluon);
     if (!t) return cudaErrorInvalidValue;
+    if (t->npar != 8) return cudaErrorInvalidValue;       // phase 3 maps lane = the helicities of particles 3 .. 7
     HsgContext* c = new HsgContext;
     c->t = t;
     struct Part { const void* src; size_t bytes; size_t off; };
@@ -331,7 +408,23 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     d.npar = t->npar; d.ncolor = t->ncolor; d.nslot = t->nslot; d.nlegsets = t->nlegsets; d.nxitem = t->nxitem;
     d.nflow = t->nflow; d.nlevel = t->nlevel;
     for (int l = 0; l < 8; l++) d.p1_level[l] = l <= t->nlevel ? t->p1_level[l] : 0;
-    c->smem = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar);
+    int p3buf = 0;
+    for (int i = 0; i < t->nentry; i++) {
+        const int w = t->entry[4 * i + 3];
+        const int lgx = ((w >> 4) & 7) + __builtin_popcount((w >> 1) & 7), lgy = t->npar - lgx;
+        bool known = false;
+#define HSG_P3_KNOWN(M, LG) known = known || (((w >> 1) & 7) == (M) && lgx == (LG));
+        HSG_P3_COMBOS(HSG_P3_KNOWN)
+#undef HSG_P3_KNOWN
+        if (!known || lgx < 4 || lgx > 6) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
+        const int b = 64 * ((1 << lgx) + (1 << lgy));
+        if (b > p3buf) p3buf = b;
+    }
+    d.p3buf = p3buf;
+    c->smem = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
+    e = cudaFuncSetAttribute(hsg_diagrams_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    if (e != cudaSuccess) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return e; }
     *out = c;
     return cudaSuccess;
 }
