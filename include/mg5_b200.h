@@ -90,7 +90,10 @@ int mg_set_parameters(mg_process* p, const char* const* keys, const double* valu
  * "graph" (1: the launch sequence of a batch is captured into a CUDA graph on its first execution and replayed while the
  * arguments and the handle's state are unchanged; ignored while "timing" = 1; mg_get_option
  * "graph_replays" counts the replays of the current graph; mg_get_option "probe_events" = the number of events of the first
- * batch the automatic helicity filter looks at, at most: 1024, or 16 for "gg_ttxgggg" whose probe goes through the jamps buffer).
+ * batch the automatic helicity filter looks at, at most: 1024, or 16 for "gg_ttxgggg" whose probe goes through the jamps buffer),
+ * "p3_tensor" ("gg_ttxgggg" only, default 1: the generic kernel contracts the pair objects with the largest branch -- phase 3,
+ * the sum over the entries of a colour flow for all 256 helicity combinations -- on the FP64 tensor path, mma.sync.m8n8k4.f64;
+ * 0: on the FP64 ALU, thread = helicity combination; same numbers up to the order of the sum; MG_EINVAL for other processes).
  * With "diagrams" = MG_DIAG_SHARED the jamps always go through the workspace and the tensor-core colour sum ("color_sum" and
  * "block" then only affect the helicity filter and MG_DIAG_THREAD).
  * Unknown key, bad value, or a combination that cannot run (helicity streams with the MG_DIAG_SHARED kernel, which has

@@ -377,6 +377,9 @@ extern "C" int mg_set_option(mg_process* p, const char* key, int value)
         p->max_streams = value;
     } else if (!strcmp(key, "graph")) {
         p->graph = value != 0;
+    } else if (!strcmp(key, "p3_tensor")) {
+        if (!p->hsg) return fail(p, MG_EINVAL, "p3_tensor applies to the generic helicity-shared kernel only (gg_ttxgggg)");
+        hsg_set_tensor(p->hsg, value != 0);
     } else return fail(p, MG_EINVAL, std::string("unknown option ") + key);
     p->epoch++;
     return MG_OK;
@@ -396,6 +399,7 @@ extern "C" int mg_get_option(const mg_process* p, const char* key, int* value)
     else if (!strcmp(key, "max_streams")) *value = p->max_streams;
     else if (!strcmp(key, "graph")) *value = p->graph;
     else if (!strcmp(key, "graph_replays")) *value = p->graph_replays;
+    else if (!strcmp(key, "p3_tensor")) *value = p->hsg ? (int)hsg_get_tensor(p->hsg) : 0;
     else if (!strcmp(key, "probe_events")) *value = p->d->launch ? 1024 : 16;      // events the automatic helicity filter uses at most
     else return MG_EINVAL;
     return MG_OK;

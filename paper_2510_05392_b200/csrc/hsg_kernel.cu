@@ -12,6 +12,12 @@
 //
 // Scratch layout: four component planes, byte(c, slot) = c * 16 * nslot + 16 * slot, so that the lanes of a warp (consecutive
 // variants) read consecutive 16-byte words of one plane.
+//
+// Phase 3 has two forms (template parameter TENSOR, option "p3_tensor"): thread = helicity combination on the FP64 ALU
+// (p3_entry8), which is bound by shared-memory bandwidth -- every lane fetches its own copies of the operands, 24 to 36 16-byte
+// loads per entry for 128 DFMA -- and the FP64 tensor path (p3t_entry, default): the entry as 8 tiles of mma.sync.m8n8k4.f64,
+// whose fragments are 8 to 10 loads per lane and entry, with the accumulator fragments in registers over a CLASS of entries
+// (gen/hsg_tables.py) and one swizzled accumulator per warp in shared memory that collects the classes of a flow.
 #include <stdint.h>
 
 #include "generated/hsg_gen.h"
@@ -23,8 +29,9 @@ namespace mg {
 struct HsgDev {
     const int4* obj; const int4* term; const int* p1_items; const int* legset_mask;
     const int2* xitem; const int4* entry; const int4* flow; const unsigned short* vtab;
+    const int4* dentry; const unsigned* ltab; const unsigned* flowL; const unsigned* flowT;       // tensor path of phase 3
     int npar, ncolor, nslot, nlegsets, nxitem, nflow, nlevel;
-    int p3buf;                 // bytes of one phase-3 operand buffer: max over the entries of 64 (2^|X| + 2^|Y|)
+    int p3buf;                 // bytes of one phase-3 operand buffer: max over the entries of 64 (2^|X| + 2^|Y|) + 128
     int p1_level[8];
 };
 
@@ -136,14 +143,147 @@ __device__ __forceinline__ void p3_stage(const char* __restrict__ area, unsigned
     }
 }
 
-// T2 = type of the jamps buffer
-template <typename T2>
+// ------------------------------------------------------------------------------------------------------------
+// phase 3 on the FP64 tensor path.  One entry = out[hp][hq] += sum_c P_c[hp] Q_c[hq] (complex, c = 4 components) for all 256
+// helicity combinations = 8 tiles of mma.sync.m8n8k4.f64: rows = the helicities of the class's three particles R (legs of P),
+// column pairs (re, im) = those of its two particles C (legs of Q), tile = those of the remaining three particles T.
+// Fragments: a = A[lane / 4][lane % 4] = P_c[row variant] (c = lane % 4; re and im in one 16-byte load), b = B[lane % 4][lane / 4]
+// = Re or Im of Q_c[column variant], c0, c1 = C[lane / 4][2 (lane % 4) + {0, 1}].  The two k-steps of a tile (Re P, Im P) go to
+// SEPARATE accumulators (no negated operand, no dependent pair): f[4t + {0, 1}] = Re P . (Re Q | Im Q), f[4t + {2, 3}] = Im P .
+// (Im Q | Re Q); re = f[4t] - f[4t + 2], im = f[4t + 1] + f[4t + 3].  MASK: tile bits whose particle is a leg of P (they select
+// the A fragment, the others the B fragment); d0..d2 = byte distance of the variants that differ in that particle's helicity.
+__device__ __forceinline__ void hsg_dmma884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__host__ __device__ constexpr int hsg_popc3(int m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1); }
+// bits of t selected by mask m, packed
+__host__ __device__ constexpr int hsg_pext3(int t, int m)
+{
+    int r = 0, k = 0;
+    for (int b = 0; b < 3; b++)
+        if ((m >> b) & 1) { r |= ((t >> b) & 1) << k; k++; }
+    return r;
+}
+
+__device__ __forceinline__ double hsg_flip(double v, unsigned smask)
+{
+    return __hiloint2double(__double2hiint(v) ^ (int)smask, __double2loint(v));
+}
+
+template <int MASK>
+__device__ __forceinline__ void p3t_entry(const char* __restrict__ bx, unsigned aoff, unsigned boff, unsigned d0, unsigned d1,
+                                          unsigned d2, unsigned smask, double (&f)[32])
+{
+    constexpr int NA = 1 << hsg_popc3(MASK), NB = 8 / NA;
+    const unsigned d[3] = { d0, d1, d2 };
+    double2 xa[NA];
+    double b0[NB], b1[NB];
+#pragma unroll
+    for (int a = 0; a < NA; a++) {
+        unsigned off = aoff;
+        int k = 0;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+            if ((MASK >> i) & 1) { if ((a >> k) & 1) off += d[i]; k++; }
+        xa[a] = *reinterpret_cast<const double2*>(bx + off);
+    }
+#pragma unroll
+    for (int b = 0; b < NB; b++) {
+        unsigned off = boff;
+        int k = 0;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+            if (!((MASK >> i) & 1)) { if ((b >> k) & 1) off += d[i]; k++; }
+        b0[b] = *reinterpret_cast<const double*>(bx + off);            // even column (re out): Re Q, odd: Im Q
+        b1[b] = *reinterpret_cast<const double*>(bx + (off ^ 8u));     // even column: Im Q, odd: Re Q
+    }
+    if constexpr (NA <= NB) {
+#pragma unroll
+        for (int a = 0; a < NA; a++) { xa[a].x = hsg_flip(xa[a].x, smask); xa[a].y = hsg_flip(xa[a].y, smask); }
+    } else {
+#pragma unroll
+        for (int b = 0; b < NB; b++) { b0[b] = hsg_flip(b0[b], smask); b1[b] = hsg_flip(b1[b], smask); }
+    }
+#pragma unroll
+    for (int t = 0; t < 8; t++) {
+        const int ai = hsg_pext3(t, MASK), bi = hsg_pext3(t, ~MASK & 7);
+        hsg_dmma884(f[4 * t], f[4 * t + 1], xa[ai].x, b0[bi]);
+        hsg_dmma884(f[4 * t + 2], f[4 * t + 3], xa[ai].y, b1[bi]);
+    }
+}
+
+// 16-byte slot of helicity combination h in a warp's flow accumulator (gen/hsg_tables.py acc_swz)
+__device__ __forceinline__ unsigned acc_swz(unsigned h)
+{
+    const unsigned hi = h >> 3;
+    return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7) ^ ((hi >> 4) & 1));
+}
+
+// a finished class: its fragments are added to the flow's accumulator (first class: plain store) and cleared.  L = swizzled slot
+// of the lane's elements for tile 0, tw0 / tw1 = the tiles' slots (one byte each), XORed on (the swizzle is linear)
+__device__ __forceinline__ void p3t_flush(char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, bool first, double (&f)[32])
+{
+#pragma unroll
+    for (int t = 0; t < 8; t++) {
+        const unsigned idx = L ^ (((t < 4 ? tw0 : tw1) >> (8 * (t & 3))) & 0xFFu);
+        double2* __restrict__ p = reinterpret_cast<double2*>(acc + 16u * idx);
+        double2 v = make_double2(0.0, 0.0);
+        if (!first) v = *p;
+        v.x += f[4 * t] - f[4 * t + 2];
+        v.y += f[4 * t + 1] + f[4 * t + 3];
+        *p = v;
+        f[4 * t] = f[4 * t + 1] = f[4 * t + 2] = f[4 * t + 3] = 0.0;
+    }
+}
+
+// variant index with bits 2 and sw exchanged (sw = 2: unchanged)
+__device__ __forceinline__ int swap2(int v, int sw)
+{
+    const int x = ((v >> 2) ^ (v >> sw)) & 1;
+    return v ^ (x << 2) ^ (x << sw);
+}
+
+// the tensor path's copy of an entry's operands: component planes of (2^LG + 1) x 16 bytes (X: four planes, then Y), and inside a
+// plane the variant index has bits 2 and swx (swy) exchanged.  With that the lanes of one shared-memory access phase of a fragment
+// load -- the four components times the helicity of the class's R[0] (16-byte A elements, 8 lanes) or of C[0] and re / im (8-byte
+// B elements, 16 lanes) -- fall into different banks (gen/hsg_tables.py staged; checked for every entry: no conflict on A, a
+// two-way one on B only where Y has two legs).
+template <int LGX>
+__device__ __forceinline__ void p3t_stage(const char* __restrict__ area, unsigned plane, int xs, int ys, unsigned dst, int lane,
+                                          int swx, int swy)
+{
+    constexpr int LGY = 8 - LGX, NX4 = 4 << LGX, NY4 = 4 << LGY;
+    constexpr unsigned PSX = (16u << LGX) + 16u, PSY = (16u << LGY) + 16u;
+#pragma unroll
+    for (int t = 0; t < NX4 / 32; t++) {
+        const int i = lane + 32 * t, c = i >> LGX, v = i & ((1 << LGX) - 1);
+        const char* src = area + ((unsigned)c * plane + 16u * (unsigned)(xs + swap2(v, swx)));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + (unsigned)c * PSX + 16u * (unsigned)v), "l"(src) : "memory");
+    }
+#pragma unroll
+    for (int t = 0; t < (NY4 + 31) / 32; t++) {
+        const int i = lane + 32 * t, c = i >> LGY, v = i & ((1 << LGY) - 1);
+        if (NY4 % 32 == 0 || i < NY4) {
+            const char* src = area + ((unsigned)c * plane + 16u * (unsigned)(ys + swap2(v, swy)));
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 4u * PSX + (unsigned)c * PSY + 16u * (unsigned)v), "l"(src)
+                         : "memory");
+        }
+    }
+}
+
+// T2 = type of the jamps buffer; TENSOR: phase 3 on the FP64 tensor path
+template <typename T2, bool TENSOR>
 __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(const HsgDev d, const HsLaunch a, char* __restrict__ scratch)
 {
     extern __shared__ __align__(16) double smd[];
     double* __restrict__ Ks = smd;                               // [nlegsets][4]
     double* __restrict__ pm = smd + 4 * d.nlegsets;              // [npar][4]
     char* __restrict__ p3base = reinterpret_cast<char*>(pm + 4 * d.npar);   // [warp][HSG_P3_STAGES][p3buf]: operands of phase 3
+    // TENSOR: [warp][2^npar][16 B] flow accumulators behind the operand buffers
+    char* __restrict__ accbase = p3base + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * d.p3buf;
     const int tid = threadIdx.x, NT = HSG_THREADS;
     const int npar = d.npar, nh = 1 << npar;
     const size_t plane = 16 * (size_t)d.nslot;
@@ -253,6 +393,112 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
         // is 3.2 MB, the L1 hit rate of direct loads was 51 %) into a shared-memory buffer of the warp by cp.async,
         // HSG_P3_STAGES - 1 entries ahead of the one being evaluated: the L2 latency, which bounded the kernel (four dependent
         // batches of loads per entry at 16 warps per SM), is off the critical path.
+        if constexpr (TENSOR) {
+            // tensor path: one warp per flow; the entries of a flow come class by class (gen/hsg_tables.py).  Staging and
+            // prefetching as in the ALU form below: the operands of entry k + 1 are copied while entry k is evaluated, the
+            // per-lane fragment offsets (ltab) of entry k + 1 and the records and class tables of the warp's NEXT flow are in
+            // flight meanwhile.
+            const int lane = tid & 31;
+            char* __restrict__ wbuf = p3base + (size_t)(tid >> 5) * (HSG_P3_STAGES * d.p3buf);
+            char* __restrict__ acc = accbase + (size_t)(tid >> 5) * (16u << 8);
+            const unsigned wbuf_s = (unsigned)__cvta_generic_to_shared(wbuf);
+            auto stage = [&](const int4 en, int b) {
+                const unsigned dst = wbuf_s + (unsigned)(b * d.p3buf);
+                const int xs = en.x & 0xFFFF, ys = (int)((unsigned)en.x >> 16), swx = (en.w >> 16) & 0xF, swy = (en.w >> 20) & 0xF;
+                switch ((en.y >> 16) & 0xF) {
+                    case 4: p3t_stage<4>(area, (unsigned)plane, xs, ys, dst, lane, swx, swy); break;
+                    case 5: p3t_stage<5>(area, (unsigned)plane, xs, ys, dst, lane, swx, swy); break;
+                    default: p3t_stage<6>(area, (unsigned)plane, xs, ys, dst, lane, swx, swy); break;
+                }
+            };
+            const int NWARP = NT >> 5;
+            auto bcast = [&](const int4 m, int k) {
+                return make_int4(__shfl_sync(0xffffffffu, m.x, k), __shfl_sync(0xffffffffu, m.y, k), __shfl_sync(0xffffffffu, m.z, k),
+                                 __shfl_sync(0xffffffffu, m.w, k));
+            };
+            const unsigned* __restrict__ lt = d.ltab + lane;
+            int f = tid >> 5;
+            int4 fl = make_int4(0, 0, 0, 0), myent = fl;
+            unsigned v = 0, myL = 0, myT = 0;
+            if (f < d.nflow) {
+                fl = __ldg(d.flow + f);
+                if (lane < fl.z) myent = __ldg(d.dentry + fl.y + lane);
+                myL = __ldg(d.flowL + 32 * f + lane);
+                myT = __ldg(d.flowT + 8 * f + (lane & 7));
+                v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent.y, 0) & 0xFFFF));
+            }
+            double fr[32];
+#pragma unroll
+            for (int i = 0; i < 32; i++) fr[i] = 0.0;
+            for (; f < d.nflow; f += NWARP) {
+                const int fn = f + NWARP;
+                int4 fl_n = make_int4(0, 0, 0, 0), myent_n = fl_n;
+                unsigned myL_n = 0, myT_n = 0;
+                if (fn < d.nflow) fl_n = __ldg(d.flow + fn);
+#pragma unroll
+                for (int k = 0; k < HSG_P3_STAGES - 1; k++) {            // one commit group per entry, empty past the end
+                    if (k < fl.z) stage(bcast(myent, k), k);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                }
+                int bcur = 0, bnew = HSG_P3_STAGES - 1, cls = 0;
+                for (int k = 0; k < fl.z; k++) {
+                    if (k + HSG_P3_STAGES - 1 < fl.z) stage(bcast(myent, k + HSG_P3_STAGES - 1), bnew);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    const int4 cur = bcast(myent, k);
+                    const unsigned cv = v;
+                    if (k == 0 && fn < d.nflow) {
+                        if (lane < fl_n.z) myent_n = __ldg(d.dentry + fl_n.y + lane);
+                        myL_n = __ldg(d.flowL + 32 * fn + lane);
+                        myT_n = __ldg(d.flowT + 8 * fn + (lane & 7));
+                    }
+                    if (k + 1 < fl.z) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent.y, k + 1) & 0xFFFF));
+                    else if (fn < d.nflow) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent_n.y, 0) & 0xFFFF));
+                    asm volatile("cp.async.wait_group %0;" ::"n"(HSG_P3_STAGES - 1) : "memory");
+                    __syncwarp();
+                    const char* __restrict__ bx = wbuf + bcur * d.p3buf;
+                    const unsigned smask = ((unsigned)cur.y << 8) & 0x80000000u;
+                    const unsigned d0 = cur.z & 0xFFFF, d1 = (unsigned)cur.z >> 16, d2 = cur.w & 0xFFFF;
+                    switch ((cur.y >> 20) & 7) {
+#define HSG_P3T_CASE(M) case M: p3t_entry<M>(bx, cv & 0xFFFFu, cv >> 16, d0, d1, d2, smask, fr); break;
+                        HSG_P3T_MASKS(HSG_P3T_CASE)
+#undef HSG_P3T_CASE
+                        default: break;                                  // (hsg_create refuses tables with another mask)
+                    }
+                    if (cur.y & (1 << 24)) {                             // last entry of its class (uniform over the warp)
+                        const unsigned tw0 = __shfl_sync(0xffffffffu, myT, 2 * cls), tw1 = __shfl_sync(0xffffffffu, myT, 2 * cls + 1);
+                        p3t_flush(acc, (myL >> (8 * cls)) & 0xFFu, tw0, tw1, cls == 0, fr);
+                        cls++;
+                    }
+                    __syncwarp();                                        // the buffer is free for the copy of entry k + STAGES
+                    bnew = bcur;
+                    bcur = bcur + 1 == HSG_P3_STAGES ? 0 : bcur + 1;
+                }
+                // the finished jamp of this flow: lane = the helicities of particles 3 .. 7 (low bits of h), q = particles 0, 1, 2
+#pragma unroll
+                for (int q = 0; q < 8; q++) {
+                    const int pos = posq[q];
+                    if (pos >= 0) {
+                        const unsigned h = (unsigned)lane | ((q & 1u) << 7) | (((q >> 1) & 1u) << 6) | (((q >> 2) & 1u) << 5);
+                        const double2 val = *reinterpret_cast<const double2*>(acc + 16u * acc_swz(h));
+                        const size_t row = (size_t)e * a.nrow_evt + pos;
+                        if (a.tile_major == 2) {
+                            if constexpr (sizeof(T2) == 4) {
+                                const unsigned m = (unsigned)(row & 127);
+                                const int jc = fl.x;
+                                float* __restrict__ o = reinterpret_cast<float*>(out) + (row >> 7) * (size_t)(256 * d.ncolor) +
+                                                        (size_t)(jc / 24) * (24 * 128) + (m >> 3) * 192 + ((jc % 24) >> 2) * 32 + (m & 7) * 4 + (jc & 3);
+                                o[0] = to_tf32((float)val.x); o[(size_t)d.ncolor * 128] = to_tf32((float)val.y);
+                            }
+                        } else {
+                            out[(size_t)fl.x * a.rows + row] = T2(val.x);
+                            out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(val.y);
+                        }
+                    }
+                }
+                __syncwarp();                                            // the next flow's first class overwrites the accumulator
+                fl = fl_n; myent = myent_n; myL = myL_n; myT = myT_n;
+            }
+        } else
         {
             const int lane = tid & 31;
             char* __restrict__ wbuf = p3base + (size_t)(tid >> 5) * (HSG_P3_STAGES * d.p3buf);
@@ -355,7 +601,8 @@ struct HsgContext {
     void* blob = nullptr;
     char* scratch = nullptr;
     int grid = 0;
-    size_t smem = 0;
+    size_t smem = 0, smem_alu = 0;   // dynamic shared memory with phase 3 on the tensor path / on the FP64 ALU
+    bool tensor = true;              // option "p3_tensor"
     // hsg_launch_static: device address of hsg_static_scratch on this context's device (hsg_static_setup)
     char* static_scratch = nullptr;
     cudaError_t static_err = cudaErrorNotReady;
@@ -382,11 +629,13 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     HsgContext* c = new HsgContext;
     c->t = t;
     struct Part { const void* src; size_t bytes; size_t off; };
-    Part parts[8] = { { t->obj, sizeof(int) * 4 * (size_t)t->nobj, 0 }, { t->term, sizeof(int) * 4 * (size_t)t->nterm, 0 },
+    Part parts[12] = { { t->obj, sizeof(int) * 4 * (size_t)t->nobj, 0 }, { t->term, sizeof(int) * 4 * (size_t)t->nterm, 0 },
                       { t->p1_items, sizeof(int) * (size_t)t->np1, 0 }, { t->legset_mask, sizeof(int) * (size_t)t->nlegsets, 0 },
                       { t->xitem, sizeof(int) * 2 * (size_t)t->nxitem, 0 }, { t->entry, sizeof(int) * 4 * (size_t)t->nentry, 0 },
                       { t->flow, sizeof(int) * 4 * (size_t)t->nflow, 0 },
-                      { t->vtab, sizeof(unsigned short) * ((size_t)t->nvrow << t->npar), 0 } };
+                      { t->vtab, sizeof(unsigned short) * ((size_t)t->nvrow << t->npar), 0 },
+                      { t->dentry, sizeof(int) * 4 * (size_t)t->nentry, 0 }, { t->ltab, sizeof(unsigned) * 32 * (size_t)t->nlrow, 0 },
+                      { t->flowL, sizeof(unsigned) * 32 * (size_t)t->nflow, 0 }, { t->flowT, sizeof(unsigned) * 8 * (size_t)t->nflow, 0 } };
     size_t total = 0;
     for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
     cudaError_t e = cudaMalloc(&c->blob, total);
@@ -405,6 +654,8 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     d.p1_items = (const int*)(b + parts[2].off); d.legset_mask = (const int*)(b + parts[3].off);
     d.xitem = (const int2*)(b + parts[4].off); d.entry = (const int4*)(b + parts[5].off);
     d.flow = (const int4*)(b + parts[6].off); d.vtab = (const unsigned short*)(b + parts[7].off);
+    d.dentry = (const int4*)(b + parts[8].off); d.ltab = (const unsigned*)(b + parts[9].off);
+    d.flowL = (const unsigned*)(b + parts[10].off); d.flowT = (const unsigned*)(b + parts[11].off);
     d.npar = t->npar; d.ncolor = t->ncolor; d.nslot = t->nslot; d.nlegsets = t->nlegsets; d.nxitem = t->nxitem;
     d.nflow = t->nflow; d.nlevel = t->nlevel;
     for (int l = 0; l < 8; l++) d.p1_level[l] = l <= t->nlevel ? t->p1_level[l] : 0;
@@ -417,16 +668,41 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
         HSG_P3_COMBOS(HSG_P3_KNOWN)
 #undef HSG_P3_KNOWN
         if (!known || lgx < 4 || lgx > 6) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
-        const int b = 64 * ((1 << lgx) + (1 << lgy));
+        const int b = 64 * ((1 << lgx) + (1 << lgy)) + 128;      // (+ 128: the tensor path's planes are 16 bytes longer)
         if (b > p3buf) p3buf = b;
+        // tensor path: the record's mask must be one the kernel is instantiated for, its leg count the entry's
+        const int w1 = t->dentry[4 * i + 1], m = (w1 >> 20) & 7;
+        bool kmask = false;
+#define HSG_P3T_KNOWN(M) kmask = kmask || m == (M);
+        HSG_P3T_MASKS(HSG_P3T_KNOWN)
+#undef HSG_P3T_KNOWN
+        if (!kmask || ((w1 >> 16) & 0xF) != lgx) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
     }
     d.p3buf = p3buf;
-    c->smem = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
-    e = cudaFuncSetAttribute(hsg_diagrams_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    c->smem_alu = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
+    c->smem = c->smem_alu + (size_t)(HSG_THREADS / 32) * (16u << t->npar);
+    e = cudaFuncSetAttribute(hsg_diagrams_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_alu);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_alu);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
     if (e != cudaSuccess) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return e; }
     *out = c;
     return cudaSuccess;
+}
+
+void hsg_set_tensor(HsgContext* c, bool on) { c->tensor = on; }
+bool hsg_get_tensor(const HsgContext* c) { return c->tensor; }
+
+static cudaError_t launch_any(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, int grid, char* scratch, cudaStream_t st)
+{
+    if (c->tensor) {
+        if (jamps_fp64) hsg_diagrams_kernel<double, true><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, scratch);
+        else hsg_diagrams_kernel<float, true><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, scratch);
+    } else {
+        if (jamps_fp64) hsg_diagrams_kernel<double, false><<<grid, HSG_THREADS, c->smem_alu, st>>>(c->d, a, scratch);
+        else hsg_diagrams_kernel<float, false><<<grid, HSG_THREADS, c->smem_alu, st>>>(c->d, a, scratch);
+    }
+    return cudaGetLastError();
 }
 
 // once per context, with the context's device current: the device address of the static scratch array on THAT device
@@ -454,9 +730,7 @@ cudaError_t hsg_launch_static(const HsgContext* c, bool jamps_fp64, const HsLaun
     const int ctas = hsg_static_ctas(c);
     if (ctas < 1) return cudaErrorInvalidValue;
     const int grid = a.nevt < ctas ? a.nevt : ctas;
-    if (jamps_fp64) hsg_diagrams_kernel<double><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->static_scratch);
-    else hsg_diagrams_kernel<float><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->static_scratch);
-    return cudaGetLastError();
+    return launch_any(c, jamps_fp64, a, grid, c->static_scratch, st);
 }
 
 void hsg_destroy(HsgContext* c)
@@ -471,9 +745,7 @@ cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, 
 {
     if (a.nevt <= 0) return cudaSuccess;
     const int grid = a.nevt < c->grid ? a.nevt : c->grid;
-    if (jamps_fp64) hsg_diagrams_kernel<double><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->scratch);
-    else hsg_diagrams_kernel<float><<<grid, HSG_THREADS, c->smem, st>>>(c->d, a, c->scratch);
-    return cudaGetLastError();
+    return launch_any(c, jamps_fp64, a, grid, c->scratch, st);
 }
 
 }  // namespace mg

@@ -8,7 +8,7 @@
 namespace mg {
 
 struct HsgTables {
-    int npar, ncolor, ns_obj, nslot, nlegsets, nobj, nterm, np1, nxitem, nentry, nflow, nvrow, nlevel, ndiagrams;
+    int npar, ncolor, ns_obj, nslot, nlegsets, nobj, nterm, np1, nxitem, nentry, nflow, nvrow, nlevel, ndiagrams, nlrow;
     int p1_level[8];
     const int* obj;
     const int* term;
@@ -18,6 +18,11 @@ struct HsgTables {
     const int* entry;
     const int* flow;
     const unsigned short* vtab;
+    // phase 3 on the FP64 tensor path: entry records in class order, per-lane fragment offsets, per-flow class tables
+    const int* dentry;
+    const unsigned* ltab;
+    const unsigned* flowL;
+    const unsigned* flowT;
     // colour matrix: numerators (over cden) of the row of the identity permutation; C[s][s'] = row0[rank(s^-1 o s')]
     const int* cmat_row0;
     int cden;
@@ -34,6 +39,9 @@ void hsg_destroy(HsgContext* c);
 const HsgTables* hsg_host_tables(const HsgContext* c);
 // jamps [2][ncolor][rows] (tile_major = 0) or, fp32 only, the tcgen05 operand layout (tile_major = 2, ncolor % 24 == 0)
 cudaError_t hsg_launch(const HsgContext* c, bool jamps_fp64, const HsLaunch& a, cudaStream_t st);
+// phase 3 on the FP64 tensor path (default) or on the FP64 ALU (option "p3_tensor" of include/mg5_b200.h)
+void hsg_set_tensor(HsgContext* c, bool on);
+bool hsg_get_tensor(const HsgContext* c);
 
 
 // The no-allocation variant (mg_sigma_batch_noalloc): the same kernel with its scratch areas in a file-scope static __device__

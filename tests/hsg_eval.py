@@ -32,8 +32,8 @@ def _x_term(op, A, B, Z, kA, kB):
     raise ValueError(op)
 
 
-def evaluate(T, mom, mt, wt):
-    """jamps[ncolor][2^npar] (without the g^n factor) of one event"""
+def _area(T, mom, mt, wt):
+    """phases 1 and 2: the scratch area of one event, [slot][component]"""
     npar = T["npar"]
     k = [mom[i] * (1 if i < 2 else -1) for i in range(npar)]
     K = [sum(k[p] for p in range(npar) if (m >> p) & 1) for m in T["legset_mask"]]
@@ -96,7 +96,13 @@ def evaluate(T, mom, mt, wt):
         assert np.isnan(area[slot]).all()
         area[slot] = G * acc if vec else acc
     assert not np.isnan(area).any()
+    return area
 
+
+def evaluate(T, mom, mt, wt):
+    """jamps[ncolor][2^npar] (without the g^n factor) of one event"""
+    npar = T["npar"]
+    area = _area(T, mom, mt, wt)
     nh = 1 << npar
     J = np.zeros((T["ncolor"], nh), dtype=complex)
     for j, e0, ne, _ in T["flow"]:
@@ -116,4 +122,94 @@ def evaluate(T, mom, mt, wt):
                 inx = (fl >> (1 + i)) & 1
                 above = sum(1 for b in range(i + 1, 3) if ((fl >> (1 + b)) & 1) == inx)       # larger fixed particles sit below
                 assert (dx, dy) == ((1 << (lx + above), 0) if inx else (0, 1 << (ly + above)))
+    return J
+
+
+def _acc_swz(h):
+    """csrc/hsg_kernel.cu acc_swz, restated"""
+    hi, g = h >> 3, 0
+    for b, pat in enumerate((3, 5, 6, 7, 1)):
+        if (hi >> b) & 1:
+            g ^= pat
+    return h ^ g
+
+
+def evaluate_tensor(T, mom, mt, wt, flows=None):
+    """the same jamps from the tables of the TENSOR path of phase 3 (dentry, ltab, flowL, flowT), executed the way a warp of
+    csrc/hsg_kernel.cu executes them: the entry's operands copied into a byte-addressed buffer (X then Y: 4 component planes of
+    2^lg + 1 slots of 16 bytes, variant bits 2 and swx / swy exchanged), fragments of mma.sync.m8n8k4.f64 gathered per lane from the table offsets (a = A[lane / 4][lane % 4],
+    b = B[lane % 4][lane / 4], c0, c1 = C[lane / 4][2 (lane % 4) + {0, 1}]), two k-steps per tile into separate accumulators,
+    classes flushed to the swizzled accumulator, read back in the order of the helicity combinations"""
+    npar = T["npar"]
+    assert npar == 8
+    area = _area(T, mom, mt, wt)
+    nh = 1 << npar
+    J = np.zeros((T["ncolor"], nh), dtype=complex)
+    lanes = np.arange(32)
+    for f, (j, e0, ne, ncls) in enumerate(T["flow"]):
+        if flows is not None and f not in flows:
+            continue
+        acc = np.full((nh, 2), np.nan)
+        frag = np.zeros((8, 32, 4))
+        cls = 0
+        for k in range(e0, e0 + ne):
+            w0, w1, w2, w3 = (int(x) & 0xFFFFFFFF for x in T["dentry"][k])
+            xs, ys = w0 & 0xFFFF, w0 >> 16
+            row, lgx, mask, neg, last = w1 & 0xFFFF, (w1 >> 16) & 0xF, (w1 >> 20) & 7, (w1 >> 23) & 1, (w1 >> 24) & 1
+            assert (xs, ys) == (int(T["entry"][k][0]), int(T["entry"][k][1])) and neg == (int(T["entry"][k][3]) & 1)
+            lgy = npar - lgx
+            d = (w2 & 0xFFFF, w2 >> 16, w3 & 0xFFFF)
+            swx, swy = (w3 >> 16) & 0xF, (w3 >> 20) & 0xF
+
+            def swap2(v, sw):          # variant index with bits 2 and sw exchanged
+                x = ((v >> 2) ^ (v >> sw)) & 1
+                return v ^ (x << 2) ^ (x << sw)
+
+            psx, psy = (16 << lgx) + 16, (16 << lgy) + 16
+            buf = np.full((4 * psx + 4 * psy) // 8, np.nan)                      # doubles
+            for c in range(4):
+                for v in range(1 << lgx):
+                    o = (c * psx + 16 * v) // 8
+                    buf[o], buf[o + 1] = area[xs + swap2(v, swx), c].real, area[xs + swap2(v, swx), c].imag
+                for v in range(1 << lgy):
+                    o = (4 * psx + c * psy + 16 * v) // 8
+                    buf[o], buf[o + 1] = area[ys + swap2(v, swy), c].real, area[ys + swap2(v, swy), c].imag
+            lt = T["ltab"][row].astype(np.int64)
+            aoff, boff = lt & 0xFFFF, lt >> 16
+            sg = -1.0 if neg else 1.0
+            for t in range(8):
+                ao, bo = aoff.copy(), boff.copy()
+                for i in range(3):
+                    if (t >> i) & 1:
+                        if (mask >> i) & 1:
+                            ao += d[i]
+                        else:
+                            bo += d[i]
+                assert (ao % 16 == 0).all() and (bo % 8 == 0).all()
+                are, aim = buf[ao // 8], buf[ao // 8 + 1]
+                b0, b1 = buf[bo // 8], buf[(bo ^ 8) // 8]
+                A0, A1, B0, B1 = np.zeros((8, 4)), np.zeros((8, 4)), np.zeros((4, 8)), np.zeros((4, 8))
+                A0[lanes >> 2, lanes & 3], A1[lanes >> 2, lanes & 3] = sg * are, sg * aim
+                B0[lanes & 3, lanes >> 2], B1[lanes & 3, lanes >> 2] = b0, b1
+                C0, C1 = A0 @ B0, A1 @ B1
+                frag[t, :, 0] += C0[lanes >> 2, 2 * (lanes & 3)]
+                frag[t, :, 1] += C0[lanes >> 2, 2 * (lanes & 3) + 1]
+                frag[t, :, 2] += C1[lanes >> 2, 2 * (lanes & 3)]
+                frag[t, :, 3] += C1[lanes >> 2, 2 * (lanes & 3) + 1]
+            if last:
+                L = (T["flowL"][f].astype(np.int64) >> (8 * cls)) & 0xFF
+                tw = int(T["flowT"][f][2 * cls]) | (int(T["flowT"][f][2 * cls + 1]) << 32)
+                for t in range(8):
+                    idx = L ^ ((tw >> (8 * t)) & 0xFF)
+                    add = np.stack([frag[t, :, 0] - frag[t, :, 2], frag[t, :, 1] + frag[t, :, 3]], axis=1)
+                    if cls == 0:
+                        assert np.isnan(acc[idx]).all()
+                        acc[idx] = add
+                    else:
+                        acc[idx] += add
+                frag[:] = 0.0
+                cls += 1
+        assert cls == ncls and not np.isnan(acc).any()
+        for h in range(nh):
+            J[j, h] = complex(*acc[_acc_swz(h)])
     return J

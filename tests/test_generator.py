@@ -130,3 +130,12 @@ def test_generic_tables_match_oracle(name, n, params):
     J = hsg_eval.evaluate(T, p[0], params["mT"], params["wT"])
     mh = np.einsum("ih,ij,jh->h", J.conj(), C, J).real * gs ** (2 * n) / oracle.DENOM[name]
     assert np.abs(mh / mh_o[0] - 1).max() < 1e-9
+    if n == 6:
+        # the tables of phase 3 on the FP64 tensor path (classes, fragment offsets, staged layout, swizzled accumulator),
+        # executed lane by lane as the kernel does, give the same jamps: every 24th colour flow, all 256 helicities
+        fl = set(range(0, len(T["flow"]), 24))
+        Jt = hsg_eval.evaluate_tensor(T, p[0], params["mT"], params["wT"], flows=fl)
+        assert set(int(x) for x in T["flow"][:, 3]) <= {3, 4}                  # classes per flow
+        for f in fl:
+            j = int(T["flow"][f][0])
+            assert np.abs(Jt[j] - J[j]).max() < 1e-12 * np.abs(J[j]).max()

@@ -455,6 +455,31 @@ def test_gg_ttxgggg_parity_and_mask(B):
     proc.close()
 
 
+def test_gg_ttxgggg_phase3_forms_agree(B):
+    """option p3_tensor: phase 3 of the generic kernel on the FP64 tensor path (default: classes of entries in mma.sync.m8n8k4.f64
+    fragments, flow accumulator in shared memory) against the thread-per-helicity form on the FP64 ALU -- same numbers up to the
+    order of the sum -- and both against the oracle; a partial helicity mask on the tensor path; the option is refused elsewhere"""
+    process, nevt = "gg_ttxgggg", 301                        # more events than the 148 persistent CTAs, ragged
+    mom = inputs.momenta(process, nevt)
+    d_mom = torch.from_numpy(mom).cuda()
+    ref = _oracle(process, mom[:40])
+    res = {}
+    for prec in ("fp64", "mixed"):
+        for tensor in (1, 0):
+            proc = B.init_process(process, prec)
+            assert proc.get_option("p3_tensor") == 1          # the default
+            proc.set_option("p3_tensor", tensor)
+            res[prec, tensor] = proc.sigma_batch(d_mom).cpu().numpy()
+            proc.close()
+    assert _relerr(res["fp64", 1], res["fp64", 0]).max() < 1e-12
+    assert _relerr(res["fp64", 1][:40], ref).max() < 1e-10 and _relerr(res["fp64", 0][:40], ref).max() < 1e-10
+    assert _relerr(res["mixed", 1], res["mixed", 0]).max() < 1e-6        # TF32 rounding of jamps that differ in the last fp64 bits
+    assert _relerr(res["mixed", 1], res["fp64", 1]).max() < 1e-3
+    with pytest.raises(Exception):
+        p5 = B.init_process("gg_ttxggg", "fp64")
+        p5.set_option("p3_tensor", 0)
+
+
 def test_gg_ttxgggg_full_batch_sampled(B):
     """the 4096-event batch bench.py times for g g -> t tbar g g g g (12 GB of jamps, one launch per kernel), oracle on 48
     sampled events (first, last, around the multiples of the 296 persistent CTAs' stride, random); then the same batch in
