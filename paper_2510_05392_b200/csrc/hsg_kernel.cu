@@ -31,6 +31,7 @@ struct HsgDev {
     const int2* xitem; const int4* entry; const int4* flow; const unsigned short* vtab;
     const int4* dentry; const unsigned* ltab; const unsigned* flowL; const unsigned* flowT;       // tensor path of phase 3
     int npar, ncolor, nslot, nlegsets, nxitem, nflow, nlevel;
+    int nslot_arg;             // slots [0, nslot_arg) = the objects of <= 3 legs: every argument of phases 1 and 2 is one of them
     int p3buf;                 // bytes of one phase-3 operand buffer: max over the entries of 64 (2^|X| + 2^|Y|) + 128
     int p1_level[8];
 };
@@ -284,6 +285,9 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
     char* __restrict__ p3base = reinterpret_cast<char*>(pm + 4 * d.npar);   // [warp][HSG_P3_STAGES][p3buf]: operands of phase 3
     // TENSOR: [warp][2^npar][16 B] flow accumulators behind the operand buffers
     char* __restrict__ accbase = p3base + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * d.p3buf;
+    // TENSOR: [2^npar] element offset of helicity combination h of the current event in the jamps buffer (without the colour's
+    // part), -1 = not computed: the write-out of a flow costs one load per element instead of the layout arithmetic
+    long long* __restrict__ rofft = reinterpret_cast<long long*>(accbase + (size_t)(HSG_THREADS / 32) * (16u << 8));
     const int tid = threadIdx.x, NT = HSG_THREADS;
     const int npar = d.npar, nh = 1 << npar;
     const size_t plane = 16 * (size_t)d.nslot;
@@ -293,11 +297,26 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
 #pragma unroll
     for (int q = 0; q < 8; q++)
         posq[q] = a.d_pos[(tid & 31) | ((q & 1) << (npar - 1)) | (((q >> 1) & 1) << (npar - 2)) | (((q >> 2) & 1) << (npar - 3))];
-    auto arg = [&](int word, int var, wf<double>& w) { ldw(area, plane, (word & 0xFFFF) + sub_variant4(var, (word >> 16) & 0xFFF), w); };
+    // Arguments of phases 1 and 2 are objects of <= 3 legs only (1 184 slots = 76 KB at 6 gluons; hsg_create checks it): they are
+    // kept in SHARED memory, in the area phase 3 uses for its operand buffers afterwards, besides their copy in the scratch area
+    // (which phase 3 reads as Y).  With them in the scratch area alone every term of phases 1 and 2 waited for an L2 round trip
+    // (L1 hit rate 14 %: the L1 left beside 210 KB of shared memory is small).
+    char* __restrict__ argarea = p3base;
+    const size_t aplane = 16 * (size_t)d.nslot_arg;
+    auto arg = [&](int word, int var, wf<double>& w) { ldw(argarea, aplane, (word & 0xFFFF) + sub_variant4(var, (word >> 16) & 0xFFF), w); };
 
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
         // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
         for (int i = tid; i < 4 * npar; i += NT) pm[i] = a.mom[(size_t)e * (4 * npar) + i];
+        if constexpr (TENSOR) {
+            for (int h = tid; h < nh; h += NT) {
+                const int pos = a.d_pos[h];
+                const size_t row = (size_t)e * a.nrow_evt + pos;
+                rofft[h] = pos < 0 ? -1ll
+                           : a.tile_major == 2 ? (long long)((row >> 7) * (size_t)(256 * d.ncolor) + ((row & 127) >> 3) * 192 + (row & 7) * 4)
+                                               : (long long)row;
+            }
+        }
         __syncthreads();
         for (int s = tid; s < d.nlegsets; s += NT) {
             const int m = __ldg(d.legset_mask + s);
@@ -344,6 +363,7 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     axpy((w.x >> 8) & 1 ? -1.0 : 1.0, r, acc);
                 }
                 stw(area, plane, o.x + var, acc);
+                if (o.x < d.nslot_arg) stw(argarea, aplane, o.x + var, acc);
             }
             __syncthreads();
         }
@@ -435,16 +455,15 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                 int4 fl_n = make_int4(0, 0, 0, 0), myent_n = fl_n;
                 unsigned myL_n = 0, myT_n = 0;
                 if (fn < d.nflow) fl_n = __ldg(d.flow + fn);
-#pragma unroll
-                for (int k = 0; k < HSG_P3_STAGES - 1; k++) {            // one commit group per entry, empty past the end
-                    if (k < fl.z) stage(bcast(myent, k), k);
-                    asm volatile("cp.async.commit_group;" ::: "memory");
-                }
-                int bcur = 0, bnew = HSG_P3_STAGES - 1, cls = 0;
+                static_assert(HSG_P3_STAGES == 2, "the record of the entry being copied is kept for the next iteration");
+                int4 nxt = bcast(myent, 0);
+                if (fl.z > 0) stage(nxt, 0);
+                asm volatile("cp.async.commit_group;" ::: "memory");     // one commit group per entry, empty past the end
+                int bcur = 0, bnew = 1, cls = 0;
                 for (int k = 0; k < fl.z; k++) {
-                    if (k + HSG_P3_STAGES - 1 < fl.z) stage(bcast(myent, k + HSG_P3_STAGES - 1), bnew);
+                    const int4 cur = nxt;
+                    if (k + 1 < fl.z) { nxt = bcast(myent, k + 1); stage(nxt, bnew); }
                     asm volatile("cp.async.commit_group;" ::: "memory");
-                    const int4 cur = bcast(myent, k);
                     const unsigned cv = v;
                     if (k == 0 && fn < d.nflow) {
                         if (lane < fl_n.z) myent_n = __ldg(d.dentry + fl_n.y + lane);
@@ -474,24 +493,27 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     bcur = bcur + 1 == HSG_P3_STAGES ? 0 : bcur + 1;
                 }
                 // the finished jamp of this flow: lane = the helicities of particles 3 .. 7 (low bits of h), q = particles 0, 1, 2
+                {
+                    const int jc = fl.x;
+                    // tcgen05 operand layout (color_sum_tf32_big.cu): per 128-row tile and part, chunks of 24 colours as K-major
+                    // core matrices [row / 8][colour quad][row % 8][colour % 4], values rounded to TF32; the row's part is in rofft
+                    const size_t joff = a.tile_major == 2 ? (size_t)(jc / 24) * (24 * 128) + ((jc % 24) >> 2) * 32 + (jc & 3)
+                                                          : (size_t)jc * a.rows;
 #pragma unroll
-                for (int q = 0; q < 8; q++) {
-                    const int pos = posq[q];
-                    if (pos >= 0) {
+                    for (int q = 0; q < 8; q++) {
                         const unsigned h = (unsigned)lane | ((q & 1u) << 7) | (((q >> 1) & 1u) << 6) | (((q >> 2) & 1u) << 5);
-                        const double2 val = *reinterpret_cast<const double2*>(acc + 16u * acc_swz(h));
-                        const size_t row = (size_t)e * a.nrow_evt + pos;
-                        if (a.tile_major == 2) {
-                            if constexpr (sizeof(T2) == 4) {
-                                const unsigned m = (unsigned)(row & 127);
-                                const int jc = fl.x;
-                                float* __restrict__ o = reinterpret_cast<float*>(out) + (row >> 7) * (size_t)(256 * d.ncolor) +
-                                                        (size_t)(jc / 24) * (24 * 128) + (m >> 3) * 192 + ((jc % 24) >> 2) * 32 + (m & 7) * 4 + (jc & 3);
-                                o[0] = to_tf32((float)val.x); o[(size_t)d.ncolor * 128] = to_tf32((float)val.y);
+                        const long long ro = rofft[h];
+                        if (ro >= 0) {
+                            const double2 val = *reinterpret_cast<const double2*>(acc + 16u * acc_swz(h));
+                            if (a.tile_major == 2) {
+                                if constexpr (sizeof(T2) == 4) {
+                                    float* __restrict__ o = reinterpret_cast<float*>(out) + (size_t)ro + joff;
+                                    o[0] = to_tf32((float)val.x); o[(size_t)d.ncolor * 128] = to_tf32((float)val.y);
+                                }
+                            } else {
+                                out[joff + (size_t)ro] = T2(val.x);
+                                out[(size_t)d.ncolor * a.rows + joff + (size_t)ro] = T2(val.y);
                             }
-                        } else {
-                            out[(size_t)fl.x * a.rows + row] = T2(val.x);
-                            out[(size_t)(d.ncolor + fl.x) * a.rows + row] = T2(val.y);
                         }
                     }
                 }
@@ -659,6 +681,20 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     d.npar = t->npar; d.ncolor = t->ncolor; d.nslot = t->nslot; d.nlegsets = t->nlegsets; d.nxitem = t->nxitem;
     d.nflow = t->nflow; d.nlevel = t->nlevel;
     for (int l = 0; l < 8; l++) d.p1_level[l] = l <= t->nlevel ? t->p1_level[l] : 0;
+    // objects are sorted by their number of legs: the arguments' area ends where the first object of more than 3 legs starts
+    d.nslot_arg = t->ns_obj;
+    for (int i = 0; i < t->nobj; i++)
+        if ((t->obj[4 * i + 1] & 0xFF) > 3 && t->obj[4 * i] < d.nslot_arg) d.nslot_arg = t->obj[4 * i];
+    bool args_ok = true;
+    for (int i = 0; i < t->nterm; i++) {
+        const int op = t->term[4 * i] & 0xFF;
+        if (op <= 2) continue;
+        const int nargs = (op == 4 || op == 12 || op == 13) ? 3 : 2;
+        for (int k = 1; k <= nargs; k++) args_ok = args_ok && (t->term[4 * i + k] & 0xFFFF) < d.nslot_arg;
+    }
+    for (int i = 0; i < t->nobj; i++)        // ... and an object of <= 3 legs lies below it entirely
+        if ((t->obj[4 * i + 1] & 0xFF) <= 3) args_ok = args_ok && t->obj[4 * i] + (1 << (t->obj[4 * i + 1] & 0xFF)) <= d.nslot_arg;
+    if (!args_ok) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
     int p3buf = 0;
     for (int i = 0; i < t->nentry; i++) {
         const int w = t->entry[4 * i + 3];
@@ -680,7 +716,8 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     }
     d.p3buf = p3buf;
     c->smem_alu = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
-    c->smem = c->smem_alu + (size_t)(HSG_THREADS / 32) * (16u << t->npar);
+    if (64 * (size_t)d.nslot_arg > (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
+    c->smem = c->smem_alu + (size_t)(HSG_THREADS / 32) * (16u << t->npar) + (sizeof(long long) << t->npar);
     e = cudaFuncSetAttribute(hsg_diagrams_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_alu);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_alu);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(hsg_diagrams_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
