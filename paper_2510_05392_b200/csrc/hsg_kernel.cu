@@ -20,6 +20,8 @@
 // (gen/hsg_tables.py) and one swizzled accumulator per warp in shared memory that collects the classes of a flow.
 #include <stdint.h>
 
+#include <vector>
+
 #include "generated/hsg_gen.h"
 #include "helas.cuh"
 #include "hsg_kernel.cuh"
@@ -31,6 +33,7 @@ struct HsgDev {
     const int2* xitem; const int4* entry; const int4* flow; const unsigned short* vtab;
     const int4* dentry; const unsigned* ltab; const unsigned* flowL; const unsigned* flowT;       // tensor path of phase 3
     int npar, ncolor, nslot, nlegsets, nxitem, nflow, nlevel;
+    const unsigned char* lut; int nlut;   // sub-variant table [nlut][HSG_LUT_VARS] (copied to shared memory), nlut * HSG_LUT_VARS % 16 == 0
     int nslot_arg;             // slots [0, nslot_arg) = the objects of <= 3 legs: every argument of phases 1 and 2 is one of them
     int p3buf;                 // bytes of one phase-3 operand buffer: max over the entries of 64 (2^|X| + 2^|Y|) + 128
     int p1_level[8];
@@ -49,11 +52,16 @@ __device__ __forceinline__ float to_tf32(float x)
     return __uint_as_float(u);
 }
 
-__device__ __forceinline__ int sub_variant4(int var, int code)
+// variant of an argument object for variant var of its parent: bit j = bit ((code >> 3j) & 7) of var (7 = none).  There are few
+// distinct codes (30 at 6 gluons): hsg_create numbers them, writes the number into the device copy of the term records in place
+// of the code and tabulates the function -- the kernel reads lut[number][var] from shared memory (one load instead of ~20
+// integer instructions per argument).
+static int sub_variant4(int var, int code)
 {
     return ((var >> (code & 7)) & 1) | (((var >> ((code >> 3) & 7)) & 1) << 1) | (((var >> ((code >> 6) & 7)) & 1) << 2) |
            (((var >> ((code >> 9) & 7)) & 1) << 3);
 }
+static constexpr int HSG_LUT_VARS = 128;          // variants of a parent: objects have <= 4 legs, pair objects <= 7
 
 __device__ __forceinline__ void ldw(const char* __restrict__ area, size_t plane, int slot, wf<double>& w)
 {
@@ -149,9 +157,10 @@ __device__ __forceinline__ void p3_stage(const char* __restrict__ area, unsigned
 // helicity combinations = 8 tiles of mma.sync.m8n8k4.f64: rows = the helicities of the class's three particles R (legs of P),
 // column pairs (re, im) = those of its two particles C (legs of Q), tile = those of the remaining three particles T.
 // Fragments: a = A[lane / 4][lane % 4] = P_c[row variant] (c = lane % 4; re and im in one 16-byte load), b = B[lane % 4][lane / 4]
-// = Re or Im of Q_c[column variant], c0, c1 = C[lane / 4][2 (lane % 4) + {0, 1}].  The two k-steps of a tile (Re P, Im P) go to
-// SEPARATE accumulators (no negated operand, no dependent pair): f[4t + {0, 1}] = Re P . (Re Q | Im Q), f[4t + {2, 3}] = Im P .
-// (Im Q | Re Q); re = f[4t] - f[4t + 2], im = f[4t + 1] + f[4t + 3].  MASK: tile bits whose particle is a leg of P (they select
+// = Re or Im of Q_c[column variant], c0, c1 = C[lane / 4][2 (lane % 4) + {0, 1}].  The two k-steps of a tile, Re P . (Re Q | Im Q)
+// and Im P . (-Im Q | Re Q), go to ONE accumulator pair f[2t + {0, 1}] = (re, im): the minus sits on the B fragment of the second
+// step (a sign bit in the lanes of the even columns), and the eight first steps are issued before the eight second ones.  (The
+// tuned kernel keeps two pairs per tile instead, hs_kernel.cu; here 32 fewer registers and half the flush.)  MASK: tile bits whose particle is a leg of P (they select
 // the A fragment, the others the B fragment); d0..d2 = byte distance of the variants that differ in that particle's helicity.
 __device__ __forceinline__ void hsg_dmma884(double& c0, double& c1, double a, double b)
 {
@@ -176,7 +185,7 @@ __device__ __forceinline__ double hsg_flip(double v, unsigned smask)
 
 template <int MASK>
 __device__ __forceinline__ void p3t_entry(const char* __restrict__ bx, unsigned aoff, unsigned boff, unsigned d0, unsigned d1,
-                                          unsigned d2, unsigned smask, double (&f)[32])
+                                          unsigned d2, unsigned smask, unsigned nmask, double (&f)[16])
 {
     constexpr int NA = 1 << hsg_popc3(MASK), NB = 8 / NA;
     const unsigned d[3] = { d0, d1, d2 };
@@ -201,19 +210,22 @@ __device__ __forceinline__ void p3t_entry(const char* __restrict__ bx, unsigned 
         b0[b] = *reinterpret_cast<const double*>(bx + off);            // even column (re out): Re Q, odd: Im Q
         b1[b] = *reinterpret_cast<const double*>(bx + (off ^ 8u));     // even column: Im Q, odd: Re Q
     }
+    // signs: the entry's (smask) on one operand; the minus of Im P . Im Q (nmask: set in the lanes of even columns) on b1 or,
+    // where the B fragments are the many, folded into the A side as a second copy of Im P is not worth it: it stays on b1
     if constexpr (NA <= NB) {
 #pragma unroll
         for (int a = 0; a < NA; a++) { xa[a].x = hsg_flip(xa[a].x, smask); xa[a].y = hsg_flip(xa[a].y, smask); }
+#pragma unroll
+        for (int b = 0; b < NB; b++) b1[b] = hsg_flip(b1[b], nmask);
     } else {
 #pragma unroll
-        for (int b = 0; b < NB; b++) { b0[b] = hsg_flip(b0[b], smask); b1[b] = hsg_flip(b1[b], smask); }
+        for (int b = 0; b < NB; b++) { b0[b] = hsg_flip(b0[b], smask); b1[b] = hsg_flip(b1[b], smask ^ nmask); }
     }
+    // all Re P products first, then the Im P ones: the two tensor instructions of a tile are 8 apart
 #pragma unroll
-    for (int t = 0; t < 8; t++) {
-        const int ai = hsg_pext3(t, MASK), bi = hsg_pext3(t, ~MASK & 7);
-        hsg_dmma884(f[4 * t], f[4 * t + 1], xa[ai].x, b0[bi]);
-        hsg_dmma884(f[4 * t + 2], f[4 * t + 3], xa[ai].y, b1[bi]);
-    }
+    for (int t = 0; t < 8; t++) hsg_dmma884(f[2 * t], f[2 * t + 1], xa[hsg_pext3(t, MASK)].x, b0[hsg_pext3(t, ~MASK & 7)]);
+#pragma unroll
+    for (int t = 0; t < 8; t++) hsg_dmma884(f[2 * t], f[2 * t + 1], xa[hsg_pext3(t, MASK)].y, b1[hsg_pext3(t, ~MASK & 7)]);
 }
 
 // 16-byte slot of helicity combination h in a warp's flow accumulator (gen/hsg_tables.py acc_swz)
@@ -225,7 +237,7 @@ __device__ __forceinline__ unsigned acc_swz(unsigned h)
 
 // a finished class: its fragments are added to the flow's accumulator (first class: plain store) and cleared.  L = swizzled slot
 // of the lane's elements for tile 0, tw0 / tw1 = the tiles' slots (one byte each), XORed on (the swizzle is linear)
-__device__ __forceinline__ void p3t_flush(char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, bool first, double (&f)[32])
+__device__ __forceinline__ void p3t_flush(char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, bool first, double (&f)[16])
 {
 #pragma unroll
     for (int t = 0; t < 8; t++) {
@@ -233,10 +245,10 @@ __device__ __forceinline__ void p3t_flush(char* __restrict__ acc, unsigned L, un
         double2* __restrict__ p = reinterpret_cast<double2*>(acc + 16u * idx);
         double2 v = make_double2(0.0, 0.0);
         if (!first) v = *p;
-        v.x += f[4 * t] - f[4 * t + 2];
-        v.y += f[4 * t + 1] + f[4 * t + 3];
+        v.x += f[2 * t];
+        v.y += f[2 * t + 1];
         *p = v;
-        f[4 * t] = f[4 * t + 1] = f[4 * t + 2] = f[4 * t + 3] = 0.0;
+        f[2 * t] = f[2 * t + 1] = 0.0;
     }
 }
 
@@ -282,7 +294,8 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
     extern __shared__ __align__(16) double smd[];
     double* __restrict__ Ks = smd;                               // [nlegsets][4]
     double* __restrict__ pm = smd + 4 * d.nlegsets;              // [npar][4]
-    char* __restrict__ p3base = reinterpret_cast<char*>(pm + 4 * d.npar);   // [warp][HSG_P3_STAGES][p3buf]: operands of phase 3
+    unsigned char* __restrict__ lut = reinterpret_cast<unsigned char*>(pm + 4 * d.npar);     // [nlut][HSG_LUT_VARS]
+    char* __restrict__ p3base = reinterpret_cast<char*>(lut) + d.nlut * HSG_LUT_VARS;        // [warp][HSG_P3_STAGES][p3buf]: operands of phase 3
     // TENSOR: [warp][2^npar][16 B] flow accumulators behind the operand buffers
     char* __restrict__ accbase = p3base + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * d.p3buf;
     // TENSOR: [2^npar] element offset of helicity combination h of the current event in the jamps buffer (without the colour's
@@ -303,7 +316,11 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
     // (L1 hit rate 14 %: the L1 left beside 210 KB of shared memory is small).
     char* __restrict__ argarea = p3base;
     const size_t aplane = 16 * (size_t)d.nslot_arg;
-    auto arg = [&](int word, int var, wf<double>& w) { ldw(argarea, aplane, (word & 0xFFFF) + sub_variant4(var, (word >> 16) & 0xFFF), w); };
+    for (int i = threadIdx.x; i < d.nlut * HSG_LUT_VARS / 4; i += HSG_THREADS)
+        reinterpret_cast<unsigned*>(lut)[i] = __ldg(reinterpret_cast<const unsigned*>(d.lut) + i);       // (first use: after a barrier)
+    auto arg = [&](int word, int var, wf<double>& w) {
+        ldw(argarea, aplane, (word & 0xFFFF) + lut[((word >> 16) & 0xFFF) * HSG_LUT_VARS + var], w);
+    };
 
     for (int e = blockIdx.x; e < a.nevt; e += gridDim.x) {
         // a0: momenta (AOS fp64) -> shared; leg-set momenta in the all-incoming convention
@@ -447,9 +464,10 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                 myT = __ldg(d.flowT + 8 * f + (lane & 7));
                 v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent.y, 0) & 0xFFFF));
             }
-            double fr[32];
+            double fr[16];
 #pragma unroll
-            for (int i = 0; i < 32; i++) fr[i] = 0.0;
+            for (int i = 0; i < 16; i++) fr[i] = 0.0;
+            const unsigned nmask = (lane & 4) ? 0u : 0x80000000u;          // lanes of the even columns of the B fragment
             for (; f < d.nflow; f += NWARP) {
                 const int fn = f + NWARP;
                 int4 fl_n = make_int4(0, 0, 0, 0), myent_n = fl_n;
@@ -460,6 +478,8 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                 if (fl.z > 0) stage(nxt, 0);
                 asm volatile("cp.async.commit_group;" ::: "memory");     // one commit group per entry, empty past the end
                 int bcur = 0, bnew = 1, cls = 0;
+                bool pend = false, pfirst = false;
+                unsigned pL = 0, ptw0 = 0, ptw1 = 0;
                 for (int k = 0; k < fl.z; k++) {
                     const int4 cur = nxt;
                     if (k + 1 < fl.z) { nxt = bcast(myent, k + 1); stage(nxt, bnew); }
@@ -472,26 +492,34 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     }
                     if (k + 1 < fl.z) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent.y, k + 1) & 0xFFFF));
                     else if (fn < d.nflow) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent_n.y, 0) & 0xFFFF));
+                    // the class that ended with the previous entry is flushed HERE, behind the copy and the prefetches of this
+                    // iteration: its last tensor instructions have ~200 cycles of latency, which the flush would wait for if it
+                    // followed them directly (measured: the flush was 5.7 of 26.8 ms)
+                    if (pend) { p3t_flush(acc, pL, ptw0, ptw1, pfirst, fr); pend = false; }
                     asm volatile("cp.async.wait_group %0;" ::"n"(HSG_P3_STAGES - 1) : "memory");
                     __syncwarp();
                     const char* __restrict__ bx = wbuf + bcur * d.p3buf;
                     const unsigned smask = ((unsigned)cur.y << 8) & 0x80000000u;
                     const unsigned d0 = cur.z & 0xFFFF, d1 = (unsigned)cur.z >> 16, d2 = cur.w & 0xFFFF;
                     switch ((cur.y >> 20) & 7) {
-#define HSG_P3T_CASE(M) case M: p3t_entry<M>(bx, cv & 0xFFFFu, cv >> 16, d0, d1, d2, smask, fr); break;
+#define HSG_P3T_CASE(M) case M: p3t_entry<M>(bx, cv & 0xFFFFu, cv >> 16, d0, d1, d2, smask, nmask, fr); break;
                         HSG_P3T_MASKS(HSG_P3T_CASE)
 #undef HSG_P3T_CASE
                         default: break;                                  // (hsg_create refuses tables with another mask)
                     }
                     if (cur.y & (1 << 24)) {                             // last entry of its class (uniform over the warp)
-                        const unsigned tw0 = __shfl_sync(0xffffffffu, myT, 2 * cls), tw1 = __shfl_sync(0xffffffffu, myT, 2 * cls + 1);
-                        p3t_flush(acc, (myL >> (8 * cls)) & 0xFFu, tw0, tw1, cls == 0, fr);
+                        ptw0 = __shfl_sync(0xffffffffu, myT, 2 * cls); ptw1 = __shfl_sync(0xffffffffu, myT, 2 * cls + 1);
+                        pL = (myL >> (8 * cls)) & 0xFFu;
+                        pfirst = cls == 0;
+                        pend = true;
                         cls++;
                     }
                     __syncwarp();                                        // the buffer is free for the copy of entry k + STAGES
                     bnew = bcur;
                     bcur = bcur + 1 == HSG_P3_STAGES ? 0 : bcur + 1;
                 }
+                if (pend) { p3t_flush(acc, pL, ptw0, ptw1, pfirst, fr); pend = false; }     // (a flow ends with the end of a class)
+                __syncwarp();
                 // the finished jamp of this flow: lane = the helicities of particles 3 .. 7 (low bits of h), q = particles 0, 1, 2
                 {
                     const int jc = fl.x;
@@ -650,14 +678,37 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     if (t->npar != 8) return cudaErrorInvalidValue;       // phase 3 maps lane = the helicities of particles 3 .. 7
     HsgContext* c = new HsgContext;
     c->t = t;
+    // device copy of the term records: the 12-bit sub-variant code of every argument replaced by its row in the lookup table
+    std::vector<int> term(t->term, t->term + 4 * (size_t)t->nterm);
+    std::vector<int> codes;
+    for (int i = 0; i < t->nterm; i++) {
+        const int op = term[4 * i] & 0xFF;
+        if (op <= 2) continue;
+        const int nargs = (op == 4 || op == 12 || op == 13) ? 3 : 2;
+        for (int k = 1; k <= nargs; k++) {
+            const int code = (term[4 * i + k] >> 16) & 0xFFF;
+            size_t r = 0;
+            while (r < codes.size() && codes[r] != code) r++;
+            if (r == codes.size()) codes.push_back(code);
+            term[4 * i + k] = (term[4 * i + k] & 0xFFFF) | ((int)r << 16);
+        }
+    }
+    while (codes.size() % 4) codes.push_back(0xFFF);                  // (rows of 128 bytes: any count is a multiple of 16 bytes)
+    std::vector<unsigned char> lut(codes.size() * HSG_LUT_VARS);
+    for (size_t r = 0; r < codes.size(); r++)
+        for (int v = 0; v < HSG_LUT_VARS; v++) lut[r * HSG_LUT_VARS + v] = (unsigned char)sub_variant4(v, codes[r]);
+    bool vars_ok = codes.size() <= 256;
+    for (int i = 0; i < t->nxitem; i++) vars_ok = vars_ok && ((t->xitem[2 * i + 1] >> 20) & 0xFF) < HSG_LUT_VARS;
+    if (!vars_ok) { delete c; return cudaErrorInvalidValue; }
     struct Part { const void* src; size_t bytes; size_t off; };
-    Part parts[12] = { { t->obj, sizeof(int) * 4 * (size_t)t->nobj, 0 }, { t->term, sizeof(int) * 4 * (size_t)t->nterm, 0 },
+    Part parts[13] = { { t->obj, sizeof(int) * 4 * (size_t)t->nobj, 0 }, { term.data(), sizeof(int) * 4 * (size_t)t->nterm, 0 },
                       { t->p1_items, sizeof(int) * (size_t)t->np1, 0 }, { t->legset_mask, sizeof(int) * (size_t)t->nlegsets, 0 },
                       { t->xitem, sizeof(int) * 2 * (size_t)t->nxitem, 0 }, { t->entry, sizeof(int) * 4 * (size_t)t->nentry, 0 },
                       { t->flow, sizeof(int) * 4 * (size_t)t->nflow, 0 },
                       { t->vtab, sizeof(unsigned short) * ((size_t)t->nvrow << t->npar), 0 },
                       { t->dentry, sizeof(int) * 4 * (size_t)t->nentry, 0 }, { t->ltab, sizeof(unsigned) * 32 * (size_t)t->nlrow, 0 },
-                      { t->flowL, sizeof(unsigned) * 32 * (size_t)t->nflow, 0 }, { t->flowT, sizeof(unsigned) * 8 * (size_t)t->nflow, 0 } };
+                      { t->flowL, sizeof(unsigned) * 32 * (size_t)t->nflow, 0 }, { t->flowT, sizeof(unsigned) * 8 * (size_t)t->nflow, 0 },
+                      { lut.data(), lut.size(), 0 } };
     size_t total = 0;
     for (auto& p : parts) { p.off = total; total += (p.bytes + 255) & ~size_t(255); }
     cudaError_t e = cudaMalloc(&c->blob, total);
@@ -678,6 +729,7 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
     d.flow = (const int4*)(b + parts[6].off); d.vtab = (const unsigned short*)(b + parts[7].off);
     d.dentry = (const int4*)(b + parts[8].off); d.ltab = (const unsigned*)(b + parts[9].off);
     d.flowL = (const unsigned*)(b + parts[10].off); d.flowT = (const unsigned*)(b + parts[11].off);
+    d.lut = (const unsigned char*)(b + parts[12].off); d.nlut = (int)codes.size();
     d.npar = t->npar; d.ncolor = t->ncolor; d.nslot = t->nslot; d.nlegsets = t->nlegsets; d.nxitem = t->nxitem;
     d.nflow = t->nflow; d.nlevel = t->nlevel;
     for (int l = 0; l < 8; l++) d.p1_level[l] = l <= t->nlevel ? t->p1_level[l] : 0;
@@ -715,7 +767,7 @@ cudaError_t hsg_create(int ngluon, HsgContext** out)
         if (!kmask || ((w1 >> 16) & 0xF) != lgx) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
     }
     d.p3buf = p3buf;
-    c->smem_alu = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
+    c->smem_alu = sizeof(double) * 4 * (size_t)(t->nlegsets + t->npar) + lut.size() + (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf;
     if (64 * (size_t)d.nslot_arg > (size_t)(HSG_THREADS / 32) * HSG_P3_STAGES * p3buf) { cudaFree(c->blob); cudaFree(c->scratch); delete c; return cudaErrorInvalidValue; }
     c->smem = c->smem_alu + (size_t)(HSG_THREADS / 32) * (16u << t->npar) + (sizeof(long long) << t->npar);
     e = cudaFuncSetAttribute(hsg_diagrams_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_alu);

@@ -34,8 +34,8 @@ Phase 3 on the FP64 tensor path (csrc/hsg_kernel.cu, p3_tensor): one entry for a
 outer-product sum out[hp][hq] = sum_c P_c[hp] Q_c[hq] over the four components, i.e. 8 tiles of mma.sync.m8n8k4.f64: rows = the
 helicities of three particles R (all legs of one operand, P), column pairs (re, im) = the helicities of two particles C (legs of
 the other operand, Q), tile index = the helicities of the remaining three particles T.  The accumulator fragments stay in
-registers as long as (R, C) do not change: the entries of a flow are grouped into CLASSES with one (R, C) each (greedy cover,
-3 or 4 classes per flow at 6 gluons) and stored class by class; a finished class is added to the flow's accumulator in shared
+registers as long as (R, C) do not change: the entries of a flow are grouped into CLASSES with one (R, C) each (smallest cover,
+3 classes per flow at 6 gluons) and stored class by class; a finished class is added to the flow's accumulator in shared
 memory (slot of combination h = swz(h), conflict-free for the class's lane order where the choice of R[0] allows it).
   dentry[e]  = { first slot of X | first slot of Y << 16, row of ltab | legs of X << 16 | MASK << 20 | negative << 23 |
                  last entry of its class << 24, d0 | d1 << 16, d2 | swx << 16 | swy << 20 }: MASK bit i = T[i] is a leg of P; d_i =
@@ -95,26 +95,39 @@ def _independent(v):
 
 
 def _class_cover(npar, xmasks):
-    """greedy cover of the entries of a flow (bit masks of the legs of X) by classes (R, C): R = three particles that are all legs
-    of one operand, C = two particles that are legs of the other one; returns [(R mask, C mask, [entry indices])]"""
+    """smallest cover of the entries of a flow (bit masks of the legs of X) by classes (R, C): R = three particles that are all
+    legs of one operand, C = two particles that are legs of the other one; returns [(R mask, C mask, [entry indices])], every
+    entry in the first class of the cover that holds it.  Exact: the sets of entries that some (R, C) covers are few once the
+    dominated ones are dropped (16 at 6 gluons), so all combinations of up to four are tried (3 classes for every flow at 6
+    gluons; a greedy cover needs 4 for 330 of the 720)"""
     import itertools
     full = (1 << npar) - 1
-    cands = []
+    by_set = {}
     for R in itertools.combinations(range(npar), 3):
         rm = sum(1 << p for p in R)
         for C in itertools.combinations([p for p in range(npar) if p not in R], 2):
-            cands.append((rm, sum(1 << p for p in C)))
-    left, out = list(range(len(xmasks))), []
-    while left:
-        best = None
-        for rm, cm in cands:
-            cov = [i for i in left if ((xmasks[i] & rm) == rm and (~xmasks[i] & full & cm) == cm) or
-                   ((~xmasks[i] & full & rm) == rm and (xmasks[i] & cm) == cm)]
-            if best is None or len(cov) > len(best[2]):
-                best = (rm, cm, cov)
-        out.append(best)
-        left = [i for i in left if i not in best[2]]
-    return out
+            cm = sum(1 << p for p in C)
+            m = 0
+            for i, x in enumerate(xmasks):
+                if ((x & rm) == rm and (~x & full & cm) == cm) or ((~x & full & rm) == rm and (x & cm) == cm):
+                    m |= 1 << i
+            if m and m not in by_set:
+                by_set[m] = (rm, cm)
+    sets = sorted(by_set, key=lambda m: (-bin(m).count("1"), m))
+    sets = [m for m in sets if not any((m | o) == o and m != o for o in sets)]
+    everything = (1 << len(xmasks)) - 1
+    for k in range(1, 5):
+        for combo in itertools.combinations(sets, k):
+            u = 0
+            for m in combo:
+                u |= m
+            if u == everything:
+                out, seen = [], 0
+                for m in combo:
+                    out.append(by_set[m] + ([i for i in range(len(xmasks)) if (m >> i) & 1 and not (seen >> i) & 1],))
+                    seen |= m
+                return out
+    raise AssertionError("no cover of the entries of a flow by <= 4 classes")
 
 
 def build(n):
