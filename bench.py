@@ -39,7 +39,7 @@ def ncu_dram_bytes_per_event(process, precision):
     for line in open(TRAFFIC_CSV):
         f = [x.strip() for x in line.split(",")]
         if len(f) >= 6 and f[0] == process and f[1] == precision:
-            last = ((float(f[3]) + float(f[4])) / float(f[2]), f[5])
+            last = ((float(f[3]) + float(f[4])) / float(f[2]), ", ".join(f[5:]))
     return last if last else (None, None)
 
 HEADLINE = "gg_ttxggg"      # BASELINE.json configs[4]: the process the north star's roofline targets are set on
