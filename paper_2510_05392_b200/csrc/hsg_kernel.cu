@@ -235,20 +235,25 @@ __device__ __forceinline__ unsigned acc_swz(unsigned h)
     return h ^ (((hi & 1) * 3) ^ (((hi >> 1) & 1) * 5) ^ (((hi >> 2) & 1) * 6) ^ (((hi >> 3) & 1) * 7) ^ ((hi >> 4) & 1));
 }
 
-// a finished class: its fragments are added to the flow's accumulator (first class: plain store) and cleared.  L = swizzled slot
-// of the lane's elements for tile 0, tw0 / tw1 = the tiles' slots (one byte each), XORed on (the swizzle is linear)
-__device__ __forceinline__ void p3t_flush(char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, bool first, double (&f)[16])
+// Class changes.  The flow's running sum lives in the accumulator fragments: when a class ends they are STORED to the warp's
+// accumulator in shared memory (slot of the lane's elements for tile t: L ^ byte t of (tw0, tw1); the swizzle is linear), and the
+// next class LOADS them back in its own (lane, tile) order -- the tensor instructions then add onto them.  No FP64 additions: a
+// flush by read-add-write put 16 DADDs per class behind the other warps' tensor instructions in the FP64 pipe's queue.
+__device__ __forceinline__ void p3t_store(char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, const double (&f)[16])
 {
 #pragma unroll
     for (int t = 0; t < 8; t++) {
         const unsigned idx = L ^ (((t < 4 ? tw0 : tw1) >> (8 * (t & 3))) & 0xFFu);
-        double2* __restrict__ p = reinterpret_cast<double2*>(acc + 16u * idx);
-        double2 v = make_double2(0.0, 0.0);
-        if (!first) v = *p;
-        v.x += f[2 * t];
-        v.y += f[2 * t + 1];
-        *p = v;
-        f[2 * t] = f[2 * t + 1] = 0.0;
+        *reinterpret_cast<double2*>(acc + 16u * idx) = make_double2(f[2 * t], f[2 * t + 1]);
+    }
+}
+__device__ __forceinline__ void p3t_load(const char* __restrict__ acc, unsigned L, unsigned tw0, unsigned tw1, double (&f)[16])
+{
+#pragma unroll
+    for (int t = 0; t < 8; t++) {
+        const unsigned idx = L ^ (((t < 4 ? tw0 : tw1) >> (8 * (t & 3))) & 0xFFu);
+        const double2 v = *reinterpret_cast<const double2*>(acc + 16u * idx);
+        f[2 * t] = v.x; f[2 * t + 1] = v.y;
     }
 }
 
@@ -478,7 +483,7 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                 if (fl.z > 0) stage(nxt, 0);
                 asm volatile("cp.async.commit_group;" ::: "memory");     // one commit group per entry, empty past the end
                 int bcur = 0, bnew = 1, cls = 0;
-                bool pend = false, pfirst = false;
+                bool pend = false;
                 unsigned pL = 0, ptw0 = 0, ptw1 = 0;
                 for (int k = 0; k < fl.z; k++) {
                     const int4 cur = nxt;
@@ -492,10 +497,16 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     }
                     if (k + 1 < fl.z) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent.y, k + 1) & 0xFFFF));
                     else if (fn < d.nflow) v = __ldg(lt + 32 * (size_t)(__shfl_sync(0xffffffffu, myent_n.y, 0) & 0xFFFF));
-                    // the class that ended with the previous entry is flushed HERE, behind the copy and the prefetches of this
-                    // iteration: its last tensor instructions have ~200 cycles of latency, which the flush would wait for if it
-                    // followed them directly (measured: the flush was 5.7 of 26.8 ms)
-                    if (pend) { p3t_flush(acc, pL, ptw0, ptw1, pfirst, fr); pend = false; }
+                    // the class that ended with the previous entry is stored HERE, behind the copy and the prefetches of this
+                    // iteration (its last tensor instructions have ~200 cycles of latency), and the running sum comes back in the
+                    // order of this entry's class
+                    if (pend) {
+                        p3t_store(acc, pL, ptw0, ptw1, fr);
+                        __syncwarp();
+                        p3t_load(acc, (myL >> (8 * cls)) & 0xFFu, __shfl_sync(0xffffffffu, myT, 2 * cls),
+                                 __shfl_sync(0xffffffffu, myT, 2 * cls + 1), fr);           // (cls = the class of entry k)
+                        pend = false;
+                    }
                     asm volatile("cp.async.wait_group %0;" ::"n"(HSG_P3_STAGES - 1) : "memory");
                     __syncwarp();
                     const char* __restrict__ bx = wbuf + bcur * d.p3buf;
@@ -510,7 +521,6 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     if (cur.y & (1 << 24)) {                             // last entry of its class (uniform over the warp)
                         ptw0 = __shfl_sync(0xffffffffu, myT, 2 * cls); ptw1 = __shfl_sync(0xffffffffu, myT, 2 * cls + 1);
                         pL = (myL >> (8 * cls)) & 0xFFu;
-                        pfirst = cls == 0;
                         pend = true;
                         cls++;
                     }
@@ -518,7 +528,9 @@ __global__ void __launch_bounds__(HSG_THREADS, HSG_CTAS) hsg_diagrams_kernel(con
                     bnew = bcur;
                     bcur = bcur + 1 == HSG_P3_STAGES ? 0 : bcur + 1;
                 }
-                if (pend) { p3t_flush(acc, pL, ptw0, ptw1, pfirst, fr); pend = false; }     // (a flow ends with the end of a class)
+                if (pend) { p3t_store(acc, pL, ptw0, ptw1, fr); pend = false; }     // (a flow ends with the end of a class)
+#pragma unroll
+                for (int i = 0; i < 16; i++) fr[i] = 0.0;                 // the next flow starts from zero
                 __syncwarp();
                 // the finished jamp of this flow: lane = the helicities of particles 3 .. 7 (low bits of h), q = particles 0, 1, 2
                 {
