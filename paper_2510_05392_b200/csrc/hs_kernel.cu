@@ -294,6 +294,35 @@ __device__ __forceinline__ void p3_flush(char* __restrict__ acc, const uint2 cl,
     }
 }
 
+// Class changes, second form (HS_STLD): the flow's running sum travels in the fragments.  A finished class STORES (re, im) = (f[4t] - f[4t+2], f[4t+1]
+// + f[4t+3]) to the flow's accumulator; the next class LOADS it back into f[4t], f[4t+1] in its own (lane, tile) order and the tensor
+// instructions add onto it.  (A read-add-write flush had 16 FP64 additions per class waiting in the FP64 pipe's queue behind the
+// other warps' tensor instructions.  Measured: generic kernel -3 % (hsg_kernel.cu), g g -> t tbar g g -2.3 % (13.34 -> 13.03 ms per
+// 262 144 events), g g -> t tbar g g g +1.4 % (36.60 -> 37.12 ms: the warp barrier and the load in front of every class's first
+// tensor instruction cost more there) -- hence per process.)
+template <int NG> struct HsStLd { static constexpr bool value = NG == 4; };
+template <int NTILE>
+__device__ __forceinline__ void p3_store(char* __restrict__ acc, const uint2 cl, const double (&f)[4 * NTILE])
+{
+#pragma unroll
+    for (int t = 0; t < NTILE; t++) {
+        const unsigned word = t < 2 ? cl.x : cl.y;
+        const unsigned off = (t & 1) ? (word >> 16) : (word & 0xFFFFu);
+        *reinterpret_cast<double2*>(acc + off) = make_double2(f[4 * t] - f[4 * t + 2], f[4 * t + 1] + f[4 * t + 3]);
+    }
+}
+template <int NTILE>
+__device__ __forceinline__ void p3_load(const char* __restrict__ acc, const uint2 cl, double (&f)[4 * NTILE])
+{
+#pragma unroll
+    for (int t = 0; t < NTILE; t++) {
+        const unsigned word = t < 2 ? cl.x : cl.y;
+        const unsigned off = (t & 1) ? (word >> 16) : (word & 0xFFFFu);
+        const double2 v = *reinterpret_cast<const double2*>(acc + off);
+        f[4 * t] = v.x; f[4 * t + 1] = v.y; f[4 * t + 2] = 0.0; f[4 * t + 3] = 0.0;
+    }
+}
+
 // accumulator slot of helicity combination h (gen/co_program.py acc_swizzle)
 __device__ __forceinline__ int acc_swizzle(int h)
 {
@@ -352,14 +381,20 @@ __device__ __forceinline__ void p3_static_class(const P3Recs<NMAX>& q, P3Recs<NM
         if (HsCfg<NG>::P3_PAD && C > 0 && hp[C] == 0) return;      // a padded flow does not have this class
         const uint2 cl = __ldg(cp + 32 * C);
         double f[4 * NTILE];
+        if constexpr (C == 0 || !HsStLd<NG>::value) {
 #pragma unroll
-        for (int i = 0; i < 4 * NTILE; i++) f[i] = 0.0;
+            for (int i = 0; i < 4 * NTILE; i++) f[i] = 0.0;
+        } else {
+            __syncwarp();                                   // the previous class's stores (other lanes' slots)
+            p3_load<NTILE>(acc, cl, f);
+        }
         constexpr int n0 = H & 15, n1 = (H >> 4) & 15, n2 = (H >> 8) & 15;
         p3_static_run<NG, H, 0, 0, NMAX>(q, objl, stgl, f);
         p3_static_run<NG, H, 1, n0, NMAX>(q, objl, stgl, f);
         p3_static_run<NG, H, 2, n0 + n1, NMAX>(q, objl, stgl, f);
         p3_static_run<NG, H, 3, n0 + n1 + n2, NMAX>(q, objl, stgl, f);
-        p3_flush<NTILE>(acc, cl, f, C == 0);
+        if constexpr (HsStLd<NG>::value) p3_store<NTILE>(acc, cl, f);
+        else p3_flush<NTILE>(acc, cl, f, C == 0);
     }
 }
 
