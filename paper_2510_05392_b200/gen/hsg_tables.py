@@ -35,8 +35,9 @@ outer-product sum out[hp][hq] = sum_c P_c[hp] Q_c[hq] over the four components, 
 helicities of three particles R (all legs of one operand, P), column pairs (re, im) = the helicities of two particles C (legs of
 the other operand, Q), tile index = the helicities of the remaining three particles T.  The accumulator fragments stay in
 registers as long as (R, C) do not change: the entries of a flow are grouped into CLASSES with one (R, C) each (smallest cover,
-3 classes per flow at 6 gluons) and stored class by class; a finished class is added to the flow's accumulator in shared
-memory (slot of combination h = swz(h), conflict-free for the class's lane order where the choice of R[0] allows it).
+3 classes per flow at 6 gluons) and stored class by class; at a class change the flow's running sum goes through the warp's
+accumulator in shared memory -- stored in the old class's (lane, tile) order, loaded back in the new one's (slot of combination h =
+swz(h), conflict-free for a class's lane order where the choice of R[0] allows it).
   dentry[e]  = { first slot of X | first slot of Y << 16, row of ltab | legs of X << 16 | MASK << 20 | negative << 23 |
                  last entry of its class << 24, d0 | d1 << 16, d2 | swx << 16 | swy << 20 }: MASK bit i = T[i] is a leg of P; d_i =
                  byte distance in the warp's operand buffer between the variants that differ in the helicity of T[i] (added to the
