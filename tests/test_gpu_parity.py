@@ -481,9 +481,10 @@ def test_gg_ttxgggg_phase3_forms_agree(B):
 
 
 def test_gg_ttxgggg_full_batch_sampled(B):
-    """the 4096-event batch bench.py times for g g -> t tbar g g g g (12 GB of jamps, one launch per kernel), oracle on 48
-    sampled events (first, last, around the multiples of the 296 persistent CTAs' stride, random); then the same batch in
-    chunks of 128 events (jamp_chunk_mib) and as a replayed CUDA graph: identical numbers"""
+    """the 4096-event batch bench.py times for g g -> t tbar g g g g (12 GB of jamps, one launch per kernel), oracle on >= 256
+    sampled events (the first and the last 64, both sides of the multiples of the 148 persistent CTAs' stride, 128 random: ~8 s
+    of oracle time on 16 cores); then the same batch in chunks of 128 events (jamp_chunk_mib) and as a replayed CUDA graph:
+    identical numbers"""
     process = "gg_ttxgggg"
     nevt = inputs.PROCESSES[process]["nevt"]
     mom = inputs.momenta(process, nevt)
@@ -492,8 +493,10 @@ def test_gg_ttxgggg_full_batch_sampled(B):
     me = proc.sigma_batch(d_mom).cpu().numpy()
     assert np.isfinite(me).all() and (me > 0).all()
     rng = np.random.default_rng(4)
-    idx = np.unique(np.concatenate([[0, 1, 15, 16, 295, 296, 297, 591, 592, nevt - 2, nevt - 1],
-                                    rng.choice(nevt, 37, replace=False)]))
+    stride = np.arange(148, nevt, 148)
+    idx = np.unique(np.concatenate([np.arange(64), np.arange(nevt - 64, nevt), stride[::3] - 1, stride[::3],
+                                    rng.choice(nevt, 128, replace=False)]))
+    assert idx.size >= 256
     ref = _oracle(process, mom[idx])
     _histogram(_relerr(me[idx], ref), "gg_ttxgggg full batch, sampled")
     _assert_fp64_parity(process, mom[idx], me[idx], _relerr(me[idx], ref))
