@@ -302,7 +302,7 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 // DMMA kernel for a colour matrix that does not fit in shared memory (720 colours: g g -> t tbar g g g g, SURVEY.md §8(f)
 // row 3; PAPER.md:580-613 makes this contraction the point of the 2 -> 6 process).  Same triangular form Z = X L.
 //   - a CTA (16 warps) = 16 rows, their Re and Im parts: M = 32 = four m8 tiles; all 32 x NC accumulators stay in
-//     registers (NC / 8 n-tiles dealt to the warps in pairs (j, NC/8 - 1 - j): equal numbers of k-steps);
+//     registers (units of two m8 tiles x one n-tile; warp w: part w % 2, n-tiles w / 2 + 8 k);
 //   - jamps AND factor stream through a 3-stage cp.async ring, 8 colours (two k-steps) per chunk: [8][32] jamps (row stride 40
 //     doubles: the A-fragment reads fall into distinct bank pairs) and, per k-step, the factor's fragments of the n-tiles on or
 //     below the diagonal.  The factor lives in global memory (4 MB, L2-resident) in FRAGMENT order, element [lane] of block
@@ -312,7 +312,7 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 template <int NC>
 struct CsBig {
     static constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 8, NCHUNK = NC / KC, STG = 3, STRIDE = 40;
-    static constexpr int SLOTS = 2 * ((NPAIR + 15) / 16);
+    static constexpr int SLOTS = (NT8 + 7) / 8;                               // n-tiles per warp: (warp / 2) + 8 k
     static constexpr size_t L_STAGE = (size_t)(KC / 4) * NT8 * 32;            // doubles: the two k-steps of a chunk, all n-tiles
     static constexpr size_t SMEM = sizeof(double) * (STG * L_STAGE + STG * KC * STRIDE + 16 * 32);
 };
@@ -352,26 +352,19 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
         }
         asm volatile("cp.async.commit_group;");
     };
-    double acc[SLOTS][4][2];
+    // Work units = (n-tile, half of the M rows): warp w takes the Re part (even w) or the Im part (odd w) of the rows -- two m8
+    // tiles -- and the n-tiles (w / 2) + 8 k, k = 0 .. SLOTS - 1.  At chunk c the n-tiles 0 .. c are on or below the diagonal, so
+    // a warp's active tiles are a PREFIX of its slots (its length picks a branch-free body: a predicated-off DMMA still occupies
+    // the tensor pipe -- measured: predication made this kernel 2x slower) and the warps' counts differ by at most one with
+    // max = ceil((c + 1) / 8) units of 4 DMMAs.  (First version: units of four m8 tiles dealt in pairs (j, NT8 - 1 - j), max =
+    // ceil((c + 1) / 16) units of 8 DMMAs: 8 % more tensor instructions on the critical path of the chunks.)
+    double acc[SLOTS][2][2];
 #pragma unroll
     for (int s = 0; s < SLOTS; s++)
 #pragma unroll
-        for (int m = 0; m < 4; m++) acc[s][m][0] = acc[s][m][1] = 0.0;
-    // the n-tiles of this warp in ASCENDING order (slot s < SLOTS / 2: pair s's low tile, then the high tiles backwards), so
-    // that the tiles on or below the diagonal at chunk c are a PREFIX of the slots: its length picks a branch-free body.
-    // (A predicated-off DMMA still occupies the tensor pipe -- measured: predication made this kernel 2x slower.)
-    int jn[SLOTS];
-#pragma unroll
-    for (int s = 0; s < SLOTS; s++) {
-        const int pr = warp + 16 * (s < SLOTS / 2 ? s : SLOTS - 1 - s);
-        jn[s] = pr < NPAIR ? (s < SLOTS / 2 ? pr : NT8 - 1 - pr) : (1 << 20);         // no such pair: never active
-    }
-    static_assert(SLOTS == 6, "the switch below lists 1 .. 6 active tiles");
-#pragma unroll
-    for (int pass = 0; pass < SLOTS - 1; pass++)                                      // (a missing third pair sorts last)
-#pragma unroll
-        for (int s = 0; s + 1 < SLOTS - pass; s++)
-            if (jn[s] > jn[s + 1]) { const int t = jn[s]; jn[s] = jn[s + 1]; jn[s + 1] = t; }
+        for (int m = 0; m < 2; m++) acc[s][m][0] = acc[s][m][1] = 0.0;
+    const int half = warp & 1, j0 = warp >> 1;
+    static_assert(SLOTS == 12, "the switch below lists 1 .. 12 active tiles");
     load_chunk(0);
     load_chunk(1);
     const int ak = lane & 3, ar = lane >> 2;
@@ -380,23 +373,22 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
         asm volatile("cp.async.wait_group 1;");
         __syncthreads();
         load_chunk(c + 2);
-        const double* __restrict__ jt = js + (size_t)(c % STG) * KC * STRIDE;
-        const double* __restrict__ lt = ls + (size_t)(c % STG) * Cfg::L_STAGE + lane;
-        int nact = 0;
-#pragma unroll
-        for (int s = 0; s < SLOTS; s++) nact += jn[s] <= c;
+        const double* __restrict__ jt = js + (size_t)(c % STG) * KC * STRIDE + 16 * half + ar;
+        const double* __restrict__ lt = ls + (size_t)(c % STG) * Cfg::L_STAGE + (size_t)j0 * 32 + lane;
+        // active slots: n-tiles j0 + 8 k <= c, and < NT8
+        int nact = c >= j0 ? (c - j0) / 8 + 1 : 0;
+        const int nmax = (NT8 - 1 - j0) / 8 + 1;
+        nact = nact < nmax ? nact : nmax;
         auto body = [&](auto NA) {
             constexpr int NACT = decltype(NA)::value;
 #pragma unroll
             for (int kk = 0; kk < KC / 4; kk++) {
-                double a[4];
-#pragma unroll
-                for (int m = 0; m < 4; m++) a[m] = jt[(4 * kk + ak) * STRIDE + 8 * m + ar];
+                const double a0 = jt[(4 * kk + ak) * STRIDE], a1 = jt[(4 * kk + ak) * STRIDE + 8];
 #pragma unroll
                 for (int s = 0; s < NACT; s++) {
-                    const double b = lt[((size_t)kk * NT8 + jn[s]) * 32];
-#pragma unroll
-                    for (int m = 0; m < 4; m++) dmma(acc[s][m][0], acc[s][m][1], a[m], b);
+                    const double b = lt[((size_t)kk * NT8 + 8 * s) * 32];
+                    dmma(acc[s][0][0], acc[s][0][1], a0, b);
+                    dmma(acc[s][1][0], acc[s][1][1], a1, b);
                 }
             }
         };
@@ -407,24 +399,30 @@ __global__ void __launch_bounds__(512, 1) color_sum_big_kernel(const double* __r
             case 4: body(std::integral_constant<int, 4>()); break;
             case 5: body(std::integral_constant<int, 5>()); break;
             case 6: body(std::integral_constant<int, 6>()); break;
+            case 7: body(std::integral_constant<int, 7>()); break;
+            case 8: body(std::integral_constant<int, 8>()); break;
+            case 9: body(std::integral_constant<int, 9>()); break;
+            case 10: body(std::integral_constant<int, 10>()); break;
+            case 11: body(std::integral_constant<int, 11>()); break;
+            case 12: body(std::integral_constant<int, 12>()); break;
             default: break;
         }
     }
-    // sum of squares per m-row: lanes of a quad hold the 8 columns of a row
+    // sum of squares per row of this warp's part: lanes of a quad hold the 8 columns of a row
 #pragma unroll
-    for (int m = 0; m < 4; m++) {
+    for (int m = 0; m < 2; m++) {
         double v = 0.0;
 #pragma unroll
         for (int s = 0; s < SLOTS; s++) v += acc[s][m][0] * acc[s][m][0] + acc[s][m][1] * acc[s][m][1];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
-        if (ak == 0) red[warp * 32 + 8 * m + ar] = v;
+        if (ak == 0) red[warp * 16 + 8 * m + ar] = v;
     }
     __syncthreads();
     if (tid < 16) {
         double v = 0.0;
 #pragma unroll
-        for (int w = 0; w < 16; w++) v += red[w * 32 + tid] + red[w * 32 + 16 + tid];       // Re part + Im part of the row
+        for (int w = 0; w < 16; w++) v += red[w * 16 + tid];                 // Re part (even warps) + Im part (odd warps) of the row
         map.store(meh, r0 + tid, v);
     }
 }
