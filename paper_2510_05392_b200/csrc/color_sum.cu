@@ -311,7 +311,7 @@ bool color_cholesky_padded(int ncolor, const int* cmat, std::vector<double>& lp,
 // C is only positive SEMI-definite at 6 gluons (rank 685 of 720): the factor has zero columns there (color_cholesky_big).
 template <int NC>
 struct CsBig {
-    static constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 8, NCHUNK = NC / KC, STG = 3, STRIDE = 40;
+    static constexpr int NT8 = NC / 8, NPAIR = NT8 / 2, KC = 8, NCHUNK = NC / KC, STG = 3, STRIDE = 36;   // (36 = 4 mod 16: the 16 lanes of an A-fragment load phase, 4 k x 4 rows, hit 16 different 8-byte banks; 40 gave a two-way conflict)
     static constexpr int SLOTS = (NT8 + 7) / 8;                               // n-tiles per warp: (warp / 2) + 8 k
     static constexpr size_t L_STAGE = (size_t)(KC / 4) * NT8 * 32;            // doubles: the two k-steps of a chunk, all n-tiles
     static constexpr size_t SMEM = sizeof(double) * (STG * L_STAGE + STG * KC * STRIDE + 16 * 32);
